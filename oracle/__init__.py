@@ -1,0 +1,149 @@
+"""CPU ORACLE -- test infrastructure, not the product.
+
+Python face of ``oracle/sph_oracle.c`` (read that file's header first).  Only
+``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package; the product package
+``paper_2302_08381_b200`` never does, and this package never imports it.
+
+Two builds of the same C file:
+
+* ``ld``  -- ``long double`` (x86 80-bit, eps 1.08e-19): the parity reference.
+  Needed because the f64 tolerance (1e-12 with a 1e-3 row-scaled floor)
+  asks for ~1e-15 of the row scale, which an f64 evaluation of Eq. 7 at l=32 does
+  not deliver itself.
+* ``f64`` -- ``double`` + OpenMP over points: the timed CPU baseline ("trivially
+  parallelized over the sample index using OpenMP").
+
+Paper citations ``P:n`` are lines of PAPER.md (arXiv 2302.08381).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+_SRC = _HERE / "sph_oracle.c"
+_LIBS = {"ld": _HERE / "liboracle_ld.so", "f64": _HERE / "liboracle_f64.so"}
+_FLAGS = {"ld": ["-DORACLE_LONG_DOUBLE"], "f64": []}
+_DTYPE = {"ld": np.longdouble, "f64": np.float64}
+_loaded: dict[str, ctypes.CDLL] = {}
+
+
+def build(force: bool = False) -> None:
+    """Compile both builds with gcc (-O2 -fopenmp, no -ffast-math)."""
+    for kind, lib in _LIBS.items():
+        if not force and lib.exists() and lib.stat().st_mtime >= _SRC.stat().st_mtime:
+            continue
+        tmp = lib.with_suffix(f".tmp{os.getpid()}.so")
+        cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", *_FLAGS[kind],
+               "-o", str(tmp), str(_SRC), "-lm"]
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, lib)
+
+
+def _lib(kind: str) -> ctypes.CDLL:
+    if kind not in _loaded:
+        build()
+        _loaded[kind] = ctypes.CDLL(str(_LIBS[kind]))
+    return _loaded[kind]
+
+
+def _fn(kind: str, name: str):
+    return getattr(_lib(kind), f"{name}_{kind}")
+
+
+def _ptr(a):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def n_sph(l_max: int) -> int:
+    return (l_max + 1) ** 2
+
+
+def num_threads(kind: str = "f64") -> int:
+    f = _fn(kind, "oracle_num_threads")
+    f.restype = ctypes.c_int
+    return int(f())
+
+
+def compute(xyz, l_max: int, normalized: bool, gradients: bool = False, hessians: bool = False,
+            kind: str = "ld", out=None):
+    """Oracle for ``sphericart_cuda_compute``.
+
+    ``xyz`` [n,3] float32/float64 (the exact values the GPU receives; widened to double, which
+    is exact).  Returns ``(sph [n,L], dsph [n,3,L] | None, ddsph [n,3,3,L] | None)`` in
+    ``np.longdouble`` (kind="ld") or ``np.float64`` (kind="f64").  ``out`` may hold preallocated
+    ``(sph, dsph, ddsph)`` of that dtype.
+    """
+    if hessians and not gradients:
+        raise ValueError("hessians need gradients (SURVEY 8(b))")
+    xyz = np.ascontiguousarray(np.asarray(xyz), dtype=np.float64).reshape(-1, 3)
+    n, L, dt = xyz.shape[0], n_sph(l_max), _DTYPE[kind]
+    if out is None:
+        sph = np.empty((n, L), dt)
+        dsph = np.empty((n, 3, L), dt) if gradients else None
+        ddsph = np.empty((n, 3, 3, L), dt) if hessians else None
+    else:
+        sph, dsph, ddsph = out
+    f = _fn(kind, "oracle_compute")
+    f.restype = ctypes.c_int
+    f.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_int,
+                  ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+    rc = f(_ptr(xyz), n, int(l_max), int(bool(normalized)), _ptr(sph), _ptr(dsph), _ptr(ddsph))
+    if rc != 0:
+        raise RuntimeError("oracle_compute failed")
+    return sph, dsph, ddsph
+
+
+def vjp(dsph, grad_sph, l_max: int, kind: str = "ld"):
+    """Oracle for ``sphericart_cuda_vjp``: grad_xyz[n,a] = sum_k dsph[n,a,k] grad_sph[n,k]."""
+    dt = _DTYPE[kind]
+    dsph = np.ascontiguousarray(np.asarray(dsph), dtype=dt)
+    grad_sph = np.ascontiguousarray(np.asarray(grad_sph), dtype=dt)
+    n = grad_sph.shape[0]
+    out = np.empty((n, 3), dt)
+    f = _fn(kind, "oracle_vjp")
+    f.restype = ctypes.c_int
+    f.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_void_p]
+    if f(_ptr(dsph), _ptr(grad_sph), n, int(l_max), _ptr(out)) != 0:
+        raise RuntimeError("oracle_vjp failed")
+    return out
+
+
+def F_table(l_max: int, kind: str = "ld"):
+    """F_l^m (Eq. C1) as a flat triangle, index l(l+1)/2+m."""
+    out = np.empty((l_max + 1) * (l_max + 2) // 2, _DTYPE[kind])
+    f = _fn(kind, "oracle_F_table")
+    f.restype = None
+    f.argtypes = [ctypes.c_int, ctypes.c_void_p]
+    f(int(l_max), _ptr(out))
+    return out
+
+
+def Q_triangle(z, r2, l_max: int):
+    """Q_l^m(z, r^2) (Eq. 7) in long double, flat triangle index l(l+1)/2+m."""
+    out = np.empty((l_max + 1) * (l_max + 2) // 2, np.longdouble)
+    zz = np.array([z], np.longdouble)
+    rr = np.array([r2], np.longdouble)
+    f = _fn("ld", "oracle_Q_p")
+    f.restype = None
+    f.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p]
+    f(_ptr(zz), _ptr(rr), int(l_max), _ptr(out))
+    return out
+
+
+def cs(x, y, l_max: int):
+    """c_m, s_m (Eq. 9) in long double."""
+    c = np.empty(l_max + 1, np.longdouble)
+    s = np.empty(l_max + 1, np.longdouble)
+    xx = np.array([x], np.longdouble)
+    yy = np.array([y], np.longdouble)
+    f = _fn("ld", "oracle_cs_p")
+    f.restype = None
+    f.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p]
+    f(_ptr(xx), _ptr(yy), int(l_max), _ptr(c), _ptr(s))
+    return c, s
