@@ -1,0 +1,103 @@
+/*
+ * sphericart_cuda.h -- C ABI of the B200-native spherical-harmonics hot path.
+ *
+ * What is computed (arXiv 2302.08381, "Fast evaluation of spherical harmonics with sphericart";
+ * P:n = line n of PAPER.md): for n Cartesian points, every real spherical harmonic with
+ * l <= l_max -- either the solid harmonics Ytilde_l^m = r^l Y_l^m or the harmonics
+ * normalised on the unit sphere, Y_l^m = Ytilde_l^m(x/r) -- by the Cartesian scheme
+ *      Ytilde_l^m = F_l^|m| Q_l^|m|(z,r) * { s_|m| (m<0) | 1/sqrt2 (m=0) | c_m (m>0) }   Eq. 5
+ * with Q from the modified Legendre recurrence Eq. 7, c_m/s_m from Eq. 9 and the
+ * prefactors of Eq. 3 / Eq. C1; optionally the Cartesian gradients (Eq. 10,
+ * P:89-92), the Hessians (Eq. 10 applied twice) and, for the normalised variant, the chain
+ * rule through x/r.  sphericart_cuda_vjp is the backward pass of P:112.
+ *
+ * Conventions common to every entry point
+ *   dtype        0 = float32, 1 = float64: element type of EVERY array of the call.
+ *   L            (l_max+1)^2 harmonics per point; inside a row the index is k = l*(l+1)+m,
+ *                l ascending, m = -l..l (m<0: sin branch, m>0: cos branch; no Condon-Shortley sign;
+ *                orthonormal on the sphere, Y_0^0 = 1/(2 sqrt(pi))).
+ *   layouts      dense row-major: xyz [n,3], sph [n,L], dsph [n,3,L] (axis order x,y,z),
+ *                ddsph [n,3,3,L] (both triangles stored, exactly equal), grad_sph [n,L],
+ *                grad_xyz [n,3].
+ *   pointers     DEVICE pointers unless the function name ends in _host; owned by the caller;
+ *                base addresses 16-byte aligned; buffers must not alias.  The library never
+ *                returns memory.  It keeps small per-device coefficient tables for the process
+ *                lifetime.
+ *   stream       a cudaStream_t passed as void* (NULL = the legacy default stream).  Device entry
+ *                points only enqueue work: no host synchronisation.  The first call on a device
+ *                uploads the tables and sets kernel attributes, so time from the second.
+ *   l_max        0 <= l_max <= SPHERICART_CUDA_MAX_L.
+ *   return       0 on success; otherwise one of the SPHERICART_CUDA_E* codes, nothing is launched
+ *                for argument errors, and sphericart_cuda_last_error() describes the failure.
+ *                n == 0 succeeds without a launch.  No exception crosses this boundary.
+ *   r = 0        normalized=1 at a point with r == 0 is mathematically undefined; that point's
+ *                outputs are NaN (IEEE), other points are unaffected.  normalized=0 is defined
+ *                there (Ytilde_0^0 = 1/(2 sqrt(pi)), the rest 0).
+ */
+#ifndef SPHERICART_CUDA_H
+#define SPHERICART_CUDA_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SPHERICART_CUDA_MAX_L 32
+
+#define SPHERICART_CUDA_F32 0
+#define SPHERICART_CUDA_F64 1
+
+#define SPHERICART_CUDA_OK 0
+#define SPHERICART_CUDA_EINVAL 1   /* bad argument (NULL, negative n, l_max out of range, bad dtype ...) */
+#define SPHERICART_CUDA_EALIGN 2   /* a base pointer is not 16-byte aligned */
+#define SPHERICART_CUDA_ECUDA 3    /* a CUDA runtime call or the launch failed; see last_error */
+#define SPHERICART_CUDA_ENOMEM 4   /* (_host entry points) device or host allocation failed */
+
+/*
+ * Forward pass ("takes a list of Cartesian coordinates and evaluates the scaled
+ * Ytilde_l^m and, optionally, their derivatives"; P:108 for normalized=1).
+ *   xyz    [n,3]      in
+ *   sph    [n,L]      out
+ *   dsph   [n,3,L]    out, or NULL: no gradients
+ *   ddsph  [n,3,3,L]  out, or NULL: no Hessians; non-NULL requires dsph non-NULL
+ *   normalized  0: solid harmonics r^l Y, derivatives of the polynomials (Eq. 10);
+ *               1: Y on the unit sphere, derivatives of x -> Ytilde(x/|x|) w.r.t. x.
+ */
+int sphericart_cuda_compute(const void* xyz, int64_t n, int l_max, int normalized, int dtype,
+                            void* sph, void* dsph, void* ddsph, void* stream);
+
+/*
+ * Backward pass ("custom backward function to compute gradients using the derivatives
+ * evaluated in the forward pass"):  grad_xyz[i,a] = sum_k dsph[i,a,k] * grad_sph[i,k].
+ *   xyz       [n,3]    accepted for symmetry with the forward call, not read; may be NULL
+ *   dsph      [n,3,L]  in (as written by sphericart_cuda_compute)
+ *   grad_sph  [n,L]    in
+ *   grad_xyz  [n,3]    out
+ * BASELINE.json writes the call as (xyz, dsph, grad_sph, grad_xyz, stream); raw pointers cannot
+ * carry n, l_max and dtype, so they follow the pointers (reading B1).
+ */
+int sphericart_cuda_vjp(const void* xyz, const void* dsph, const void* grad_sph, void* grad_xyz,
+                        int64_t n, int l_max, int dtype, void* stream);
+
+/*
+ * The same two operations on HOST buffers: the library copies xyz (and dsph/grad_sph) to the
+ * device, runs the kernels above and copies the results back, in chunks on two streams so that
+ * transfers overlap compute; returns after everything has landed (synchronises internally).
+ * Pinned host memory gives full PCIe rate; pageable memory works.  Pointers need no alignment.
+ */
+int sphericart_cuda_compute_host(const void* xyz, int64_t n, int l_max, int normalized, int dtype,
+                                 void* sph, void* dsph, void* ddsph);
+int sphericart_cuda_vjp_host(const void* xyz, const void* dsph, const void* grad_sph,
+                             void* grad_xyz, int64_t n, int l_max, int dtype);
+
+/* Message for the last non-zero return on the calling thread ("" if none).  Never NULL. */
+const char* sphericart_cuda_last_error(void);
+
+/* Number of kernels this library has launched in this process (all threads); for harnesses. */
+int64_t sphericart_cuda_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPHERICART_CUDA_H */

@@ -1,0 +1,163 @@
+"""B200-native real spherical harmonics (arXiv 2302.08381's Cartesian scheme): Python binding.
+
+A thin ``ctypes`` face of ``libsphericart_cuda.so`` (``include/sphericart_cuda.h``).  The
+functions below carry the C names and do argument marshalling only -- every step of the path runs
+in the library's sm_100a kernels.  PyTorch supplies device memory and streams, nothing else.
+There is no CPU fallback: if the library is missing or the call fails, an exception is raised.
+
+    sphericart_cuda_compute(xyz, n, l_max, normalized, dtype, sph, dsph, ddsph, stream)
+    sphericart_cuda_vjp(xyz, dsph, grad_sph, grad_xyz, n, l_max, dtype, stream)
+    sphericart_cuda_compute_host(...), sphericart_cuda_vjp_host(...)      host buffers
+    compute(xyz, l_max, ...), vjp(dsph, grad_sph)                         torch.Tensor convenience
+"""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+
+_PKG = Path(__file__).resolve().parent
+_LIB_PATH = _PKG / "libsphericart_cuda.so"
+_lib = None
+
+F32, F64 = 0, 1
+MAX_L = 32
+
+
+class SphericartCudaError(RuntimeError):
+    pass
+
+
+def library_path() -> Path:
+    return _LIB_PATH
+
+
+def load():
+    """Load the CUDA library; raises if it has not been built (no fallback)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not _LIB_PATH.exists():
+        raise SphericartCudaError(
+            f"{_LIB_PATH} is missing: build it with `python -m paper_2302_08381_b200.build` "
+            "(there is no CPU fallback)")
+    lib = ctypes.CDLL(str(_LIB_PATH))
+    vp, i64, ci = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int
+    lib.sphericart_cuda_compute.restype = ci
+    lib.sphericart_cuda_compute.argtypes = [vp, i64, ci, ci, ci, vp, vp, vp, vp]
+    lib.sphericart_cuda_vjp.restype = ci
+    lib.sphericart_cuda_vjp.argtypes = [vp, vp, vp, vp, i64, ci, ci, vp]
+    lib.sphericart_cuda_compute_host.restype = ci
+    lib.sphericart_cuda_compute_host.argtypes = [vp, i64, ci, ci, ci, vp, vp, vp]
+    lib.sphericart_cuda_vjp_host.restype = ci
+    lib.sphericart_cuda_vjp_host.argtypes = [vp, vp, vp, vp, i64, ci, ci]
+    lib.sphericart_cuda_last_error.restype = ctypes.c_char_p
+    lib.sphericart_cuda_last_error.argtypes = []
+    lib.sphericart_cuda_launch_count.restype = i64
+    lib.sphericart_cuda_launch_count.argtypes = []
+    _lib = lib
+    return lib
+
+
+def _ptr(a):
+    """Address of a torch tensor / numpy array / int / None."""
+    if a is None:
+        return None
+    if isinstance(a, int):
+        return a
+    if hasattr(a, "data_ptr"):
+        return a.data_ptr()
+    return a.ctypes.data
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        msg = load().sphericart_cuda_last_error().decode()
+        raise SphericartCudaError(f"{what} failed (code {rc}): {msg}")
+
+
+# --- the C entry points, same names, same argument order ---------------------------------------
+def sphericart_cuda_compute(xyz, n, l_max, normalized, dtype, sph, dsph, ddsph, stream):
+    rc = load().sphericart_cuda_compute(_ptr(xyz), n, l_max, int(normalized), dtype, _ptr(sph),
+                                        _ptr(dsph), _ptr(ddsph), _ptr(stream))
+    _check(rc, "sphericart_cuda_compute")
+
+
+def sphericart_cuda_vjp(xyz, dsph, grad_sph, grad_xyz, n, l_max, dtype, stream):
+    rc = load().sphericart_cuda_vjp(_ptr(xyz), _ptr(dsph), _ptr(grad_sph), _ptr(grad_xyz), n, l_max,
+                                    dtype, _ptr(stream))
+    _check(rc, "sphericart_cuda_vjp")
+
+
+def sphericart_cuda_compute_host(xyz, n, l_max, normalized, dtype, sph, dsph, ddsph):
+    rc = load().sphericart_cuda_compute_host(_ptr(xyz), n, l_max, int(normalized), dtype, _ptr(sph),
+                                             _ptr(dsph), _ptr(ddsph))
+    _check(rc, "sphericart_cuda_compute_host")
+
+
+def sphericart_cuda_vjp_host(xyz, dsph, grad_sph, grad_xyz, n, l_max, dtype):
+    rc = load().sphericart_cuda_vjp_host(_ptr(xyz), _ptr(dsph), _ptr(grad_sph), _ptr(grad_xyz), n,
+                                         l_max, dtype)
+    _check(rc, "sphericart_cuda_vjp_host")
+
+
+def sphericart_cuda_last_error() -> str:
+    return load().sphericart_cuda_last_error().decode()
+
+
+def sphericart_cuda_launch_count() -> int:
+    return int(load().sphericart_cuda_launch_count())
+
+
+# --- torch.Tensor convenience (allocation + marshalling only) -----------------------------------
+def _dtype_code(t):
+    import torch
+
+    if t.dtype == torch.float32:
+        return F32
+    if t.dtype == torch.float64:
+        return F64
+    raise TypeError(f"unsupported dtype {t.dtype}: float32 or float64")
+
+
+def compute(xyz, l_max: int, normalized: bool = True, gradients: bool = False, hessians: bool = False,
+            out=None):
+    """``xyz`` [n,3] CUDA tensor -> ``(sph [n,L], dsph [n,3,L] | None, ddsph [n,3,3,L] | None)``.
+
+    Enqueued on torch's current stream.  ``out`` may hold preallocated ``(sph, dsph, ddsph)``.
+    """
+    import torch
+
+    if not xyz.is_cuda:
+        raise SphericartCudaError("xyz must be a CUDA tensor (no CPU fallback)")
+    if hessians and not gradients:
+        raise ValueError("hessians need gradients")
+    xyz = xyz.contiguous()
+    n, L = xyz.shape[0], (l_max + 1) ** 2
+    if out is None:
+        sph = torch.empty((n, L), dtype=xyz.dtype, device=xyz.device)
+        dsph = torch.empty((n, 3, L), dtype=xyz.dtype, device=xyz.device) if gradients else None
+        ddsph = torch.empty((n, 3, 3, L), dtype=xyz.dtype, device=xyz.device) if hessians else None
+    else:
+        sph, dsph, ddsph = out
+    with torch.cuda.device(xyz.device):
+        stream = torch.cuda.current_stream().cuda_stream
+        sphericart_cuda_compute(xyz, n, l_max, normalized, _dtype_code(xyz), sph, dsph, ddsph, stream)
+    return sph, dsph, ddsph
+
+
+def vjp(dsph, grad_sph, out=None):
+    """``grad_xyz[n,a] = sum_k dsph[n,a,k] grad_sph[n,k]`` on torch's current stream."""
+    import torch
+
+    if not dsph.is_cuda:
+        raise SphericartCudaError("dsph must be a CUDA tensor (no CPU fallback)")
+    dsph, grad_sph = dsph.contiguous(), grad_sph.contiguous()
+    n, L = grad_sph.shape
+    l_max = int(round(L ** 0.5)) - 1
+    if (l_max + 1) ** 2 != L or dsph.shape != (n, 3, L) or dsph.dtype != grad_sph.dtype:
+        raise ValueError("shapes: dsph [n,3,L], grad_sph [n,L], L a perfect square, same dtype")
+    gx = torch.empty((n, 3), dtype=dsph.dtype, device=dsph.device) if out is None else out
+    with torch.cuda.device(dsph.device):
+        stream = torch.cuda.current_stream().cuda_stream
+        sphericart_cuda_vjp(None, dsph, grad_sph, gx, n, l_max, _dtype_code(dsph), stream)
+    return gx

@@ -1,0 +1,429 @@
+// C ABI of the library (include/sphericart_cuda.h): argument checks, one-time per-device setup,
+// kernel selection and launch.  No torch types, no exceptions across the boundary.
+#include "../../include/sphericart_cuda.h"
+
+#include <atomic>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <mutex>
+
+#include <cuda_runtime.h>
+
+#include "kernel_tp.cuh"
+#include "kernel_vjp.cuh"
+#include "kernel_w.cuh"
+
+namespace sphb200 {
+
+static thread_local char g_err[512] = "";
+static std::atomic<int64_t> g_launches{0};
+
+static int fail(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CUDA_TRY(call)                                                                      \
+    do {                                                                                    \
+        cudaError_t e_ = (call);                                                            \
+        if (e_ != cudaSuccess)                                                              \
+            return fail(SPHERICART_CUDA_ECUDA, "%s failed: %s", #call, cudaGetErrorString(e_)); \
+    } while (0)
+
+// ---------------------------------------------------------------------------------------------
+// per-device state
+// ---------------------------------------------------------------------------------------------
+constexpr int MAX_DEVICES = 64;
+struct DeviceState {
+    bool ready = false;
+    int sm_count = 0;
+    int smem_optin = 0;          // max dynamic shared memory per block
+    SphTables* d_tables = nullptr;   // copy of the tables in global memory (warp kernel)
+};
+static DeviceState g_dev[MAX_DEVICES];
+static std::mutex g_mutex;
+static SphTables g_host_tables;
+static std::once_flag g_tables_once;
+
+static int device_state(DeviceState** out) {
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= MAX_DEVICES) return fail(SPHERICART_CUDA_ECUDA, "device index %d out of range", dev);
+    DeviceState& st = g_dev[dev];
+    std::lock_guard<std::mutex> lock(g_mutex);
+    if (!st.ready) {
+        std::call_once(g_tables_once, [] { sph_build_tables(&g_host_tables); });
+        cudaDeviceProp prop;
+        CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
+        if (prop.major < 10)
+            return fail(SPHERICART_CUDA_ECUDA, "device %d is sm_%d%d; this library is built for sm_100a only",
+                        dev, prop.major, prop.minor);
+        st.sm_count = prop.multiProcessorCount;
+        st.smem_optin = (int)prop.sharedMemPerBlockOptin;
+        CUDA_TRY(cudaMemcpyToSymbol(c_tables, &g_host_tables, sizeof(SphTables)));
+        CUDA_TRY(cudaMalloc(&st.d_tables, sizeof(SphTables)));
+        CUDA_TRY(cudaMemcpy(st.d_tables, &g_host_tables, sizeof(SphTables), cudaMemcpyHostToDevice));
+        st.ready = true;
+    }
+    *out = &st;
+    return 0;
+}
+
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) once per (device, kernel)
+static int allow_smem(const void* func, int bytes) {
+    static std::mutex m;
+    static const void* done[MAX_DEVICES][64];
+    static int n_done[MAX_DEVICES];
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    std::lock_guard<std::mutex> lock(m);
+    for (int i = 0; i < n_done[dev]; ++i)
+        if (done[dev][i] == func) return 0;
+    (void)bytes;
+    CUDA_TRY(cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, g_dev[dev].smem_optin));
+    if (n_done[dev] < 64) done[dev][n_done[dev]++] = func;
+    return 0;
+}
+
+static int env_int(const char* name, int dflt) {
+    const char* s = getenv(name);
+    return (s && *s) ? atoi(s) : dflt;
+}
+
+// ---------------------------------------------------------------------------------------------
+// forward: thread-per-point kernel
+// ---------------------------------------------------------------------------------------------
+typedef void (*TpKernel)(const TpParams);
+
+template <typename T, typename R> static TpKernel tp_pick(int deriv, int norm) {
+    if (deriv == 0) return norm ? sph_tp_kernel<T, R, 0, true> : sph_tp_kernel<T, R, 0, false>;
+    return norm ? sph_tp_kernel<T, R, 1, true> : sph_tp_kernel<T, R, 1, false>;
+}
+
+// Can the tp kernel run this shape, and with how many warps?  Returns 0 if not.
+static int tp_plan(const DeviceState& st, int64_t n, int l_max, int deriv, int esize, TpParams* prm,
+                   int* grid, size_t* smem) {
+    if (deriv > 1) return 0;
+    const int L = (l_max + 1) * (l_max + 1);
+    const uint32_t tile_bytes = 32u * L * esize * (deriv ? 4 : 1);
+    const int budget = st.smem_optin - 1024;
+    int max_warps = TP_MAX_THREADS / 32;
+    int nbuf = env_int("SPHB200_TP_NBUF", 0);
+    int warps = env_int("SPHB200_TP_WARPS", 0);
+    if (nbuf <= 0) nbuf = ((int64_t)2 * tile_bytes * 8 <= budget) ? 2 : 1;  // 2 images if >= 8 warps still fit
+    if (warps <= 0) warps = max_warps;
+    int fit = (int)(budget / ((int64_t)nbuf * tile_bytes));
+    if (fit < 1 && nbuf == 2) {
+        nbuf = 1;
+        fit = (int)(budget / (int64_t)tile_bytes);
+    }
+    if (fit < 1) return 0;
+    if (warps > fit) warps = fit;
+    const int64_t n_tiles = (n + 31) / 32;
+    // small problems: spread the tiles over the SMs instead of stacking warps on a few of them
+    int64_t per_sm = (n_tiles + st.sm_count - 1) / st.sm_count;
+    if (per_sm < warps) warps = (int)(per_sm < 1 ? 1 : per_sm);
+    int64_t ctas = (n_tiles + warps - 1) / warps;
+    if (ctas > st.sm_count) ctas = st.sm_count;
+    prm->warps_per_cta = warps;
+    prm->nbuf = nbuf;
+    prm->tile_bytes = tile_bytes;
+    *grid = (int)ctas;
+    *smem = (size_t)warps * nbuf * tile_bytes;
+    return warps;
+}
+
+static int launch_tp(const DeviceState& st, const void* xyz, int64_t n, int l_max, int normalized, int dtype,
+                     void* sph, void* dsph, cudaStream_t stream, bool* handled) {
+    TpParams prm{};
+    int grid = 0;
+    size_t smem = 0;
+    const int deriv = dsph ? 1 : 0;
+    const int esize = dtype == SPHERICART_CUDA_F32 ? 4 : 8;
+    const int warps = tp_plan(st, n, l_max, deriv, esize, &prm, &grid, &smem);
+    *handled = warps > 0;
+    if (!*handled) return 0;
+    prm.xyz = xyz;
+    prm.sph = sph;
+    prm.dsph = dsph;
+    prm.n = n;
+    prm.l_max = l_max;
+    TpKernel k = dtype == SPHERICART_CUDA_F32 ? tp_pick<float, double>(deriv, normalized)
+                                              : tp_pick<double, dd>(deriv, normalized);
+    int rc = allow_smem((const void*)k, (int)smem);
+    if (rc) return rc;
+    k<<<grid, warps * 32, smem, stream>>>(prm);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    CUDA_TRY(cudaGetLastError());
+    return 0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// forward: warp-per-point kernel (any l_max <= 32, Hessians)
+// ---------------------------------------------------------------------------------------------
+static int launch_w(const DeviceState& st, const void* xyz, int64_t n, int l_max, int normalized, int dtype,
+                    void* sph, void* dsph, void* ddsph, cudaStream_t stream) {
+    WkLaunch lw{};
+    int rc = wk_plan(st.sm_count, st.smem_optin, n, l_max, normalized, dtype, sph, dsph, ddsph, xyz,
+                     st.d_tables, &lw);
+    if (rc) return fail(SPHERICART_CUDA_ECUDA, "warp kernel: no launch configuration fits (l_max=%d)", l_max);
+    rc = allow_smem(lw.func, (int)lw.smem);
+    if (rc) return rc;
+    wk_launch(lw, stream);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    CUDA_TRY(cudaGetLastError());
+    return 0;
+}
+
+static bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+
+static int check_common(int64_t n, int l_max, int dtype) {
+    if (n < 0) return fail(SPHERICART_CUDA_EINVAL, "n = %lld is negative", (long long)n);
+    if (l_max < 0 || l_max > SPHERICART_CUDA_MAX_L)
+        return fail(SPHERICART_CUDA_EINVAL, "l_max = %d outside [0, %d]", l_max, SPHERICART_CUDA_MAX_L);
+    if (dtype != SPHERICART_CUDA_F32 && dtype != SPHERICART_CUDA_F64)
+        return fail(SPHERICART_CUDA_EINVAL, "dtype = %d is neither 0 (f32) nor 1 (f64)", dtype);
+    return 0;
+}
+
+static int compute_device(const void* xyz, int64_t n, int l_max, int normalized, int dtype, void* sph,
+                          void* dsph, void* ddsph, cudaStream_t stream) {
+    int rc = check_common(n, l_max, dtype);
+    if (rc) return rc;
+    if (normalized != 0 && normalized != 1)
+        return fail(SPHERICART_CUDA_EINVAL, "normalized = %d is neither 0 nor 1", normalized);
+    if (ddsph && !dsph) return fail(SPHERICART_CUDA_EINVAL, "ddsph given without dsph");
+    if (n == 0) return 0;
+    if (!xyz || !sph) return fail(SPHERICART_CUDA_EINVAL, "xyz and sph must not be NULL when n > 0");
+    if (misaligned(xyz) || misaligned(sph) || misaligned(dsph) || misaligned(ddsph))
+        return fail(SPHERICART_CUDA_EALIGN, "device pointers must be 16-byte aligned");
+    DeviceState* st = nullptr;
+    rc = device_state(&st);
+    if (rc) return rc;
+
+    const char* force = getenv("SPHB200_FORCE_KERNEL");  // "tp" | "w": experiments only
+    const bool force_w = force && force[0] == 'w';
+    if (!ddsph && !force_w) {
+        // the tp kernel wants an odd row length (conflict-free staging) and >= 4 warps per SM
+        TpParams probe{};
+        int grid;
+        size_t smem;
+        const int L = (l_max + 1) * (l_max + 1);
+        const int64_t tile_bytes = 32LL * L * (dtype == SPHERICART_CUDA_F32 ? 4 : 8) * (dsph ? 4 : 1);
+        const bool fits = tile_bytes * 4 <= st->smem_optin - 1024;
+        const bool want_tp = (force && force[0] == 't') || ((L & 1) && fits);
+        if (want_tp && tp_plan(*st, n, l_max, dsph ? 1 : 0, dtype == SPHERICART_CUDA_F32 ? 4 : 8, &probe, &grid, &smem)) {
+            bool handled = false;
+            rc = launch_tp(*st, xyz, n, l_max, normalized, dtype, sph, dsph, stream, &handled);
+            if (rc || handled) return rc;
+        }
+    }
+    return launch_w(*st, xyz, n, l_max, normalized, dtype, sph, dsph, ddsph, stream);
+}
+
+static int vjp_device(const void* dsph, const void* grad_sph, void* grad_xyz, int64_t n, int l_max, int dtype,
+                      cudaStream_t stream) {
+    int rc = check_common(n, l_max, dtype);
+    if (rc) return rc;
+    if (n == 0) return 0;
+    if (!dsph || !grad_sph || !grad_xyz)
+        return fail(SPHERICART_CUDA_EINVAL, "dsph, grad_sph and grad_xyz must not be NULL when n > 0");
+    if (misaligned(dsph) || misaligned(grad_sph) || misaligned(grad_xyz))
+        return fail(SPHERICART_CUDA_EALIGN, "device pointers must be 16-byte aligned");
+    DeviceState* st = nullptr;
+    rc = device_state(&st);
+    if (rc) return rc;
+
+    const int L = (l_max + 1) * (l_max + 1);
+    const int esize = dtype == SPHERICART_CUDA_F32 ? 4 : 8;
+    VjpParams prm{};
+    prm.dsph = dsph;
+    prm.grad_sph = grad_sph;
+    prm.grad_xyz = grad_xyz;
+    prm.n = n;
+    prm.L = L;
+    prm.tile_bytes = 4u * 32u * L * esize;
+    const int budget = st->smem_optin - 1024;
+    int warps = (int)(budget / ((int64_t)VJP_NBUF * prm.tile_bytes + VJP_NBUF * 8));
+    const int want = env_int("SPHB200_VJP_WARPS", VJP_MAX_THREADS / 32);
+    if (warps > want) warps = want;
+    const int64_t n_tiles = (n + 31) / 32;
+    void (*kern)(const VjpParams);
+    if (warps >= 1) {
+        kern = dtype == SPHERICART_CUDA_F32 ? sph_vjp_kernel<float> : sph_vjp_kernel<double>;
+    } else {
+        // rows too long to stage a 32-point tile: warp-per-point streaming kernel
+        return wk_launch_vjp(st->sm_count, dsph, grad_sph, grad_xyz, n, L, dtype, stream, &g_launches) == 0
+                   ? 0
+                   : fail(SPHERICART_CUDA_ECUDA, "vjp launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    }
+    int64_t per_sm = (n_tiles + st->sm_count - 1) / st->sm_count;
+    if (per_sm < warps) warps = (int)(per_sm < 1 ? 1 : per_sm);
+    int64_t ctas = (n_tiles + warps - 1) / warps;
+    if (ctas > st->sm_count) ctas = st->sm_count;
+    prm.warps_per_cta = warps;
+    const size_t smem = (size_t)warps * VJP_NBUF * (prm.tile_bytes + 8);
+    rc = allow_smem((const void*)kern, (int)smem);
+    if (rc) return rc;
+    kern<<<(int)ctas, warps * 32, smem, stream>>>(prm);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    CUDA_TRY(cudaGetLastError());
+    return 0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// host-buffer entry points: chunked, two streams, transfers overlap compute
+// ---------------------------------------------------------------------------------------------
+struct HostWs {  // grow-only device workspace, one set per stream slot
+    void* buf[2][5] = {{nullptr}};
+    size_t cap[2][5] = {{0}};
+    cudaStream_t stream[2] = {nullptr, nullptr};
+    int device = -1;
+};
+static HostWs g_ws;
+static std::mutex g_ws_mutex;
+
+static int ws_reserve(int slot, int which, size_t bytes) {
+    if (g_ws.cap[slot][which] >= bytes) return 0;
+    if (g_ws.buf[slot][which]) cudaFree(g_ws.buf[slot][which]);
+    g_ws.buf[slot][which] = nullptr;
+    g_ws.cap[slot][which] = 0;
+    if (cudaMalloc(&g_ws.buf[slot][which], bytes) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(SPHERICART_CUDA_ENOMEM, "cudaMalloc of %zu bytes failed", bytes);
+    }
+    g_ws.cap[slot][which] = bytes;
+    return 0;
+}
+
+static int ws_streams() {
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (g_ws.device != dev) {
+        for (int s = 0; s < 2; ++s) {
+            for (int w = 0; w < 5; ++w) {
+                if (g_ws.buf[s][w]) cudaFree(g_ws.buf[s][w]);
+                g_ws.buf[s][w] = nullptr;
+                g_ws.cap[s][w] = 0;
+            }
+            if (g_ws.stream[s]) cudaStreamDestroy(g_ws.stream[s]);
+            CUDA_TRY(cudaStreamCreateWithFlags(&g_ws.stream[s], cudaStreamNonBlocking));
+        }
+        g_ws.device = dev;
+    }
+    return 0;
+}
+
+// points per chunk so that one chunk's buffers stay near `target` bytes
+static int64_t chunk_points(int64_t n, size_t bytes_per_point, size_t target) {
+    int64_t c = (int64_t)(target / (bytes_per_point ? bytes_per_point : 1));
+    c &= ~(int64_t)31;
+    if (c < 32) c = 32;
+    return c < n ? c : n;
+}
+
+}  // namespace sphb200
+
+using namespace sphb200;
+
+extern "C" {
+
+int sphericart_cuda_compute(const void* xyz, int64_t n, int l_max, int normalized, int dtype, void* sph,
+                            void* dsph, void* ddsph, void* stream) {
+    return compute_device(xyz, n, l_max, normalized, dtype, sph, dsph, ddsph, static_cast<cudaStream_t>(stream));
+}
+
+int sphericart_cuda_vjp(const void* xyz, const void* dsph, const void* grad_sph, void* grad_xyz, int64_t n,
+                        int l_max, int dtype, void* stream) {
+    (void)xyz;  // reserved (reading B1)
+    return vjp_device(dsph, grad_sph, grad_xyz, n, l_max, dtype, static_cast<cudaStream_t>(stream));
+}
+
+int sphericart_cuda_compute_host(const void* xyz, int64_t n, int l_max, int normalized, int dtype, void* sph,
+                                 void* dsph, void* ddsph) {
+    int rc = check_common(n, l_max, dtype);
+    if (rc) return rc;
+    if (ddsph && !dsph) return fail(SPHERICART_CUDA_EINVAL, "ddsph given without dsph");
+    if (n == 0) return 0;
+    if (!xyz || !sph) return fail(SPHERICART_CUDA_EINVAL, "xyz and sph must not be NULL when n > 0");
+    std::lock_guard<std::mutex> lock(g_ws_mutex);
+    rc = ws_streams();
+    if (rc) return rc;
+    const size_t es = dtype == SPHERICART_CUDA_F32 ? 4 : 8;
+    const size_t L = (size_t)(l_max + 1) * (l_max + 1);
+    const size_t bpp = es * L * (1 + (dsph ? 3 : 0) + (ddsph ? 9 : 0));
+    const int64_t chunk = chunk_points(n, bpp, (size_t)256 << 20);
+    int slot = 0;
+    for (int64_t p0 = 0; p0 < n; p0 += chunk, slot ^= 1) {
+        const int64_t np = (n - p0 < chunk) ? n - p0 : chunk;
+        cudaStream_t s = g_ws.stream[slot];
+        if ((rc = ws_reserve(slot, 0, (size_t)np * 3 * es))) return rc;
+        if ((rc = ws_reserve(slot, 1, (size_t)np * L * es))) return rc;
+        if (dsph && (rc = ws_reserve(slot, 2, (size_t)np * 3 * L * es))) return rc;
+        if (ddsph && (rc = ws_reserve(slot, 3, (size_t)np * 9 * L * es))) return rc;
+        void** b = g_ws.buf[slot];
+        CUDA_TRY(cudaMemcpyAsync(b[0], (const char*)xyz + (size_t)p0 * 3 * es, (size_t)np * 3 * es,
+                                 cudaMemcpyHostToDevice, s));
+        rc = compute_device(b[0], np, l_max, normalized, dtype, b[1], dsph ? b[2] : nullptr,
+                            ddsph ? b[3] : nullptr, s);
+        if (rc) return rc;
+        CUDA_TRY(cudaMemcpyAsync((char*)sph + (size_t)p0 * L * es, b[1], (size_t)np * L * es,
+                                 cudaMemcpyDeviceToHost, s));
+        if (dsph)
+            CUDA_TRY(cudaMemcpyAsync((char*)dsph + (size_t)p0 * 3 * L * es, b[2], (size_t)np * 3 * L * es,
+                                     cudaMemcpyDeviceToHost, s));
+        if (ddsph)
+            CUDA_TRY(cudaMemcpyAsync((char*)ddsph + (size_t)p0 * 9 * L * es, b[3], (size_t)np * 9 * L * es,
+                                     cudaMemcpyDeviceToHost, s));
+    }
+    CUDA_TRY(cudaStreamSynchronize(g_ws.stream[0]));
+    CUDA_TRY(cudaStreamSynchronize(g_ws.stream[1]));
+    return 0;
+}
+
+int sphericart_cuda_vjp_host(const void* xyz, const void* dsph, const void* grad_sph, void* grad_xyz, int64_t n,
+                             int l_max, int dtype) {
+    (void)xyz;
+    int rc = check_common(n, l_max, dtype);
+    if (rc) return rc;
+    if (n == 0) return 0;
+    if (!dsph || !grad_sph || !grad_xyz)
+        return fail(SPHERICART_CUDA_EINVAL, "dsph, grad_sph and grad_xyz must not be NULL when n > 0");
+    std::lock_guard<std::mutex> lock(g_ws_mutex);
+    rc = ws_streams();
+    if (rc) return rc;
+    const size_t es = dtype == SPHERICART_CUDA_F32 ? 4 : 8;
+    const size_t L = (size_t)(l_max + 1) * (l_max + 1);
+    const int64_t chunk = chunk_points(n, 4 * L * es, (size_t)256 << 20);
+    int slot = 0;
+    for (int64_t p0 = 0; p0 < n; p0 += chunk, slot ^= 1) {
+        const int64_t np = (n - p0 < chunk) ? n - p0 : chunk;
+        cudaStream_t s = g_ws.stream[slot];
+        if ((rc = ws_reserve(slot, 2, (size_t)np * 3 * L * es))) return rc;
+        if ((rc = ws_reserve(slot, 1, (size_t)np * L * es))) return rc;
+        if ((rc = ws_reserve(slot, 4, (size_t)np * 3 * es))) return rc;
+        void** b = g_ws.buf[slot];
+        CUDA_TRY(cudaMemcpyAsync(b[2], (const char*)dsph + (size_t)p0 * 3 * L * es, (size_t)np * 3 * L * es,
+                                 cudaMemcpyHostToDevice, s));
+        CUDA_TRY(cudaMemcpyAsync(b[1], (const char*)grad_sph + (size_t)p0 * L * es, (size_t)np * L * es,
+                                 cudaMemcpyHostToDevice, s));
+        rc = vjp_device(b[2], b[1], b[4], np, l_max, dtype, s);
+        if (rc) return rc;
+        CUDA_TRY(cudaMemcpyAsync((char*)grad_xyz + (size_t)p0 * 3 * es, b[4], (size_t)np * 3 * es,
+                                 cudaMemcpyDeviceToHost, s));
+    }
+    CUDA_TRY(cudaStreamSynchronize(g_ws.stream[0]));
+    CUDA_TRY(cudaStreamSynchronize(g_ws.stream[1]));
+    return 0;
+}
+
+const char* sphericart_cuda_last_error(void) { return g_err; }
+
+int64_t sphericart_cuda_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+}  // extern "C"

@@ -1,0 +1,359 @@
+// "w" forward kernel: one WARP per point.  Any l_max <= 32, values / +gradients / +Hessians.
+//
+// Used when a point's outputs are too large for the thread-per-point kernel (config C4:
+// 13 * 1089 * 8 B = 113 KB per point) or its row length is even.  Per point the warp runs
+//   phase A  lane = m: c_m, s_m by square-and-multiply and column m of the Legendre triangle by the
+//            integer-coefficient form of Eq. 7 (tables.h), all lanes stepping l together; the
+//            triangle Qt and (c,s) go to a per-warp scratch in shared memory as f64;
+//   phase B  lane = output index k inside a chunk of CH consecutive harmonics: each lane assembles
+//            ALL components (Y, 3 gradient, 6 unique Hessian) of its (l,m) from the scratch
+//            (assemble_element) and writes them into per-component staging rows in shared memory;
+//   store    each of the 1/4/13 global rows of the chunk is a contiguous run of CH elements; lane j
+//            issues row j as one 1-D TMA bulk store.  A run starts at element (n*rows+j)*L + k0,
+//            which is 16-byte aligned only up to an element offset sigma_j; the staging row holds
+//            the run at offset sigma_j so that shared and global addresses agree mod 16, the
+//            aligned body goes out by TMA and at most AL-1 elements at either end by plain stores.
+// Staging rows are double-buffered, so phase B of the next chunk overlaps the drain of this one.
+#pragma once
+#include <atomic>
+
+#include "ptx.cuh"
+#include "sph_core.cuh"
+
+namespace sphb200 {
+
+struct WkParams {
+    const void* xyz;
+    void* sph;
+    void* dsph;
+    void* ddsph;
+    const SphTables* tab;   // global-memory copy of the tables
+    int64_t n;
+    int l_max;
+    int warps_per_cta;
+    int chunk;              // CH, multiple of 32
+    int nbuf;               // staging images per warp
+};
+
+struct WkTabView {  // phase-B coefficient tables, copied to shared memory once per CTA
+    const double *G1, *Gz, *H2, *Hxz, *Hzz;
+};
+
+constexpr int WK_MAX_THREADS = 512;
+
+template <int DERIV> struct wk_rows {  // global rows per point / staging rows
+    static constexpr int n = DERIV == 0 ? 1 : (DERIV == 1 ? 4 : 13);
+};
+
+// shared-memory carve-up (bytes), identical on host and device
+struct WkSmem {
+    int tsz;            // (l_max+1)(l_max+2)/2
+    int ntab;           // coefficient tables kept in smem: Np + {0,2,5}
+    size_t tab_bytes;
+    size_t scratch_bytes;   // per warp: Qt[tsz] + cs[2(l_max+1)], rounded to 16
+    size_t row_bytes;       // one staging row: (CH + AL) elements
+    size_t stage_bytes;     // per warp: nbuf * rows * row_bytes
+    size_t warp_bytes;
+    __host__ __device__ WkSmem(int l_max, int deriv, int esize, int chunk, int nbuf) {
+        tsz = (l_max + 1) * (l_max + 2) / 2;
+        ntab = 1 + (deriv == 0 ? 0 : (deriv == 1 ? 2 : 5));
+        tab_bytes = ((size_t)ntab * tsz * 8 + 15) & ~(size_t)15;
+        scratch_bytes = ((size_t)(tsz + 2 * (l_max + 1)) * 8 + 15) & ~(size_t)15;
+        const int al = 16 / esize;
+        row_bytes = (size_t)(chunk + al) * esize;
+        const int rows = deriv == 0 ? 1 : (deriv == 1 ? 4 : 13);
+        stage_bytes = (size_t)nbuf * rows * row_bytes;
+        warp_bytes = scratch_bytes + stage_bytes;
+    }
+};
+
+template <typename T, typename R, int DERIV, bool NORM>
+__global__ void __launch_bounds__(WK_MAX_THREADS, 1) sph_w_kernel(const WkParams prm) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    constexpr int ROWS = wk_rows<DERIV>::n;
+    constexpr int AL = 16 / (int)sizeof(T);
+    using RT = rec<R>;
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    const int l_max = prm.l_max;
+    const int L = (l_max + 1) * (l_max + 1);
+    const int CH = prm.chunk;
+    const WkSmem lay(l_max, DERIV, (int)sizeof(T), CH, prm.nbuf);
+
+    // ---- coefficient tables -> shared memory (once per CTA) -----------------------------------
+    double* tabs = reinterpret_cast<double*>(smem);
+    {
+        const double* src[6] = {prm.tab->Np, prm.tab->G1, prm.tab->Gz, prm.tab->H2, prm.tab->Hxz, prm.tab->Hzz};
+        for (int t = 0; t < lay.ntab; ++t)
+            for (int i = threadIdx.x; i < lay.tsz; i += blockDim.x) tabs[t * lay.tsz + i] = src[t][i];
+    }
+    __syncthreads();
+    const double* Np = tabs;
+    WkTabView tv;
+    tv.G1 = tabs + 1 * lay.tsz;
+    tv.Gz = tabs + 2 * lay.tsz;
+    tv.H2 = tabs + 3 * lay.tsz;   // only dereferenced when DERIV == 2
+    tv.Hxz = tabs + 4 * lay.tsz;
+    tv.Hzz = tabs + 5 * lay.tsz;
+
+    unsigned char* my = smem + lay.tab_bytes + (size_t)warp * lay.warp_bytes;
+    double* Qt = reinterpret_cast<double*>(my);
+    double* cs = Qt + lay.tsz;
+    unsigned char* stage = my + lay.scratch_bytes;
+    const int row_elems = CH + AL;
+
+    const T* __restrict__ xyz = static_cast<const T*>(prm.xyz);
+    T* __restrict__ out_base[3] = {static_cast<T*>(prm.sph), static_cast<T*>(prm.dsph), static_cast<T*>(prm.ddsph)};
+    const uint64_t policy = policy_evict_first();
+
+    int nbits = 0;
+    while ((1 << nbits) <= (l_max < 31 ? l_max : 31)) ++nbits;
+
+    const int64_t stride = (int64_t)gridDim.x * prm.warps_per_cta;
+    int buf = 0;
+    for (int64_t pt = (int64_t)warp * gridDim.x + blockIdx.x; pt < prm.n; pt += stride) {
+        const double x = static_cast<double>(xyz[3 * pt + 0]);
+        const double y = static_cast<double>(xyz[3 * pt + 1]);
+        const double z = static_cast<double>(xyz[3 * pt + 2]);
+        R X, Y, Z, r2;
+        double rinv = 1.0;
+        if (NORM) {
+            RT::normalize(x, y, z, X, Y, Z, rinv);
+            r2 = RT::make(1.0, 0.0);
+        } else {
+            X = RT::make(x, 0.0);
+            Y = RT::make(y, 0.0);
+            Z = RT::make(z, 0.0);
+            r2 = RT::r2_of(X, Y, Z);
+        }
+        const double xd = to_double(X), yd = to_double(Y), zd = to_double(Z);
+
+        // ---- phase A: lane = m ---------------------------------------------------------------
+        __syncwarp();  // the previous point's phase B has finished reading the scratch
+        {
+            const int m = lane;
+            R c, s;
+            cs_power<R>(m, X, Y, nbits, c, s);
+            if (m <= l_max) {
+                cs[2 * m] = to_double(c);
+                cs[2 * m + 1] = to_double(s);
+            }
+            if (l_max == 32 && lane == 31) {  // the 33rd column: (c,s)_32 and Qt_32^32 = Np_32^32 * 1
+                const R c32 = X * c - Y * s;
+                const R s32 = X * s + Y * c;
+                cs[64] = to_double(c32);
+                cs[65] = to_double(s32);
+                Qt[SPH_TRI(32, 32)] = Np[SPH_TRI(32, 32)];
+            }
+            R w = RT::make(0.0, 0.0), wp = RT::make(0.0, 0.0);
+            for (int l = 0; l <= l_max; ++l) {
+                const R wn = column_step_int<R, NORM>(l, m, Z, r2, w, wp);
+                wp = w;
+                w = wn;
+                if (m <= l) Qt[SPH_TRI(l, m)] = to_double(w) * Np[SPH_TRI(l, m)];
+            }
+        }
+        __syncwarp();
+
+        // ---- phase B + store: chunks of CH harmonics -----------------------------------------
+        for (int k0 = 0; k0 < L; k0 += CH) {
+            // the staging image we are about to fill must have been drained
+            if (prm.nbuf == 1) bulk_wait_read<0>();
+            else bulk_wait_read<1>();
+            __syncwarp();
+            T* img = reinterpret_cast<T*>(stage + (size_t)buf * ROWS * lay.row_bytes);
+            const int cnt = (L - k0 < CH) ? L - k0 : CH;
+
+            // element offset of row j of this point inside its array, low bits only
+            // rows: 0 = sph; 1..3 = dsph[a]; 4..12 = ddsph[a][b]
+            uint32_t sig[ROWS];
+            {
+                const uint32_t Lu = (uint32_t)L, k0u = (uint32_t)k0;
+                const uint32_t ptl = (uint32_t)pt;  // low 32 bits are enough modulo AL
+                sig[0] = (ptl * Lu + k0u) & (AL - 1);
+                if (DERIV >= 1) {
+#pragma unroll
+                    for (int a = 0; a < 3; ++a) sig[1 + a] = ((ptl * 3u + a) * Lu + k0u) & (AL - 1);
+                }
+                if (DERIV >= 2) {
+#pragma unroll
+                    for (int a = 0; a < 9; ++a) sig[4 + a] = ((ptl * 9u + a) * Lu + k0u) & (AL - 1);
+                }
+            }
+
+            for (int i = lane; i < cnt; i += 32) {
+                const int k = k0 + i;
+                int l = (int)sqrtf((float)k);
+                l += ((l + 1) * (l + 1) <= k);
+                l -= (l * l > k);
+                const int mm = k - l * (l + 1);
+                double o[10];
+                assemble_element<DERIV, NORM>(l, mm, Qt, cs, xd, yd, zd, rinv, tv, o);
+                img[0 * row_elems + sig[0] + i] = static_cast<T>(o[0]);
+                if (DERIV >= 1) {
+                    img[1 * row_elems + sig[1] + i] = static_cast<T>(o[1]);
+                    img[2 * row_elems + sig[2] + i] = static_cast<T>(o[2]);
+                    img[3 * row_elems + sig[3] + i] = static_cast<T>(o[3]);
+                }
+                if (DERIV >= 2) {
+                    // o[4..9] = xx xy xz yy yz zz ; rows 4.. = xx xy xz yx yy yz zx zy zz
+                    img[4 * row_elems + sig[4] + i] = static_cast<T>(o[4]);
+                    img[5 * row_elems + sig[5] + i] = static_cast<T>(o[5]);
+                    img[6 * row_elems + sig[6] + i] = static_cast<T>(o[6]);
+                    img[7 * row_elems + sig[7] + i] = static_cast<T>(o[5]);
+                    img[8 * row_elems + sig[8] + i] = static_cast<T>(o[7]);
+                    img[9 * row_elems + sig[9] + i] = static_cast<T>(o[8]);
+                    img[10 * row_elems + sig[10] + i] = static_cast<T>(o[6]);
+                    img[11 * row_elems + sig[11] + i] = static_cast<T>(o[8]);
+                    img[12 * row_elems + sig[12] + i] = static_cast<T>(o[9]);
+                }
+            }
+            fence_proxy_async_smem();
+            __syncwarp();
+
+            if (lane < ROWS) {
+                const int j = lane;
+                // which array, which row inside the point
+                const int arr = (j == 0) ? 0 : (j < 4 ? 1 : 2);
+                const int rows_in_arr = (arr == 0) ? 1 : (arr == 1 ? 3 : 9);
+                const int jj = (arr == 0) ? 0 : (arr == 1 ? j - 1 : j - 4);
+                const int64_t e = (pt * rows_in_arr + jj) * (int64_t)L + k0;  // first element of the run
+                T* g = out_base[arr] + e;
+                const uint32_t sg = (uint32_t)e & (AL - 1);
+                const T* srow = img + j * row_elems + sg;  // srow[i] <-> g[i]
+                int head = (int)((AL - sg) & (AL - 1));   // elements before the first 16-byte boundary
+                if (head > cnt) head = cnt;
+                const int body = (cnt - head) & ~(AL - 1);
+                for (int i = 0; i < head; ++i) st_cs(g + i, srow[i]);
+                if (body > 0) bulk_store_hint(g + head, srow + head, (uint32_t)body * sizeof(T), policy);
+                for (int i = head + body; i < cnt; ++i) st_cs(g + i, srow[i]);
+                bulk_commit();
+            }
+            buf = (buf + 1 == prm.nbuf) ? 0 : buf + 1;
+        }
+    }
+    bulk_wait_all<0>();
+}
+
+// ---------------------------------------------------------------------------------------------
+// generic VJP for rows too long to stage 32 points: one warp per point, lanes stride over k
+// ---------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(256) sph_vjp_warp_kernel(const T* __restrict__ dsph, const T* __restrict__ gsph,
+                                                           T* __restrict__ gxyz, int64_t n, int L) {
+    const int lane = threadIdx.x & 31;
+    const int64_t warps = (int64_t)gridDim.x * (blockDim.x >> 5);
+    for (int64_t p = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); p < n; p += warps) {
+        const T* g = gsph + p * L;
+        const T* d = dsph + p * 3 * L;
+        double ax = 0.0, ay = 0.0, az = 0.0;
+        for (int k = lane; k < L; k += 32) {
+            const double w = static_cast<double>(__ldcs(g + k));
+            ax = fma(static_cast<double>(__ldcs(d + k)), w, ax);
+            ay = fma(static_cast<double>(__ldcs(d + L + k)), w, ay);
+            az = fma(static_cast<double>(__ldcs(d + 2 * L + k)), w, az);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            ax += __shfl_xor_sync(0xffffffffu, ax, o);
+            ay += __shfl_xor_sync(0xffffffffu, ay, o);
+            az += __shfl_xor_sync(0xffffffffu, az, o);
+        }
+        if (lane == 0) {
+            gxyz[3 * p + 0] = static_cast<T>(ax);
+            gxyz[3 * p + 1] = static_cast<T>(ay);
+            gxyz[3 * p + 2] = static_cast<T>(az);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------
+typedef void (*WkKernel)(const WkParams);
+
+struct WkLaunch {
+    const void* func;
+    WkKernel kern;
+    WkParams prm;
+    int grid, threads;
+    size_t smem;
+};
+
+template <typename T, typename R> static WkKernel wk_pick(int deriv, int norm) {
+    if (deriv == 0) return norm ? sph_w_kernel<T, R, 0, true> : sph_w_kernel<T, R, 0, false>;
+    if (deriv == 1) return norm ? sph_w_kernel<T, R, 1, true> : sph_w_kernel<T, R, 1, false>;
+    return norm ? sph_w_kernel<T, R, 2, true> : sph_w_kernel<T, R, 2, false>;
+}
+
+static inline int wk_env(const char* name, int dflt) {
+    const char* s = getenv(name);
+    return (s && *s) ? atoi(s) : dflt;
+}
+
+static inline int wk_plan(int sm_count, int smem_optin, int64_t n, int l_max, int normalized, int dtype,
+                          void* sph, void* dsph, void* ddsph, const void* xyz, const SphTables* d_tab,
+                          WkLaunch* out) {
+    const int deriv = ddsph ? 2 : (dsph ? 1 : 0);
+    const int esize = dtype == 0 ? 4 : 8;
+    const int L = (l_max + 1) * (l_max + 1);
+    int chunk = wk_env("SPHB200_W_CHUNK", 128);
+    chunk = (chunk + 31) & ~31;
+    if (chunk > ((L + 31) & ~31)) chunk = (L + 31) & ~31;
+    int nbuf = wk_env("SPHB200_W_NBUF", 2);
+    if (nbuf < 1) nbuf = 1;
+    if (nbuf > 2) nbuf = 2;
+    const int budget = smem_optin - 1024;
+    int warps = 0;
+    for (;;) {
+        WkSmem lay(l_max, deriv, esize, chunk, nbuf);
+        warps = (int)(((size_t)budget - lay.tab_bytes) / lay.warp_bytes);
+        if (warps >= 4 || (chunk == 32 && nbuf == 1)) break;
+        if (nbuf == 2 && chunk <= 64) nbuf = 1;
+        else if (chunk > 32) chunk -= 32;
+    }
+    if (warps < 1) return 1;
+    const int want = wk_env("SPHB200_W_WARPS", WK_MAX_THREADS / 32);
+    if (warps > want) warps = want;
+    int64_t per_sm = (n + sm_count - 1) / sm_count;
+    if (per_sm < warps) warps = (int)(per_sm < 1 ? 1 : per_sm);
+    int64_t ctas = (n + warps - 1) / warps;
+    if (ctas > sm_count) ctas = sm_count;
+    WkSmem lay(l_max, deriv, esize, chunk, nbuf);
+    out->kern = dtype == 0 ? wk_pick<float, double>(deriv, normalized) : wk_pick<double, dd>(deriv, normalized);
+    out->func = (const void*)out->kern;
+    out->prm.xyz = xyz;
+    out->prm.sph = sph;
+    out->prm.dsph = dsph;
+    out->prm.ddsph = ddsph;
+    out->prm.tab = d_tab;
+    out->prm.n = n;
+    out->prm.l_max = l_max;
+    out->prm.warps_per_cta = warps;
+    out->prm.chunk = chunk;
+    out->prm.nbuf = nbuf;
+    out->grid = (int)ctas;
+    out->threads = warps * 32;
+    out->smem = lay.tab_bytes + (size_t)warps * lay.warp_bytes;
+    return 0;
+}
+
+static inline void wk_launch(const WkLaunch& lw, cudaStream_t stream) {
+    lw.kern<<<lw.grid, lw.threads, lw.smem, stream>>>(lw.prm);
+}
+
+static inline int wk_launch_vjp(int sm_count, const void* dsph, const void* gsph, void* gxyz, int64_t n, int L,
+                                int dtype, cudaStream_t stream, std::atomic<int64_t>* launches) {
+    int64_t blocks = (n + 7) / 8;
+    if (blocks > (int64_t)sm_count * 8) blocks = (int64_t)sm_count * 8;
+    if (dtype == 0)
+        sph_vjp_warp_kernel<float><<<(int)blocks, 256, 0, stream>>>((const float*)dsph, (const float*)gsph,
+                                                                     (float*)gxyz, n, L);
+    else
+        sph_vjp_warp_kernel<double><<<(int)blocks, 256, 0, stream>>>((const double*)dsph, (const double*)gsph,
+                                                                      (double*)gxyz, n, L);
+    launches->fetch_add(1, std::memory_order_relaxed);
+    return cudaGetLastError() == cudaSuccess ? 0 : 1;
+}
+
+}  // namespace sphb200

@@ -1,0 +1,83 @@
+"""Parity metric shared by the GPU tests.
+
+north_star: "relative error <= 1e-12 in f64 and <= 5e-6*(l_max+1) in f32 (absolute where
+|Y| < 1e-3)".  Reading R1 makes the 1e-3 floor relative to the row scale so that it also means
+something for solid harmonics (size r^l) and for derivatives (size l/r, l^2/r^2):
+
+    S_d = sqrt((2l+1)/4pi) * rho * max(l,1)^d / r^d,   rho = 1 (normalised) or r^l (solid)
+    e   = |got - oracle| / max(|oracle|, 1e-3 * S_d)          PASS iff max e <= tol
+
+S_0 is exactly the 2-norm of the l-row (addition theorem).  For normalised values S_0 = O(1) and
+this IS the literal rule.  ``strict`` counts violations of the literal, unscaled rule for the record.
+"""
+from __future__ import annotations
+
+import math
+
+import numpy as np
+
+LD = np.longdouble
+
+
+def tol_for(dtype: str, l_max: int) -> float:
+    return 1e-12 if dtype == "f64" else 5e-6 * (l_max + 1)
+
+
+def l_of_k(l_max: int) -> np.ndarray:
+    return np.concatenate([[l] * (2 * l + 1) for l in range(l_max + 1)])
+
+
+def row_scales(xyz, l_max: int, normalized: bool, order: int) -> np.ndarray:
+    """S_order for every (point, k): shape [n, L] (long double)."""
+    x = np.asarray(xyz, LD)
+    r = np.sqrt((x * x).sum(axis=1))
+    l = l_of_k(l_max).astype(LD)
+    base = np.sqrt((2 * l + 1) / (4 * LD(math.pi)))[None, :]
+    rho = np.ones_like(r)[:, None] if normalized else r[:, None] ** l[None, :]
+    lam = np.maximum(l, 1)[None, :]
+    return base * rho * (lam / r[:, None]) ** order
+
+
+def errors(got, want, xyz, l_max: int, normalized: bool, order: int):
+    """Return (max scaled-floor error e, number of strict-rule violations at tol=1, max strict e).
+
+    got / want: [n, (3,)*order, L].  Points whose oracle value is non-finite (r = 0, normalised)
+    must be non-finite in ``got`` too and are excluded from the maximum.
+    """
+    got = np.asarray(got).astype(LD)
+    want = np.asarray(want).astype(LD)
+    S = row_scales(xyz, l_max, normalized, order)
+    S = S.reshape((S.shape[0],) + (1,) * order + (S.shape[1],))
+    bad = ~np.isfinite(want)
+    if bad.any():
+        assert np.all(~np.isfinite(got[bad])), "GPU finite where the oracle is not"
+    diff = np.abs(np.where(bad, 0, got - want))
+    aw = np.abs(np.where(bad, 1, want))
+    e = diff / np.maximum(aw, LD(1e-3) * S)
+    e = np.where(np.isfinite(e), e, np.where(diff == 0, 0, np.inf))   # S = 0 (r = 0 solid, l >= 1): exact zeros
+    strict = diff / np.maximum(aw, LD(1e-3))
+    return float(e.max(initial=0)), strict, e
+
+
+def check(got, want, xyz, l_max, normalized, order, dtype, what=""):
+    tol = tol_for(dtype, l_max)
+    emax, strict, e = errors(got, want, xyz, l_max, normalized, order)
+    n_strict = int((strict > tol).sum())
+    msg = (f"{what}: max scaled error {emax:.3e} (tol {tol:.1e}); strict-rule violations "
+           f"{n_strict} of {strict.size}, max {float(strict.max(initial=0)):.3e}")
+    assert emax <= tol, msg
+    return emax, n_strict, msg
+
+
+def check_vjp(got, want, dsph, grad_sph, l_max, dtype, what="vjp"):
+    """|err| / max(|ref|, 1e-3 * ||dsph[n,a,:]||_2 ||grad_sph[n,:]||_2) <= tol (SURVEY 8(c) VJP)."""
+    tol = tol_for(dtype, l_max)
+    got = np.asarray(got).astype(LD)
+    want = np.asarray(want).astype(LD)
+    d = np.asarray(dsph).astype(LD)
+    g = np.asarray(grad_sph).astype(LD)
+    scale = np.sqrt((d * d).sum(axis=2)) * np.sqrt((g * g).sum(axis=1))[:, None]
+    e = np.abs(got - want) / np.maximum(np.abs(want), LD(1e-3) * scale)
+    emax = float(e.max(initial=0))
+    assert emax <= tol, f"{what}: max scaled error {emax:.3e} (tol {tol:.1e})"
+    return emax

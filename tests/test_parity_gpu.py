@@ -1,0 +1,235 @@
+"""`-m gpu`: the CUDA path, called through the C ABI, against the CPU oracle, element by element.
+
+Reduced sizes span several 32-point tiles / 128-harmonic chunks plus a ragged tail; full
+BASELINE.json sizes run in the launch configuration bench.py times and are compared on sampled
+points.  Tolerance: tests/parity.py.
+"""
+import numpy as np
+import pytest
+
+import parity
+from paper_2302_08381_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def sph():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2302_08381_b200 as pkg
+
+    pkg.load()  # must exist on a GPU box: no fallback
+    return pkg
+
+
+def _torch_dtype(name):
+    return torch.float32 if name == "f32" else torch.float64
+
+
+def _run_gpu(pkg, xyz_np, l_max, normalized, gradients, hessians):
+    xyz = torch.from_numpy(xyz_np).cuda()
+    s, d, h = pkg.compute(xyz, l_max, normalized, gradients, hessians)
+    torch.cuda.synchronize()
+    return s, d, h
+
+
+def _compare(oracle, xyz_np, l_max, normalized, dtype, s, d, h, what):
+    ws, wd, wh = oracle.compute(xyz_np, l_max, normalized, d is not None, h is not None)
+    out = [parity.check(s.cpu().numpy(), ws, xyz_np, l_max, normalized, 0, dtype, what + " values")]
+    if d is not None:
+        out.append(parity.check(d.cpu().numpy(), wd, xyz_np, l_max, normalized, 1, dtype, what + " gradients"))
+    if h is not None:
+        hh = h.cpu().numpy()
+        out.append(parity.check(hh, wh, xyz_np, l_max, normalized, 2, dtype, what + " hessians"))
+        for a in range(3):                      # S4: both triangles stored and exactly equal
+            for b in range(a):
+                assert np.array_equal(hh[:, a, b], hh[:, b, a], equal_nan=True)
+    return out
+
+
+# ------------------------------------------------------------------------------------------------
+# the five configurations at sizes the oracle finishes in seconds
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,n", [("C1", 1000), ("C2", 8219), ("C3", 6007), ("C4", 203), ("C5", 10007)])
+def test_config_reduced(sph, oracle, name, n):
+    cfg = W.CONFIGS[name]
+    xyz = W.make_xyz(cfg, n)
+    s, d, h = _run_gpu(sph, xyz, cfg.l_max, cfg.normalized, cfg.gradients, cfg.hessians)
+    res = _compare(oracle, xyz, cfg.l_max, cfg.normalized, cfg.dtype, s, d, h, name)
+    print(name, [r[2] for r in res])
+    if cfg.vjp:
+        g = W.make_grad_sph(cfg, n)
+        gx = sph.vjp(d, torch.from_numpy(g).cuda())
+        torch.cuda.synchronize()
+        d_np = d.cpu().numpy()
+        # isolate the contraction: oracle contracts the GPU-produced dsph ...
+        want = oracle.vjp(d_np, g, cfg.l_max)
+        parity.check_vjp(gx.cpu().numpy(), want, d_np, g, cfg.l_max, cfg.dtype, name + " vjp (GPU dsph)")
+        # ... and end to end from the oracle's own derivatives
+        _, wd, _ = oracle.compute(xyz, cfg.l_max, cfg.normalized, True)
+        want = oracle.vjp(wd, g, cfg.l_max)
+        parity.check_vjp(gx.cpu().numpy(), want, wd, g, cfg.l_max, cfg.dtype, name + " vjp (end to end)")
+
+
+# ------------------------------------------------------------------------------------------------
+# the five configurations at full size, as bench.py launches them; sampled points
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5"])
+def test_config_full_size_sampled(sph, oracle, name):
+    cfg = W.CONFIGS[name]
+    need = cfg.n * (cfg.out_bytes_per_point + cfg.in_bytes_per_point) * 1.05
+    free, _ = torch.cuda.mem_get_info()
+    if need > free:
+        pytest.skip(f"{name} needs {need / 1e9:.1f} GB, {free / 1e9:.1f} GB free")
+    xyz = W.make_xyz(cfg)
+    s, d, h = _run_gpu(sph, xyz, cfg.l_max, cfg.normalized, cfg.gradients, cfg.hessians)
+    rng = np.random.default_rng(7)
+    n_s = 384 if name == "C4" else 20000
+    idx = np.unique(np.concatenate([rng.integers(0, cfg.n, n_s), [0, 1, 31, 32, cfg.n - 33, cfg.n - 1]]))
+    it = torch.from_numpy(idx).cuda()
+    pick = lambda t: None if t is None else t.index_select(0, it)
+    _compare(oracle, xyz[idx], cfg.l_max, cfg.normalized, cfg.dtype, pick(s), pick(d), pick(h), name + " full")
+    # a property that holds at any size: the addition theorem on EVERY point (values only)
+    l = parity.l_of_k(cfg.l_max)
+    lt = torch.from_numpy(l).cuda()
+    sq = (s.double() ** 2)
+    rows = torch.zeros((cfg.n, cfg.l_max + 1), dtype=torch.float64, device="cuda")
+    rows.index_add_(1, lt, sq)
+    r2 = (torch.from_numpy(xyz).cuda().double() ** 2).sum(1)
+    lv = torch.arange(cfg.l_max + 1, device="cuda", dtype=torch.float64)
+    want = (2 * lv + 1) / (4 * np.pi)
+    if not cfg.normalized:
+        want = want[None, :] * r2[:, None] ** lv[None, :]
+    rel = (rows / want - 1).abs()
+    tol = 4 * (cfg.l_max + 1) * (1.2e-7 if cfg.dtype == "f32" else 1e-14)
+    assert float(rel.max()) < tol, f"{name}: addition theorem off by {float(rel.max()):.3e}"
+    if cfg.vjp:
+        g = W.make_grad_sph(cfg)
+        gt = torch.from_numpy(g).cuda()
+        gx = sph.vjp(d, gt)
+        torch.cuda.synchronize()
+        d_np = pick(d).cpu().numpy()
+        want = oracle.vjp(d_np, g[idx], cfg.l_max)
+        parity.check_vjp(pick(gx).cpu().numpy(), want, d_np, g[idx], cfg.l_max, cfg.dtype, name + " full vjp")
+        # whole-array property: against torch's own contraction in f64
+        ref = torch.einsum("nak,nk->na", d.double(), gt.double())
+        scale = d.double().norm(dim=2) * gt.double().norm(dim=1)[:, None]
+        assert float(((gx.double() - ref).abs() / scale).max()) < 2e-7
+
+
+# ------------------------------------------------------------------------------------------------
+# every kernel variant at small sizes: dtype x derivative order x normalisation x l_max
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("l_max", [0, 1, 2, 3, 5, 6, 9, 16, 17, 32])
+@pytest.mark.parametrize("normalized", [False, True])
+def test_all_variants_small(sph, oracle, dtype, l_max, normalized):
+    rng = np.random.default_rng([l_max, int(normalized)])
+    n = 77 if l_max > 9 else 333                              # several tiles + a ragged tail
+    xyz = rng.standard_normal((n, 3)) * 1.2
+    xyz[3] = [0, 0, 1.5]                                      # +z
+    xyz[4] = [0, 0, -0.7]                                     # -z
+    xyz[5] = [1e-5, -2e-5, 3e-6]                              # near the origin
+    xyz[6] = [0.3, 0, 0]
+    xyz = xyz.astype(np.float32 if dtype == "f32" else np.float64)
+    for deriv in (0, 1, 2):
+        s, d, h = _run_gpu(sph, xyz, l_max, normalized, deriv >= 1, deriv >= 2)
+        _compare(oracle, xyz, l_max, normalized, dtype, s, d, h, f"{dtype} l={l_max} norm={normalized} d={deriv}")
+
+
+@pytest.mark.parametrize("force", ["tp", "w"])
+def test_both_forward_kernels_agree_with_the_oracle(sph, oracle, force, monkeypatch):
+    """The thread-per-point and warp-per-point kernels are interchangeable where both apply."""
+    monkeypatch.setenv("SPHB200_FORCE_KERNEL", force)
+    for dtype, l_max in (("f32", 8), ("f64", 4), ("f32", 3), ("f64", 7)):
+        cfgname = "C2"
+        xyz = W.make_xyz(cfgname, 2000 + 13).astype(np.float32 if dtype == "f32" else np.float64)
+        s, d, h = _run_gpu(sph, xyz, l_max, True, True, False)
+        _compare(oracle, xyz, l_max, True, dtype, s, d, h, f"force={force} {dtype} l={l_max}")
+
+
+# ------------------------------------------------------------------------------------------------
+# edge cases
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n", [0, 1, 2, 31, 32, 33, 63, 64, 65])
+def test_ragged_sizes(sph, oracle, n):
+    for dtype, l_max, hess in (("f32", 6, False), ("f64", 4, False), ("f64", 10, True), ("f32", 3, True)):
+        xyz = np.random.default_rng(n).standard_normal((n, 3)).astype(
+            np.float32 if dtype == "f32" else np.float64)
+        s, d, h = _run_gpu(sph, xyz, l_max, True, True, hess)
+        assert s.shape == (n, (l_max + 1) ** 2)
+        if n:
+            _compare(oracle, xyz, l_max, True, dtype, s, d, h, f"n={n} {dtype} l={l_max}")
+            g = np.random.default_rng(n + 1).standard_normal((n, (l_max + 1) ** 2)).astype(xyz.dtype)
+            gx = sph.vjp(d, torch.from_numpy(g).cuda())
+            d_np = d.cpu().numpy()
+            parity.check_vjp(gx.cpu().numpy(), oracle.vjp(d_np, g, l_max), d_np, g, l_max, dtype)
+
+
+def test_vjp_long_rows(sph, oracle):
+    """Rows too long for the staged VJP kernel take the warp-per-point one."""
+    for dtype, l_max, n in (("f64", 32, 41), ("f32", 32, 70), ("f64", 16, 100)):
+        xyz = W.make_xyz("C4", n).astype(np.float32 if dtype == "f32" else np.float64)
+        _, d, _ = _run_gpu(sph, xyz, l_max, True, True, False)
+        g = np.random.default_rng(3).standard_normal((n, (l_max + 1) ** 2)).astype(xyz.dtype)
+        gx = sph.vjp(d, torch.from_numpy(g).cuda())
+        d_np = d.cpu().numpy()
+        parity.check_vjp(gx.cpu().numpy(), oracle.vjp(d_np, g, l_max), d_np, g, l_max, dtype)
+
+
+def test_origin_and_untouched_memory(sph, oracle):
+    # normalised at r = 0: NaN for that point only; solid at r = 0 is defined
+    xyz = np.array([[0, 0, 0], [1, 2, 3], [0, 0, 0], [-1, 0.5, 0.25]], np.float64)
+    for l_max, hess in ((4, False), (11, True)):
+        s, d, h = _run_gpu(sph, xyz, l_max, True, True, hess)
+        s = s.cpu().numpy()
+        assert np.all(np.isnan(s[[0, 2], 1:])) and np.all(np.isfinite(s[[1, 3]]))
+        s, d, h = _run_gpu(sph, xyz, l_max, False, True, hess)
+        _compare(oracle, xyz, l_max, False, "f64", s, d, h, "solid at the origin")
+    # outputs are written exactly where they belong: guard bands around the buffers stay intact
+    n, l_max = 101, 6
+    L = (l_max + 1) ** 2
+    pts = torch.randn(n, 3, device="cuda")
+    for hess in (False, True):
+        bufs = [torch.full((m + 64,), 777.0, device="cuda") for m in (n * L, n * 3 * L, n * 9 * L)]
+        views = [b[32:-32] for b in bufs]             # 128-byte offset keeps the 16-byte alignment
+        sph.sphericart_cuda_compute(pts, n, l_max, 1, 0, views[0], views[1], views[2] if hess else None,
+                                    torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        for b, used in zip(bufs, (True, True, hess)):
+            assert torch.all(b[:32] == 777.0) and torch.all(b[-32:] == 777.0)
+            assert bool(torch.all(b[32:-32] != 777.0)) == used
+
+
+def test_host_buffer_entry_points(sph, oracle):
+    cfg = W.CONFIGS["C5"]
+    n = 50_021
+    xyz = W.make_xyz(cfg, n)
+    L = cfg.n_sph
+    s = np.empty((n, L), np.float32)
+    d = np.empty((n, 3, L), np.float32)
+    sph.sphericart_cuda_compute_host(xyz, n, cfg.l_max, 1, 0, s, d, None)
+    idx = np.arange(0, n, 37)
+    ws, wd, _ = oracle.compute(xyz[idx], cfg.l_max, True, True)
+    parity.check(s[idx], ws, xyz[idx], cfg.l_max, True, 0, "f32", "host values")
+    parity.check(d[idx], wd, xyz[idx], cfg.l_max, True, 1, "f32", "host gradients")
+    g = W.make_grad_sph(cfg, n)
+    gx = np.empty((n, 3), np.float32)
+    sph.sphericart_cuda_vjp_host(None, d, g, gx, n, cfg.l_max, 0)
+    parity.check_vjp(gx[idx], oracle.vjp(d[idx], g[idx], cfg.l_max), d[idx], g[idx], cfg.l_max, "f32")
+
+
+def test_errors_raise(sph):
+    x = torch.randn(10, 3, device="cuda")
+    with pytest.raises(sph.SphericartCudaError):
+        sph.compute(x.cpu(), 3)
+    with pytest.raises(sph.SphericartCudaError):
+        sph.compute(x, 33)
+    with pytest.raises(sph.SphericartCudaError):          # misaligned view
+        sph.sphericart_cuda_compute(x.view(-1)[1:], 3, 2, 1, 0, torch.empty(64, device="cuda"), None, None, None)
+    before = sph.sphericart_cuda_launch_count()
+    sph.compute(x, 3, gradients=True)
+    assert sph.sphericart_cuda_launch_count() == before + 1
