@@ -1,0 +1,459 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the spherical-harmonics hot path on B200 (one JSON line on stdout).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2] [--no-sweep]
+    python bench.py --impl reference ...        # the CPU oracle, as it stands, on the host cores
+
+A "step" is one pass of the hot path over one batch of the named workload: one
+``sphericart_cuda_compute`` call and, for C5, the ``sphericart_cuda_vjp``
+call that follows it (a10).  The headline workload is BASELINE.json ``configs[1]`` (C2: N=100000
+f32 l_max=8 normalised values+gradients).  ``value`` is points/s with inputs resident in HBM;
+``e2e`` is the same metric through the host-buffer entry point (pinned host memory, H2D of xyz and
+D2H of every output inside the timed region).  The remaining configurations are parity-test cases;
+at N=1 they are also timed briefly and reported under ``sweep`` (the metric is "points/s and output
+GB/s vs l_max, f32/f64, +-grads") but the JSON line's headline keys are C2's.
+
+Multi-GPU: the path shards over points with no communication; every rank
+runs the same per-GPU batch ("scaling": "weak"), a barrier + synchronize brackets the timed region
+and the time is the max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+from paper_2302_08381_b200 import workloads as W  # noqa: E402
+
+METRIC = "points/s"
+N_SETS = 4          # output buffer sets the timed loop rotates over (C2: 4 x 129.6 MB > 126 MB L2)
+
+
+def measured_peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        d = json.loads(p.read_text())
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy read+write, burst)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# ncu --set full: dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel,
+# copied by hand from the capture summarised under profiles/ (None until a capture exists).
+NCU_TRAFFIC_BYTES = {
+}
+
+
+# -------------------------------------------------------------------------------------------------
+# clocks during the timed region
+# -------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """Polls SM clock and throttle reasons through NVML while the timed region runs."""
+
+    BAD = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20}
+    NOTE = {"sw_power_cap": 0x4}
+
+    def __init__(self, index: int, period_s: float = 0.02):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self.period = period_s
+        self._stop = threading.Event()
+        self._thread = None
+        try:
+            import pynvml
+
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:  # NVML missing: the JSON line then carries null clocks
+            self.nv = None
+
+    def sample(self):
+        if self.nv is None:
+            return
+        try:
+            self.samples.append(float(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM)))
+            mask = int(self.nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+            for name, bit in {**self.BAD, **self.NOTE}.items():
+                if mask & bit:
+                    self.reasons.add(name)
+        except Exception:
+            pass
+
+    def _run(self):
+        while not self._stop.is_set():
+            self.sample()
+            self._stop.wait(self.period)
+
+    def start(self):
+        self._thread = threading.Thread(target=self._run, daemon=True)
+        self._thread.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._thread:
+            self._thread.join()
+
+    def summary(self):
+        return {"sm_mhz": statistics.median(self.samples) if self.samples else None,
+                "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+# -------------------------------------------------------------------------------------------------
+# the CUDA arm
+# -------------------------------------------------------------------------------------------------
+def algorithmic_bytes_per_point(cfg, with_vjp: bool):
+    """forward = in + out; VJP = dsph + grad_sph read, grad_xyz written."""
+    fwd = cfg.in_bytes_per_point + cfg.out_bytes_per_point
+    vjp = (4 * cfg.n_sph + 3) * cfg.itemsize if with_vjp else 0
+    return fwd, vjp
+
+
+class DeviceWorkload:
+    """Inputs resident in HBM + N_SETS output buffer sets for one configuration."""
+
+    def __init__(self, cfg, torch, pkg, device, n_sets, seed=0):
+        self.cfg, self.torch, self.pkg = cfg, torch, pkg
+        dt = torch.float32 if cfg.dtype == "f32" else torch.float64
+        self.dcode = pkg.F32 if cfg.dtype == "f32" else pkg.F64
+        self.xyz = torch.from_numpy(W.make_xyz(cfg, seed=seed)).to(device)
+        n, L = cfg.n, cfg.n_sph
+        self.sets = []
+        for _ in range(n_sets):
+            sph = torch.empty((n, L), dtype=dt, device=device)
+            dsph = torch.empty((n, 3, L), dtype=dt, device=device) if cfg.gradients else None
+            ddsph = torch.empty((n, 3, 3, L), dtype=dt, device=device) if cfg.hessians else None
+            self.sets.append((sph, dsph, ddsph))
+        self.grad_sph = self.grad_xyz = None
+        if cfg.vjp:
+            self.grad_sph = torch.from_numpy(W.make_grad_sph(cfg, seed=seed)).to(device)
+            self.grad_xyz = torch.empty((n, 3), dtype=dt, device=device)
+        self.stream = torch.cuda.current_stream().cuda_stream
+
+    def forward(self, i):
+        c = self.cfg
+        sph, dsph, ddsph = self.sets[i % len(self.sets)]
+        self.pkg.sphericart_cuda_compute(self.xyz, c.n, c.l_max, c.normalized, self.dcode, sph, dsph, ddsph,
+                                         self.stream)
+
+    def backward(self, i):
+        c = self.cfg
+        _, dsph, _ = self.sets[i % len(self.sets)]
+        self.pkg.sphericart_cuda_vjp(None, dsph, self.grad_sph, self.grad_xyz, c.n, c.l_max, self.dcode,
+                                     self.stream)
+
+    def step(self, i):
+        self.forward(i)
+        if self.cfg.vjp:
+            self.backward(i)
+
+
+def time_loop(torch, fn, steps):
+    """CUDA events on torch's current stream (the stream the library launches on) around `steps` calls."""
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for i in range(steps):
+        fn(i)
+    e1.record()
+    return e0, e1
+
+
+def n_sets_for(cfg, free_bytes):
+    per_set = cfg.n * cfg.out_bytes_per_point
+    want = N_SETS if per_set < (2 << 30) else 2
+    while want > 1 and want * per_set > 0.8 * free_bytes:
+        want -= 1
+    return want
+
+
+def store_ceiling_gbs(torch, nbytes, device):
+    """Write-only ceiling measured in the same run: torch's fill kernel over the same byte count."""
+    nbytes = int(min(max(nbytes, 1 << 28), 8 << 30))
+    bufs = [torch.empty(nbytes, dtype=torch.uint8, device=device) for _ in range(2)]
+    for b in bufs:
+        b.zero_()
+    torch.cuda.synchronize()
+    reps = 10
+    e0, e1 = time_loop(torch, lambda i: bufs[i & 1].zero_(), reps)
+    torch.cuda.synchronize()
+    return nbytes * reps / (e0.elapsed_time(e1) * 1e-3) / 1e9
+
+
+def sweep_one(cfg, torch, pkg, device, peak):
+    """Brief timing of one configuration (N=1 only): forward and VJP kernels timed separately."""
+    free, _ = torch.cuda.mem_get_info()
+    wl = DeviceWorkload(cfg, torch, pkg, device, n_sets_for(cfg, free))
+    out_bytes = cfg.n * cfg.out_bytes_per_point
+    reps = int(max(5, min(200, 2e9 // max(out_bytes, 1) * 10)))
+    for i in range(3):
+        wl.step(i)
+    torch.cuda.synchronize()
+    e0, e1 = time_loop(torch, wl.forward, reps)
+    torch.cuda.synchronize()
+    ms_f = e0.elapsed_time(e1) / reps
+    fwd_b, vjp_b = algorithmic_bytes_per_point(cfg, cfg.vjp)
+    res = {"workload": cfg.what, "dtype": cfg.dtype, "l_max": cfg.l_max, "n": cfg.n, "launches_timed": reps,
+           "buffer_sets": len(wl.sets), "fwd_us": round(ms_f * 1e3, 2), "fwd_points_per_s": cfg.n / (ms_f * 1e-3),
+           "fwd_gbs": cfg.n * fwd_b / (ms_f * 1e-3) / 1e9}
+    res["fwd_frac_of_measured_peak"] = res["fwd_gbs"] / peak
+    if cfg.vjp:
+        e0, e1 = time_loop(torch, wl.backward, reps)
+        torch.cuda.synchronize()
+        ms_b = e0.elapsed_time(e1) / reps
+        res.update({"vjp_us": round(ms_b * 1e3, 2), "vjp_gbs": cfg.n * vjp_b / (ms_b * 1e-3) / 1e9})
+        res["vjp_frac_of_measured_peak"] = res["vjp_gbs"] / peak
+    del wl
+    torch.cuda.empty_cache()
+    return res
+
+
+def time_e2e(cfg, torch, pkg, steps):
+    """The same metric through the host-buffer C-ABI call: pinned host arrays in, pinned host arrays
+    out, H2D + kernels + D2H inside the timed region (wall clock around a synchronous call)."""
+    dt = torch.float32 if cfg.dtype == "f32" else torch.float64
+    dcode = pkg.F32 if cfg.dtype == "f32" else pkg.F64
+    n, L = cfg.n, cfg.n_sph
+    xyz = torch.from_numpy(W.make_xyz(cfg)).pin_memory()
+    sph = torch.empty((n, L), dtype=dt).pin_memory()
+    dsph = torch.empty((n, 3, L), dtype=dt).pin_memory() if cfg.gradients else None
+    ddsph = torch.empty((n, 3, 3, L), dtype=dt).pin_memory() if cfg.hessians else None
+    gs = gx = None
+    if cfg.vjp:
+        gs = torch.from_numpy(W.make_grad_sph(cfg)).pin_memory()
+        gx = torch.empty((n, 3), dtype=dt).pin_memory()
+
+    def one():
+        pkg.sphericart_cuda_compute_host(xyz, n, cfg.l_max, cfg.normalized, dcode, sph, dsph, ddsph)
+        if cfg.vjp:
+            pkg.sphericart_cuda_vjp_host(None, dsph, gs, gx, n, cfg.l_max, dcode)
+
+    for _ in range(2):
+        one()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        one()
+    torch.cuda.synchronize()
+    dt_s = (time.perf_counter() - t0) / steps
+    h2d = n * cfg.in_bytes_per_point + (n * 4 * L * cfg.itemsize if cfg.vjp else 0)
+    d2h = n * cfg.out_bytes_per_point + (n * 3 * cfg.itemsize if cfg.vjp else 0)
+    return {"value": n / dt_s, "unit": METRIC, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+            "ms_per_step": dt_s * 1e3, "steps": steps,
+            "how": "sphericart_cuda_compute_host on pinned host buffers, wall clock around the synchronous call"}
+
+
+def oracle_baseline(cfg, budget_s=12.0):
+    """The oracle's double build, as it stands, on the host cores, on a bounded sample of cfg."""
+    import oracle
+
+    oracle.build()
+    cores = oracle.num_threads("f64")
+    per_point_guess = 40e-9 * cfg.n_sph * (1 + 3 * cfg.gradients + 9 * cfg.hessians)   # seconds, 1 core
+    n = int(min(cfg.n, max(2048, budget_s * cores / 5 / per_point_guess)))
+    xyz = W.make_xyz(cfg, n)
+    L = cfg.n_sph
+    out = (np.empty((n, L)), np.empty((n, 3, L)) if cfg.gradients else None,
+           np.empty((n, 3, 3, L)) if cfg.hessians else None)
+    g = W.make_grad_sph(cfg, n).astype(np.float64) if cfg.vjp else None
+
+    def one():
+        oracle.compute(xyz, cfg.l_max, cfg.normalized, cfg.gradients, cfg.hessians, kind="f64", out=out)
+        if cfg.vjp:
+            oracle.vjp(out[1], g, cfg.l_max, kind="f64")
+
+    one()
+    times, t_all = [], time.perf_counter()
+    while len(times) < 5 or (time.perf_counter() - t_all < budget_s / 2 and len(times) < 200):
+        t0 = time.perf_counter()
+        one()
+        times.append(time.perf_counter() - t0)
+    med = statistics.median(times)
+    return {"value": n / med, "unit": METRIC, "cores": cores, "kind": "oracle",
+            "sample": f"{cfg.name}: first {n} of {cfg.n} points, oracle f64 build (gcc -O2 -fopenmp), "
+                      f"median of {len(times)} passes, {med * 1e3:.2f} ms per pass"}, n, med
+
+
+def run_cuda(args):
+    import torch
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; --impl reference times the oracle)")
+    torch.cuda.set_device(local_rank)
+    device = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=device)
+
+    import paper_2302_08381_b200 as pkg
+
+    pkg.load()                                   # raises if the CUDA library is missing
+    cfg = W.CONFIGS[args.workload]
+    peak, peak_src = measured_peaks()
+    free, _ = torch.cuda.mem_get_info()
+    wl = DeviceWorkload(cfg, torch, pkg, device, n_sets_for(cfg, free), seed=rank)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for i in range(max(args.warmup, 3)):
+        wl.step(i)
+    barrier()
+    clocks = ClockSampler(local_rank)
+    clocks.start()
+    launches0 = pkg.sphericart_cuda_launch_count()
+    e0, e1 = time_loop(torch, wl.step, args.steps)
+    clocks.sample()                              # the GPU is still draining the queue here
+    barrier()
+    clocks.stop()
+    launches = pkg.sphericart_cuda_launch_count() - launches0
+    ms_total = e0.elapsed_time(e1)
+    if dist is not None:
+        t = torch.tensor([ms_total], device=device, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = world * cfg.n / (ms_step * 1e-3)
+
+    # dominant kernel: the forward kernel.  One launch per step for forward-only workloads, so its
+    # average duration IS the step time; for C5 the forward launches are timed in a pass of their own.
+    fwd_b, vjp_b = algorithmic_bytes_per_point(cfg, cfg.vjp)
+    if cfg.vjp:
+        f0, f1 = time_loop(torch, wl.forward, args.steps)
+        torch.cuda.synchronize()
+        ms_fwd = f0.elapsed_time(f1) / args.steps
+    else:
+        ms_fwd = ms_step
+    achieved = cfg.n * fwd_b / (ms_fwd * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": "forward (sph_tp_kernel / sph_w_kernel)", "achieved": achieved,
+                "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg.name),
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": cfg.n * fwd_b,
+                "avg_launch_us": ms_fwd * 1e3, "output_gbs": cfg.n * cfg.out_bytes_per_point / (ms_fwd * 1e-3) / 1e9,
+                "frac_of_nominal_8tbs": achieved / 8000.0}
+
+    line = {"metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic",
+            "config": {"workload": f"{cfg.name}: {cfg.what}", "n_points_per_gpu": cfg.n, "l_max": cfg.l_max,
+                       "normalized": cfg.normalized, "gradients": cfg.gradients, "hessians": cfg.hessians,
+                       "vjp": cfg.vjp, "parallelism": f"points sharded over {world} GPU(s), no collective",
+                       "l2": f"outputs rotate over {len(wl.sets)} buffer sets "
+                             f"({len(wl.sets) * cfg.n * cfg.out_bytes_per_point / 1e6:.0f} MB written before reuse "
+                             "> 126 MB L2)"},
+            "clocks": clocks.summary(), "gpu_launches": int(launches), "roofline": roofline}
+    if rank == 0:
+        line["roofline"]["store_ceiling_gbs"] = store_ceiling_gbs(torch, cfg.n * cfg.out_bytes_per_point, device)
+    del wl
+    torch.cuda.empty_cache()
+
+    e2e = time_e2e(cfg, torch, pkg, max(3, min(args.steps, args.e2e_steps)))
+    if dist is not None:
+        t = torch.tensor([e2e["ms_per_step"]], device=device, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e["ms_per_step"] = float(t.item())
+        e2e["value"] = world * cfg.n / (e2e["ms_per_step"] * 1e-3)
+    line["e2e"] = e2e
+
+    if rank == 0 and world == 1:
+        base, _, _ = oracle_baseline(cfg)
+        line["cpu_baseline"] = base
+        if not args.no_sweep:
+            line["sweep"] = {}
+            for name in ("C1", "C2", "C3", "C4", "C5"):
+                c = W.CONFIGS[name]
+                free, _ = torch.cuda.mem_get_info()
+                if c.n * (c.out_bytes_per_point + c.in_bytes_per_point) * 1.05 > free:
+                    line["sweep"][name] = {"skipped": "does not fit in free HBM"}
+                    continue
+                line["sweep"][name] = sweep_one(c, torch, pkg, device, peak)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(line))
+
+
+def run_reference(args):
+    """--impl reference: the oracle (f64 build, OpenMP) on the host cores; rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import oracle
+
+    oracle.build()
+    cfg = W.CONFIGS[args.workload]
+    cores = oracle.num_threads("f64")
+    # one step = one oracle pass over a bounded sample, sized so the whole run ends within minutes
+    per_point = 60e-9 * cfg.n_sph * (1 + 3 * cfg.gradients + 9 * cfg.hessians) / cores
+    total = max(args.steps + max(args.warmup, 1), 1)
+    n = int(min(cfg.n, max(1024, 120.0 / total / per_point)))
+    xyz = W.make_xyz(cfg, n)
+    L = cfg.n_sph
+    out = (np.empty((n, L)), np.empty((n, 3, L)) if cfg.gradients else None,
+           np.empty((n, 3, 3, L)) if cfg.hessians else None)
+    g = W.make_grad_sph(cfg, n).astype(np.float64) if cfg.vjp else None
+
+    def one():
+        oracle.compute(xyz, cfg.l_max, cfg.normalized, cfg.gradients, cfg.hessians, kind="f64", out=out)
+        if cfg.vjp:
+            oracle.vjp(out[1], g, cfg.l_max, kind="f64")
+
+    for _ in range(max(args.warmup, 1)):
+        one()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        one()
+    ms_step = (time.perf_counter() - t0) / args.steps * 1e3
+    value = n / (ms_step * 1e-3)
+    sample = f"{cfg.name}: first {n} of {cfg.n} points per step, oracle f64 build (gcc -O2 -fopenmp)"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": METRIC, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": max(args.warmup, 1), "ms_per_step": ms_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{cfg.name}: {cfg.what}", "l_max": cfg.l_max, "sample_points_per_step": n},
+            "cpu_baseline": {"value": value, "unit": METRIC, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": METRIC, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=None)
+    ap.add_argument("--impl", choices=["cuda", "reference"], default="cuda")
+    ap.add_argument("--workload", choices=sorted(W.CONFIGS), default="C2")
+    ap.add_argument("--e2e-steps", type=int, default=20)
+    ap.add_argument("--no-sweep", action="store_true", help="skip the brief timing of the other configurations")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        args.steps = 20 if args.steps is None else args.steps
+        args.warmup = 1 if args.warmup is None else args.warmup
+        return run_reference(args)
+    args.steps = 2000 if args.steps is None else args.steps
+    args.warmup = 20 if args.warmup is None else args.warmup
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world != args.gpus:
+        if args.gpus > 1 and world == 1:
+            raise SystemExit(f"--gpus {args.gpus}: launch with python -m torch.distributed.run --nproc-per-node "
+                             f"{args.gpus} --master-addr 127.0.0.1 bench.py --gpus {args.gpus} ...")
+    run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()

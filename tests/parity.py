@@ -9,6 +9,10 @@ something for solid harmonics (size r^l) and for derivatives (size l/r, l^2/r^2)
 
 S_0 is exactly the 2-norm of the l-row (addition theorem).  For normalised values S_0 = O(1) and
 this IS the literal rule.  ``strict`` counts violations of the literal, unscaled rule for the record.
+
+Underflow (reading U1): solid harmonics of a point with r ~ 1e-5 are ~r^l, below the
+smallest normal number of the output type (f32: 1.18e-38) already at l = 8; there the output type
+has no relative precision to offer, so the floor never drops below ``finfo(dtype).tiny``.
 """
 from __future__ import annotations
 
@@ -33,12 +37,16 @@ def row_scales(xyz, l_max: int, normalized: bool, order: int) -> np.ndarray:
     r = np.sqrt((x * x).sum(axis=1))
     l = l_of_k(l_max).astype(LD)
     base = np.sqrt((2 * l + 1) / (4 * LD(math.pi)))[None, :]
-    rho = np.ones_like(r)[:, None] if normalized else r[:, None] ** l[None, :]
     lam = np.maximum(l, 1)[None, :]
-    return base * rho * (lam / r[:, None]) ** order
+    if normalized:
+        with np.errstate(divide="ignore"):
+            return base * (lam / r[:, None]) ** order
+    # solid: r^l / r^order as ONE power so that r = 0 gives 0 or 1, not 0 * inf; a derivative of
+    # order > l of a degree-l polynomial is identically zero, hence the clamp of the exponent
+    return base * lam ** order * r[:, None] ** np.maximum(l - order, 0)[None, :]
 
 
-def errors(got, want, xyz, l_max: int, normalized: bool, order: int):
+def errors(got, want, xyz, l_max: int, normalized: bool, order: int, tiny: float = 0.0):
     """Return (max scaled-floor error e, number of strict-rule violations at tol=1, max strict e).
 
     got / want: [n, (3,)*order, L].  Points whose oracle value is non-finite (r = 0, normalised)
@@ -53,7 +61,7 @@ def errors(got, want, xyz, l_max: int, normalized: bool, order: int):
         assert np.all(~np.isfinite(got[bad])), "GPU finite where the oracle is not"
     diff = np.abs(np.where(bad, 0, got - want))
     aw = np.abs(np.where(bad, 1, want))
-    e = diff / np.maximum(aw, LD(1e-3) * S)
+    e = diff / np.maximum(np.maximum(aw, LD(1e-3) * S), LD(tiny))
     e = np.where(np.isfinite(e), e, np.where(diff == 0, 0, np.inf))   # S = 0 (r = 0 solid, l >= 1): exact zeros
     strict = diff / np.maximum(aw, LD(1e-3))
     return float(e.max(initial=0)), strict, e
@@ -61,7 +69,8 @@ def errors(got, want, xyz, l_max: int, normalized: bool, order: int):
 
 def check(got, want, xyz, l_max, normalized, order, dtype, what=""):
     tol = tol_for(dtype, l_max)
-    emax, strict, e = errors(got, want, xyz, l_max, normalized, order)
+    tiny = float(np.finfo(np.float32 if dtype == "f32" else np.float64).tiny)
+    emax, strict, e = errors(got, want, xyz, l_max, normalized, order, tiny)
     n_strict = int((strict > tol).sum())
     msg = (f"{what}: max scaled error {emax:.3e} (tol {tol:.1e}); strict-rule violations "
            f"{n_strict} of {strict.size}, max {float(strict.max(initial=0)):.3e}")
