@@ -357,10 +357,17 @@ def run_cuda(args):
                              f"({len(wl.sets) * cfg.n * cfg.out_bytes_per_point / 1e6:.0f} MB written before reuse "
                              "> 126 MB L2)"},
             "clocks": clocks.summary(), "gpu_launches": int(launches), "roofline": roofline}
-    if rank == 0:
+    if rank == 0 and not args.kernels_only:
         line["roofline"]["store_ceiling_gbs"] = store_ceiling_gbs(torch, cfg.n * cfg.out_bytes_per_point, device)
     del wl
     torch.cuda.empty_cache()
+    if args.kernels_only:                        # profiling runs (ncu): the timed kernels and nothing else
+        if dist is not None:
+            dist.barrier()
+            dist.destroy_process_group()
+        if rank == 0:
+            print(json.dumps(line))
+        return
 
     e2e = time_e2e(cfg, torch, pkg, max(3, min(args.steps, args.e2e_steps)))
     if dist is not None:
@@ -440,6 +447,8 @@ def main():
     ap.add_argument("--workload", choices=sorted(W.CONFIGS), default="C2")
     ap.add_argument("--e2e-steps", type=int, default=20)
     ap.add_argument("--no-sweep", action="store_true", help="skip the brief timing of the other configurations")
+    ap.add_argument("--kernels-only", action="store_true",
+                    help="time the device-resident step only (no e2e, no oracle, no sweep): the command ncu wraps")
     args = ap.parse_args()
     if args.impl == "reference":
         args.steps = 20 if args.steps is None else args.steps
