@@ -14,6 +14,7 @@
 #include "kernel_tp.cuh"
 #include "kernel_vjp.cuh"
 #include "kernel_w.cuh"
+#include "tpb_api.h"
 
 namespace sphb200 {
 
@@ -66,6 +67,9 @@ static int device_state(DeviceState** out) {
         st.sm_count = prop.multiProcessorCount;
         st.smem_optin = (int)prop.sharedMemPerBlockOptin;
         CUDA_TRY(cudaMemcpyToSymbol(c_tables, &g_host_tables, sizeof(SphTables)));
+        if (sph_tpb_upload_f32_v(&g_host_tables) || sph_tpb_upload_f32_g(&g_host_tables) ||
+            sph_tpb_upload_f64_v(&g_host_tables) || sph_tpb_upload_f64_g(&g_host_tables))
+            return fail(SPHERICART_CUDA_ECUDA, "table upload failed: %s", cudaGetErrorString(cudaGetLastError()));
         CUDA_TRY(cudaMalloc(&st.d_tables, sizeof(SphTables)));
         CUDA_TRY(cudaMemcpy(st.d_tables, &g_host_tables, sizeof(SphTables), cudaMemcpyHostToDevice));
         st.ready = true;
@@ -206,8 +210,22 @@ static int compute_device(const void* xyz, int64_t n, int l_max, int normalized,
     rc = device_state(&st);
     if (rc) return rc;
 
-    const char* force = getenv("SPHB200_FORCE_KERNEL");  // "tp" | "w": experiments only
+    const char* force = getenv("SPHB200_FORCE_KERNEL");  // "tpb" | "tp" | "w": experiments only
     const bool force_w = force && force[0] == 'w';
+    const bool force_tp = force && force[0] == 't' && force[1] == 'p' && force[2] == '\0';
+    if (!ddsph && !force_w && !force_tp) {
+        // compile-time-l_max kernels (two threads per point): every l_max that has an instantiation
+        const bool f32 = dtype == SPHERICART_CUDA_F32;
+        int r = dsph ? (f32 ? sph_tpb_launch_f32_g : sph_tpb_launch_f64_g)(st->sm_count, xyz, n, l_max, normalized,
+                                                                            sph, dsph, stream)
+                     : (f32 ? sph_tpb_launch_f32_v : sph_tpb_launch_f64_v)(st->sm_count, xyz, n, l_max, normalized,
+                                                                            sph, nullptr, stream);
+        if (r < 0) return fail(SPHERICART_CUDA_ECUDA, "tpb launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+        if (r == 0) {
+            g_launches.fetch_add(1, std::memory_order_relaxed);
+            return 0;
+        }
+    }
     if (!ddsph && !force_w) {
         // the tp kernel wants an odd row length (conflict-free staging) and >= 4 warps per SM
         TpParams probe{};
@@ -216,7 +234,7 @@ static int compute_device(const void* xyz, int64_t n, int l_max, int normalized,
         const int L = (l_max + 1) * (l_max + 1);
         const int64_t tile_bytes = 32LL * L * (dtype == SPHERICART_CUDA_F32 ? 4 : 8) * (dsph ? 4 : 1);
         const bool fits = tile_bytes * 4 <= st->smem_optin - 1024;
-        const bool want_tp = (force && force[0] == 't') || ((L & 1) && fits);
+        const bool want_tp = force_tp || ((L & 1) && fits);
         if (want_tp && tp_plan(*st, n, l_max, dsph ? 1 : 0, dtype == SPHERICART_CUDA_F32 ? 4 : 8, &probe, &grid, &smem)) {
             bool handled = false;
             rc = launch_tp(*st, xyz, n, l_max, normalized, dtype, sph, dsph, stream, &handled);

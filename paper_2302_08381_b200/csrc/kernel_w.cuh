@@ -300,7 +300,7 @@ static inline int wk_plan(int sm_count, int smem_optin, int64_t n, int l_max, in
     int chunk = wk_env("SPHB200_W_CHUNK", 128);
     chunk = (chunk + 31) & ~31;
     if (chunk > ((L + 31) & ~31)) chunk = (L + 31) & ~31;
-    int nbuf = wk_env("SPHB200_W_NBUF", 2);
+    int nbuf = wk_env("SPHB200_W_NBUF", 1);   // measured on C4: one image per warp and more warps beats two images
     if (nbuf < 1) nbuf = 1;
     if (nbuf > 2) nbuf = 2;
     const int budget = smem_optin - 1024;

@@ -1,0 +1,19 @@
+// Host entry points of the tpb translation units (tpb_inst.cu, compiled once per element type
+// and derivative order).  Return: 0 launched, 1 no instantiation for this l_max, -1 CUDA error.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "tables.h"
+
+namespace sphb200 {
+#define SPH_TPB_DECL(sfx)                                                                                   \
+    int sph_tpb_launch_##sfx(int sm_count, const void* xyz, int64_t n, int l_max, int normalized, void* sph, \
+                             void* dsph, cudaStream_t stream);                                              \
+    int sph_tpb_upload_##sfx(const SphTables* host_tables);
+SPH_TPB_DECL(f32_v)
+SPH_TPB_DECL(f32_g)
+SPH_TPB_DECL(f64_v)
+SPH_TPB_DECL(f64_g)
+#undef SPH_TPB_DECL
+}  // namespace sphb200

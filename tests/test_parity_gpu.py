@@ -124,7 +124,7 @@ def test_config_full_size_sampled(sph, oracle, name):
 # every kernel variant at small sizes: dtype x derivative order x normalisation x l_max
 # ------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
-@pytest.mark.parametrize("l_max", [0, 1, 2, 3, 5, 6, 9, 16, 17, 32])
+@pytest.mark.parametrize("l_max", [0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 12, 16, 17, 32])
 @pytest.mark.parametrize("normalized", [False, True])
 def test_all_variants_small(sph, oracle, dtype, l_max, normalized):
     rng = np.random.default_rng([l_max, int(normalized)])
@@ -140,10 +140,12 @@ def test_all_variants_small(sph, oracle, dtype, l_max, normalized):
         _compare(oracle, xyz, l_max, normalized, dtype, s, d, h, f"{dtype} l={l_max} norm={normalized} d={deriv}")
 
 
-@pytest.mark.parametrize("force", ["tp", "w"])
-def test_both_forward_kernels_agree_with_the_oracle(sph, oracle, force, monkeypatch):
-    """The thread-per-point and warp-per-point kernels are interchangeable where both apply."""
-    monkeypatch.setenv("SPHB200_FORCE_KERNEL", force)
+@pytest.mark.parametrize("force", ["auto", "tp", "w"])
+def test_all_forward_kernels_agree_with_the_oracle(sph, oracle, force, monkeypatch):
+    """The compile-time-l_max (auto picks it for l_max <= 8), thread-per-point and warp-per-point
+    kernels are interchangeable where they all apply."""
+    if force != "auto":
+        monkeypatch.setenv("SPHB200_FORCE_KERNEL", force)
     for dtype, l_max in (("f32", 8), ("f64", 4), ("f32", 3), ("f64", 7)):
         cfgname = "C2"
         xyz = W.make_xyz(cfgname, 2000 + 13).astype(np.float32 if dtype == "f32" else np.float64)
