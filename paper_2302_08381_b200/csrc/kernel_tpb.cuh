@@ -1,5 +1,5 @@
 // "tpb" forward kernel: TWO threads per point (one per branch of Eq. 5), l_max a compile-time
-// constant, 16 points per warp.  Values, or values + gradients.
+// constant, 16 points per tile.  Values, or values + gradients.
 //
 // Why (profiles/r1_*): the path is bound by the HBM write of the row-major
 // outputs, and a tile of consecutive points owns one contiguous byte range of sph and one of dsph.
@@ -41,34 +41,62 @@ struct TpbParams {
     void* sph;
     void* dsph;
     int64_t n;
+    int tiles_per_cta;   // consecutive tiles one CTA works through
 };
 
-constexpr int TPB_PTS = 16;            // points per warp tile
-constexpr int TPB_SMEM_BUDGET = 226 * 1024;
+constexpr int TPB_PTS = 16;                 // points per tile
+constexpr int TPB_SMEM_PER_SM = 228 * 1024; // B200: 228 KB per SM, 1 KB of it reserved per resident CTA
 
-// launch shape fixed by (element size, DERIV, LMAX)
-template <int ESIZE, int DERIV, int LMAX> struct TpbShape {
+// Launch shape fixed by (element size, DERIV, LMAX, SPLIT).
+//
+// The grid is NOT persistent: a CTA owns `tiles_per_cta` consecutive tiles and there are many more
+// CTAs than fit on the machine, so the hardware block scheduler hands tiles out as SMs free up.
+// Measured on B200 with a store-only probe: under a static, equal split of a large output the SMs
+// finish at 247k / 283k / 346k cycles depending on where they sit (6.2 TB/s overall); handing the
+// same tiles out dynamically reaches 7.3-7.4 TB/s.
+//
+// SPLIT = warps that share one tile.  SPLIT == 2: warp 0 takes the columns m < cut, warp 1 the
+// columns m >= cut of the (l,m) triangle (balanced by the number of (l,m) pairs), so a tile's
+// latency halves for the same shared-memory footprint; the only duplicated work is column `cut`
+// and the first `cut` steps of Eq. 9.
+template <int LMAX, int SPLIT> struct TpbCut {
+    static constexpr int pairs(int m0, int m1) {   // (l,m) pairs with m0 <= m < m1
+        int s = 0;
+        for (int m = m0; m < m1; ++m) s += LMAX + 1 - m;
+        return s;
+    }
+    static constexpr int cut() {
+        if (SPLIT == 1) return LMAX + 1;
+        const int total = pairs(0, LMAX + 1);
+        int c = 1;
+        while (c < LMAX && 2 * pairs(0, c) < total) ++c;
+        // the nearer of c-1 and c to an even split
+        const int over = 2 * pairs(0, c) - total, under = total - 2 * pairs(0, c - 1);
+        return (c > 1 && under < over) ? c - 1 : c;
+    }
+};
+
+template <int ESIZE, int DERIV, int LMAX, int SPLIT> struct TpbShape {
     static constexpr int L = (LMAX + 1) * (LMAX + 1);
     static constexpr int tile_bytes = TPB_PTS * L * ESIZE * (DERIV ? 4 : 1);
-    static constexpr int fit = TPB_SMEM_BUDGET / tile_bytes;
-    static constexpr int nbuf = (fit >= 32) ? 2 : 1;                       // two images if 16 warps still fit
-    static constexpr int warps = (fit / nbuf) >= 16 ? 16 : (fit / nbuf);   // 0 => does not fit
-    static constexpr int smem = warps * nbuf * tile_bytes;
+    static constexpr int fit = TPB_SMEM_PER_SM / (tile_bytes + 1024);   // resident CTAs per SM by shared memory
+    static constexpr int cap = 16 / SPLIT;                              // ... and by registers (<= 128 each)
+    static constexpr int min_ctas = fit < 1 ? 1 : (fit < cap ? fit : cap);
+    static constexpr int cut = TpbCut<LMAX, SPLIT>::cut();
 };
 
-template <typename T, typename R, int DERIV, bool NORM, int LMAX>
-__global__ void __launch_bounds__(TpbShape<sizeof(T), DERIV, LMAX>::warps * 32, 1)
+template <typename T, typename R, int DERIV, bool NORM, int LMAX, int SPLIT>
+__global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, SPLIT>::min_ctas)
     sph_tpb_kernel(const TpbParams prm) {
     using RT = rec<R>;
-    using Shape = TpbShape<sizeof(T), DERIV, LMAX>;
+    using Shape = TpbShape<sizeof(T), DERIV, LMAX, SPLIT>;
     constexpr int L = Shape::L;
-    constexpr int WARPS = Shape::warps;
-    constexpr int NBUF = Shape::nbuf;
+    constexpr int CUT = Shape::cut;
     constexpr uint32_t S_BYTES = TPB_PTS * L * sizeof(T);
     const SphTables& TB = c_tables_tpb;
     extern __shared__ __align__(128) unsigned char smem[];
     const int lane = threadIdx.x & 31;
-    const int warp = threadIdx.x >> 5;
+    const int part = threadIdx.x >> 5;     // which share of the columns (warp-uniform)
     const int pl = lane & (TPB_PTS - 1);   // point inside the tile
     const bool sinb = lane >= TPB_PTS;     // branch
     const int64_t n = prm.n;
@@ -76,19 +104,32 @@ __global__ void __launch_bounds__(TpbShape<sizeof(T), DERIV, LMAX>::warps * 32, 
     const T* __restrict__ xyz = static_cast<const T*>(prm.xyz);
     T* __restrict__ sph = static_cast<T*>(prm.sph);
     T* __restrict__ dsph = static_cast<T*>(prm.dsph);
-    unsigned char* my = smem + (size_t)warp * NBUF * Shape::tile_bytes;
     const uint64_t policy = policy_evict_first();
+    auto cta_sync = [&]() {
+        if constexpr (SPLIT == 1) __syncwarp();
+        else __syncthreads();
+    };
 
-    const int64_t stride = (int64_t)gridDim.x * WARPS;
-    int buf = 0;
-    for (int64_t tile = (int64_t)warp * gridDim.x + blockIdx.x; tile < n_tiles; tile += stride) {
+    const int64_t t_begin = (int64_t)blockIdx.x * prm.tiles_per_cta;
+    int64_t t_end = t_begin + prm.tiles_per_cta;
+    if (t_end > n_tiles) t_end = n_tiles;
+
+    // lanes past the end compute a harmless point
+    auto load_xyz = [&](int64_t tile, T& a, T& b, T& c) {
         const int64_t p = tile * TPB_PTS + pl;
-        double x = 0.0, y = 0.0, z = 1.0;  // lanes past the end compute a harmless point
+        a = T(0), b = T(0), c = T(1);
         if (p < n) {
-            x = static_cast<double>(__ldg(xyz + 3 * p + 0));
-            y = static_cast<double>(__ldg(xyz + 3 * p + 1));
-            z = static_cast<double>(__ldg(xyz + 3 * p + 2));
+            a = __ldg(xyz + 3 * p + 0);
+            b = __ldg(xyz + 3 * p + 1);
+            c = __ldg(xyz + 3 * p + 2);
         }
+    };
+    T xn, yn, zn;
+    if (t_begin < t_end) load_xyz(t_begin, xn, yn, zn);
+
+    for (int64_t tile = t_begin; tile < t_end; ++tile) {
+        const double x = static_cast<double>(xn), y = static_cast<double>(yn), z = static_cast<double>(zn);
+        if (tile + 1 < t_end) load_xyz(tile + 1, xn, yn, zn);   // in flight while this tile computes
         R X, Y, Z, r2;
         double rinv = 1.0;
         if (NORM) {
@@ -103,10 +144,12 @@ __global__ void __launch_bounds__(TpbShape<sizeof(T), DERIV, LMAX>::warps * 32, 
         const double xd = to_double(X), yd = to_double(Y), zd = to_double(Z);
 
         // the image we are about to overwrite must have been read out by its bulk store
-        if (lane == 0) bulk_wait_read<NBUF - 1>();
-        __syncwarp();
-        T* S = reinterpret_cast<T*>(my + (size_t)buf * Shape::tile_bytes) + pl * L;
-        T* G = reinterpret_cast<T*>(my + (size_t)buf * Shape::tile_bytes + S_BYTES) + pl * 3 * L;
+        if (tile > t_begin) {
+            if (threadIdx.x == 0) bulk_wait_read<0>();
+            cta_sync();
+        }
+        T* S = reinterpret_cast<T*>(smem) + pl * L;
+        T* G = reinterpret_cast<T*>(smem + S_BYTES) + pl * 3 * L;
 
         double Qc[LMAX + 1];   // column m:   Qc[l] = Qt_l^m     (0 for l < m)
         double Qn[LMAX + 1];   // column m+1: Qn[l] = Qt_l^{m+1} (0 for l < m+1)
@@ -133,93 +176,111 @@ __global__ void __launch_bounds__(TpbShape<sizeof(T), DERIV, LMAX>::warps * 32, 
                 }
             });
         };
-        column(std::integral_constant<int, 0>{}, Qc);
-        R c = RT::make(1.0, 0.0), s = RT::make(0.0, 0.0);
-        double c1 = 0.0, s1 = 0.0;  // c_{m-1}, s_{m-1}
-        static_for<0, LMAX + 1>([&](auto mc) {
-            constexpr int m = decltype(mc)::value;
-            // column m+1, computed once: Eq. 10 needs Qt_{l-1}^{m+1} now, and it is the next column
-            if constexpr (m < LMAX) column(std::integral_constant<int, m + 1>{}, Qn);
-            // azimuthal factor of this lane's branch and its x/y derivatives (Eq. 9, Eq. 10)
-            const double cd = to_double(c), sd = to_double(s);
-            const double dm = (double)m;
-            const double A = sinb ? sd : (m == 0 ? SPH_INV_SQRT2 : cd);
-            double Ax = dm * (sinb ? s1 : c1);
-            double Ay = dm * (sinb ? c1 : -s1);
-            double xA = xd * A, yA = yd * A, Az = A;
-            if (NORM && DERIV >= 1) {
-                xA *= rinv;
-                yA *= rinv;
-                Az *= rinv;
-                Ax *= rinv;
-                Ay *= rinv;
-            }
-            const bool emit = (m > 0) || !sinb;   // the sin branch has no m = 0 output
-            static_for<m, LMAX + 1>([&](auto lc) {
-                constexpr int l = decltype(lc)::value;
-                constexpr int kc = l * (l + 1) + m, ks = l * (l + 1) - m;
-                const int k = sinb ? ks : kc;
-                const double Q = Qc[l];
-                if (emit) S[k] = static_cast<T>(Q * A);
-                if constexpr (DERIV >= 1) {
-                    constexpr int t = SPH_TRI(l, m);
-                    double q1 = 0.0, qz = 0.0;
-                    if constexpr (l >= m + 2) q1 = TB.G1[t] * Qn[l - 1];   // F_l^m Q_{l-1}^{m+1}
-                    if constexpr (l >= m + 1) qz = TB.Gz[t] * Qc[l - 1];   // F_l^m (l+m) Q_{l-1}^m
-                    double gx, gy, gz;
-                    if (NORM) {
-                        const double lQ = (double)l * Q;
-                        const double t1 = q1 - lQ;
-                        const double tz = SPH_FMA(-lQ, zd, qz);
-                        gx = SPH_FMA(t1, xA, Q * Ax);
-                        gy = SPH_FMA(t1, yA, Q * Ay);
-                        gz = tz * Az;
-                    } else {
-                        gx = SPH_FMA(q1, xA, Q * Ax);
-                        gy = SPH_FMA(q1, yA, Q * Ay);
-                        gz = qz * Az;
-                    }
-                    if (emit) {
-                        G[k] = static_cast<T>(gx);
-                        G[L + k] = static_cast<T>(gy);
-                        G[2 * L + k] = static_cast<T>(gz);
-                    }
-                }
-            });
-            // next column, next power of (x + i y): Eq. 9
-            if constexpr (m < LMAX) {
-                static_for<m + 1, LMAX + 1>([&](auto lc) { Qc[decltype(lc)::value] = Qn[decltype(lc)::value]; });
-                c1 = cd;
-                s1 = sd;
+        // the columns M0 <= m < M1 of the triangle: values (Eq. 5) and gradients (Eq. 10) of this
+        // lane's branch into the image
+        auto columns = [&](auto M0c, auto M1c) {
+            constexpr int M0 = decltype(M0c)::value, M1 = decltype(M1c)::value;
+            R c = RT::make(1.0, 0.0), s = RT::make(0.0, 0.0);
+            double c1 = 0.0, s1 = 0.0;  // c_{m-1}, s_{m-1}
+            static_for<0, M0>([&](auto) {   // Eq. 9 up to (x + i y)^M0
+                c1 = to_double(c);
+                s1 = to_double(s);
                 const R cn = X * c - Y * s;
                 const R sn = X * s + Y * c;
                 c = cn;
                 s = sn;
-            }
-        });
+            });
+            column(std::integral_constant<int, M0>{}, Qc);
+            static_for<M0, M1>([&](auto mc) {
+                constexpr int m = decltype(mc)::value;
+                // column m+1, computed once: Eq. 10 needs Qt_{l-1}^{m+1} now, and it is the next column
+                if constexpr (m < LMAX && (DERIV >= 1 || m + 1 < M1)) column(std::integral_constant<int, m + 1>{}, Qn);
+                // azimuthal factor of this lane's branch and its x/y derivatives (Eq. 9, Eq. 10)
+                const double cd = to_double(c), sd = to_double(s);
+                const double dm = (double)m;
+                const double A = sinb ? sd : (m == 0 ? SPH_INV_SQRT2 : cd);
+                double Ax = dm * (sinb ? s1 : c1);
+                double Ay = dm * (sinb ? c1 : -s1);
+                double xA = xd * A, yA = yd * A, Az = A;
+                if (NORM && DERIV >= 1) {
+                    xA *= rinv;
+                    yA *= rinv;
+                    Az *= rinv;
+                    Ax *= rinv;
+                    Ay *= rinv;
+                }
+                const bool emit = (m > 0) || !sinb;   // the sin branch has no m = 0 output
+                static_for<m, LMAX + 1>([&](auto lc) {
+                    constexpr int l = decltype(lc)::value;
+                    constexpr int kc = l * (l + 1) + m, ks = l * (l + 1) - m;
+                    const int k = sinb ? ks : kc;
+                    const double Q = Qc[l];
+                    if (emit) S[k] = static_cast<T>(Q * A);
+                    if constexpr (DERIV >= 1) {
+                        constexpr int t = SPH_TRI(l, m);
+                        double q1 = 0.0, qz = 0.0;
+                        if constexpr (l >= m + 2) q1 = TB.G1[t] * Qn[l - 1];   // F_l^m Q_{l-1}^{m+1}
+                        if constexpr (l >= m + 1) qz = TB.Gz[t] * Qc[l - 1];   // F_l^m (l+m) Q_{l-1}^m
+                        double gx, gy, gz;
+                        if (NORM) {
+                            const double lQ = (double)l * Q;
+                            const double t1 = q1 - lQ;
+                            const double tz = SPH_FMA(-lQ, zd, qz);
+                            gx = SPH_FMA(t1, xA, Q * Ax);
+                            gy = SPH_FMA(t1, yA, Q * Ay);
+                            gz = tz * Az;
+                        } else {
+                            gx = SPH_FMA(q1, xA, Q * Ax);
+                            gy = SPH_FMA(q1, yA, Q * Ay);
+                            gz = qz * Az;
+                        }
+                        if (emit) {
+                            G[k] = static_cast<T>(gx);
+                            G[L + k] = static_cast<T>(gy);
+                            G[2 * L + k] = static_cast<T>(gz);
+                        }
+                    }
+                });
+                // next column, next power of (x + i y): Eq. 9
+                if constexpr (m + 1 < M1) {
+                    static_for<m + 1, LMAX + 1>([&](auto lc) { Qc[decltype(lc)::value] = Qn[decltype(lc)::value]; });
+                    c1 = cd;
+                    s1 = sd;
+                    const R cn = X * c - Y * s;
+                    const R sn = X * s + Y * c;
+                    c = cn;
+                    s = sn;
+                }
+            });
+        };
+        if constexpr (SPLIT == 1) {
+            columns(std::integral_constant<int, 0>{}, std::integral_constant<int, LMAX + 1>{});
+        } else {
+            if (part == 0) columns(std::integral_constant<int, 0>{}, std::integral_constant<int, CUT>{});
+            else columns(std::integral_constant<int, CUT>{}, std::integral_constant<int, LMAX + 1>{});
+        }
 
         fence_proxy_async_smem();
-        __syncwarp();
+        cta_sync();
         const int64_t p0 = tile * TPB_PTS;
-        T* S0 = reinterpret_cast<T*>(my + (size_t)buf * Shape::tile_bytes);
-        T* G0 = reinterpret_cast<T*>(my + (size_t)buf * Shape::tile_bytes + S_BYTES);
+        T* S0 = reinterpret_cast<T*>(smem);
+        T* G0 = reinterpret_cast<T*>(smem + S_BYTES);
         if (n - p0 >= TPB_PTS) {
-            if (lane == 0) {
+            if (threadIdx.x == 0) {
                 bulk_store_hint(sph + p0 * L, S0, S_BYTES, policy);
                 if (DERIV >= 1) bulk_store_hint(dsph + p0 * 3 * L, G0, 3u * S_BYTES, policy);
                 bulk_commit();
             }
         } else {  // ragged last tile: byte count need not be a multiple of 16 -> plain stores
             const int np = (int)(n - p0);
-            for (int i = lane; i < np * L; i += 32) st_cs(sph + p0 * L + i, S0[i]);
+            for (int i = threadIdx.x; i < np * L; i += SPLIT * 32) st_cs(sph + p0 * L + i, S0[i]);
             if (DERIV >= 1)
-                for (int i = lane; i < np * 3 * L; i += 32) st_cs(dsph + p0 * 3 * L + i, G0[i]);
-            __syncwarp();
+                for (int i = threadIdx.x; i < np * 3 * L; i += SPLIT * 32) st_cs(dsph + p0 * 3 * L + i, G0[i]);
+            cta_sync();
         }
-        buf = (buf + 1 == NBUF) ? 0 : buf + 1;
     }
-    // shared memory must outlive the bulk stores that read it
-    if (lane == 0) bulk_wait_all<0>();
+    // shared memory must outlive the bulk stores' reads of it
+    if (threadIdx.x == 0) bulk_wait_read<0>();
 }
 
 }  // namespace sphb200

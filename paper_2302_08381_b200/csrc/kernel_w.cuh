@@ -33,6 +33,7 @@ struct WkParams {
     int warps_per_cta;
     int chunk;              // CH, multiple of 32
     int nbuf;               // staging images per warp
+    int pts_per_warp;       // consecutive rounds of warps_per_cta points one CTA works through
 };
 
 struct WkTabView {  // phase-B coefficient tables, copied to shared memory once per CTA
@@ -109,9 +110,14 @@ __global__ void __launch_bounds__(WK_MAX_THREADS, 1) sph_w_kernel(const WkParams
     int nbits = 0;
     while ((1 << nbits) <= (l_max < 31 ? l_max : 31)) ++nbits;
 
-    const int64_t stride = (int64_t)gridDim.x * prm.warps_per_cta;
+    // NOT persistent: CTA b owns the points [b W P, (b+1) W P) (W warps, P points per warp) and the
+    // grid has many more CTAs than the machine holds, so the block scheduler balances SMs that
+    // drain their stores at different rates (kernel_tpb.cuh has the measurement).
+    const int64_t pt_begin = (int64_t)blockIdx.x * prm.warps_per_cta * prm.pts_per_warp;
+    int64_t pt_end = pt_begin + (int64_t)prm.warps_per_cta * prm.pts_per_warp;
+    if (pt_end > prm.n) pt_end = prm.n;
     int buf = 0;
-    for (int64_t pt = (int64_t)warp * gridDim.x + blockIdx.x; pt < prm.n; pt += stride) {
+    for (int64_t pt = pt_begin + warp; pt < pt_end; pt += prm.warps_per_cta) {
         const double x = static_cast<double>(xyz[3 * pt + 0]);
         const double y = static_cast<double>(xyz[3 * pt + 1]);
         const double z = static_cast<double>(xyz[3 * pt + 2]);
@@ -232,7 +238,7 @@ __global__ void __launch_bounds__(WK_MAX_THREADS, 1) sph_w_kernel(const WkParams
             buf = (buf + 1 == prm.nbuf) ? 0 : buf + 1;
         }
     }
-    bulk_wait_all<0>();
+    bulk_wait_read<0>();   // shared memory must outlive the bulk stores' reads of it
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -317,8 +323,15 @@ static inline int wk_plan(int sm_count, int smem_optin, int64_t n, int l_max, in
     if (warps > want) warps = want;
     int64_t per_sm = (n + sm_count - 1) / sm_count;
     if (per_sm < warps) warps = (int)(per_sm < 1 ? 1 : per_sm);
-    int64_t ctas = (n + warps - 1) / warps;
-    if (ctas > sm_count) ctas = sm_count;
+    // points per warp: amortise the per-CTA table copy, but keep >= ~16 waves of CTAs
+    int64_t ppw = wk_env("SPHB200_W_PPW", 0);
+    if (ppw <= 0) {
+        ppw = n / ((int64_t)sm_count * warps * 16);
+        if (ppw > 8) ppw = 8;
+    }
+    if (ppw < 1) ppw = 1;
+    const int64_t ctas = (n + warps * ppw - 1) / (warps * ppw);
+    if (ctas > 0x7fffffff) return 1;
     WkSmem lay(l_max, deriv, esize, chunk, nbuf);
     out->kern = dtype == 0 ? wk_pick<float, double>(deriv, normalized) : wk_pick<double, dd>(deriv, normalized);
     out->func = (const void*)out->kern;
@@ -332,6 +345,7 @@ static inline int wk_plan(int sm_count, int smem_optin, int64_t n, int l_max, in
     out->prm.warps_per_cta = warps;
     out->prm.chunk = chunk;
     out->prm.nbuf = nbuf;
+    out->prm.pts_per_warp = (int)ppw;
     out->grid = (int)ctas;
     out->threads = warps * 32;
     out->smem = lay.tab_bytes + (size_t)warps * lay.warp_bytes;

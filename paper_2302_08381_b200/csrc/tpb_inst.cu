@@ -6,6 +6,8 @@
 #include "kernel_tpb.cuh"
 #include "tpb_api.h"
 
+#include <cstdlib>
+
 #ifndef TPB_F64
 #error "compile with -DTPB_F64=0|1 -DTPB_DERIV=0|1"
 #endif
@@ -30,24 +32,49 @@ typedef double tpb_R;
 #define TPB_NAME(f) f##_f32_v
 #endif
 
-template <int LMAX, bool NORM>
-static int launch_one(int sm_count, const TpbParams& prm, cudaStream_t stream) {
-    using Shape = TpbShape<sizeof(tpb_T), TPB_DERIV, LMAX>;
-    static_assert(Shape::warps >= 1, "tile does not fit in shared memory");
-    auto kern = sph_tpb_kernel<tpb_T, tpb_R, TPB_DERIV, NORM, LMAX>;
+static int env_int(const char* name, int dflt) {
+    const char* s = getenv(name);
+    return (s && *s) ? atoi(s) : dflt;
+}
+
+template <int LMAX, bool NORM, int SPLIT>
+static int launch_split(int sm_count, TpbParams prm, cudaStream_t stream) {
+    using Shape = TpbShape<sizeof(tpb_T), TPB_DERIV, LMAX, SPLIT>;
+    static_assert(Shape::fit >= 1, "tile does not fit in shared memory");
+    auto kern = sph_tpb_kernel<tpb_T, tpb_R, TPB_DERIV, NORM, LMAX, SPLIT>;
     static bool attr_done[64] = {false};   // per device; benign race (idempotent call)
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return -1;
     if (dev >= 0 && dev < 64 && !attr_done[dev]) {
-        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Shape::smem) != cudaSuccess)
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Shape::tile_bytes) != cudaSuccess)
             return -1;
         attr_done[dev] = true;
     }
+    // one tile per CTA measured best on every config (C3: 166 us against 172 us with four, C5: 476
+    // against 508): the CTA launch is cheap next to a tile; the knob stays for experiments
     const int64_t n_tiles = (prm.n + TPB_PTS - 1) / TPB_PTS;
-    int64_t ctas = (n_tiles + Shape::warps - 1) / Shape::warps;
-    if (ctas > sm_count) ctas = sm_count;
-    kern<<<(int)ctas, Shape::warps * 32, Shape::smem, stream>>>(prm);
+    static const int k_env = env_int("SPHB200_TPB_TILES", 1);
+    const int64_t k = k_env > 0 ? k_env : 1;
+    prm.tiles_per_cta = (int)k;
+    const int64_t ctas = (n_tiles + k - 1) / k;
+    if (ctas > 0x7fffffff) return 1;
+    kern<<<(unsigned)ctas, SPLIT * 32, Shape::tile_bytes, stream>>>(prm);
     return cudaGetLastError() == cudaSuccess ? 0 : -1;
+}
+
+// Two warps per tile where shared memory, not registers, limits the tiles in flight (<= 12 per
+// SM): the second warp then fills issue slots that would idle and halves a tile's latency.
+// Measured: C2 24.7 -> 22.8 us, C3 166 -> 164 us; C5 (17 tiles fit) 476 -> 562 us, so not there.
+template <int LMAX, bool NORM>
+static int launch_one(int sm_count, const TpbParams& prm, cudaStream_t stream) {
+    static const int split_env = env_int("SPHB200_TPB_SPLIT", 0);
+    constexpr bool can_split = LMAX >= 4;
+    if constexpr (can_split) {
+        constexpr bool dflt = TpbShape<sizeof(tpb_T), TPB_DERIV, LMAX, 1>::fit <= 12;
+        const bool want = split_env ? split_env == 2 : dflt;
+        if (want) return launch_split<LMAX, NORM, 2>(sm_count, prm, stream);
+    }
+    return launch_split<LMAX, NORM, 1>(sm_count, prm, stream);
 }
 
 #define TPB_CASE(LM) \
@@ -56,7 +83,7 @@ static int launch_one(int sm_count, const TpbParams& prm, cudaStream_t stream) {
 
 int TPB_NAME(sph_tpb_launch)(int sm_count, const void* xyz, int64_t n, int l_max, int normalized, void* sph,
                              void* dsph, cudaStream_t stream) {
-    TpbParams prm{xyz, sph, dsph, n};
+    TpbParams prm{xyz, sph, dsph, n, 1};
     switch (l_max) {
         TPB_CASE(1)
         TPB_CASE(2)
