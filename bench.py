@@ -50,6 +50,11 @@ def measured_peaks():
 # ncu --set full: dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel,
 # copied by hand from the capture summarised under profiles/ (None until a capture exists).
 NCU_TRAFFIC_BYTES = {
+    # profiles/r1b_kernels.md
+    "C2": 71.43e6,     # 70.19 MB written + 1.24 MB read (a single launch's 129.6 MB output is L2-sized)
+    "C3": 1108.6e6,    # 1096.6 MB written + 12.05 MB read
+    "C4": 29.918e9,    # 29.807 GB written + 0.111 GB read
+    "C5": 3124.6e6,    # forward kernel: 3076.6 MB written + 48.0 MB read
 }
 
 
@@ -177,14 +182,26 @@ def n_sets_for(cfg, free_bytes):
 
 
 def store_ceiling_gbs(torch, nbytes, device):
-    """Write-only ceiling measured in the same run: torch's fill kernel over the same byte count."""
-    nbytes = int(min(max(nbytes, 1 << 28), 8 << 30))
-    bufs = [torch.empty(nbytes, dtype=torch.uint8, device=device) for _ in range(2)]
-    for b in bufs:
-        b.zero_()
+    """Write-only ceiling measured in the same run: cudaMemsetAsync over the same byte count,
+    rotating over buffers larger than L2 (torch's fill kernel if libcudart cannot be reached)."""
+    import ctypes
+
+    nbytes = int(min(max(nbytes, 1 << 20), 8 << 30))
+    n_bufs = max(2, int(600e6 // nbytes) + 1)
+    bufs = [torch.empty(nbytes, dtype=torch.uint8, device=device) for _ in range(n_bufs)]
+    fill = lambda i: bufs[i % n_bufs].zero_()
+    try:
+        rt = ctypes.CDLL("libcudart.so.12")
+        rt.cudaMemsetAsync.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t, ctypes.c_void_p]
+        stream = torch.cuda.current_stream().cuda_stream
+        fill = lambda i: rt.cudaMemsetAsync(bufs[i % n_bufs].data_ptr(), 0, nbytes, stream)
+    except OSError:
+        pass
+    for i in range(3):
+        fill(i)
     torch.cuda.synchronize()
-    reps = 10
-    e0, e1 = time_loop(torch, lambda i: bufs[i & 1].zero_(), reps)
+    reps = int(max(10, min(200, 4e9 // nbytes)))
+    e0, e1 = time_loop(torch, fill, reps)
     torch.cuda.synchronize()
     return nbytes * reps / (e0.elapsed_time(e1) * 1e-3) / 1e9
 
@@ -341,7 +358,7 @@ def run_cuda(args):
     else:
         ms_fwd = ms_step
     achieved = cfg.n * fwd_b / (ms_fwd * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "forward (sph_tp_kernel / sph_w_kernel)", "achieved": achieved,
+    roofline = {"bound": "hbm", "kernel": "forward (sph_tpb_kernel; sph_w_kernel for C4)", "achieved": achieved,
                 "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg.name),
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": cfg.n * fwd_b,
                 "avg_launch_us": ms_fwd * 1e3, "output_gbs": cfg.n * cfg.out_bytes_per_point / (ms_fwd * 1e-3) / 1e9,

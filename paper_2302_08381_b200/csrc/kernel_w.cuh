@@ -5,15 +5,15 @@
 //   phase A  lane = m: c_m, s_m by square-and-multiply and column m of the Legendre triangle by the
 //            integer-coefficient form of Eq. 7 (tables.h), all lanes stepping l together; the
 //            triangle Qt and (c,s) go to a per-warp scratch in shared memory as f64;
-//   phase B  lane = output index k inside a chunk of CH consecutive harmonics: each lane assembles
-//            ALL components (Y, 3 gradient, 6 unique Hessian) of its (l,m) from the scratch
-//            (assemble_element) and writes them into per-component staging rows in shared memory;
-//   store    each of the 1/4/13 global rows of the chunk is a contiguous run of CH elements; lane j
+//   phase B  a chunk = a few whole l-rows (<= CH harmonics); lane = one (l, m >= 0) of the chunk's
+//            part of the triangle: it assembles ALL components (Y, 3 gradient, 6 unique Hessian) of
+//            BOTH harmonics (l, +m) and (l, -m) from the scratch (assemble_pair: the Legendre side
+//            of Eq. 10 is shared by the two) and writes them into per-component staging rows;
+//   store    each of the 1/4/13 global rows of the chunk is a contiguous run of elements; lane j
 //            issues row j as one 1-D TMA bulk store.  A run starts at element (n*rows+j)*L + k0,
-//            which is 16-byte aligned only up to an element offset sigma_j; the staging row holds
-//            the run at offset sigma_j so that shared and global addresses agree mod 16, the
-//            aligned body goes out by TMA and at most AL-1 elements at either end by plain stores.
-// Staging rows are double-buffered, so phase B of the next chunk overlaps the drain of this one.
+//            which is 16-byte aligned only up to an element offset; the staging image (WkStage)
+//            places every run so that shared and global addresses agree mod 16, the aligned body
+//            goes out by TMA and at most AL-1 elements at either end by plain stores.
 #pragma once
 #include <atomic>
 
@@ -31,20 +31,50 @@ struct WkParams {
     int64_t n;
     int l_max;
     int warps_per_cta;
-    int chunk;              // CH, multiple of 32
     int nbuf;               // staging images per warp
     int pts_per_warp;       // consecutive rounds of warps_per_cta points one CTA works through
+    int n_chunks;
+    unsigned char row0[SPH_MAX_L + 3];   // chunk i = the l-rows [row0[i], row0[i+1])
 };
 
 struct WkTabView {  // phase-B coefficient tables, copied to shared memory once per CTA
     const double *G1, *Gz, *H2, *Hxz, *Hzz;
 };
 
-constexpr int WK_MAX_THREADS = 512;
+constexpr int WK_MAX_THREADS = 384;
+constexpr int WK_CH = 128;   // most harmonics in a chunk (whole l-rows; the row l = 32 has 65)
 
 template <int DERIV> struct wk_rows {  // global rows per point / staging rows
     static constexpr int n = DERIV == 0 ? 1 : (DERIV == 1 ? 4 : 13);
 };
+
+// Staging image of one chunk: one row per output component, laid out so that EVERY row's
+// shared-memory address agrees with its global address modulo 16 bytes (what a bulk store needs)
+// while the rows of one array sit a COMPILE-TIME stride apart:
+//   row jj of array a (a = 0 sph, 1 dsph, 2 ddsph) starts at global element
+//       e(a, jj) = (pt rows_a + jj) L + k0,            so  e(a, jj) = e(a, 0) + jj L;
+//   it is staged at element  A_a + d_a + jj RS  with  d_a = e(a, 0) mod AL  (AL = elements per
+//   16 bytes) and a row stride RS = L (mod AL): RS = CH + 1 for odd L (odd squares are 1 mod 8),
+//   RS = CH + AL for even L (even squares are 0 mod 4).
+// One base register per array then addresses all of its rows with immediate offsets.
+__host__ __device__ constexpr int wk_round_up(int v, int a) { return (v + a - 1) / a * a; }
+template <int ESIZE, int DERIV, bool LODD> struct WkStage {
+    static constexpr int AL = 16 / ESIZE;
+    static constexpr int RS = LODD ? WK_CH + 1 : WK_CH + AL;
+    static constexpr int A1 = wk_round_up(RS + AL - 1, AL);              // after the 1 row of sph
+    static constexpr int A2 = wk_round_up(A1 + 3 * RS + AL - 1, AL);     // after the 3 rows of dsph
+    static constexpr int A3 = wk_round_up(A2 + 9 * RS + AL - 1, AL);     // after the 9 rows of ddsph
+    static constexpr int elems = DERIV == 0 ? A1 : (DERIV == 1 ? A2 : A3);
+    static constexpr int bytes = elems * ESIZE;
+};
+__host__ __device__ constexpr int wk_stage_bytes(int esize, int deriv, bool lodd) {
+    return esize == 4 ? (deriv == 0 ? (lodd ? WkStage<4, 0, true>::bytes : WkStage<4, 0, false>::bytes)
+                                    : deriv == 1 ? (lodd ? WkStage<4, 1, true>::bytes : WkStage<4, 1, false>::bytes)
+                                                 : (lodd ? WkStage<4, 2, true>::bytes : WkStage<4, 2, false>::bytes))
+                      : (deriv == 0 ? (lodd ? WkStage<8, 0, true>::bytes : WkStage<8, 0, false>::bytes)
+                                    : deriv == 1 ? (lodd ? WkStage<8, 1, true>::bytes : WkStage<8, 1, false>::bytes)
+                                                 : (lodd ? WkStage<8, 2, true>::bytes : WkStage<8, 2, false>::bytes));
+}
 
 // shared-memory carve-up (bytes), identical on host and device
 struct WkSmem {
@@ -52,34 +82,40 @@ struct WkSmem {
     int ntab;           // coefficient tables kept in smem: Np + {0,2,5}
     size_t tab_bytes;
     size_t scratch_bytes;   // per warp: Qt[tsz] + cs[2(l_max+1)], rounded to 16
-    size_t row_bytes;       // one staging row: (CH + AL) elements
-    size_t stage_bytes;     // per warp: nbuf * rows * row_bytes
+    size_t stage_bytes;     // per warp: nbuf staging images
     size_t warp_bytes;
-    __host__ __device__ WkSmem(int l_max, int deriv, int esize, int chunk, int nbuf) {
+    __host__ __device__ WkSmem(int l_max, int deriv, int esize, int nbuf) {
         tsz = (l_max + 1) * (l_max + 2) / 2;
         ntab = 1 + (deriv == 0 ? 0 : (deriv == 1 ? 2 : 5));
         tab_bytes = ((size_t)ntab * tsz * 8 + 15) & ~(size_t)15;
         scratch_bytes = ((size_t)(tsz + 2 * (l_max + 1)) * 8 + 15) & ~(size_t)15;
-        const int al = 16 / esize;
-        row_bytes = (size_t)(chunk + al) * esize;
-        const int rows = deriv == 0 ? 1 : (deriv == 1 ? 4 : 13);
-        stage_bytes = (size_t)nbuf * rows * row_bytes;
+        stage_bytes = (size_t)nbuf * wk_stage_bytes(esize, deriv, (l_max & 1) == 0);
         warp_bytes = scratch_bytes + stage_bytes;
     }
 };
 
-template <typename T, typename R, int DERIV, bool NORM>
+// shared-memory stores through 32-bit shared addresses with an immediate byte offset
+template <int OFF> __device__ __forceinline__ void sts_off(uint32_t addr, float v) {
+    asm volatile("st.shared.f32 [%0+%2], %1;" ::"r"(addr), "f"(v), "n"(OFF) : "memory");
+}
+template <int OFF> __device__ __forceinline__ void sts_off(uint32_t addr, double v) {
+    asm volatile("st.shared.f64 [%0+%2], %1;" ::"r"(addr), "d"(v), "n"(OFF) : "memory");
+}
+
+template <typename T, typename R, int DERIV, bool NORM, bool LODD>
 __global__ void __launch_bounds__(WK_MAX_THREADS, 1) sph_w_kernel(const WkParams prm) {
     extern __shared__ __align__(128) unsigned char smem[];
     constexpr int ROWS = wk_rows<DERIV>::n;
-    constexpr int AL = 16 / (int)sizeof(T);
+    constexpr int ES = (int)sizeof(T);
+    using Stage = WkStage<ES, DERIV, LODD>;
+    constexpr int AL = Stage::AL;
+    constexpr int RS = Stage::RS;
     using RT = rec<R>;
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
     const int l_max = prm.l_max;
     const int L = (l_max + 1) * (l_max + 1);
-    const int CH = prm.chunk;
-    const WkSmem lay(l_max, DERIV, (int)sizeof(T), CH, prm.nbuf);
+    const WkSmem lay(l_max, DERIV, ES, prm.nbuf);
 
     // ---- coefficient tables -> shared memory (once per CTA) -----------------------------------
     double* tabs = reinterpret_cast<double*>(smem);
@@ -101,7 +137,11 @@ __global__ void __launch_bounds__(WK_MAX_THREADS, 1) sph_w_kernel(const WkParams
     double* Qt = reinterpret_cast<double*>(my);
     double* cs = Qt + lay.tsz;
     unsigned char* stage = my + lay.scratch_bytes;
-    const int row_elems = CH + AL;
+    const uint32_t stage_s = smem_u32(stage);
+    // neighbour reads of assemble_pair may touch the padding behind cs (times a zero coefficient):
+    // it only has to be finite
+    for (int i = lane; i < (int)(lay.scratch_bytes / 8); i += 32) Qt[i] = 0.0;
+    __syncwarp();
 
     const T* __restrict__ xyz = static_cast<const T*>(prm.xyz);
     T* __restrict__ out_base[3] = {static_cast<T*>(prm.sph), static_cast<T*>(prm.dsph), static_cast<T*>(prm.ddsph)};
@@ -161,58 +201,63 @@ __global__ void __launch_bounds__(WK_MAX_THREADS, 1) sph_w_kernel(const WkParams
         }
         __syncwarp();
 
-        // ---- phase B + store: chunks of CH harmonics -----------------------------------------
-        for (int k0 = 0; k0 < L; k0 += CH) {
+        // ---- phase B + store: chunks of whole l-rows ---------------------------------------------
+        const uint32_t ptl = (uint32_t)pt;   // low 32 bits are enough modulo AL
+        for (int ci = 0; ci < prm.n_chunks; ++ci) {
+            const int l0 = prm.row0[ci], l1 = prm.row0[ci + 1];   // rows [l0, l1)
+            const int k0 = l0 * l0;
+            const int cnt = l1 * l1 - k0;
+            const int tA = SPH_TRI(l0, 0), tB = SPH_TRI(l1, 0);   // this chunk's part of the triangle
             // the staging image we are about to fill must have been drained
             if (prm.nbuf == 1) bulk_wait_read<0>();
             else bulk_wait_read<1>();
             __syncwarp();
-            T* img = reinterpret_cast<T*>(stage + (size_t)buf * ROWS * lay.row_bytes);
-            const int cnt = (L - k0 < CH) ? L - k0 : CH;
+            // d_a = e(a, 0) mod AL, and the 32-bit shared address of row 0 of each array
+            const uint32_t d0 = (ptl * (uint32_t)L + (uint32_t)k0) & (AL - 1);
+            const uint32_t d1 = (ptl * 3u * (uint32_t)L + (uint32_t)k0) & (AL - 1);
+            const uint32_t d2 = (ptl * 9u * (uint32_t)L + (uint32_t)k0) & (AL - 1);
+            const uint32_t img_s = stage_s + (uint32_t)buf * Stage::bytes;
+            const uint32_t b0 = img_s + d0 * ES;
+            const uint32_t b1 = img_s + (Stage::A1 + d1) * ES;
+            const uint32_t b2 = img_s + (Stage::A2 + d2) * ES;
+            auto put = [&](int i, const double* o) {
+                const uint32_t ib = (uint32_t)i * ES;
+                sts_off<0>(b0 + ib, static_cast<T>(o[0]));
+                if constexpr (DERIV >= 1) {
+                    const uint32_t a1 = b1 + ib;
+                    sts_off<0 * RS * ES>(a1, static_cast<T>(o[1]));
+                    sts_off<1 * RS * ES>(a1, static_cast<T>(o[2]));
+                    sts_off<2 * RS * ES>(a1, static_cast<T>(o[3]));
+                }
+                if constexpr (DERIV >= 2) {
+                    // o[4..9] = xx xy xz yy yz zz ; rows = xx xy xz yx yy yz zx zy zz
+                    const uint32_t a2 = b2 + ib;
+                    sts_off<0 * RS * ES>(a2, static_cast<T>(o[4]));
+                    sts_off<1 * RS * ES>(a2, static_cast<T>(o[5]));
+                    sts_off<2 * RS * ES>(a2, static_cast<T>(o[6]));
+                    sts_off<3 * RS * ES>(a2, static_cast<T>(o[5]));
+                    sts_off<4 * RS * ES>(a2, static_cast<T>(o[7]));
+                    sts_off<5 * RS * ES>(a2, static_cast<T>(o[8]));
+                    sts_off<6 * RS * ES>(a2, static_cast<T>(o[6]));
+                    sts_off<7 * RS * ES>(a2, static_cast<T>(o[8]));
+                    sts_off<8 * RS * ES>(a2, static_cast<T>(o[9]));
+                }
+            };
 
-            // element offset of row j of this point inside its array, low bits only
-            // rows: 0 = sph; 1..3 = dsph[a]; 4..12 = ddsph[a][b]
-            uint32_t sig[ROWS];
-            {
-                const uint32_t Lu = (uint32_t)L, k0u = (uint32_t)k0;
-                const uint32_t ptl = (uint32_t)pt;  // low 32 bits are enough modulo AL
-                sig[0] = (ptl * Lu + k0u) & (AL - 1);
-                if (DERIV >= 1) {
-#pragma unroll
-                    for (int a = 0; a < 3; ++a) sig[1 + a] = ((ptl * 3u + a) * Lu + k0u) & (AL - 1);
-                }
-                if (DERIV >= 2) {
-#pragma unroll
-                    for (int a = 0; a < 9; ++a) sig[4 + a] = ((ptl * 9u + a) * Lu + k0u) & (AL - 1);
-                }
-            }
-
-            for (int i = lane; i < cnt; i += 32) {
-                const int k = k0 + i;
-                int l = (int)sqrtf((float)k);
-                l += ((l + 1) * (l + 1) <= k);
-                l -= (l * l > k);
-                const int mm = k - l * (l + 1);
-                double o[10];
-                assemble_element<DERIV, NORM>(l, mm, Qt, cs, xd, yd, zd, rinv, tv, o);
-                img[0 * row_elems + sig[0] + i] = static_cast<T>(o[0]);
-                if (DERIV >= 1) {
-                    img[1 * row_elems + sig[1] + i] = static_cast<T>(o[1]);
-                    img[2 * row_elems + sig[2] + i] = static_cast<T>(o[2]);
-                    img[3 * row_elems + sig[3] + i] = static_cast<T>(o[3]);
-                }
-                if (DERIV >= 2) {
-                    // o[4..9] = xx xy xz yy yz zz ; rows 4.. = xx xy xz yx yy yz zx zy zz
-                    img[4 * row_elems + sig[4] + i] = static_cast<T>(o[4]);
-                    img[5 * row_elems + sig[5] + i] = static_cast<T>(o[5]);
-                    img[6 * row_elems + sig[6] + i] = static_cast<T>(o[6]);
-                    img[7 * row_elems + sig[7] + i] = static_cast<T>(o[5]);
-                    img[8 * row_elems + sig[8] + i] = static_cast<T>(o[7]);
-                    img[9 * row_elems + sig[9] + i] = static_cast<T>(o[8]);
-                    img[10 * row_elems + sig[10] + i] = static_cast<T>(o[6]);
-                    img[11 * row_elems + sig[11] + i] = static_cast<T>(o[8]);
-                    img[12 * row_elems + sig[12] + i] = static_cast<T>(o[9]);
-                }
+            auto lm_of = [](int t, int& l, int& m) {   // (l, m) of triangle index t
+                l = (int)((sqrtf((float)(8 * t + 1)) - 1.0f) * 0.5f);
+                l += (SPH_TRI(l + 1, 0) <= t);
+                l -= (SPH_TRI(l, 0) > t);
+                m = t - SPH_TRI(l, 0);
+            };
+            for (int t = tA + lane; t < tB; t += 32) {
+                int l, m;
+                lm_of(t, l, m);
+                double oc[10], os[10];
+                assemble_pair<DERIV, NORM>(l, m, t, Qt, cs, xd, yd, zd, rinv, tv, oc, os);
+                const int ic = l * (l + 1) + m - k0;   // (l, +m) inside the chunk; (l, -m) sits 2m before it
+                put(ic, oc);
+                if (m > 0) put(ic - 2 * m, os);
             }
             fence_proxy_async_smem();
             __syncwarp();
@@ -224,9 +269,12 @@ __global__ void __launch_bounds__(WK_MAX_THREADS, 1) sph_w_kernel(const WkParams
                 const int rows_in_arr = (arr == 0) ? 1 : (arr == 1 ? 3 : 9);
                 const int jj = (arr == 0) ? 0 : (arr == 1 ? j - 1 : j - 4);
                 const int64_t e = (pt * rows_in_arr + jj) * (int64_t)L + k0;  // first element of the run
-                T* g = out_base[arr] + e;
+                T* g = (arr == 0 ? out_base[0] : (arr == 1 ? out_base[1] : out_base[2])) + e;
                 const uint32_t sg = (uint32_t)e & (AL - 1);
-                const T* srow = img + j * row_elems + sg;  // srow[i] <-> g[i]
+                // where the run was staged: A_a + d_a + jj RS; by construction this is sg modulo AL
+                const uint32_t da = (arr == 0) ? d0 : (arr == 1 ? d1 : d2);
+                const int aoff = (arr == 0) ? 0 : (arr == 1 ? Stage::A1 : Stage::A2);
+                const T* srow = reinterpret_cast<const T*>(stage + (size_t)buf * Stage::bytes) + aoff + da + jj * RS;
                 int head = (int)((AL - sg) & (AL - 1));   // elements before the first 16-byte boundary
                 if (head > cnt) head = cnt;
                 const int body = (cnt - head) & ~(AL - 1);
@@ -286,10 +334,13 @@ struct WkLaunch {
     size_t smem;
 };
 
-template <typename T, typename R> static WkKernel wk_pick(int deriv, int norm) {
-    if (deriv == 0) return norm ? sph_w_kernel<T, R, 0, true> : sph_w_kernel<T, R, 0, false>;
-    if (deriv == 1) return norm ? sph_w_kernel<T, R, 1, true> : sph_w_kernel<T, R, 1, false>;
-    return norm ? sph_w_kernel<T, R, 2, true> : sph_w_kernel<T, R, 2, false>;
+template <typename T, typename R, bool LODD> static WkKernel wk_pick2(int deriv, int norm) {
+    if (deriv == 0) return norm ? sph_w_kernel<T, R, 0, true, LODD> : sph_w_kernel<T, R, 0, false, LODD>;
+    if (deriv == 1) return norm ? sph_w_kernel<T, R, 1, true, LODD> : sph_w_kernel<T, R, 1, false, LODD>;
+    return norm ? sph_w_kernel<T, R, 2, true, LODD> : sph_w_kernel<T, R, 2, false, LODD>;
+}
+template <typename T, typename R> static WkKernel wk_pick(int deriv, int norm, bool lodd) {
+    return lodd ? wk_pick2<T, R, true>(deriv, norm) : wk_pick2<T, R, false>(deriv, norm);
 }
 
 static inline int wk_env(const char* name, int dflt) {
@@ -302,21 +353,16 @@ static inline int wk_plan(int sm_count, int smem_optin, int64_t n, int l_max, in
                           WkLaunch* out) {
     const int deriv = ddsph ? 2 : (dsph ? 1 : 0);
     const int esize = dtype == 0 ? 4 : 8;
-    const int L = (l_max + 1) * (l_max + 1);
-    int chunk = wk_env("SPHB200_W_CHUNK", 128);
-    chunk = (chunk + 31) & ~31;
-    if (chunk > ((L + 31) & ~31)) chunk = (L + 31) & ~31;
     int nbuf = wk_env("SPHB200_W_NBUF", 1);   // measured on C4: one image per warp and more warps beats two images
     if (nbuf < 1) nbuf = 1;
     if (nbuf > 2) nbuf = 2;
     const int budget = smem_optin - 1024;
     int warps = 0;
     for (;;) {
-        WkSmem lay(l_max, deriv, esize, chunk, nbuf);
+        WkSmem lay(l_max, deriv, esize, nbuf);
         warps = (int)(((size_t)budget - lay.tab_bytes) / lay.warp_bytes);
-        if (warps >= 4 || (chunk == 32 && nbuf == 1)) break;
-        if (nbuf == 2 && chunk <= 64) nbuf = 1;
-        else if (chunk > 32) chunk -= 32;
+        if (warps >= 4 || nbuf == 1) break;
+        nbuf = 1;
     }
     if (warps < 1) return 1;
     const int want = wk_env("SPHB200_W_WARPS", WK_MAX_THREADS / 32);
@@ -332,8 +378,9 @@ static inline int wk_plan(int sm_count, int smem_optin, int64_t n, int l_max, in
     if (ppw < 1) ppw = 1;
     const int64_t ctas = (n + warps * ppw - 1) / (warps * ppw);
     if (ctas > 0x7fffffff) return 1;
-    WkSmem lay(l_max, deriv, esize, chunk, nbuf);
-    out->kern = dtype == 0 ? wk_pick<float, double>(deriv, normalized) : wk_pick<double, dd>(deriv, normalized);
+    WkSmem lay(l_max, deriv, esize, nbuf);
+    const bool lodd = (l_max & 1) == 0;
+    out->kern = dtype == 0 ? wk_pick<float, double>(deriv, normalized, lodd) : wk_pick<double, dd>(deriv, normalized, lodd);
     out->func = (const void*)out->kern;
     out->prm.xyz = xyz;
     out->prm.sph = sph;
@@ -343,9 +390,25 @@ static inline int wk_plan(int sm_count, int smem_optin, int64_t n, int l_max, in
     out->prm.n = n;
     out->prm.l_max = l_max;
     out->prm.warps_per_cta = warps;
-    out->prm.chunk = chunk;
     out->prm.nbuf = nbuf;
     out->prm.pts_per_warp = (int)ppw;
+    // chunks of whole l-rows, at most WK_CH harmonics each: the partition that minimises
+    // (32-pair assembly passes) x ~320 instructions + (chunks) x ~290 instructions, by dynamic programming
+    int best[SPH_MAX_L + 2], from[SPH_MAX_L + 2];
+    best[0] = 0;
+    for (int e = 1; e <= l_max + 1; ++e) {   // rows [0, e) covered
+        best[e] = 1 << 30;
+        for (int b = e - 1; b >= 0 && e * e - b * b <= WK_CH; --b) {
+            const int pairs = e * (e + 1) / 2 - b * (b + 1) / 2;
+            const int c = best[b] + (pairs + 31) / 32 * 320 + 290;
+            if (c < best[e]) best[e] = c, from[e] = b;
+        }
+    }
+    int nc = 0;
+    for (int e = l_max + 1; e > 0; e = from[e]) ++nc;
+    out->prm.row0[nc] = (unsigned char)(l_max + 1);
+    for (int e = l_max + 1, i = nc; e > 0; e = from[e]) out->prm.row0[--i] = (unsigned char)from[e];
+    out->prm.n_chunks = nc;
     out->grid = (int)ctas;
     out->threads = warps * 32;
     out->smem = lay.tab_bytes + (size_t)warps * lay.warp_bytes;

@@ -275,4 +275,91 @@ SPH_HD void assemble_element(int l, int mm, const double* Qt, const double* cs, 
     out[9] = Hzz;
 }
 
+// Assembly of every requested output of the PAIR of harmonics (l, +m) and (l, -m), m >= 0, from
+// the per-point scratch.  Both share Qt_l^m and every Legendre-side factor of Eq. 10 (the five
+// neighbours in the triangle, the coefficient tables, the second-derivative tensor of Q); only the
+// azimuthal factor A = c_m | s_m and its derivatives differ, so a pair costs little more than one
+// element.  t = SPH_TRI(l, m).  oc[] = outputs of (l, +m), os[] = outputs of (l, -m) (meaningless
+// for m == 0), both in the order of assemble_element.
+// The neighbours' indices need no clamping: with t1 = t - l (= TRI(l-1, m)) and
+// t2 = t - 2l + 1 (= TRI(l-2, m)) every index below lies in [0, t + 1] and the table entry is 0
+// whenever the neighbour does not exist, so what is read there only has to be finite.
+template <int DERIV, bool NORM, typename Tab>
+SPH_HD void assemble_pair(int l, int m, int t, const double* Qt, const double* cs, double x, double y,
+                          double z, double rinv, const Tab& T, double* oc, double* os) {
+    const double Q = Qt[t];
+    const double c0 = (m == 0) ? SPH_INV_SQRT2 : cs[2 * m];
+    const double s0 = cs[2 * m + 1];
+    oc[0] = Q * c0;
+    os[0] = Q * s0;
+    if (DERIV < 1) return;
+
+    const double dm = (double)m, dl = (double)l;
+    const int m1 = m >= 1 ? m - 1 : 0;  // c_{m-1}, s_{m-1}; multiplied by m = 0 when absent
+    const double c1 = cs[2 * m1], s1 = cs[2 * m1 + 1];
+    const int t1 = t - l;
+    const double q1 = T.G1[t] * Qt[t1 + 1];   // F_l^m Q_{l-1}^{m+1}
+    const double qz = T.Gz[t] * Qt[t1];       // F_l^m (l+m) Q_{l-1}^m
+    const double a1 = x * q1, a2 = y * q1;
+    // Eq. 10: cos branch A_x = m c_{m-1}, A_y = -m s_{m-1}; sin branch A_x = m s_{m-1}, A_y = m c_{m-1}
+    const double Acx = dm * c1, Acy = -dm * s1, Asx = dm * s1, Asy = dm * c1;
+    const double gcx = SPH_FMA(a1, c0, Q * Acx), gcy = SPH_FMA(a2, c0, Q * Acy), gcz = qz * c0;
+    const double gsx = SPH_FMA(a1, s0, Q * Asx), gsy = SPH_FMA(a2, s0, Q * Asy), gsz = qz * s0;
+    const double lYc = dl * oc[0], lYs = dl * os[0];
+    if (NORM) {
+        oc[1] = SPH_FMA(-lYc, x, gcx) * rinv;
+        oc[2] = SPH_FMA(-lYc, y, gcy) * rinv;
+        oc[3] = SPH_FMA(-lYc, z, gcz) * rinv;
+        os[1] = SPH_FMA(-lYs, x, gsx) * rinv;
+        os[2] = SPH_FMA(-lYs, y, gsy) * rinv;
+        os[3] = SPH_FMA(-lYs, z, gsz) * rinv;
+    } else {
+        oc[1] = gcx, oc[2] = gcy, oc[3] = gcz;
+        os[1] = gsx, os[2] = gsy, os[3] = gsz;
+    }
+    if (DERIV < 2) return;
+
+    const double dmm = dm * (dm - 1.0);
+    const int m2 = m >= 2 ? m - 2 : 0;
+    const double c2 = cs[2 * m2], s2 = cs[2 * m2 + 1];
+    const int t2 = t1 - l + 1;
+    const double q2 = T.H2[t] * Qt[t2 + 2];
+    const double qxz = T.Hxz[t] * Qt[t2 + 1];
+    const double qzz = T.Hzz[t] * Qt[t2];
+    // second derivatives of Q (Eq. 10 twice): Q1 + x^2 Q2, xy Q2, (l+m) x Qxz, (l+m)(l+m-1) Qzz
+    const double Qxx = SPH_FMA(x * x, q2, q1), Qyy = SPH_FMA(y * y, q2, q1), Qxy = (x * y) * q2;
+    const double Qxz = x * qxz, Qyz = y * qxz;
+    const double b1 = 2.0 * a1, b2 = 2.0 * a2;
+    const double r2inv = rinv * rinv;
+    const double w2 = dl + 2.0;
+    // one branch: A, its first derivatives (Ax, Ay), second derivatives Axx (= -Ayy), Axy
+    auto branch = [&](double A, double Ax, double Ay, double Axx, double Axy, double gx, double gy, double gz,
+                      double lY, double* o) {
+        const double QAxx = Q * Axx;
+        double Hxx = SPH_FMA(Qxx, A, SPH_FMA(b1, Ax, QAxx));
+        double Hyy = SPH_FMA(Qyy, A, SPH_FMA(b2, Ay, -QAxx));
+        double Hxy = SPH_FMA(Qxy, A, SPH_FMA(a1, Ay, SPH_FMA(a2, Ax, Q * Axy)));
+        double Hxz = SPH_FMA(Qxz, A, qz * Ax);
+        double Hyz = SPH_FMA(Qyz, A, qz * Ay);
+        double Hzz = qzz * A;
+        if (NORM) {
+            // hess Y = (H - l(u g^T + g u^T) + l(l+2) Y u u^T - l Y I) / r^2   with g, H, Y at u
+            const double lgx = dl * gx, lgy = dl * gy, lgz = dl * gz;
+            const double w = w2 * lY;
+            const double wx = w * x, wy = w * y, wz = w * z;
+            Hxx = (SPH_FMA(x, SPH_FMA(-2.0, lgx, wx), Hxx) - lY) * r2inv;
+            Hyy = (SPH_FMA(y, SPH_FMA(-2.0, lgy, wy), Hyy) - lY) * r2inv;
+            Hzz = (SPH_FMA(z, SPH_FMA(-2.0, lgz, wz), Hzz) - lY) * r2inv;
+            Hxy = SPH_FMA(x, wy - lgy, SPH_FMA(-y, lgx, Hxy)) * r2inv;
+            Hxz = SPH_FMA(x, wz - lgz, SPH_FMA(-z, lgx, Hxz)) * r2inv;
+            Hyz = SPH_FMA(y, wz - lgz, SPH_FMA(-z, lgy, Hyz)) * r2inv;
+        }
+        o[4] = Hxx, o[5] = Hxy, o[6] = Hxz, o[7] = Hyy, o[8] = Hyz, o[9] = Hzz;
+    };
+    // Eq. 10 twice: cos: A_xx = m(m-1) c_{m-2}, A_xy = -m(m-1) s_{m-2}; sin: m(m-1) s_{m-2}, m(m-1) c_{m-2}
+    branch(c0, Acx, Acy, dmm * c2, -dmm * s2, gcx, gcy, gcz, lYc, oc);
+    branch(s0, Asx, Asy, dmm * s2, dmm * c2, gsx, gsy, gsz, lYs, os);
+}
+
+
 }  // namespace sphb200
