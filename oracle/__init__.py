@@ -114,6 +114,15 @@ def vjp(dsph, grad_sph, l_max: int, kind: str = "ld"):
     return out
 
 
+def vjp_recompute(xyz, grad_sph, l_max: int, normalized: bool, kind: str = "ld"):
+    """Oracle for ``sphericart_cuda_vjp_recompute``: the backward pass of P:112
+    with the derivatives evaluated again from ``xyz`` instead of stored in the forward pass.  It is
+    the composition of the two oracle routines above and nothing else:
+    grad_xyz[n,a] = sum_k (d sph[n,k] / d xyz[n,a]) grad_sph[n,k]."""
+    _, dsph, _ = compute(xyz, l_max, normalized, gradients=True, kind=kind)
+    return vjp(dsph, grad_sph, l_max, kind=kind)
+
+
 def F_table(l_max: int, kind: str = "ld"):
     """F_l^m (Eq. C1) as a flat triangle, index l(l+1)/2+m."""
     out = np.empty((l_max + 1) * (l_max + 2) // 2, _DTYPE[kind])

@@ -595,6 +595,37 @@ def test_vjp_against_einsum_and_closed_forms(oracle):
     assert float(np.max(np.abs(lhs - rhs) / (np.abs(rhs) + 1))) < 1e-15
 
 
+@pytest.mark.parametrize("normalized", [False, True])
+def test_vjp_recompute_is_gradient_of_weighted_sum(oracle, normalized):
+    """N1 pin: vjp_recompute(x, w) is the Cartesian gradient of the scalar f(x) = sum_k w_k Y_k(x);
+    checked against 4th-order central differences of f built from the oracle's VALUES only
+    (the gradients under test never enter the reference), poles included."""
+    l_max = 12
+    L = (l_max + 1) ** 2
+    pts = random_points(40, 11)
+    pts = np.concatenate([pts, [[0, 0, 1.5], [0, 0, -0.75]]])
+    rng = np.random.default_rng(12)
+    w = rng.standard_normal((len(pts), L)).astype(LD)
+    got = oracle.vjp_recompute(pts, w, l_max, normalized)
+    assert got.shape == (len(pts), 3) and got.dtype == LD
+    h = 2.0 ** -22
+    f = lambda x: (oracle.compute(x, l_max, normalized)[0] * w).sum(axis=1)
+    r = np.linalg.norm(pts, axis=1)
+    # scale of one term of the sum: |w| * row scale * l / r (times r^l for solid harmonics)
+    scale = np.zeros(len(pts), LD)
+    for l in range(l_max + 1):
+        rho = r ** l if not normalized else np.ones_like(r)
+        scale += row_scale(l) * rho * max(l, 1) / r * np.abs(w[:, l * l:(l + 1) ** 2]).max(axis=1)
+    for a in range(3):
+        e = np.zeros(3)
+        e[a] = h
+        fd = (8 * (f(pts + e) - f(pts - e)) - (f(pts + 2 * e) - f(pts - 2 * e))) / (12 * LD(h))
+        assert float(np.max(np.abs(fd - got[:, a]) / scale)) < 1e-11, a
+    # and it is exactly the two-step route
+    _, d, _ = oracle.compute(pts, l_max, normalized, gradients=True)
+    assert np.array_equal(got, oracle.vjp(d, w, l_max))
+
+
 # --------------------------------------------------------------------------------------------
 # edge cases of the oracle's interface
 # --------------------------------------------------------------------------------------------
