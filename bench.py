@@ -157,6 +157,17 @@ class DeviceWorkload:
         self.pkg.sphericart_cuda_vjp(None, dsph, self.grad_sph, self.grad_xyz, c.n, c.l_max, self.dcode,
                                      self.stream)
 
+    def forward_values_only(self, i):
+        c = self.cfg
+        sph, _, _ = self.sets[i % len(self.sets)]
+        self.pkg.sphericart_cuda_compute(self.xyz, c.n, c.l_max, c.normalized, self.dcode, sph, None, None,
+                                         self.stream)
+
+    def backward_recompute(self, i):
+        c = self.cfg
+        self.pkg.sphericart_cuda_vjp_recompute(self.xyz, self.grad_sph, self.grad_xyz, c.n, c.l_max, c.normalized,
+                                               self.dcode, self.stream)
+
     def step(self, i):
         self.forward(i)
         if self.cfg.vjp:
@@ -229,6 +240,17 @@ def sweep_one(cfg, torch, pkg, device, peak):
         ms_b = e0.elapsed_time(e1) / reps
         res.update({"vjp_us": round(ms_b * 1e3, 2), "vjp_gbs": cfg.n * vjp_b / (ms_b * 1e-3) / 1e9})
         res["vjp_frac_of_measured_peak"] = res["vjp_gbs"] / peak
+        # the same backward without stored derivatives (reads xyz + grad_sph only), and
+        # the values-only forward it pairs with
+        esize = 4 if cfg.dtype == "f32" else 8
+        for key, fn, bytes_pt in (("vjp_recompute", wl.backward_recompute, (cfg.n_sph + 6) * esize),
+                                  ("fwd_values_only", wl.forward_values_only, (cfg.n_sph + 3) * esize)):
+            for i in range(3):
+                fn(i)
+            e0, e1 = time_loop(torch, fn, reps)
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / reps
+            res.update({key + "_us": round(ms * 1e3, 2), key + "_gbs": cfg.n * bytes_pt / (ms * 1e-3) / 1e9})
     del wl
     torch.cuda.empty_cache()
     return res

@@ -81,6 +81,24 @@ int sphericart_cuda_vjp(const void* xyz, const void* dsph, const void* grad_sph,
                         int64_t n, int l_max, int dtype, void* stream);
 
 /*
+ * Backward pass WITHOUT stored derivatives (the paper's own backward, P:112,
+ * contracts derivatives "evaluated in the forward pass"): the derivatives of Eq. 10 --
+ * through x/r for normalized = 1 -- are evaluated again from xyz inside the kernel and
+ * contracted on the fly:
+ *     grad_xyz[i,a] = sum_k (d sph[i,k] / d xyz[i,a]) * grad_sph[i,k].
+ * Same result as sphericart_cuda_compute(..., dsph, ...) followed by sphericart_cuda_vjp up to
+ * rounding, reading 3 + L values per point instead of 4 L + 3, and the forward pass need not write
+ * dsph.  Device pointers, caller-owned, 16-byte aligned; asynchronous on `stream`.
+ *   xyz       [n,3]    in
+ *   grad_sph  [n,L]    in
+ *   grad_xyz  [n,3]    out
+ * Any 0 <= l_max <= SPHERICART_CUDA_MAX_L (compile-time-specialised kernels for l_max <= 8, f32 <= 12).
+ * Errors as for sphericart_cuda_compute; normalized = 1 at r = 0 gives NaN for that point only.
+ */
+int sphericart_cuda_vjp_recompute(const void* xyz, const void* grad_sph, void* grad_xyz, int64_t n,
+                                  int l_max, int normalized, int dtype, void* stream);
+
+/*
  * The same two operations on HOST buffers: the library copies xyz (and dsph/grad_sph) to the
  * device, runs the kernels above and copies the results back, in chunks on two streams so that
  * transfers overlap compute; returns after everything has landed (synchronises internally).

@@ -48,6 +48,8 @@ def load():
     lib.sphericart_cuda_vjp.argtypes = [vp, vp, vp, vp, i64, ci, ci, vp]
     lib.sphericart_cuda_compute_host.restype = ci
     lib.sphericart_cuda_compute_host.argtypes = [vp, i64, ci, ci, ci, vp, vp, vp]
+    lib.sphericart_cuda_vjp_recompute.restype = ci
+    lib.sphericart_cuda_vjp_recompute.argtypes = [vp, vp, vp, i64, ci, ci, ci, vp]
     lib.sphericart_cuda_vjp_host.restype = ci
     lib.sphericart_cuda_vjp_host.argtypes = [vp, vp, vp, vp, i64, ci, ci]
     lib.sphericart_cuda_last_error.restype = ctypes.c_char_p
@@ -92,6 +94,12 @@ def sphericart_cuda_compute_host(xyz, n, l_max, normalized, dtype, sph, dsph, dd
     rc = load().sphericart_cuda_compute_host(_ptr(xyz), n, l_max, int(normalized), dtype, _ptr(sph),
                                              _ptr(dsph), _ptr(ddsph))
     _check(rc, "sphericart_cuda_compute_host")
+
+
+def sphericart_cuda_vjp_recompute(xyz, grad_sph, grad_xyz, n, l_max, normalized, dtype, stream):
+    rc = load().sphericart_cuda_vjp_recompute(_ptr(xyz), _ptr(grad_sph), _ptr(grad_xyz), n, l_max,
+                                              int(bool(normalized)), dtype, _ptr(stream))
+    _check(rc, "sphericart_cuda_vjp_recompute")
 
 
 def sphericart_cuda_vjp_host(xyz, dsph, grad_sph, grad_xyz, n, l_max, dtype):
@@ -160,4 +168,23 @@ def vjp(dsph, grad_sph, out=None):
     with torch.cuda.device(dsph.device):
         stream = torch.cuda.current_stream().cuda_stream
         sphericart_cuda_vjp(None, dsph, grad_sph, gx, n, l_max, _dtype_code(dsph), stream)
+    return gx
+
+
+def vjp_recompute(xyz, grad_sph, normalized: bool, out=None):
+    """``grad_xyz[n,a] = sum_k (d sph[n,k] / d xyz[n,a]) grad_sph[n,k]`` evaluated from ``xyz``
+    (no stored derivatives), on torch's current stream."""
+    import torch
+
+    if not xyz.is_cuda:
+        raise SphericartCudaError("xyz must be a CUDA tensor (no CPU fallback)")
+    xyz, grad_sph = xyz.contiguous(), grad_sph.contiguous()
+    n, L = grad_sph.shape
+    l_max = int(round(L ** 0.5)) - 1
+    if (l_max + 1) ** 2 != L or xyz.shape != (n, 3) or xyz.dtype != grad_sph.dtype:
+        raise ValueError("shapes: xyz [n,3], grad_sph [n,L], L a perfect square, same dtype")
+    gx = torch.empty((n, 3), dtype=xyz.dtype, device=xyz.device) if out is None else out
+    with torch.cuda.device(xyz.device):
+        stream = torch.cuda.current_stream().cuda_stream
+        sphericart_cuda_vjp_recompute(xyz, grad_sph, gx, n, l_max, normalized, _dtype_code(xyz), stream)
     return gx

@@ -68,7 +68,8 @@ static int device_state(DeviceState** out) {
         st.smem_optin = (int)prop.sharedMemPerBlockOptin;
         CUDA_TRY(cudaMemcpyToSymbol(c_tables, &g_host_tables, sizeof(SphTables)));
         if (sph_tpb_upload_f32_v(&g_host_tables) || sph_tpb_upload_f32_g(&g_host_tables) ||
-            sph_tpb_upload_f64_v(&g_host_tables) || sph_tpb_upload_f64_g(&g_host_tables))
+            sph_tpb_upload_f64_v(&g_host_tables) || sph_tpb_upload_f64_g(&g_host_tables) ||
+            sph_vjpr_upload_f32(&g_host_tables) || sph_vjpr_upload_f64(&g_host_tables))
             return fail(SPHERICART_CUDA_ECUDA, "table upload failed: %s", cudaGetErrorString(cudaGetLastError()));
         CUDA_TRY(cudaMalloc(&st.d_tables, sizeof(SphTables)));
         CUDA_TRY(cudaMemcpy(st.d_tables, &g_host_tables, sizeof(SphTables), cudaMemcpyHostToDevice));
@@ -244,6 +245,71 @@ static int compute_device(const void* xyz, int64_t n, int l_max, int normalized,
     return launch_w(*st, xyz, n, l_max, normalized, dtype, sph, dsph, ddsph, stream);
 }
 
+// ---------------------------------------------------------------------------------------------
+// recompute-in-backward VJP, any l_max: one thread per point, runtime l_max, grad_sph read straight
+// from global memory.  The compile-time-l_max kernels of kernel_vjpr.cuh cover the l_max that
+// matter for speed; this one keeps the entry point total.
+// ---------------------------------------------------------------------------------------------
+template <typename T> struct VjprEmit {
+    const T* w;
+    double a[3];
+    __device__ __forceinline__ void val(int, double) {}
+    __device__ __forceinline__ void grad(int c, int k, double v) { a[c] = fma(v, static_cast<double>(w[k]), a[c]); }
+};
+
+template <typename T, typename R, bool NORM>
+__global__ void __launch_bounds__(128) sph_vjpr_generic_kernel(const T* __restrict__ xyz, const T* __restrict__ gsph,
+                                                               T* __restrict__ gxyz, int64_t n, int l_max) {
+    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    const int L = (l_max + 1) * (l_max + 1);
+    VjprEmit<T> e{gsph + p * L, {0.0, 0.0, 0.0}};
+    eval_point_columns<R, 1, NORM>(static_cast<double>(xyz[3 * p]), static_cast<double>(xyz[3 * p + 1]),
+                                   static_cast<double>(xyz[3 * p + 2]), l_max, c_tables, e);
+    gxyz[3 * p + 0] = static_cast<T>(e.a[0]);
+    gxyz[3 * p + 1] = static_cast<T>(e.a[1]);
+    gxyz[3 * p + 2] = static_cast<T>(e.a[2]);
+}
+
+static int vjp_recompute_device(const void* xyz, const void* grad_sph, void* grad_xyz, int64_t n, int l_max,
+                                int normalized, int dtype, cudaStream_t stream) {
+    int rc = check_common(n, l_max, dtype);
+    if (rc) return rc;
+    if (normalized != 0 && normalized != 1)
+        return fail(SPHERICART_CUDA_EINVAL, "normalized = %d is neither 0 nor 1", normalized);
+    if (n == 0) return 0;
+    if (!xyz || !grad_sph || !grad_xyz)
+        return fail(SPHERICART_CUDA_EINVAL, "xyz, grad_sph and grad_xyz must not be NULL when n > 0");
+    if (misaligned(xyz) || misaligned(grad_sph) || misaligned(grad_xyz))
+        return fail(SPHERICART_CUDA_EALIGN, "device pointers must be 16-byte aligned");
+    DeviceState* st = nullptr;
+    rc = device_state(&st);
+    if (rc) return rc;
+    const bool f32 = dtype == SPHERICART_CUDA_F32;
+    const char* force = getenv("SPHB200_FORCE_KERNEL");  // "generic": experiments and tests only
+    const bool force_generic = force && force[0] == 'g';
+    if (!force_generic) {
+        int r = (f32 ? sph_vjpr_launch_f32 : sph_vjpr_launch_f64)(xyz, grad_sph, grad_xyz, n, l_max, normalized, stream);
+        if (r < 0) return fail(SPHERICART_CUDA_ECUDA, "vjpr launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+        if (r == 0) {
+            g_launches.fetch_add(1, std::memory_order_relaxed);
+            return 0;
+        }
+    }
+    const int64_t blocks = (n + 127) / 128;
+    if (blocks > 0x7fffffff) return fail(SPHERICART_CUDA_EINVAL, "n = %lld is too large", (long long)n);
+    if (f32) {
+        auto k = normalized ? sph_vjpr_generic_kernel<float, double, true> : sph_vjpr_generic_kernel<float, double, false>;
+        k<<<(unsigned)blocks, 128, 0, stream>>>((const float*)xyz, (const float*)grad_sph, (float*)grad_xyz, n, l_max);
+    } else {
+        auto k = normalized ? sph_vjpr_generic_kernel<double, dd, true> : sph_vjpr_generic_kernel<double, dd, false>;
+        k<<<(unsigned)blocks, 128, 0, stream>>>((const double*)xyz, (const double*)grad_sph, (double*)grad_xyz, n, l_max);
+    }
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    CUDA_TRY(cudaGetLastError());
+    return 0;
+}
+
 static int vjp_device(const void* dsph, const void* grad_sph, void* grad_xyz, int64_t n, int l_max, int dtype,
                       cudaStream_t stream) {
     int rc = check_common(n, l_max, dtype);
@@ -360,6 +426,12 @@ int sphericart_cuda_vjp(const void* xyz, const void* dsph, const void* grad_sph,
                         int l_max, int dtype, void* stream) {
     (void)xyz;  // reserved (reading B1)
     return vjp_device(dsph, grad_sph, grad_xyz, n, l_max, dtype, static_cast<cudaStream_t>(stream));
+}
+
+int sphericart_cuda_vjp_recompute(const void* xyz, const void* grad_sph, void* grad_xyz, int64_t n, int l_max,
+                                  int normalized, int dtype, void* stream) {
+    return vjp_recompute_device(xyz, grad_sph, grad_xyz, n, l_max, normalized, dtype,
+                                static_cast<cudaStream_t>(stream));
 }
 
 int sphericart_cuda_compute_host(const void* xyz, int64_t n, int l_max, int normalized, int dtype, void* sph,

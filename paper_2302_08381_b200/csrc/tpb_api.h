@@ -16,4 +16,12 @@ SPH_TPB_DECL(f32_g)
 SPH_TPB_DECL(f64_v)
 SPH_TPB_DECL(f64_g)
 #undef SPH_TPB_DECL
+// recompute-in-backward VJP (vjpr_inst.cu, compiled once per element type); same return codes
+#define SPH_VJPR_DECL(sfx)                                                                              \
+    int sph_vjpr_launch_##sfx(const void* xyz, const void* grad_sph, void* grad_xyz, int64_t n, int l_max, \
+                              int normalized, cudaStream_t stream);                                      \
+    int sph_vjpr_upload_##sfx(const SphTables* host_tables);
+SPH_VJPR_DECL(f32)
+SPH_VJPR_DECL(f64)
+#undef SPH_VJPR_DECL
 }  // namespace sphb200

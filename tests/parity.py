@@ -78,15 +78,28 @@ def check(got, want, xyz, l_max, normalized, order, dtype, what=""):
     return emax, n_strict, msg
 
 
-def check_vjp(got, want, dsph, grad_sph, l_max, dtype, what="vjp"):
-    """|err| / max(|ref|, 1e-3 * ||dsph[n,a,:]||_2 ||grad_sph[n,:]||_2) <= tol (SURVEY 8(c) VJP)."""
+def check_vjp(got, want, dsph, grad_sph, l_max, dtype, what="vjp", point_scale=False):
+    """|err| / max(|ref|, 1e-3 * ||dsph[n,a,:]||_2 ||grad_sph[n,:]||_2) <= tol (SURVEY 8(c) VJP).
+
+    ``point_scale``: the floor uses max_a ||dsph[n,a,:]||_2 instead (reading R3, used for
+    the recompute route: like R1's row scale S_1 it does not depend on the component a, so a
+    component whose derivatives all vanish identically -- d/dz of normalised Y for a point ON the z
+    axis -- is held to the size of that point's gradient, not to an exact zero)."""
     tol = tol_for(dtype, l_max)
     got = np.asarray(got).astype(LD)
     want = np.asarray(want).astype(LD)
     d = np.asarray(dsph).astype(LD)
     g = np.asarray(grad_sph).astype(LD)
-    scale = np.sqrt((d * d).sum(axis=2)) * np.sqrt((g * g).sum(axis=1))[:, None]
-    e = np.abs(got - want) / np.maximum(np.abs(want), LD(1e-3) * scale)
+    dn = np.sqrt((d * d).sum(axis=2))
+    if point_scale:
+        dn = np.broadcast_to(dn.max(axis=1, keepdims=True), dn.shape)
+    scale = dn * np.sqrt((g * g).sum(axis=1))[:, None]
+    diff = np.abs(got - want)
+    with np.errstate(invalid="ignore", divide="ignore"):
+        e = diff / np.maximum(np.abs(want), LD(1e-3) * scale)
+    # scale = 0 (every d/dx_a vanishes, e.g. d/dz of normalised Y for a point ON the z axis): the
+    # reference is an exact zero and only an exact zero passes
+    e = np.where(np.isfinite(e), e, np.where(diff == 0, 0, np.inf))
     emax = float(e.max(initial=0))
     assert emax <= tol, f"{what}: max scaled error {emax:.3e} (tol {tol:.1e})"
     return emax

@@ -30,7 +30,7 @@ def lib():
 def test_header_declares_the_boundary():
     names = _declared_symbols()
     for must in ("sphericart_cuda_compute", "sphericart_cuda_vjp", "sphericart_cuda_last_error",
-                 "sphericart_cuda_compute_host", "sphericart_cuda_vjp_host"):
+                 "sphericart_cuda_compute_host", "sphericart_cuda_vjp_host", "sphericart_cuda_vjp_recompute"):
         assert must in names
 
 
@@ -60,6 +60,11 @@ def test_argument_errors_do_not_need_a_gpu(lib):
     assert c.sphericart_cuda_vjp(None, None, None, None, 5, 4, 0, None) == 1
     assert c.sphericart_cuda_vjp(None, None, None, None, 0, 4, 0, None) == 0
     assert c.sphericart_cuda_vjp(None, 16, 16, 4, 5, 4, 0, None) == 2
+    assert c.sphericart_cuda_vjp_recompute(None, None, None, 5, 4, 1, 0, None) == 1              # NULL pointers
+    assert c.sphericart_cuda_vjp_recompute(None, None, None, 0, 4, 1, 0, None) == 0              # n == 0
+    assert c.sphericart_cuda_vjp_recompute(16, 16, 16, 5, 4, 3, 0, None) == 1                    # normalized
+    assert c.sphericart_cuda_vjp_recompute(16, 16, 16, 5, 40, 1, 0, None) == 1                   # l_max
+    assert c.sphericart_cuda_vjp_recompute(16, 8, 16, 5, 4, 1, 0, None) == 2                     # misaligned
     with pytest.raises(lib.SphericartCudaError):
         lib.sphericart_cuda_compute(None, -1, 4, 1, 0, None, None, None, None)
 

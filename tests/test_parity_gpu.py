@@ -182,6 +182,63 @@ def test_vjp_long_rows(sph, oracle):
         parity.check_vjp(gx.cpu().numpy(), oracle.vjp(d_np, g, l_max), d_np, g, l_max, dtype)
 
 
+def _check_vjp_recompute(sph, oracle, xyz, l_max, normalized, dtype, what):
+    n = xyz.shape[0]
+    g = np.random.default_rng(l_max + 100 * n).standard_normal((n, (l_max + 1) ** 2)).astype(xyz.dtype)
+    gx = sph.vjp_recompute(torch.from_numpy(xyz).cuda(), torch.from_numpy(g).cuda(), normalized)
+    torch.cuda.synchronize()
+    _, wd, _ = oracle.compute(xyz, l_max, normalized, True)
+    want = oracle.vjp_recompute(xyz, g, l_max, normalized)
+    return parity.check_vjp(gx.cpu().numpy(), want, wd, g, l_max, dtype, what, point_scale=True)
+
+
+@pytest.mark.parametrize("name,n", [("C1", 1000), ("C2", 4099), ("C5", 6000), ("C2", 7), ("C3", 2049)])
+def test_vjp_recompute_configs(sph, oracle, name, n):
+    """N1: backward without stored derivatives against the oracle's compute + vjp, on the configs'
+    own point clouds (C2: points on +-z and |r| down to 1e-6), both variants."""
+    cfg = W.CONFIGS[name]
+    l_max = min(cfg.l_max, 12)
+    xyz = W.make_xyz(cfg, n)
+    for normalized in (True, False):
+        _check_vjp_recompute(sph, oracle, xyz, l_max, normalized, cfg.dtype, f"{name} vjp_recompute norm={normalized}")
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_vjp_recompute_every_l_max(sph, oracle, dtype):
+    """Specialised kernels (l_max <= 8, f32 <= 12), the generic one above that, l_max = 0, ragged n."""
+    for l_max in (0, 1, 2, 3, 5, 7, 8, 9, 12, 13, 20, 32):
+        n = 3 * 16 + 5
+        xyz = W.make_xyz("C4" if l_max > 12 else "C2", n).astype(np.float32 if dtype == "f32" else np.float64)
+        for normalized in (True, False):
+            _check_vjp_recompute(sph, oracle, xyz, l_max, normalized, dtype, f"{dtype} l_max={l_max} norm={normalized}")
+
+
+def test_vjp_recompute_matches_stored_route_and_generic(sph, oracle, monkeypatch):
+    """Same numbers as forward-with-gradients followed by the stored-derivative VJP (to rounding),
+    and the generic kernel agrees with the specialised one."""
+    cfg = W.CONFIGS["C5"]
+    n = 20_000
+    xyz = W.make_xyz(cfg, n)
+    g = W.make_grad_sph(cfg, n)
+    x_d, g_d = torch.from_numpy(xyz).cuda(), torch.from_numpy(g).cuda()
+    _, d, _ = sph.compute(x_d, cfg.l_max, True, True)
+    stored = sph.vjp(d, g_d).cpu().numpy()
+    before = sph.sphericart_cuda_launch_count()
+    rec = sph.vjp_recompute(x_d, g_d, True).cpu().numpy()
+    assert sph.sphericart_cuda_launch_count() == before + 1
+    scale = np.abs(stored).max()
+    assert np.max(np.abs(rec - stored)) <= 2e-6 * scale
+    monkeypatch.setenv("SPHB200_FORCE_KERNEL", "generic")
+    gen = sph.vjp_recompute(x_d, g_d, True).cpu().numpy()
+    assert np.max(np.abs(gen - rec)) <= 2e-6 * scale
+    # guard bands: grad_xyz is written exactly where it belongs
+    buf = torch.full((n * 3 + 64,), 777.0, device="cuda")
+    monkeypatch.delenv("SPHB200_FORCE_KERNEL")
+    sph.sphericart_cuda_vjp_recompute(x_d, g_d, buf[32:-32], n, cfg.l_max, 1, 0, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert torch.all(buf[:32] == 777.0) and torch.all(buf[-32:] == 777.0) and torch.all(buf[32:-32] != 777.0)
+
+
 def test_origin_and_untouched_memory(sph, oracle):
     # normalised at r = 0: NaN for that point only; solid at r = 0 is defined
     xyz = np.array([[0, 0, 0], [1, 2, 3], [0, 0, 0], [-1, 0.5, 0.25]], np.float64)
