@@ -14,6 +14,7 @@
 #include "kernel_tp.cuh"
 #include "kernel_vjp.cuh"
 #include "kernel_w.cuh"
+#include "kernel_wc.cuh"
 #include "tpb_api.h"
 
 namespace sphb200 {
@@ -173,6 +174,19 @@ static int launch_tp(const DeviceState& st, const void* xyz, int64_t n, int l_ma
 // ---------------------------------------------------------------------------------------------
 static int launch_w(const DeviceState& st, const void* xyz, int64_t n, int l_max, int normalized, int dtype,
                     void* sph, void* dsph, void* ddsph, cudaStream_t stream) {
+    const char* force = getenv("SPHB200_FORCE_KERNEL");  // "w1": the one-warp-per-point kernel even for long rows
+    if (!(force && force[0] == 'w' && force[1] == '1')) {
+        // long rows: the warps of a CTA share one point, chunks of half a row, ~4 KB bulk stores
+        WcLaunch lc{};
+        if (wc_plan(st.smem_optin, n, l_max, normalized, dtype, sph, dsph, ddsph, xyz, st.d_tables, &lc) == 0) {
+            int rc = allow_smem(lc.func, (int)lc.smem);
+            if (rc) return rc;
+            wc_launch(lc, stream);
+            g_launches.fetch_add(1, std::memory_order_relaxed);
+            CUDA_TRY(cudaGetLastError());
+            return 0;
+        }
+    }
     WkLaunch lw{};
     int rc = wk_plan(st.sm_count, st.smem_optin, n, l_max, normalized, dtype, sph, dsph, ddsph, xyz,
                      st.d_tables, &lw);

@@ -239,6 +239,39 @@ def test_vjp_recompute_matches_stored_route_and_generic(sph, oracle, monkeypatch
     assert torch.all(buf[:32] == 777.0) and torch.all(buf[-32:] == 777.0) and torch.all(buf[32:-32] != 777.0)
 
 
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_cooperative_kernel_long_rows(sph, oracle, dtype, monkeypatch):
+    """Rows with l_max >= 19 take the CTA-cooperative kernel (kernel_wc.cuh): every derivative order,
+    both variants, odd and even row lengths, n below / across / not a multiple of the 128 points a
+    CTA owns; and it writes the same numbers as the one-warp-per-point kernel."""
+    np_dt = np.float32 if dtype == "f32" else np.float64
+    cases = [(32, 1, True, True, True), (32, 127, True, True, False), (31, 129, True, True, True),
+             (19, 300, True, False, True), (20, 77, False, False, False), (26, 257, True, True, True),
+             (25, 130, True, False, False)]
+    for l_max, n, grads, hess, normalized in cases:
+        xyz = W.make_xyz("C4", n).astype(np_dt)
+        s, d, h = _run_gpu(sph, xyz, l_max, normalized, grads, hess)
+        _compare(oracle, xyz, l_max, normalized, dtype, s, d, h, f"wc {dtype} l_max={l_max} n={n}")
+        monkeypatch.setenv("SPHB200_FORCE_KERNEL", "w1")
+        s1, d1, h1 = _run_gpu(sph, xyz, l_max, normalized, grads, hess)
+        monkeypatch.delenv("SPHB200_FORCE_KERNEL")
+        for a, b in ((s, s1), (d, d1), (h, h1)):
+            if a is not None:
+                assert torch.equal(a, b), "cooperative and one-warp kernels disagree bit-wise"
+    # guard bands around the three outputs
+    n, l_max = 131, 32
+    L = (l_max + 1) ** 2
+    t_dt = torch.float32 if dtype == "f32" else torch.float64
+    pts = torch.from_numpy(W.make_xyz("C4", n).astype(np_dt)).cuda()
+    bufs = [torch.full((m + 64,), 777.0, device="cuda", dtype=t_dt) for m in (n * L, n * 3 * L, n * 9 * L)]
+    views = [b[32:-32] for b in bufs]
+    sph.sphericart_cuda_compute(pts, n, l_max, 1, 0 if dtype == "f32" else 1, views[0], views[1], views[2],
+                                torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    for b in bufs:
+        assert torch.all(b[:32] == 777.0) and torch.all(b[-32:] == 777.0) and torch.all(b[32:-32] != 777.0)
+
+
 def test_origin_and_untouched_memory(sph, oracle):
     # normalised at r = 0: NaN for that point only; solid at r = 0 is defined
     xyz = np.array([[0, 0, 0], [1, 2, 3], [0, 0, 0], [-1, 0.5, 0.25]], np.float64)
