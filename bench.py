@@ -53,7 +53,7 @@ NCU_TRAFFIC_BYTES = {
     # profiles/r1b_kernels.md
     "C2": 71.43e6,     # 70.19 MB written + 1.24 MB read (a single launch's 129.6 MB output is L2-sized)
     "C3": 1108.6e6,    # 1096.6 MB written + 12.05 MB read
-    "C4": 29.918e9,    # 29.807 GB written + 0.111 GB read
+    "C4": 29.689e9,    # sph_wc_kernel: 29.676 GB written + 0.013 GB read
     "C5": 3124.6e6,    # forward kernel: 3076.6 MB written + 48.0 MB read
 }
 
@@ -380,7 +380,7 @@ def run_cuda(args):
     else:
         ms_fwd = ms_step
     achieved = cfg.n * fwd_b / (ms_fwd * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "forward (sph_tpb_kernel; sph_w_kernel for C4)", "achieved": achieved,
+    roofline = {"bound": "hbm", "kernel": "forward (sph_tpb_kernel; sph_wc_kernel for C4)", "achieved": achieved,
                 "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg.name),
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": cfg.n * fwd_b,
                 "avg_launch_us": ms_fwd * 1e3, "output_gbs": cfg.n * cfg.out_bytes_per_point / (ms_fwd * 1e-3) / 1e9,

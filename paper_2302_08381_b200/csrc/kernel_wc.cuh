@@ -33,7 +33,7 @@ constexpr int WC_AW = 4;        // recurrence warps (phase A of a point takes ~4
 constexpr int WC_SLOTS = 6;     // triangles in flight
 constexpr int WC_CH = 368;      // most harmonics in a chunk: l_max = 32 splits into l < 19, 19 <= l < 27, l >= 27
                                 // (361 / 368 / 360 harmonics, 190 / 188 / 183 pairs: one pass each)
-constexpr int WC_PTS = 128;     // points per CTA (the first point's phase A is not overlapped)
+constexpr int WC_PTS = 256;     // points per CTA (the first point's phase A is not overlapped)
 constexpr int WC_THREADS = (WC_BW + WC_AW) * 32;
 
 // Staging image: as WkStage (kernel_w.cuh), rows of one array a compile-time stride apart and
