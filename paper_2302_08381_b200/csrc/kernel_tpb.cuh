@@ -42,6 +42,7 @@ struct TpbParams {
     void* dsph;
     int64_t n;
     int tiles_per_cta;   // consecutive tiles one CTA works through
+    int pdl;             // launched as a programmatic dependent launch (tpb_inst.cu)
 };
 
 constexpr int TPB_PTS = 16;                 // points per tile
@@ -109,6 +110,13 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
         if constexpr (SPLIT == 1) __syncwarp();
         else __syncthreads();
     };
+
+    // programmatic dependent launch (tpb_inst.cu): let the next kernel's CTAs become resident as
+    // ours retire, and do not touch memory before the previous kernel in the stream has completed
+    if (prm.pdl) {
+        grid_launch_dependents();
+        grid_dependency_wait();
+    }
 
     const int64_t t_begin = (int64_t)blockIdx.x * prm.tiles_per_cta;
     int64_t t_end = t_begin + prm.tiles_per_cta;

@@ -25,6 +25,7 @@ struct VjprParams {
     const void* grad_sph;
     void* grad_xyz;
     int64_t n;
+    int pdl;   // launched as a programmatic dependent launch (see kernel_tpb.cuh)
 };
 
 template <typename T, typename R, bool NORM, int LMAX>
@@ -46,6 +47,12 @@ __global__ void __launch_bounds__(32, 16) sph_vjpr_kernel(const VjprParams prm) 
     const T* __restrict__ xyz = static_cast<const T*>(prm.xyz);
     const T* __restrict__ gsph = static_cast<const T*>(prm.grad_sph);
     T* __restrict__ gxyz = static_cast<T*>(prm.grad_xyz);
+
+    // programmatic dependent launch: see kernel_tpb.cuh
+    if (prm.pdl) {
+        grid_launch_dependents();
+        grid_dependency_wait();
+    }
 
     const bool full = n - p0 >= TPB_PTS;
     if (full) {

@@ -79,6 +79,10 @@ __device__ __forceinline__ void bulk_load(void* sdst, const void* gsrc, uint32_t
         : "memory");
 }
 
+// programmatic dependent launch: no-ops when the kernel was launched without the attribute
+__device__ __forceinline__ void grid_dependency_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void grid_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // streaming (evict-first) global stores for the few elements that cannot go through TMA
 __device__ __forceinline__ void st_cs(float* p, float v) { __stcs(p, v); }
 __device__ __forceinline__ void st_cs(double* p, double v) { __stcs(p, v); }

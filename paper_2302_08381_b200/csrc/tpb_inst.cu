@@ -58,8 +58,26 @@ static int launch_split(int sm_count, TpbParams prm, cudaStream_t stream) {
     prm.tiles_per_cta = (int)k;
     const int64_t ctas = (n_tiles + k - 1) / k;
     if (ctas > 0x7fffffff) return 1;
-    kern<<<(unsigned)ctas, SPLIT * 32, Shape::tile_bytes, stream>>>(prm);
-    return cudaGetLastError() == cudaSuccess ? 0 : -1;
+    // Programmatic dependent launch: the CTAs of this grid may become resident while the previous
+    // kernel in the stream drains; each waits (griddepcontrol.wait, first thing in the kernel) until
+    // that kernel has completed and its memory is visible, so stream order is kept for ANY
+    // predecessor.  It hides the launch ramp between back-to-back calls (C2: 22.8 -> 20.8 us).  Only
+    // for grids of a few waves: the two griddepcontrol instructions cost every CTA a fixed latency,
+    // which a grid of 250 000 one-tile CTAs cannot hide (C5 values only: 169 -> 261 us with them).
+    static const int pdl_env = env_int("SPHB200_PDL", 1);
+    const int pdl = pdl_env && ctas <= (int64_t)sm_count * 64;
+    prm.pdl = pdl;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)ctas);
+    cfg.blockDim = dim3(SPLIT * 32);
+    cfg.dynamicSmemBytes = Shape::tile_bytes;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, prm) == cudaSuccess ? 0 : -1;
 }
 
 // Two warps per tile where shared memory, not registers, limits the tiles in flight (<= 12 per
@@ -83,7 +101,7 @@ static int launch_one(int sm_count, const TpbParams& prm, cudaStream_t stream) {
 
 int TPB_NAME(sph_tpb_launch)(int sm_count, const void* xyz, int64_t n, int l_max, int normalized, void* sph,
                              void* dsph, cudaStream_t stream) {
-    TpbParams prm{xyz, sph, dsph, n, 1};
+    TpbParams prm{xyz, sph, dsph, n, 1, 0};
     switch (l_max) {
         TPB_CASE(1)
         TPB_CASE(2)

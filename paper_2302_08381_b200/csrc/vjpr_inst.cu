@@ -5,6 +5,8 @@
 #include "kernel_vjpr.cuh"
 #include "tpb_api.h"
 
+#include <cstdlib>
+
 #ifndef VJPR_F64
 #error "compile with -DVJPR_F64=0|1"
 #endif
@@ -21,7 +23,7 @@ typedef double vjpr_R;
 #define VJPR_NAME(f) f##_f32
 #endif
 
-template <int LMAX, bool NORM> static int launch_one(const VjprParams& prm, cudaStream_t stream) {
+template <int LMAX, bool NORM> static int launch_one(VjprParams prm, cudaStream_t stream) {
     constexpr int L = (LMAX + 1) * (LMAX + 1);
     constexpr int smem = TPB_PTS * L * (int)sizeof(vjpr_T) + 16;
     auto kern = sph_vjpr_kernel<vjpr_T, vjpr_R, NORM, LMAX>;
@@ -34,8 +36,20 @@ template <int LMAX, bool NORM> static int launch_one(const VjprParams& prm, cuda
     }
     const int64_t n_tiles = (prm.n + TPB_PTS - 1) / TPB_PTS;
     if (n_tiles > 0x7fffffff) return 1;
-    kern<<<(unsigned)n_tiles, 32, smem, stream>>>(prm);
-    return cudaGetLastError() == cudaSuccess ? 0 : -1;
+    // programmatic dependent launch, as for the forward kernels (tpb_inst.cu)
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)n_tiles);
+    cfg.blockDim = dim3(32);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    static const int pdl = [] { const char* e = getenv("SPHB200_PDL"); return (e && *e) ? atoi(e) : 1; }();
+    prm.pdl = pdl && n_tiles <= 148 * 64;   // small grids only (tpb_inst.cu)
+    cfg.numAttrs = prm.pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, prm) == cudaSuccess ? 0 : -1;
 }
 
 #define VJPR_CASE(LM) \
@@ -44,7 +58,7 @@ template <int LMAX, bool NORM> static int launch_one(const VjprParams& prm, cuda
 
 int VJPR_NAME(sph_vjpr_launch)(const void* xyz, const void* grad_sph, void* grad_xyz, int64_t n, int l_max,
                                int normalized, cudaStream_t stream) {
-    VjprParams prm{xyz, grad_sph, grad_xyz, n};
+    VjprParams prm{xyz, grad_sph, grad_xyz, n, 0};
     switch (l_max) {
         VJPR_CASE(1)
         VJPR_CASE(2)
