@@ -272,6 +272,39 @@ def test_cooperative_kernel_long_rows(sph, oracle, dtype, monkeypatch):
         assert torch.all(b[:32] == 777.0) and torch.all(b[-32:] == 777.0) and torch.all(b[32:-32] != 777.0)
 
 
+def test_stream_order_with_programmatic_dependent_launch(sph):
+    """The small-grid kernels are launched as programmatic dependent launches: their CTAs may become
+    resident while the previous kernel in the stream still runs, but must not read or write
+    anything before it has completed.  RAW, WAR and WAW hazards against torch kernels and against
+    the library's own kernels, without any synchronisation in between."""
+    n, l_max = 60_000, 8
+    L = (l_max + 1) ** 2
+    x1 = torch.randn(n, 3, device="cuda")
+    x2 = torch.randn(n, 3, device="cuda")
+    ref1 = sph.compute(x1, l_max, True, True)
+    ref2 = sph.compute(x2, l_max, True, True)
+    torch.cuda.synchronize()
+    st = torch.cuda.current_stream().cuda_stream
+    for _ in range(20):
+        x = x1.clone()
+        s = torch.empty((n, L), device="cuda")
+        d = torch.empty((n, 3, L), device="cuda")
+        big = torch.randn(64 << 20, device="cuda")
+        big.mul_(1.0001)                                   # something long-running in front
+        x.copy_(x2)                                        # RAW: the forward must see x2
+        sph.sphericart_cuda_compute(x, n, l_max, 1, 0, s, d, None, st)
+        keep = s.clone()                                   # WAR: the clone must see this forward's values
+        sph.sphericart_cuda_compute(x1, n, l_max, 1, 0, s, d, None, st)   # WAW on s, d
+        g = torch.ones((n, L), device="cuda")
+        g.mul_(2.0)                                        # RAW for the recompute VJP
+        gx = sph.vjp_recompute(x1, g, True)
+        torch.cuda.synchronize()
+        assert torch.equal(keep, ref2[0])
+        assert torch.equal(s, ref1[0]) and torch.equal(d, ref1[1])
+        want = sph.vjp(ref1[1], torch.full((n, L), 2.0, device="cuda"))
+        assert torch.allclose(gx, want, rtol=1e-4, atol=1e-4 * float(want.abs().max()))
+
+
 def test_origin_and_untouched_memory(sph, oracle):
     # normalised at r = 0: NaN for that point only; solid at r = 0 is defined
     xyz = np.array([[0, 0, 0], [1, 2, 3], [0, 0, 0], [-1, 0.5, 0.25]], np.float64)
