@@ -50,11 +50,15 @@ static int launch_split(int sm_count, TpbParams prm, cudaStream_t stream) {
             return -1;
         attr_done[dev] = true;
     }
-    // one tile per CTA measured best on every config (C3: 166 us against 172 us with four, C5: 476
-    // against 508): the CTA launch is cheap next to a tile; the knob stays for experiments
+    // One tile per CTA where a tile is >= ~12 KB (C3: 166 us against 172 us with four tiles, C5 with
+    // gradients: 476 against 508): the CTA launch is cheap next to such a tile.  Small tiles (values
+    // only, low l_max) take up to four per CTA, or the launch rate of the block scheduler shows
+    // (C5 values only, 3.1 KB tiles: 170 us with one, 147 with two, 136 with four or eight).
     const int64_t n_tiles = (prm.n + TPB_PTS - 1) / TPB_PTS;
-    static const int k_env = env_int("SPHB200_TPB_TILES", 1);
-    const int64_t k = k_env > 0 ? k_env : 1;
+    static const int k_env = env_int("SPHB200_TPB_TILES", 0);
+    int64_t k = k_env > 0 ? k_env : 12288 / Shape::tile_bytes;
+    if (k < 1) k = 1;
+    if (k_env <= 0 && k > 4) k = 4;
     prm.tiles_per_cta = (int)k;
     const int64_t ctas = (n_tiles + k - 1) / k;
     if (ctas > 0x7fffffff) return 1;
