@@ -123,6 +123,30 @@ def vjp_recompute(xyz, grad_sph, l_max: int, normalized: bool, kind: str = "ld")
     return vjp(dsph, grad_sph, l_max, kind=kind)
 
 
+def expand(xyz, radial, seg_ptr, l_max: int):
+    """Oracle for ``sphericart_cuda_expand`` (Eq. 1):
+
+        c[s, n, lm] = sum over the points k of segment s of  R[k, n, l] * Y_l^m(r_k / |r_k|),
+
+    ``xyz`` [N,3] the points r_k, ``radial`` [N, n_rad, l_max+1] the values R_nl(r_k) (the paper
+    leaves the radial basis to the application: they are an input), ``seg_ptr`` [S+1] ascending
+    offsets: segment s (e.g. the neighbours of centre s) is the points seg_ptr[s] .. seg_ptr[s+1]-1.
+    Plain loops over segments, long double throughout; Y from ``compute`` (normalised)."""
+    xyz = np.ascontiguousarray(np.asarray(xyz), dtype=np.float64).reshape(-1, 3)
+    radial = np.asarray(radial)
+    seg_ptr = np.asarray(seg_ptr, dtype=np.int64)
+    n, n_rad = xyz.shape[0], radial.shape[1]
+    assert radial.shape == (n, n_rad, l_max + 1) and seg_ptr[0] == 0 and seg_ptr[-1] == n
+    Y, _, _ = compute(xyz, l_max, True)
+    l_of = np.concatenate([[l] * (2 * l + 1) for l in range(l_max + 1)])
+    R = radial.astype(np.longdouble)[:, :, l_of]            # [N, n_rad, L]: R_nl repeated over m
+    out = np.zeros((len(seg_ptr) - 1, n_rad, n_sph(l_max)), np.longdouble)
+    for s in range(len(seg_ptr) - 1):
+        for k in range(seg_ptr[s], seg_ptr[s + 1]):
+            out[s] += R[k] * Y[k][None, :]
+    return out
+
+
 def F_table(l_max: int, kind: str = "ld"):
     """F_l^m (Eq. C1) as a flat triangle, index l(l+1)/2+m."""
     out = np.empty((l_max + 1) * (l_max + 2) // 2, _DTYPE[kind])

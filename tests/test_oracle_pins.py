@@ -626,6 +626,52 @@ def test_vjp_recompute_is_gradient_of_weighted_sum(oracle, normalized):
     assert np.array_equal(got, oracle.vjp(d, w, l_max))
 
 
+def test_expand_eq1(oracle):
+    """N2 pins for the density expansion of Eq. 1: one-point segments, brute force, order
+    independence, parity of antipodal pairs, rotation invariance of the power spectrum."""
+    l_max, n_rad = 6, 3
+    L = (l_max + 1) ** 2
+    rng = np.random.default_rng(21)
+    pts = rng.standard_normal((37, 3))
+    rad = rng.standard_normal((37, n_rad, l_max + 1))
+    Y = oracle.compute(pts, l_max, True)[0]
+    l_of = np.concatenate([[l] * (2 * l + 1) for l in range(l_max + 1)])
+    # (1) one point per segment: c = R_nl Y_lm, nothing summed
+    c1 = oracle.expand(pts, rad, np.arange(38), l_max)
+    assert c1.shape == (37, n_rad, L)
+    for k in (0, 5, 36):
+        for n in range(n_rad):
+            assert np.array_equal(c1[k, n], rad[k, n].astype(LD)[l_of] * Y[k])
+    # (2) brute force with python scalars over ragged segments, one of them empty
+    seg = np.array([0, 4, 4, 20, 37])
+    c = oracle.expand(pts, rad, seg, l_max)
+    assert np.all(c[1] == 0)
+    for s_, n, lm in ((0, 0, 0), (2, 1, 17), (3, 2, L - 1), (2, 0, 30)):
+        want = LD(0)
+        for k in range(seg[s_], seg[s_ + 1]):
+            want += LD(rad[k, n, l_of[lm]]) * Y[k, lm]
+        assert abs(c[s_, n, lm] - want) <= 1e-17 * 37
+    # (3) the sum does not depend on the order of the points (to rounding)
+    perm = rng.permutation(37)
+    cp = oracle.expand(pts[perm], rad[perm], np.array([0, 37]), l_max)
+    ca = oracle.expand(pts, rad, np.array([0, 37]), l_max)
+    assert float(np.max(np.abs(cp - ca))) < 1e-16 * 37
+    # (4) antipodal pair with equal radial values: odd l cancel, even l double (P9: Y(-x) = (-1)^l Y(x))
+    pair = np.stack([pts[3], -pts[3]])
+    c2 = oracle.expand(pair, np.stack([rad[3], rad[3]]), np.array([0, 2]), l_max)[0]
+    odd = (l_of % 2) == 1
+    assert float(np.max(np.abs(c2[:, odd]))) < 1e-17
+    assert float(np.max(np.abs(c2[:, ~odd] - 2 * c1[3][:, ~odd]))) < 1e-17
+    # (5) rotating every point leaves the power spectrum p_nl = sum_m c_nlm^2 unchanged (P4)
+    Rm = _random_rotation(rng)
+    cr = oracle.expand(pts @ Rm.T, rad, np.array([0, 37]), l_max)[0]
+    for l in range(l_max + 1):
+        sl = slice(l * l, (l + 1) ** 2)
+        p0 = (ca[0][:, sl] ** 2).sum(axis=1)
+        p1 = (cr[:, sl] ** 2).sum(axis=1)
+        assert float(np.max(np.abs(p0 - p1) / (np.abs(p0) + 1e-30))) < 1e-13, l
+
+
 # --------------------------------------------------------------------------------------------
 # edge cases of the oracle's interface
 # --------------------------------------------------------------------------------------------
