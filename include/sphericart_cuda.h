@@ -53,6 +53,7 @@ extern "C" {
 #define SPHERICART_CUDA_EALIGN 2   /* a base pointer is not 16-byte aligned */
 #define SPHERICART_CUDA_ECUDA 3    /* a CUDA runtime call or the launch failed; see last_error */
 #define SPHERICART_CUDA_ENOMEM 4   /* (_host entry points) device or host allocation failed */
+#define SPHERICART_CUDA_ENOTSUP 5  /* valid arguments this build has no kernel for (sphericart_cuda_expand) */
 
 /*
  * Forward pass ("takes a list of Cartesian coordinates and evaluates the scaled
@@ -97,6 +98,24 @@ int sphericart_cuda_vjp(const void* xyz, const void* dsph, const void* grad_sph,
  */
 int sphericart_cuda_vjp_recompute(const void* xyz, const void* grad_sph, void* grad_xyz, int64_t n,
                                   int l_max, int normalized, int dtype, void* stream);
+
+/*
+ * Fused density expansion (the use the paper motivates, Eq. 1):
+ *     coeff[s, n, lm] = sum over the points k of segment s of  radial[k, n, l] * Y_l^m(r_k / |r_k|),
+ * lm = l(l+1)+m as everywhere, Y normalised (Eq. 1 evaluates Y at the direction of r_k).  The
+ * harmonics are evaluated inside the kernel and never written to memory.
+ *   xyz      [N,3]               in   the points r_k (e.g. neighbour vectors), N = seg_ptr[n_seg]
+ *   radial   [N, n_rad, l_max+1] in   R_nl(r_k): the radial basis is the caller's (the paper fixes none)
+ *   seg_ptr  [n_seg+1] int64     in   DEVICE array of ascending offsets into the points: segment s
+ *                                     (e.g. the neighbours of centre s) is seg_ptr[s] .. seg_ptr[s+1]-1;
+ *                                     an empty segment gives zeros
+ *   coeff    [n_seg, n_rad, L]   out
+ * Device pointers, caller-owned, 16-byte aligned (seg_ptr: 8); asynchronous on `stream`.
+ * This build has kernels for l_max <= 8 and n_rad <= 16: otherwise SPHERICART_CUDA_ENOTSUP, no launch.
+ * A point with r = 0 makes its segment's coefficients NaN.
+ */
+int sphericart_cuda_expand(const void* xyz, const void* radial, const int64_t* seg_ptr, int64_t n_seg,
+                           int l_max, int n_rad, int dtype, void* coeff, void* stream);
 
 /*
  * The same two operations on HOST buffers: the library copies xyz (and dsph/grad_sph) to the

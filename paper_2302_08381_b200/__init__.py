@@ -50,6 +50,8 @@ def load():
     lib.sphericart_cuda_compute_host.argtypes = [vp, i64, ci, ci, ci, vp, vp, vp]
     lib.sphericart_cuda_vjp_recompute.restype = ci
     lib.sphericart_cuda_vjp_recompute.argtypes = [vp, vp, vp, i64, ci, ci, ci, vp]
+    lib.sphericart_cuda_expand.restype = ci
+    lib.sphericart_cuda_expand.argtypes = [vp, vp, vp, i64, ci, ci, ci, vp, vp]
     lib.sphericart_cuda_vjp_host.restype = ci
     lib.sphericart_cuda_vjp_host.argtypes = [vp, vp, vp, vp, i64, ci, ci]
     lib.sphericart_cuda_last_error.restype = ctypes.c_char_p
@@ -100,6 +102,12 @@ def sphericart_cuda_vjp_recompute(xyz, grad_sph, grad_xyz, n, l_max, normalized,
     rc = load().sphericart_cuda_vjp_recompute(_ptr(xyz), _ptr(grad_sph), _ptr(grad_xyz), n, l_max,
                                               int(bool(normalized)), dtype, _ptr(stream))
     _check(rc, "sphericart_cuda_vjp_recompute")
+
+
+def sphericart_cuda_expand(xyz, radial, seg_ptr, n_seg, l_max, n_rad, dtype, coeff, stream):
+    rc = load().sphericart_cuda_expand(_ptr(xyz), _ptr(radial), _ptr(seg_ptr), n_seg, l_max, n_rad, dtype,
+                                       _ptr(coeff), _ptr(stream))
+    _check(rc, "sphericart_cuda_expand")
 
 
 def sphericart_cuda_vjp_host(xyz, dsph, grad_sph, grad_xyz, n, l_max, dtype):
@@ -188,3 +196,22 @@ def vjp_recompute(xyz, grad_sph, normalized: bool, out=None):
         stream = torch.cuda.current_stream().cuda_stream
         sphericart_cuda_vjp_recompute(xyz, grad_sph, gx, n, l_max, normalized, _dtype_code(xyz), stream)
     return gx
+
+
+def expand(xyz, radial, seg_ptr, out=None):
+    """``coeff[s,n,lm] = sum_{k in segment s} radial[k,n,l] Y_lm(xyz[k]/|xyz[k]|)`` (Eq. 1 of the paper)
+    on torch's current stream; ``seg_ptr`` an int64 CUDA tensor of ascending offsets."""
+    import torch
+
+    if not xyz.is_cuda:
+        raise SphericartCudaError("xyz must be a CUDA tensor (no CPU fallback)")
+    xyz, radial, seg_ptr = xyz.contiguous(), radial.contiguous(), seg_ptr.contiguous()
+    n, n_rad, lp1 = radial.shape
+    if xyz.shape != (n, 3) or xyz.dtype != radial.dtype or seg_ptr.dtype != torch.int64:
+        raise ValueError("shapes: xyz [n,3], radial [n,n_rad,l_max+1] of the same dtype, seg_ptr int64")
+    n_seg, L = seg_ptr.numel() - 1, lp1 * lp1
+    c = torch.empty((n_seg, n_rad, L), dtype=xyz.dtype, device=xyz.device) if out is None else out
+    with torch.cuda.device(xyz.device):
+        stream = torch.cuda.current_stream().cuda_stream
+        sphericart_cuda_expand(xyz, radial, seg_ptr, n_seg, lp1 - 1, n_rad, _dtype_code(xyz), c, stream)
+    return c

@@ -70,7 +70,8 @@ static int device_state(DeviceState** out) {
         CUDA_TRY(cudaMemcpyToSymbol(c_tables, &g_host_tables, sizeof(SphTables)));
         if (sph_tpb_upload_f32_v(&g_host_tables) || sph_tpb_upload_f32_g(&g_host_tables) ||
             sph_tpb_upload_f64_v(&g_host_tables) || sph_tpb_upload_f64_g(&g_host_tables) ||
-            sph_vjpr_upload_f32(&g_host_tables) || sph_vjpr_upload_f64(&g_host_tables))
+            sph_vjpr_upload_f32(&g_host_tables) || sph_vjpr_upload_f64(&g_host_tables) ||
+            sph_expand_upload_f32(&g_host_tables) || sph_expand_upload_f64(&g_host_tables))
             return fail(SPHERICART_CUDA_ECUDA, "table upload failed: %s", cudaGetErrorString(cudaGetLastError()));
         CUDA_TRY(cudaMalloc(&st.d_tables, sizeof(SphTables)));
         CUDA_TRY(cudaMemcpy(st.d_tables, &g_host_tables, sizeof(SphTables), cudaMemcpyHostToDevice));
@@ -446,6 +447,29 @@ int sphericart_cuda_vjp_recompute(const void* xyz, const void* grad_sph, void* g
                                   int normalized, int dtype, void* stream) {
     return vjp_recompute_device(xyz, grad_sph, grad_xyz, n, l_max, normalized, dtype,
                                 static_cast<cudaStream_t>(stream));
+}
+
+int sphericart_cuda_expand(const void* xyz, const void* radial, const int64_t* seg_ptr, int64_t n_seg, int l_max,
+                           int n_rad, int dtype, void* coeff, void* stream) {
+    int rc = check_common(n_seg, l_max, dtype);
+    if (rc) return rc;
+    if (n_rad < 1) return fail(SPHERICART_CUDA_EINVAL, "n_rad = %d must be at least 1", n_rad);
+    if (n_seg == 0) return 0;
+    if (!xyz || !radial || !seg_ptr || !coeff)
+        return fail(SPHERICART_CUDA_EINVAL, "xyz, radial, seg_ptr and coeff must not be NULL when n_seg > 0");
+    if (misaligned(xyz) || misaligned(radial) || misaligned(coeff) || (reinterpret_cast<uintptr_t>(seg_ptr) & 7u))
+        return fail(SPHERICART_CUDA_EALIGN, "device pointers must be 16-byte aligned (seg_ptr: 8)");
+    DeviceState* st = nullptr;
+    rc = device_state(&st);
+    if (rc) return rc;
+    const int r = (dtype == SPHERICART_CUDA_F32 ? sph_expand_launch_f32 : sph_expand_launch_f64)(
+        st->smem_optin, xyz, radial, seg_ptr, n_seg, l_max, n_rad, coeff, static_cast<cudaStream_t>(stream));
+    if (r < 0) return fail(SPHERICART_CUDA_ECUDA, "expand launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    if (r > 0)
+        return fail(SPHERICART_CUDA_ENOTSUP, "expand: l_max = %d (max 8) or n_rad = %d (max %d) has no kernel in this build",
+                    l_max, n_rad, 16);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return 0;
 }
 
 int sphericart_cuda_compute_host(const void* xyz, int64_t n, int l_max, int normalized, int dtype, void* sph,

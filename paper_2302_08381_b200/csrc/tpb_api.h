@@ -24,4 +24,12 @@ SPH_TPB_DECL(f64_g)
 SPH_VJPR_DECL(f32)
 SPH_VJPR_DECL(f64)
 #undef SPH_VJPR_DECL
+// fused density expansion of Eq. 1 (expand_inst.cu, compiled once per element type); same return codes
+#define SPH_EXPAND_DECL(sfx)                                                                                   \
+    int sph_expand_launch_##sfx(int smem_optin, const void* xyz, const void* radial, const int64_t* seg_ptr,  \
+                                int64_t n_seg, int l_max, int n_rad, void* coeff, cudaStream_t stream);       \
+    int sph_expand_upload_##sfx(const SphTables* host_tables);
+SPH_EXPAND_DECL(f32)
+SPH_EXPAND_DECL(f64)
+#undef SPH_EXPAND_DECL
 }  // namespace sphb200

@@ -116,3 +116,22 @@ def make_grad_sph(cfg: Config | str, n: int | None = None, seed: int = 0) -> np.
     if cfg.dtype == "f32":
         return rng.standard_normal((n, cfg.n_sph), dtype=np.float32)
     return rng.standard_normal((n, cfg.n_sph))
+
+
+def make_expand_inputs(n_seg: int, l_max: int, n_rad: int, dtype: str = "f32", mean_neighbours: float = 32.0,
+                       seed: int = 0):
+    """Synthetic input of the density expansion of Eq. 1, shaped like an atomistic
+    neighbour list: ``n_seg`` centres with Poisson(``mean_neighbours``) neighbours each (some
+    centres have none), neighbour vectors uniform in a ball of radius 5 (as C3), radial values
+    i.i.d. N(0,1) -- the paper fixes no radial basis, so they are plain numbers here.
+    Returns ``(xyz [N,3], radial [N,n_rad,l_max+1], seg_ptr [n_seg+1] int64)``."""
+    rng = np.random.default_rng([200 + l_max, n_rad, seed])
+    counts = rng.poisson(mean_neighbours, size=n_seg).astype(np.int64)
+    seg_ptr = np.concatenate([[0], np.cumsum(counts)]).astype(np.int64)
+    n = int(seg_ptr[-1])
+    d = rng.standard_normal((n, 3))
+    d /= np.linalg.norm(d, axis=1, keepdims=True)
+    xyz = d * (5.0 * rng.random(n) ** (1.0 / 3.0))[:, None]
+    np_dt = np.float32 if dtype == "f32" else np.float64
+    radial = rng.standard_normal((n, n_rad, l_max + 1)).astype(np_dt)
+    return xyz.astype(np_dt), radial, seg_ptr

@@ -103,3 +103,26 @@ def check_vjp(got, want, dsph, grad_sph, l_max, dtype, what="vjp", point_scale=F
     emax = float(e.max(initial=0))
     assert emax <= tol, f"{what}: max scaled error {emax:.3e} (tol {tol:.1e})"
     return emax
+
+
+def check_expand(got, want, radial, seg_ptr, l_max, dtype, what="expand"):
+    """Density expansion (Eq. 1): |err| / max(|ref|, 1e-3 S) <= tol with the scale of one row of the
+    sum, S[s,n,l] = sqrt((2l+1)/4pi) * sum_{k in s} |R[k,n,l]|  (R1's row scale S_0 weighted by the
+    radial values: the size the terms have before they cancel).  Empty segments must be exact zeros."""
+    tol = tol_for(dtype, l_max)
+    got = np.asarray(got).astype(LD)
+    want = np.asarray(want).astype(LD)
+    R = np.abs(np.asarray(radial).astype(LD))
+    n_seg = len(seg_ptr) - 1
+    l_of = np.concatenate([[l] * (2 * l + 1) for l in range(l_max + 1)])
+    S = np.zeros_like(want)
+    for s_ in range(n_seg):
+        S[s_] = R[seg_ptr[s_]:seg_ptr[s_ + 1]].sum(axis=0)[:, l_of]
+    S *= np.sqrt((2 * l_of + 1) / (4 * np.pi)).astype(LD)[None, None, :]
+    diff = np.abs(got - want)
+    with np.errstate(invalid="ignore", divide="ignore"):
+        e = diff / np.maximum(np.abs(want), LD(1e-3) * S)
+    e = np.where(np.isfinite(e), e, np.where(diff == 0, 0, np.inf))
+    emax = float(e.max(initial=0))
+    assert emax <= tol, f"{what}: max scaled error {emax:.3e} (tol {tol:.1e})"
+    return emax

@@ -30,7 +30,7 @@ def lib():
 def test_header_declares_the_boundary():
     names = _declared_symbols()
     for must in ("sphericart_cuda_compute", "sphericart_cuda_vjp", "sphericart_cuda_last_error",
-                 "sphericart_cuda_compute_host", "sphericart_cuda_vjp_host", "sphericart_cuda_vjp_recompute"):
+                 "sphericart_cuda_compute_host", "sphericart_cuda_vjp_host", "sphericart_cuda_vjp_recompute", "sphericart_cuda_expand"):
         assert must in names
 
 
@@ -65,6 +65,10 @@ def test_argument_errors_do_not_need_a_gpu(lib):
     assert c.sphericart_cuda_vjp_recompute(16, 16, 16, 5, 4, 3, 0, None) == 1                    # normalized
     assert c.sphericart_cuda_vjp_recompute(16, 16, 16, 5, 40, 1, 0, None) == 1                   # l_max
     assert c.sphericart_cuda_vjp_recompute(16, 8, 16, 5, 4, 1, 0, None) == 2                     # misaligned
+    assert c.sphericart_cuda_expand(None, None, None, 5, 4, 2, 0, None, None) == 1                # NULL pointers
+    assert c.sphericart_cuda_expand(None, None, None, 0, 4, 2, 0, None, None) == 0                # n_seg == 0
+    assert c.sphericart_cuda_expand(16, 16, 16, 5, 4, 0, 0, 16, None) == 1                        # n_rad
+    assert c.sphericart_cuda_expand(16, 16, 12, 5, 4, 2, 0, 16, None) == 2                        # seg_ptr alignment
     with pytest.raises(lib.SphericartCudaError):
         lib.sphericart_cuda_compute(None, -1, 4, 1, 0, None, None, None, None)
 

@@ -305,6 +305,33 @@ def test_stream_order_with_programmatic_dependent_launch(sph):
         assert torch.allclose(gx, want, rtol=1e-4, atol=1e-4 * float(want.abs().max()))
 
 
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_expand_eq1(sph, oracle, dtype):
+    """N2: the fused density expansion against the oracle; every l_max with a kernel, n_rad across
+    the three register variants, ragged / empty / long segments."""
+    for l_max, n_rad, n_seg, mean in ((8, 8, 300, 32.0), (6, 3, 200, 5.0), (4, 16, 64, 70.0), (1, 1, 50, 2.0),
+                                     (0, 2, 40, 3.0), (7, 5, 33, 17.0), (8, 12, 20, 40.0)):
+        xyz, rad, seg = W.make_expand_inputs(n_seg, l_max, n_rad, dtype, mean)
+        c = sph.expand(torch.from_numpy(xyz).cuda(), torch.from_numpy(rad).cuda(), torch.from_numpy(seg).cuda())
+        torch.cuda.synchronize()
+        want = oracle.expand(xyz, rad, seg, l_max)
+        parity.check_expand(c.cpu().numpy(), want, rad, seg, l_max, dtype, f"expand {dtype} l_max={l_max} n_rad={n_rad}")
+        empty = np.nonzero(np.diff(seg) == 0)[0]
+        assert np.all(c.cpu().numpy()[empty] == 0)
+    # the same numbers as compute() followed by a segment sum in torch (f64 accumulation)
+    xyz, rad, seg = W.make_expand_inputs(100, 6, 4, dtype, 20.0)
+    x_d, r_d = torch.from_numpy(xyz).cuda(), torch.from_numpy(rad).cuda()
+    c = sph.expand(x_d, r_d, torch.from_numpy(seg).cuda())
+    Y = sph.compute(x_d, 6, True)[0].double()
+    l_of = torch.tensor(np.concatenate([[l] * (2 * l + 1) for l in range(7)]), device="cuda")
+    terms = r_d.double()[:, :, l_of] * Y[:, None, :]
+    ref = torch.stack([terms[seg[i]:seg[i + 1]].sum(dim=0) for i in range(100)])
+    assert torch.allclose(c.double(), ref, rtol=1e-5 if dtype == "f32" else 1e-12, atol=1e-5 if dtype == "f32" else 1e-12)
+    # unsupported sizes are refused, nothing is launched
+    with pytest.raises(sph.SphericartCudaError):
+        sph.expand(x_d, torch.zeros((x_d.shape[0], 17, 7), device="cuda", dtype=x_d.dtype), torch.from_numpy(seg).cuda())
+
+
 def test_origin_and_untouched_memory(sph, oracle):
     # normalised at r = 0: NaN for that point only; solid at r = 0 is defined
     xyz = np.array([[0, 0, 0], [1, 2, 3], [0, 0, 0], [-1, 0.5, 0.25]], np.float64)
