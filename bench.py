@@ -256,6 +256,36 @@ def sweep_one(cfg, torch, pkg, device, peak):
     return res
 
 
+def sweep_expand(torch, pkg, device):
+    """the fused density expansion of Eq. 1 on a neighbour-list-shaped input
+    (32768 centres x Poisson(32) neighbours, l_max = 8, n_rad = 8, f32), and the values-only forward
+    over the same points as context (what an unfused consumer would have to run first)."""
+    l_max, n_rad, n_seg = 8, 8, 32768
+    xyz, rad, seg = W.make_expand_inputs(n_seg, l_max, n_rad, "f32", 32.0)
+    n = xyz.shape[0]
+    x_d, r_d, s_d = (torch.from_numpy(a).to(device) for a in (xyz, rad, seg))
+    L = (l_max + 1) ** 2
+    outs = [torch.empty((n_seg, n_rad, L), dtype=torch.float32, device=device) for _ in range(4)]
+    sphs = [torch.empty((n, L), dtype=torch.float32, device=device) for _ in range(2)]
+    stream = torch.cuda.current_stream().cuda_stream
+    fused = lambda i: pkg.sphericart_cuda_expand(x_d, r_d, s_d, n_seg, l_max, n_rad, pkg.F32, outs[i % 4], stream)
+    fwd = lambda i: pkg.sphericart_cuda_compute(x_d, n, l_max, 1, pkg.F32, sphs[i % 2], None, None, stream)
+    res = {"workload": f"Eq. 1: {n_seg} segments, {n} points (Poisson(32) per segment), l_max={l_max}, n_rad={n_rad}, f32",
+           "n_points": n}
+    for key, fn in (("expand", fused), ("fwd_values_only", fwd)):
+        for i in range(3):
+            fn(i)
+        torch.cuda.synchronize()
+        e0, e1 = time_loop(torch, fn, 50)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / 50
+        res[key + "_us"] = round(ms * 1e3, 2)
+        res[key + "_points_per_s"] = n / (ms * 1e-3)
+    in_bytes = n * (12 + n_rad * (l_max + 1) * 4) + n_seg * (8 + n_rad * L * 4)
+    res["expand_algorithmic_gbs"] = in_bytes / (res["expand_us"] * 1e-6) / 1e9
+    return res
+
+
 def time_e2e(cfg, torch, pkg, steps):
     """The same metric through the host-buffer C-ABI call: pinned host arrays in, pinned host arrays
     out, H2D + kernels + D2H inside the timed region (wall clock around a synchronous call)."""
@@ -428,6 +458,7 @@ def run_cuda(args):
                     line["sweep"][name] = {"skipped": "does not fit in free HBM"}
                     continue
                 line["sweep"][name] = sweep_one(c, torch, pkg, device, peak)
+            line["sweep"]["N2_expand"] = sweep_expand(torch, pkg, device)
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()

@@ -24,9 +24,9 @@ typedef double exp_R;
 template <int LMAX, int NRAD_MAX> static int launch_nr(int smem_optin, ExpandParams prm, cudaStream_t stream) {
     using Shape = ExpandShape<sizeof(exp_T), LMAX>;
     auto kern = sph_expand_kernel<exp_T, exp_R, LMAX, NRAD_MAX>;
-    int warps = 4;
-    while (warps > 1 && warps * Shape::warp_bytes(prm.n_rad) > smem_optin - 1024) warps >>= 1;
-    const int smem = warps * Shape::warp_bytes(prm.n_rad);
+    int warps = 2;   // small CTAs: more of them fit beside each other in shared memory
+    while (warps > 1 && warps * Shape::warp_bytes(prm.n_rad, NRAD_MAX) > smem_optin - 1024) warps >>= 1;
+    const int smem = warps * Shape::warp_bytes(prm.n_rad, NRAD_MAX);
     if (smem > smem_optin - 1024) return 1;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return -1;
     prm.warps_per_cta = warps;

@@ -9,8 +9,11 @@
 // One warp per segment.  Per tile of 16 points of the segment
 //   1. two lanes per point (cos | sin branch of Eq. 5, as in kernel_tpb.cuh, l_max compile-time)
 //      evaluate the normalised harmonics into a [16][L] image in shared memory (f64 / double-double
-//      recurrences, stored in the I/O type), while the tile's radial values ([16][n_rad][l_max+1], one contiguous
-//      range) are copied next to it;
+//      recurrences, stored in the I/O type), while the tile's radial values ([16][n_rad][l_max+1],
+//      one contiguous range) are copied next to it, widened to double ONCE here: the contraction
+//      runs in f64 and reads every radial value 2l+1 times (ncu on the first version, which widened
+//      each operand where it was used: the XU pipe of the f32->f64 conversions 63 % busy, the top
+//      pipe of the kernel);
 //   2. lane = harmonic index lm (ceil(L/32) passes): acc[pass][n] += R[p][n][l(lm)] * Y[p][lm] over
 //      the tile's points, in f64 registers;
 // and at the end of the segment the accumulators go out, coalesced along lm.
@@ -34,10 +37,14 @@ constexpr int EXP_MAX_RAD = 16;   // accumulators per pass held in registers
 template <int ESIZE, int LMAX> struct ExpandShape {
     static constexpr int L = (LMAX + 1) * (LMAX + 1);
     static constexpr int passes = (L + 31) / 32;
-    // per warp: Y image [16][L] + radial image [16][n_rad][LMAX+1], both in the I/O type
-    static constexpr int y_bytes = TPB_PTS * L * ESIZE;
-    __host__ __device__ static constexpr int r_bytes(int n_rad) { return TPB_PTS * n_rad * (LMAX + 1) * ESIZE; }
-    __host__ __device__ static constexpr int warp_bytes(int n_rad) { return (y_bytes + r_bytes(n_rad) + 15) & ~15; }
+    // per warp: Y image [16][L] in the I/O type + radial image [16][n_rad][LMAX+1] in double, the
+    // latter followed by nrad_max rows of padding (the unrolled contraction reads nrad_max rows per
+    // point whatever n_rad is; what it reads past n_rad only feeds accumulators that are dropped)
+    static constexpr int y_bytes = (TPB_PTS * L * ESIZE + 15) & ~15;
+    __host__ __device__ static constexpr int r_bytes(int n_rad, int nrad_max) {
+        return (TPB_PTS * n_rad + nrad_max) * (LMAX + 1) * 8;
+    }
+    __host__ __device__ static constexpr int warp_bytes(int n_rad, int nrad_max) { return y_bytes + r_bytes(n_rad, nrad_max); }
 };
 
 template <typename T, typename R, int LMAX, int NRAD_MAX>
@@ -53,8 +60,9 @@ __global__ void __launch_bounds__(128) sph_expand_kernel(const ExpandParams prm)
     const int n_rad = prm.n_rad;
     const int64_t seg = (int64_t)blockIdx.x * prm.warps_per_cta + warp;
     if (seg >= prm.n_seg) return;
-    T* Ys = reinterpret_cast<T*>(smem + (size_t)warp * Shape::warp_bytes(n_rad));
-    T* Rs = Ys + TPB_PTS * L;
+    unsigned char* my = smem + (size_t)warp * Shape::warp_bytes(n_rad, NRAD_MAX);
+    T* Ys = reinterpret_cast<T*>(my);
+    double* Rs = reinterpret_cast<double*>(my + Shape::y_bytes);
     const int pl = lane & (TPB_PTS - 1);   // point inside the tile
     const bool sinb = lane >= TPB_PTS;     // branch
     const T* __restrict__ xyz = static_cast<const T*>(prm.xyz);
@@ -83,7 +91,7 @@ __global__ void __launch_bounds__(128) sph_expand_kernel(const ExpandParams prm)
         const int np = (int)((k_end - k0 < TPB_PTS) ? k_end - k0 : TPB_PTS);
         __syncwarp();   // the previous tile's accumulation is done with both images
         // ---- radial values of the tile: one contiguous range -----------------------------------
-        for (int i = lane; i < np * rstride; i += 32) Rs[i] = __ldg(radial + k0 * rstride + i);
+        for (int i = lane; i < np * rstride; i += 32) Rs[i] = static_cast<double>(__ldg(radial + k0 * rstride + i));
         // ---- harmonics of the tile: two lanes per point ----------------------------------------
         double x = 0.0, y = 0.0, z = 1.0;  // lanes past the end compute a harmless point
         if (pl < np) {
@@ -138,10 +146,9 @@ __global__ void __launch_bounds__(128) sph_expand_kernel(const ExpandParams prm)
                 const int lm = lane + 32 * ps;
                 if (lm < L) {
                     const double yv = static_cast<double>(Ys[p * L + lm]);
-                    const T* rp = Rs + p * rstride + l_of[ps];
+                    const double* rp = Rs + p * rstride + l_of[ps];
 #pragma unroll
-                    for (int nr = 0; nr < NRAD_MAX; ++nr)
-                        if (nr < n_rad) acc[ps][nr] = fma(static_cast<double>(rp[nr * (LMAX + 1)]), yv, acc[ps][nr]);
+                    for (int nr = 0; nr < NRAD_MAX; ++nr) acc[ps][nr] = fma(rp[nr * (LMAX + 1)], yv, acc[ps][nr]);
                 }
             }
         }
