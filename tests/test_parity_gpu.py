@@ -118,6 +118,40 @@ def test_config_full_size_sampled(sph, oracle, name):
         ref = torch.einsum("nak,nk->na", d.double(), gt.double())
         scale = d.double().norm(dim=2) * gt.double().norm(dim=1)[:, None]
         assert float(((gx.double() - ref).abs() / scale).max()) < 2e-7
+        # N1 at full size, as bench.py launches it: sampled against the oracle, every point against
+        # the stored-derivative route
+        gr = sph.vjp_recompute(torch.from_numpy(xyz).cuda(), gt, cfg.normalized)
+        torch.cuda.synchronize()
+        _, wd, _ = oracle.compute(xyz[idx], cfg.l_max, cfg.normalized, True)
+        parity.check_vjp(pick(gr).cpu().numpy(), oracle.vjp_recompute(xyz[idx], g[idx], cfg.l_max, cfg.normalized),
+                         wd, g[idx], cfg.l_max, cfg.dtype, name + " full vjp_recompute", point_scale=True)
+        pscale = scale.max(dim=1, keepdim=True).values
+        assert float(((gr.double() - ref).abs() / pscale).max()) < 4e-7
+
+
+def test_expand_full_size_sampled(sph, oracle):
+    """N2 at the size and launch configuration bench.py times (32768 segments, ~1.05 M points,
+    l_max = 8, n_rad = 8, f32): sampled segments against the oracle, every segment against
+    compute() + a segment sum in torch."""
+    l_max, n_rad, n_seg = 8, 8, 32768
+    xyz, rad, seg = W.make_expand_inputs(n_seg, l_max, n_rad, "f32", 32.0)
+    x_d, r_d, s_d = (torch.from_numpy(a).cuda() for a in (xyz, rad, seg))
+    c = sph.expand(x_d, r_d, s_d)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(9)
+    pick = np.unique(np.concatenate([rng.integers(0, n_seg, 300), [0, 1, n_seg - 1]]))
+    lo, hi = seg[pick], seg[pick + 1]
+    sub_idx = np.concatenate([np.arange(a, b) for a, b in zip(lo, hi)])
+    sub_seg = np.concatenate([[0], np.cumsum(hi - lo)])
+    want = oracle.expand(xyz[sub_idx], rad[sub_idx], sub_seg, l_max)
+    parity.check_expand(c.cpu().numpy()[pick], want, rad[sub_idx], sub_seg, l_max, "f32", "expand full")
+    Y = sph.compute(x_d, l_max, True)[0].double()
+    l_of = torch.from_numpy(parity.l_of_k(l_max)).cuda()
+    terms = r_d.double()[:, :, l_of] * Y[:, None, :]
+    owner = torch.repeat_interleave(torch.arange(n_seg, device="cuda"), torch.from_numpy(np.diff(seg)).cuda())
+    ref = torch.zeros((n_seg, n_rad, (l_max + 1) ** 2), dtype=torch.float64, device="cuda").index_add_(0, owner, terms)
+    mag = torch.zeros_like(ref).index_add_(0, owner, terms.abs())
+    assert float(((c.double() - ref).abs() / (mag + 1e-30)).max()) < 1e-6
 
 
 # ------------------------------------------------------------------------------------------------
