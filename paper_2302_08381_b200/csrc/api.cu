@@ -13,6 +13,7 @@
 
 #include "kernel_tp.cuh"
 #include "kernel_vjp.cuh"
+#include "kernel_tpg.cuh"
 #include "kernel_w.cuh"
 #include "kernel_wc.cuh"
 #include "tpb_api.h"
@@ -229,7 +230,8 @@ static int compute_device(const void* xyz, int64_t n, int l_max, int normalized,
     const char* force = getenv("SPHB200_FORCE_KERNEL");  // "tpb" | "tp" | "w": experiments only
     const bool force_w = force && force[0] == 'w';
     const bool force_tp = force && force[0] == 't' && force[1] == 'p' && force[2] == '\0';
-    if (!ddsph && !force_w && !force_tp) {
+    const bool force_tpg = force && force[0] == 't' && force[1] == 'p' && force[2] == 'g';
+    if (!ddsph && !force_w && !force_tp && !force_tpg) {
         // compile-time-l_max kernels (two threads per point): every l_max that has an instantiation
         const bool f32 = dtype == SPHERICART_CUDA_F32;
         int r = dsph ? (f32 ? sph_tpb_launch_f32_g : sph_tpb_launch_f64_g)(st->sm_count, xyz, n, l_max, normalized,
@@ -239,6 +241,18 @@ static int compute_device(const void* xyz, int64_t n, int l_max, int normalized,
         if (r < 0) return fail(SPHERICART_CUDA_ECUDA, "tpb launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         if (r == 0) {
             g_launches.fetch_add(1, std::memory_order_relaxed);
+            return 0;
+        }
+    }
+    if (!ddsph && !force_w && !force_tp) {
+        // any other l_max without Hessians: several lanes per point, run-time l_max
+        TpgLaunch lg{};
+        if (tpg_plan(st->smem_optin, n, l_max, normalized, dtype, sph, dsph, xyz, st->d_tables, &lg) == 0) {
+            rc = allow_smem(lg.func, (int)lg.smem);
+            if (rc) return rc;
+            tpg_launch(lg, stream);
+            g_launches.fetch_add(1, std::memory_order_relaxed);
+            CUDA_TRY(cudaGetLastError());
             return 0;
         }
     }

@@ -1,0 +1,331 @@
+// "tpg" forward kernel: SEVERAL lanes per point, any l_max at run time.  Values, or values +
+// gradients, for the l_max that have no compile-time-unrolled tpb kernel (kernel_tpb.cuh).
+//
+// Why: the path is bound by the HBM write of the row-major outputs and wants many small tiles in
+// flight (kernel_tpb.cuh).  With gradients at l_max = 16 a 16-point f32 tile is already 74 KB; the
+// one-warp-per-point kernels (kernel_w.cuh, kernel_wc.cuh) are built for rows of ~100 KB per point
+// and reach ~1 TB/s here.  So a point is given LP = 2, 4 or 8 lanes:
+//     lane = p + PTS (b + 2 c),   PTS = 32 / LP points per tile,
+//     b = branch of Eq. 5 (0: the m >= 0 / cos outputs, 1: the m < 0 / sin outputs),
+//     c = column class: the lane owns the columns m = c, c + C, c + 2C, ... of the (l,m) triangle,
+//         C = LP / 2.
+// A column is run with O(1) state as in eval_point_columns (sph_core.cuh): Qt_l^m by the folded
+// Eq. 7 and, for the gradients, column m+1 one row behind it (Eq. 10 needs Qt_{l-1}^{m+1}); the
+// powers (x + i y)^m of Eq. 9 advance C at a time.  All lanes run the same loops (trip counts
+// differ by < C), the tile's image is laid out exactly like global memory and leaves as 1-D TMA
+// bulk stores; non-persistent grid, one tile per warp.
+#pragma once
+#include <cstdlib>
+
+#include "ptx.cuh"
+#include "sph_core.cuh"
+
+namespace sphb200 {
+
+struct TpgParams {
+    const void* xyz;
+    void* sph;
+    void* dsph;
+    const SphTables* tab;   // global-memory copy of the tables
+    int64_t n;
+    int l_max;
+    int warps_per_cta;
+};
+
+// coefficient tables in shared memory (lanes of a warp sit on different (l,m): a constant bank
+// would serialise them)
+template <typename R> struct TpgTabs;
+template <> struct TpgTabs<double> {
+    const double *A, *B, *D, *G1, *Gz;
+    static constexpr int n_tri = 4, n_col = 1;
+    __device__ void carve(double* base, int tsz, int ncol) {
+        A = base, B = A + tsz, G1 = B + tsz, Gz = G1 + tsz, D = Gz + tsz;
+    }
+    __device__ void fill(double* base, const SphTables* t, int tsz, int ncol) {
+        for (int i = threadIdx.x; i < tsz; i += blockDim.x) {
+            base[i] = t->A_hi[i], base[tsz + i] = t->B_hi[i], base[2 * tsz + i] = t->G1[i], base[3 * tsz + i] = t->Gz[i];
+        }
+        for (int i = threadIdx.x; i < ncol; i += blockDim.x) base[4 * tsz + i] = t->D_hi[i];
+    }
+    __device__ double a(int t) const { return A[t]; }
+    __device__ double b(int t) const { return B[t]; }
+    __device__ double d(int m) const { return D[m]; }
+};
+template <> struct TpgTabs<dd> {
+    const double *Ah, *Al, *Bh, *Bl, *Dh, *Dl, *G1, *Gz;
+    static constexpr int n_tri = 6, n_col = 2;
+    __device__ void carve(double* base, int tsz, int ncol) {
+        Ah = base, Al = Ah + tsz, Bh = Al + tsz, Bl = Bh + tsz, G1 = Bl + tsz, Gz = G1 + tsz, Dh = Gz + tsz, Dl = Dh + ncol;
+    }
+    __device__ void fill(double* base, const SphTables* t, int tsz, int ncol) {
+        for (int i = threadIdx.x; i < tsz; i += blockDim.x) {
+            base[i] = t->A_hi[i], base[tsz + i] = t->A_lo[i], base[2 * tsz + i] = t->B_hi[i], base[3 * tsz + i] = t->B_lo[i];
+            base[4 * tsz + i] = t->G1[i], base[5 * tsz + i] = t->Gz[i];
+        }
+        for (int i = threadIdx.x; i < ncol; i += blockDim.x) base[6 * tsz + i] = t->D_hi[i], base[6 * tsz + ncol + i] = t->D_lo[i];
+    }
+    __device__ dd a(int t) const { return dd{Ah[t], Al[t]}; }
+    __device__ dd b(int t) const { return dd{Bh[t], Bl[t]}; }
+    __device__ dd d(int m) const { return dd{Dh[m], Dl[m]}; }
+};
+
+__host__ __device__ inline int tpg_tab_bytes(int l_max, bool is_dd) {
+    const int tsz = (l_max + 1) * (l_max + 2) / 2, ncol = l_max + 1;
+    return (((is_dd ? 6 : 4) * tsz + (is_dd ? 2 : 1) * ncol) * 8 + 15) & ~15;
+}
+
+template <typename T, typename R, int DERIV, bool NORM, int LP>
+__global__ void __launch_bounds__(128, 4) sph_tpg_kernel(const TpgParams prm) {
+    using RT = rec<R>;
+    constexpr int PTS = 32 / LP;   // points per tile
+    constexpr int C = LP / 2;      // column classes
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    const int l_max = prm.l_max;
+    const int L = (l_max + 1) * (l_max + 1);
+    const int tsz = (l_max + 1) * (l_max + 2) / 2;
+    const int64_t n = prm.n;
+
+    // ---- coefficient tables -> shared memory (once per CTA) -----------------------------------
+    TpgTabs<R> TB;
+    TB.fill(reinterpret_cast<double*>(smem), prm.tab, tsz, l_max + 1);
+    TB.carve(reinterpret_cast<double*>(smem), tsz, l_max + 1);
+    __syncthreads();
+
+    const int64_t tile = (int64_t)blockIdx.x * prm.warps_per_cta + warp;
+    const int64_t p0 = tile * PTS;
+    if (p0 >= n) return;
+    const uint32_t S_BYTES = (uint32_t)(PTS * L * sizeof(T));
+    unsigned char* img = smem + tpg_tab_bytes(l_max, sizeof(R) == sizeof(dd)) + (size_t)warp * S_BYTES * (DERIV ? 4 : 1);
+    const int pl = lane % PTS;          // point inside the tile
+    const int role = lane / PTS;
+    const bool sinb = role & 1;         // branch
+    const int cls = role >> 1;          // column class
+    const T* __restrict__ xyz = static_cast<const T*>(prm.xyz);
+    T* __restrict__ sph = static_cast<T*>(prm.sph);
+    T* __restrict__ dsph = static_cast<T*>(prm.dsph);
+    const int64_t p = p0 + pl;
+
+    double x = 0.0, y = 0.0, z = 1.0;  // lanes past the end compute a harmless point
+    if (p < n) {
+        x = static_cast<double>(__ldg(xyz + 3 * p + 0));
+        y = static_cast<double>(__ldg(xyz + 3 * p + 1));
+        z = static_cast<double>(__ldg(xyz + 3 * p + 2));
+    }
+    R X, Y, Z, r2;
+    double rinv = 1.0;
+    if (NORM) {
+        RT::normalize(x, y, z, X, Y, Z, rinv);
+        r2 = RT::make(1.0, 0.0);
+    } else {
+        X = RT::make(x, 0.0);
+        Y = RT::make(y, 0.0);
+        Z = RT::make(z, 0.0);
+        r2 = RT::r2_of(X, Y, Z);
+    }
+    const double xd = to_double(X), yd = to_double(Y), zd = to_double(Z);
+
+    // powers of (x + i y) (Eq. 9): w^cls and w^(cls-1) to start with, w^C to advance by,
+    // w^(C-1) for the class that starts at m = 0 (its "w^(m-1)" exists from the second column on)
+    R cm = RT::make(1.0, 0.0), sm = RT::make(0.0, 0.0);     // w^m
+    R cm1 = RT::make(0.0, 0.0), sm1 = RT::make(0.0, 0.0);   // w^(m-1)
+    R cC = RT::make(1.0, 0.0), sC = RT::make(0.0, 0.0);     // w^C
+    R cCm = RT::make(1.0, 0.0), sCm = RT::make(0.0, 0.0);   // w^(C-1)
+#pragma unroll
+    for (int j = 0; j < C; ++j) {
+        if (j == cls) cm = cC, sm = sC;
+        if (j + 1 == cls) cm1 = cC, sm1 = sC;
+        if (j == C - 1) cCm = cC, sCm = sC;
+        const R cn = X * cC - Y * sC;
+        const R sn = X * sC + Y * cC;
+        cC = cn;
+        sC = sn;
+    }
+
+    T* S = reinterpret_cast<T*>(img) + pl * L;
+    T* G = reinterpret_cast<T*>(img + S_BYTES) + pl * 3 * L;
+
+    for (int m = cls; m <= l_max; m += C) {
+        const double cd = to_double(cm), sd = to_double(sm);
+        const double c1 = to_double(cm1), s1 = to_double(sm1);
+        const double dm = (double)m;
+        // azimuthal factor of this lane's branch and its x/y derivatives (Eq. 9, Eq. 10)
+        const double A = sinb ? sd : (m == 0 ? SPH_INV_SQRT2 : cd);
+        double Ax = dm * (sinb ? s1 : c1);
+        double Ay = dm * (sinb ? c1 : -s1);
+        double xA = xd * A, yA = yd * A, Az = A;
+        if (NORM && DERIV >= 1) {
+            xA *= rinv;
+            yA *= rinv;
+            Az *= rinv;
+            Ax *= rinv;
+            Ay *= rinv;
+        }
+        const bool emit = (m > 0) || !sinb;   // the sin branch has no m = 0 output
+        R q = TB.d(m);                   // Qt_l^m, starting at Qt_m^m
+        R qp = RT::make(0.0, 0.0);       // Qt_{l-1}^m
+        R pc = RT::make(0.0, 0.0);       // Qt_{l-1}^{m+1}
+        R pp = RT::make(0.0, 0.0);       // Qt_{l-2}^{m+1}
+        int k0 = m * (m + 1);            // l (l + 1)
+        for (int l = m; l <= l_max; ++l) {
+            const double Q = to_double(q);
+            const int k = sinb ? k0 - m : k0 + m;
+            if (emit) S[k] = static_cast<T>(Q * A);   // Eq. 5
+            if (DERIV >= 1) {
+                const int t = SPH_TRI(l, m);
+                const double q1 = TB.G1[t] * to_double(pc);   // F_l^m Q_{l-1}^{m+1}
+                const double qz = TB.Gz[t] * to_double(qp);   // F_l^m (l+m) Q_{l-1}^m
+                double gx, gy, gz;
+                if (NORM) {
+                    const double lQ = (double)l * Q;
+                    const double t1 = q1 - lQ;
+                    const double tz = SPH_FMA(-lQ, zd, qz);
+                    gx = SPH_FMA(t1, xA, Q * Ax);
+                    gy = SPH_FMA(t1, yA, Q * Ay);
+                    gz = tz * Az;
+                } else {
+                    gx = SPH_FMA(q1, xA, Q * Ax);
+                    gy = SPH_FMA(q1, yA, Q * Ay);
+                    gz = qz * Az;
+                }
+                if (emit) {
+                    G[k] = static_cast<T>(gx);
+                    G[L + k] = static_cast<T>(gy);
+                    G[2 * L + k] = static_cast<T>(gz);
+                }
+            }
+            if (l < l_max) {
+                const int t1 = SPH_TRI(l + 1, m);
+                R qn;
+                if (l == m) {
+                    qn = TB.a(t1) * (Z * q);
+                } else {
+                    const R w = NORM ? qp : r2 * qp;
+                    qn = TB.a(t1) * (Z * q) - TB.b(t1) * w;
+                }
+                qp = q;
+                q = qn;
+                if (DERIV >= 1) {  // column m+1 reaches row l
+                    R pn;
+                    if (l == m) {
+                        pn = RT::make(0.0, 0.0);
+                    } else if (l == m + 1) {
+                        pn = TB.d(m + 1);
+                    } else {
+                        const int t2 = SPH_TRI(l, m + 1);
+                        const R w2 = NORM ? pp : r2 * pp;
+                        pn = TB.a(t2) * (Z * pc) - TB.b(t2) * w2;
+                    }
+                    pp = pc;
+                    pc = pn;
+                }
+            }
+            k0 += 2 * (l + 1);
+        }
+        // the next column of this class: w^(m+C), w^(m+C-1)
+        if (m == 0) {
+            cm1 = cCm, sm1 = sCm;
+        } else {
+            const R cn1 = cm1 * cC - sm1 * sC;
+            const R sn1 = cm1 * sC + sm1 * cC;
+            cm1 = cn1, sm1 = sn1;
+        }
+        const R cn = cm * cC - sm * sC;
+        const R sn = cm * sC + sm * cC;
+        cm = cn, sm = sn;
+    }
+
+    fence_proxy_async_smem();
+    __syncwarp();
+    T* S0 = reinterpret_cast<T*>(img);
+    T* G0 = reinterpret_cast<T*>(img + S_BYTES);
+    if (n - p0 >= PTS) {
+        if (lane == 0) {
+            const uint64_t policy = policy_evict_first();
+            bulk_store_hint(sph + p0 * L, S0, S_BYTES, policy);
+            if (DERIV >= 1) bulk_store_hint(dsph + p0 * 3 * L, G0, 3u * S_BYTES, policy);
+            bulk_commit();
+            bulk_wait_read<0>();   // shared memory must outlive the bulk stores' reads of it
+        }
+    } else {  // ragged last tile: byte count need not be a multiple of 16 -> plain stores
+        const int np = (int)(n - p0);
+        for (int i = lane; i < np * L; i += 32) st_cs(sph + p0 * L + i, S0[i]);
+        if (DERIV >= 1)
+            for (int i = lane; i < np * 3 * L; i += 32) st_cs(dsph + p0 * 3 * L + i, G0[i]);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------
+typedef void (*TpgKernel)(const TpgParams);
+
+struct TpgLaunch {
+    const void* func;
+    TpgKernel kern;
+    TpgParams prm;
+    int64_t grid;
+    int threads;
+    size_t smem;
+};
+
+template <typename T, typename R, int LP> static TpgKernel tpg_pick2(int deriv, int norm) {
+    if (deriv == 0) return norm ? sph_tpg_kernel<T, R, 0, true, LP> : sph_tpg_kernel<T, R, 0, false, LP>;
+    return norm ? sph_tpg_kernel<T, R, 1, true, LP> : sph_tpg_kernel<T, R, 1, false, LP>;
+}
+template <typename T, typename R> static TpgKernel tpg_pick(int deriv, int norm, int lp) {
+    if (lp == 2) return tpg_pick2<T, R, 2>(deriv, norm);
+    if (lp == 4) return tpg_pick2<T, R, 4>(deriv, norm);
+    return tpg_pick2<T, R, 8>(deriv, norm);
+}
+
+static inline int tpg_env(const char* name, int dflt) {
+    const char* s = getenv(name);
+    return (s && *s) ? atoi(s) : dflt;
+}
+
+// returns 0 and fills *out if the kernel applies: values or values + gradients whose smallest tile
+// (4 points) still leaves room for several tiles per SM; 1 otherwise
+static inline int tpg_plan(int smem_optin, int64_t n, int l_max, int normalized, int dtype, void* sph, void* dsph,
+                           const void* xyz, const SphTables* d_tab, TpgLaunch* out) {
+    const int deriv = dsph ? 1 : 0;
+    const int esize = dtype == 0 ? 4 : 8;
+    const int L = (l_max + 1) * (l_max + 1);
+    const int64_t per_pt = (int64_t)L * esize * (deriv ? 4 : 1);
+    // lanes per point: the most points per tile (16, 8, 4) whose image stays under 16 KB (measured:
+    // the kernel is latency-bound, so small tiles = more warps in flight wins almost everywhere)
+    int lp = tpg_env("SPHB200_TPG_LP", 0);
+    if (lp != 2 && lp != 4 && lp != 8) {
+        lp = 2;
+        while (lp < 8 && (32 / lp) * per_pt > 16 * 1024) lp *= 2;
+    }
+    const int64_t tile_bytes = (32 / lp) * per_pt;
+    if (tile_bytes > 48 * 1024) return 1;
+    const int tab_bytes = tpg_tab_bytes(l_max, dtype != 0);
+    int warps = 4;
+    while (warps > 1 && tab_bytes + warps * tile_bytes > (smem_optin - 1024) / 2) warps >>= 1;   // >= 2 CTAs per SM
+    if (tab_bytes + warps * tile_bytes > smem_optin - 1024) return 1;
+    out->kern = dtype == 0 ? tpg_pick<float, double>(deriv, normalized, lp) : tpg_pick<double, dd>(deriv, normalized, lp);
+    out->func = (const void*)out->kern;
+    out->prm.xyz = xyz;
+    out->prm.sph = sph;
+    out->prm.dsph = dsph;
+    out->prm.tab = d_tab;
+    out->prm.n = n;
+    out->prm.l_max = l_max;
+    out->prm.warps_per_cta = warps;
+    const int pts = 32 / lp;
+    const int64_t n_tiles = (n + pts - 1) / pts;
+    out->grid = (n_tiles + warps - 1) / warps;
+    if (out->grid > 0x7fffffff) return 1;
+    out->threads = warps * 32;
+    out->smem = (size_t)tab_bytes + (size_t)warps * tile_bytes;
+    return 0;
+}
+
+static inline void tpg_launch(const TpgLaunch& lw, cudaStream_t stream) {
+    lw.kern<<<(unsigned)lw.grid, lw.threads, lw.smem, stream>>>(lw.prm);
+}
+
+}  // namespace sphb200

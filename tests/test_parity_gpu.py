@@ -286,6 +286,9 @@ def test_cooperative_kernel_long_rows(sph, oracle, dtype, monkeypatch):
         xyz = W.make_xyz("C4", n).astype(np_dt)
         s, d, h = _run_gpu(sph, xyz, l_max, normalized, grads, hess)
         _compare(oracle, xyz, l_max, normalized, dtype, s, d, h, f"wc {dtype} l_max={l_max} n={n}")
+        monkeypatch.setenv("SPHB200_FORCE_KERNEL", "wc")   # (without Hessians the default route is tpg)
+        s, d, h = _run_gpu(sph, xyz, l_max, normalized, grads, hess)
+        _compare(oracle, xyz, l_max, normalized, dtype, s, d, h, f"forced wc {dtype} l_max={l_max} n={n}")
         monkeypatch.setenv("SPHB200_FORCE_KERNEL", "w1")
         s1, d1, h1 = _run_gpu(sph, xyz, l_max, normalized, grads, hess)
         monkeypatch.delenv("SPHB200_FORCE_KERNEL")
@@ -304,6 +307,25 @@ def test_cooperative_kernel_long_rows(sph, oracle, dtype, monkeypatch):
     torch.cuda.synchronize()
     for b in bufs:
         assert torch.all(b[:32] == 777.0) and torch.all(b[-32:] == 777.0) and torch.all(b[32:-32] != 777.0)
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("lp", [2, 4, 8])
+def test_lanes_per_point_kernel(sph, oracle, dtype, lp, monkeypatch):
+    """kernel_tpg.cuh (several lanes per point, run-time l_max): forced for every l_max it can take,
+    every lanes-per-point variant, values and values + gradients, both variants, ragged n; C2-style
+    points (on the z axis, tiny r) included."""
+    np_dt = np.float32 if dtype == "f32" else np.float64
+    monkeypatch.setenv("SPHB200_FORCE_KERNEL", "tpg")
+    monkeypatch.setenv("SPHB200_TPG_LP", str(lp))
+    for l_max, n, grads, normalized in ((0, 5, True, True), (1, 33, True, False), (3, 100, False, True),
+                                        (9, 131, True, True), (10, 64, True, False), (13, 77, False, False),
+                                        (16, 203, True, True), (21, 50, False, True), (32, 37, False, False)):
+        xyz = W.make_xyz("C2" if l_max <= 10 else "C4", n).astype(np_dt)
+        before = sph.sphericart_cuda_launch_count()
+        s, d, _ = _run_gpu(sph, xyz, l_max, normalized, grads, False)
+        assert sph.sphericart_cuda_launch_count() == before + 1
+        _compare(oracle, xyz, l_max, normalized, dtype, s, d, None, f"tpg {dtype} lp={lp} l_max={l_max} n={n}")
 
 
 def test_stream_order_with_programmatic_dependent_launch(sph):
