@@ -286,6 +286,38 @@ def sweep_expand(torch, pkg, device):
     return res
 
 
+def lmax_sweep(torch, pkg, device, peak):
+    """`--lmax-sweep`: the metric's own axis -- output GB/s and points/s against l_max, f32 / f64,
+    with and without gradients (normalised harmonics, xyz ~ N(0,1), n sized for ~1.5 GB of output,
+    two rotating output sets).  One JSON object; not part of the default run."""
+    st = torch.cuda.current_stream().cuda_stream
+    rows = {}
+    for dtype, tdt, es in (("f32", torch.float32, 4), ("f64", torch.float64, 8)):
+        for grads in (False, True):
+            key = f"{dtype}_{'grads' if grads else 'values'}"
+            rows[key] = {}
+            for l_max in (1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12, 13, 14, 15, 16, 20, 24, 28, 32):
+                L = (l_max + 1) ** 2
+                per_pt = L * es * (4 if grads else 1)
+                n = int(min(4_000_000, 1.5e9 // per_pt)) // 256 * 256
+                x = torch.randn(n, 3, device=device, dtype=tdt)
+                outs = [(torch.empty((n, L), device=device, dtype=tdt),
+                         torch.empty((n, 3, L), device=device, dtype=tdt) if grads else None) for _ in range(2)]
+                fn = lambda i: pkg.sphericart_cuda_compute(x, n, l_max, 1, pkg.F32 if dtype == "f32" else pkg.F64,
+                                                           outs[i & 1][0], outs[i & 1][1], None, st)
+                for i in range(3):
+                    fn(i)
+                torch.cuda.synchronize()
+                e0, e1 = time_loop(torch, fn, 10)
+                torch.cuda.synchronize()
+                sec = e0.elapsed_time(e1) / 10 * 1e-3
+                rows[key][str(l_max)] = {"n": n, "us": round(sec * 1e6, 1), "points_per_s": n / sec,
+                                         "out_gbs": round(n * per_pt / sec / 1e9, 1),
+                                         "frac_of_measured_peak": round(n * per_pt / sec / 1e9 / peak, 3)}
+                del outs, x
+    return rows
+
+
 def time_e2e(cfg, torch, pkg, steps):
     """The same metric through the host-buffer C-ABI call: pinned host arrays in, pinned host arrays
     out, H2D + kernels + D2H inside the timed region (wall clock around a synchronous call)."""
@@ -373,6 +405,11 @@ def run_cuda(args):
     pkg.load()                                   # raises if the CUDA library is missing
     cfg = W.CONFIGS[args.workload]
     peak, peak_src = measured_peaks()
+    if args.lmax_sweep:
+        if rank == 0:
+            print(json.dumps({"lmax_sweep": lmax_sweep(torch, pkg, device, peak), "peak_gbs": peak,
+                              "peak_source": peak_src}))
+        return
     free, _ = torch.cuda.mem_get_info()
     wl = DeviceWorkload(cfg, torch, pkg, device, n_sets_for(cfg, free), seed=rank)
 
@@ -517,6 +554,8 @@ def main():
     ap.add_argument("--workload", choices=sorted(W.CONFIGS), default="C2")
     ap.add_argument("--e2e-steps", type=int, default=20)
     ap.add_argument("--no-sweep", action="store_true", help="skip the brief timing of the other configurations")
+    ap.add_argument("--lmax-sweep", action="store_true",
+                    help="print output GB/s against l_max (f32/f64, +-gradients) as one JSON object and exit")
     ap.add_argument("--kernels-only", action="store_true",
                     help="time the device-resident step only (no e2e, no oracle, no sweep): the command ncu wraps")
     args = ap.parse_args()

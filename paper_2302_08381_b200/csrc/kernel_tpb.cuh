@@ -79,7 +79,18 @@ template <int LMAX, int SPLIT> struct TpbCut {
 
 template <int ESIZE, int DERIV, int LMAX, int SPLIT> struct TpbShape {
     static constexpr int L = (LMAX + 1) * (LMAX + 1);
-    static constexpr int tile_bytes = TPB_PTS * L * ESIZE * (DERIV ? 4 : 1);
+    // Shared-memory banks: lane p writes word p * (row pitch) + k; the lanes of a branch collide 8- or
+    // 16-way when the pitch in 32-bit words is 0 or 16 modulo 32, i.e. for l_max = 3 (mod 4)
+    // (measured: f32 l_max = 7 ran at 2.0 TB/s where l_max = 6 and 8 reach 6.7 and 6.9).  Those row
+    // lengths get 16 bytes of padding per point (pitch = 4 or 20 mod 32: 2-way), the image is then
+    // no longer byte-identical to global memory and leaves by 16-byte vector stores instead of TMA.
+    static constexpr int words = L * ESIZE / 4;
+    static constexpr bool pad = (words % 32 == 0) || (words % 32 == 16);
+    static constexpr int pad_elems = pad ? 16 / ESIZE : 0;
+    static constexpr int pitch_s = L + pad_elems;          // elements between the points' rows of sph
+    static constexpr int pitch_g = 3 * L + pad_elems;      // ... of dsph
+    static constexpr int s_bytes = TPB_PTS * pitch_s * ESIZE;
+    static constexpr int tile_bytes = s_bytes + (DERIV ? TPB_PTS * pitch_g * ESIZE : 0);
     static constexpr int fit = TPB_SMEM_PER_SM / (tile_bytes + 1024);   // resident CTAs per SM by shared memory
     static constexpr int cap = 16 / SPLIT;                              // ... and by registers (<= 128 each)
     static constexpr int min_ctas = fit < 1 ? 1 : (fit < cap ? fit : cap);
@@ -93,7 +104,8 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
     using Shape = TpbShape<sizeof(T), DERIV, LMAX, SPLIT>;
     constexpr int L = Shape::L;
     constexpr int CUT = Shape::cut;
-    constexpr uint32_t S_BYTES = TPB_PTS * L * sizeof(T);
+    constexpr uint32_t S_BYTES = Shape::s_bytes;
+    constexpr int PS = Shape::pitch_s, PG = Shape::pitch_g;
     const SphTables& TB = c_tables_tpb;
     extern __shared__ __align__(128) unsigned char smem[];
     const int lane = threadIdx.x & 31;
@@ -156,8 +168,8 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
             if (threadIdx.x == 0) bulk_wait_read<0>();
             cta_sync();
         }
-        T* S = reinterpret_cast<T*>(smem) + pl * L;
-        T* G = reinterpret_cast<T*>(smem + S_BYTES) + pl * 3 * L;
+        T* S = reinterpret_cast<T*>(smem) + pl * PS;
+        T* G = reinterpret_cast<T*>(smem + S_BYTES) + pl * PG;
 
         double Qc[LMAX + 1];   // column m:   Qc[l] = Qt_l^m     (0 for l < m)
         double Qn[LMAX + 1];   // column m+1: Qn[l] = Qt_l^{m+1} (0 for l < m+1)
@@ -273,7 +285,23 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
         const int64_t p0 = tile * TPB_PTS;
         T* S0 = reinterpret_cast<T*>(smem);
         T* G0 = reinterpret_cast<T*>(smem + S_BYTES);
-        if (n - p0 >= TPB_PTS) {
+        if constexpr (Shape::pad) {
+            // padded image: rows leave as 16-byte vectors (row lengths are multiples of 16 bytes here)
+            constexpr int VE = 16 / (int)sizeof(T);        // elements per vector
+            const int np = (int)((n - p0 < TPB_PTS) ? n - p0 : TPB_PTS);
+            constexpr int VS = L / VE, VG = 3 * L / VE;    // vectors per point
+            for (int i = threadIdx.x; i < np * VS; i += SPLIT * 32) {
+                const int r = i / VS, v = i - r * VS;
+                __stcs(reinterpret_cast<float4*>(sph + (p0 + r) * L) + v, reinterpret_cast<const float4*>(S0 + r * PS)[v]);
+            }
+            if (DERIV >= 1)
+                for (int i = threadIdx.x; i < np * VG; i += SPLIT * 32) {
+                    const int r = i / VG, v = i - r * VG;
+                    __stcs(reinterpret_cast<float4*>(dsph + (p0 + r) * 3 * L) + v,
+                           reinterpret_cast<const float4*>(G0 + r * PG)[v]);
+                }
+            cta_sync();
+        } else if (n - p0 >= TPB_PTS) {
             if (threadIdx.x == 0) {
                 bulk_store_hint(sph + p0 * L, S0, S_BYTES, policy);
                 if (DERIV >= 1) bulk_store_hint(dsph + p0 * 3 * L, G0, 3u * S_BYTES, policy);

@@ -69,6 +69,18 @@ template <> struct TpgTabs<dd> {
     __device__ dd d(int m) const { return dd{Dh[m], Dl[m]}; }
 };
 
+// bytes of one tile's image; rows whose pitch in 32-bit words would be 0 or 16 modulo 32
+// (l_max = 3 mod 4) get 16 bytes of padding per point against 8/16-way bank conflicts, and such an
+// image leaves by vector stores instead of TMA (see TpbShape in kernel_tpb.cuh)
+__host__ __device__ inline int tpg_pad_elems(int L, int esize) {
+    const int words = L * esize / 4;
+    return (words % 32 == 0 || words % 32 == 16) ? 16 / esize : 0;
+}
+__host__ __device__ inline int tpg_tile_bytes(int pts, int L, int esize, int deriv) {
+    const int pe = tpg_pad_elems(L, esize);
+    return pts * (L + pe) * esize + (deriv ? pts * (3 * L + pe) * esize : 0);
+}
+
 __host__ __device__ inline int tpg_tab_bytes(int l_max, bool is_dd) {
     const int tsz = (l_max + 1) * (l_max + 2) / 2, ncol = l_max + 1;
     return (((is_dd ? 6 : 4) * tsz + (is_dd ? 2 : 1) * ncol) * 8 + 15) & ~15;
@@ -96,8 +108,11 @@ __global__ void __launch_bounds__(128, 4) sph_tpg_kernel(const TpgParams prm) {
     const int64_t tile = (int64_t)blockIdx.x * prm.warps_per_cta + warp;
     const int64_t p0 = tile * PTS;
     if (p0 >= n) return;
-    const uint32_t S_BYTES = (uint32_t)(PTS * L * sizeof(T));
-    unsigned char* img = smem + tpg_tab_bytes(l_max, sizeof(R) == sizeof(dd)) + (size_t)warp * S_BYTES * (DERIV ? 4 : 1);
+    const int pad_e = tpg_pad_elems(L, (int)sizeof(T));
+    const int PS = L + pad_e, PG = 3 * L + pad_e;   // elements between the points' rows of sph / dsph
+    const uint32_t S_BYTES = (uint32_t)(PTS * PS * sizeof(T));
+    unsigned char* img = smem + tpg_tab_bytes(l_max, sizeof(R) == sizeof(dd)) +
+                         (size_t)warp * tpg_tile_bytes(PTS, L, (int)sizeof(T), DERIV);
     const int pl = lane % PTS;          // point inside the tile
     const int role = lane / PTS;
     const bool sinb = role & 1;         // branch
@@ -143,8 +158,8 @@ __global__ void __launch_bounds__(128, 4) sph_tpg_kernel(const TpgParams prm) {
         sC = sn;
     }
 
-    T* S = reinterpret_cast<T*>(img) + pl * L;
-    T* G = reinterpret_cast<T*>(img + S_BYTES) + pl * 3 * L;
+    T* S = reinterpret_cast<T*>(img) + pl * PS;
+    T* G = reinterpret_cast<T*>(img + S_BYTES) + pl * PG;
 
     for (int m = cls; m <= l_max; m += C) {
         const double cd = to_double(cm), sd = to_double(sm);
@@ -167,13 +182,16 @@ __global__ void __launch_bounds__(128, 4) sph_tpg_kernel(const TpgParams prm) {
         R qp = RT::make(0.0, 0.0);       // Qt_{l-1}^m
         R pc = RT::make(0.0, 0.0);       // Qt_{l-1}^{m+1}
         R pp = RT::make(0.0, 0.0);       // Qt_{l-2}^{m+1}
-        int k0 = m * (m + 1);            // l (l + 1)
+        // running indices: t = TRI(l, m) (so TRI(l+1, m) = t + l + 1 and TRI(l, m+1) = t + 1) and
+        // this lane's output index k = l (l + 1) +- m, which advances by 2 (l + 1)
+        int t = SPH_TRI(m, m);
+        int k = m * (m + 1) + (sinb ? -m : m);
+        T* Sk = S + k;
+        T* Gk = G + k;
         for (int l = m; l <= l_max; ++l) {
             const double Q = to_double(q);
-            const int k = sinb ? k0 - m : k0 + m;
-            if (emit) S[k] = static_cast<T>(Q * A);   // Eq. 5
+            if (emit) *Sk = static_cast<T>(Q * A);   // Eq. 5
             if (DERIV >= 1) {
-                const int t = SPH_TRI(l, m);
                 const double q1 = TB.G1[t] * to_double(pc);   // F_l^m Q_{l-1}^{m+1}
                 const double qz = TB.Gz[t] * to_double(qp);   // F_l^m (l+m) Q_{l-1}^m
                 double gx, gy, gz;
@@ -190,13 +208,13 @@ __global__ void __launch_bounds__(128, 4) sph_tpg_kernel(const TpgParams prm) {
                     gz = qz * Az;
                 }
                 if (emit) {
-                    G[k] = static_cast<T>(gx);
-                    G[L + k] = static_cast<T>(gy);
-                    G[2 * L + k] = static_cast<T>(gz);
+                    Gk[0] = static_cast<T>(gx);
+                    Gk[L] = static_cast<T>(gy);
+                    Gk[2 * L] = static_cast<T>(gz);
                 }
             }
             if (l < l_max) {
-                const int t1 = SPH_TRI(l + 1, m);
+                const int t1 = t + l + 1;   // TRI(l + 1, m)
                 R qn;
                 if (l == m) {
                     qn = TB.a(t1) * (Z * q);
@@ -213,15 +231,16 @@ __global__ void __launch_bounds__(128, 4) sph_tpg_kernel(const TpgParams prm) {
                     } else if (l == m + 1) {
                         pn = TB.d(m + 1);
                     } else {
-                        const int t2 = SPH_TRI(l, m + 1);
                         const R w2 = NORM ? pp : r2 * pp;
-                        pn = TB.a(t2) * (Z * pc) - TB.b(t2) * w2;
+                        pn = TB.a(t + 1) * (Z * pc) - TB.b(t + 1) * w2;   // TRI(l, m + 1) = t + 1
                     }
                     pp = pc;
                     pc = pn;
                 }
             }
-            k0 += 2 * (l + 1);
+            t += l + 1;
+            Sk += 2 * (l + 1);
+            Gk += 2 * (l + 1);
         }
         // the next column of this class: w^(m+C), w^(m+C-1)
         if (m == 0) {
@@ -240,7 +259,21 @@ __global__ void __launch_bounds__(128, 4) sph_tpg_kernel(const TpgParams prm) {
     __syncwarp();
     T* S0 = reinterpret_cast<T*>(img);
     T* G0 = reinterpret_cast<T*>(img + S_BYTES);
-    if (n - p0 >= PTS) {
+    if (pad_e) {
+        // padded image: rows leave as 16-byte vectors (row lengths are multiples of 16 bytes here)
+        const int VE = 16 / (int)sizeof(T);
+        const int np = (int)((n - p0 < PTS) ? n - p0 : PTS);
+        const int VS = L / VE, VG = 3 * L / VE;
+        for (int i = lane; i < np * VS; i += 32) {
+            const int r = i / VS, v = i - r * VS;
+            __stcs(reinterpret_cast<float4*>(sph + (p0 + r) * L) + v, reinterpret_cast<const float4*>(S0 + r * PS)[v]);
+        }
+        if (DERIV >= 1)
+            for (int i = lane; i < np * VG; i += 32) {
+                const int r = i / VG, v = i - r * VG;
+                __stcs(reinterpret_cast<float4*>(dsph + (p0 + r) * 3 * L) + v, reinterpret_cast<const float4*>(G0 + r * PG)[v]);
+            }
+    } else if (n - p0 >= PTS) {
         if (lane == 0) {
             const uint64_t policy = policy_evict_first();
             bulk_store_hint(sph + p0 * L, S0, S_BYTES, policy);
@@ -300,7 +333,7 @@ static inline int tpg_plan(int smem_optin, int64_t n, int l_max, int normalized,
         lp = 2;
         while (lp < 8 && (32 / lp) * per_pt > 16 * 1024) lp *= 2;
     }
-    const int64_t tile_bytes = (32 / lp) * per_pt;
+    const int64_t tile_bytes = tpg_tile_bytes(32 / lp, L, esize, deriv);
     if (tile_bytes > 48 * 1024) return 1;
     const int tab_bytes = tpg_tab_bytes(l_max, dtype != 0);
     int warps = 4;
