@@ -115,11 +115,13 @@ int TPB_NAME(sph_tpb_launch)(int sm_count, const void* xyz, int64_t n, int l_max
         TPB_CASE(6)
         TPB_CASE(7)
         TPB_CASE(8)
-#if !TPB_DERIV && !TPB_F64   // long value-only rows: f32 only (C3 is l_max = 16)
+#if !TPB_F64 || !TPB_DERIV    // f32 (C3 is l_max = 16 values) and f64 values: up to l_max = 16 / 12
         TPB_CASE(9)
         TPB_CASE(10)
         TPB_CASE(11)
         TPB_CASE(12)
+#endif
+#if !TPB_F64
         TPB_CASE(13)
         TPB_CASE(14)
         TPB_CASE(15)
