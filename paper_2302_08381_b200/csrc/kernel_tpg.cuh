@@ -188,6 +188,7 @@ __global__ void __launch_bounds__(128, 4) sph_tpg_kernel(const TpgParams prm) {
         int k = m * (m + 1) + (sinb ? -m : m);
         T* Sk = S + k;
         T* Gk = G + k;
+#pragma unroll 2
         for (int l = m; l <= l_max; ++l) {
             const double Q = to_double(q);
             if (emit) *Sk = static_cast<T>(Q * A);   // Eq. 5
