@@ -37,7 +37,6 @@ template <int LMAX, int NRAD_MAX> static int launch_nr(int smem_optin, ExpandPar
 }
 
 template <int LMAX> static int launch_one(int smem_optin, const ExpandParams& prm, cudaStream_t stream) {
-    if (prm.n_rad <= 4) return launch_nr<LMAX, 4>(smem_optin, prm, stream);
     if (prm.n_rad <= 8) return launch_nr<LMAX, 8>(smem_optin, prm, stream);
     if (prm.n_rad <= EXP_MAX_RAD) return launch_nr<LMAX, EXP_MAX_RAD>(smem_optin, prm, stream);
     return 1;

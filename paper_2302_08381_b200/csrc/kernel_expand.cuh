@@ -14,9 +14,15 @@
 //      runs in f64 and reads every radial value 2l+1 times (ncu on the first version, which widened
 //      each operand where it was used: the XU pipe of the f32->f64 conversions 63 % busy, the top
 //      pipe of the kernel);
-//   2. lane = harmonic index lm (ceil(L/32) passes): acc[pass][n] += R[p][n][l(lm)] * Y[p][lm] over
-//      the tile's points, in f64 registers;
-// and at the end of the segment the accumulators go out, coalesced along lm.
+//   2. the contraction over the tile's points is, for every degree l, a small dense product
+//          C_l [n_rad x (2l+1)]  +=  R_l^T [n_rad x 16]  .  Y_l [16 x (2l+1)]
+//      and runs on the f64 tensor-core path: mma.sync m8n8k4 (SASS DMMA), M = radial index n, N = 8
+//      consecutive m of one l, K = 4 points per step; fragments come straight from the two images,
+//      accumulators stay in registers for the whole segment.  (Measured on B200: DMMA sustains the
+//      same 18 T FMA/s as DFMA, but one instruction does 256 FMAs instead of 32 and needs 2 operand
+//      loads instead of 2 per 32: the first version of this kernel, lane = harmonic with one LDS per
+//      DFMA, was bound by the LSU pipe and by issue slots, not by f64 throughput.)
+// At the end of the segment the accumulators go out.
 #pragma once
 #include "kernel_tpb.cuh"
 
@@ -32,7 +38,26 @@ struct ExpandParams {
     int warps_per_cta;
 };
 
-constexpr int EXP_MAX_RAD = 16;   // accumulators per pass held in registers
+constexpr int EXP_MAX_RAD = 16;   // two M-tiles of 8 radial indices
+
+// N-tiles of the contraction: degree l has ceil((2l+1)/8) tiles of 8 consecutive m
+template <int LMAX> struct ExpandTiles {
+    __host__ __device__ static constexpr int of(int l) { return (2 * l + 1 + 7) / 8; }
+    __host__ __device__ static constexpr int first(int l) {
+        int s = 0;
+        for (int i = 0; i < l; ++i) s += of(i);
+        return s;
+    }
+    static constexpr int total = first(LMAX + 1);
+};
+
+// D (8x8, f64) += A (8x4, row) * B (4x8, col): lane holds A[lane/4][lane%4], B[lane%4][lane/4],
+// D[lane/4][2 (lane%4) + {0,1}]
+__device__ __forceinline__ void dmma_m8n8k4(double (&d)[2], double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(d[0]), "+d"(d[1])
+                 : "d"(a), "d"(b));
+}
 
 template <int ESIZE, int LMAX> struct ExpandShape {
     static constexpr int L = (LMAX + 1) * (LMAX + 1);
@@ -52,7 +77,6 @@ __global__ void __launch_bounds__(128) sph_expand_kernel(const ExpandParams prm)
     using RT = rec<R>;
     using Shape = ExpandShape<sizeof(T), LMAX>;
     constexpr int L = Shape::L;
-    constexpr int PASSES = Shape::passes;
     const SphTables& TB = c_tables_tpb;
     extern __shared__ __align__(128) unsigned char smem[];
     const int lane = threadIdx.x & 31;
@@ -71,27 +95,22 @@ __global__ void __launch_bounds__(128) sph_expand_kernel(const ExpandParams prm)
     const int64_t k_begin = prm.seg_ptr[seg], k_end = prm.seg_ptr[seg + 1];
     const int rstride = n_rad * (LMAX + 1);   // radial values per point
 
-    // this lane's harmonics in the accumulation: lm = lane + 32 pass, and their degree l
-    int l_of[PASSES];
+    using Tiles = ExpandTiles<LMAX>;
+    constexpr int MT = NRAD_MAX / 8;   // M-tiles
+    constexpr int NT = Tiles::total;   // N-tiles
+    const int fr = lane >> 2, fk = lane & 3;   // fragment coordinates of this lane
+    double acc[MT][NT][2];
 #pragma unroll
-    for (int ps = 0; ps < PASSES; ++ps) {
-        const int lm = lane + 32 * ps;
-        int l = (int)sqrtf((float)lm);
-        l += ((l + 1) * (l + 1) <= lm);
-        l -= (l * l > lm);
-        l_of[ps] = lm < L ? l : 0;
-    }
-    double acc[PASSES][NRAD_MAX];
+    for (int mt = 0; mt < MT; ++mt)
 #pragma unroll
-    for (int ps = 0; ps < PASSES; ++ps)
-#pragma unroll
-        for (int nr = 0; nr < NRAD_MAX; ++nr) acc[ps][nr] = 0.0;
+        for (int t = 0; t < NT; ++t) acc[mt][t][0] = acc[mt][t][1] = 0.0;
 
     for (int64_t k0 = k_begin; k0 < k_end; k0 += TPB_PTS) {
         const int np = (int)((k_end - k0 < TPB_PTS) ? k_end - k0 : TPB_PTS);
         __syncwarp();   // the previous tile's accumulation is done with both images
         // ---- radial values of the tile: one contiguous range -----------------------------------
         for (int i = lane; i < np * rstride; i += 32) Rs[i] = static_cast<double>(__ldg(radial + k0 * rstride + i));
+        for (int i = np * rstride + lane; i < TPB_PTS * rstride; i += 32) Rs[i] = 0.0;   // absent points contribute 0
         // ---- harmonics of the tile: two lanes per point ----------------------------------------
         double x = 0.0, y = 0.0, z = 1.0;  // lanes past the end compute a harmless point
         if (pl < np) {
@@ -139,31 +158,48 @@ __global__ void __launch_bounds__(128) sph_expand_kernel(const ExpandParams prm)
             }
         });
         __syncwarp();
-        // ---- accumulate: lane = harmonic, over the tile's points --------------------------------
-        for (int p = 0; p < np; ++p) {
+        // ---- contract over the tile's points, 4 at a time (K of the DMMA) --------------------------
+        // What a fragment reads outside the valid ranges (n >= n_rad: the next point's radial values
+        // or the padding; m beyond 2l+1: the next degree's harmonics) only reaches rows / columns of
+        // C that are never stored.
 #pragma unroll
-            for (int ps = 0; ps < PASSES; ++ps) {
-                const int lm = lane + 32 * ps;
-                if (lm < L) {
-                    const double yv = static_cast<double>(Ys[p * L + lm]);
-                    const double* rp = Rs + p * rstride + l_of[ps];
+        for (int ks = 0; ks < TPB_PTS / 4; ++ks) {
+            if (4 * ks < np) {
+                const int p = 4 * ks + fk;
+                static_for<0, LMAX + 1>([&](auto lc) {
+                    constexpr int l = decltype(lc)::value;
+                    double a[MT];
 #pragma unroll
-                    for (int nr = 0; nr < NRAD_MAX; ++nr) acc[ps][nr] = fma(rp[nr * (LMAX + 1)], yv, acc[ps][nr]);
+                    for (int mt = 0; mt < MT; ++mt) a[mt] = Rs[p * rstride + (fr + 8 * mt) * (LMAX + 1) + l];
+                    constexpr int NTL = Tiles::of(l), T0 = Tiles::first(l);
+                    static_for<0, NTL>([&](auto tc) {
+                        constexpr int t = decltype(tc)::value;
+                        const double bv = static_cast<double>(Ys[p * L + l * l + 8 * t + fr]);
+#pragma unroll
+                        for (int mt = 0; mt < MT; ++mt) dmma_m8n8k4(acc[mt][T0 + t], a[mt], bv);
+                    });
+                });
+            }
+        }
+    }
+    // ---- c[seg, n, lm]: lane holds C[n = fr + 8 mt][m-index 8 t + 2 fk + {0, 1}] of every tile ------
+    static_for<0, LMAX + 1>([&](auto lc) {
+        constexpr int l = decltype(lc)::value;
+        constexpr int NTL = Tiles::of(l), T0 = Tiles::first(l);
+        static_for<0, NTL>([&](auto tc) {
+            constexpr int t = decltype(tc)::value;
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt) {
+                const int n = fr + 8 * mt;
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int j = 8 * t + 2 * fk + e;
+                    if (n < n_rad && j < 2 * l + 1)
+                        coeff[(seg * n_rad + n) * L + l * l + j] = static_cast<T>(acc[mt][T0 + t][e]);
                 }
             }
-        }
-    }
-    // ---- c[seg, n, lm], coalesced along lm ----------------------------------------------------------
-#pragma unroll
-    for (int nr = 0; nr < NRAD_MAX; ++nr) {
-        if (nr < n_rad) {
-#pragma unroll
-            for (int ps = 0; ps < PASSES; ++ps) {
-                const int lm = lane + 32 * ps;
-                if (lm < L) coeff[(seg * n_rad + nr) * L + lm] = static_cast<T>(acc[ps][nr]);
-            }
-        }
-    }
+        });
+    });
 }
 
 }  // namespace sphb200
