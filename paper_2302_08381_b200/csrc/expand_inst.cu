@@ -30,7 +30,8 @@ template <int LMAX, int NRAD_MAX> static int launch_nr(int smem_optin, ExpandPar
     if (smem > smem_optin - 1024) return 1;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return -1;
     prm.warps_per_cta = warps;
-    const int64_t ctas = (prm.n_seg + warps - 1) / warps;
+    const int64_t per_cta = (int64_t)warps * EXP_SPW;   // segments per CTA
+    const int64_t ctas = (prm.n_seg + per_cta - 1) / per_cta;
     if (ctas > 0x7fffffff) return 1;
     kern<<<(unsigned)ctas, warps * 32, smem, stream>>>(prm);
     return cudaGetLastError() == cudaSuccess ? 0 : -1;

@@ -39,6 +39,7 @@ struct ExpandParams {
 };
 
 constexpr int EXP_MAX_RAD = 16;   // two M-tiles of 8 radial indices
+constexpr int EXP_SPW = 4;        // consecutive segments one warp works through
 
 // N-tiles of the contraction: degree l has ceil((2l+1)/8) tiles of 8 consecutive m
 template <int LMAX> struct ExpandTiles {
@@ -62,14 +63,18 @@ __device__ __forceinline__ void dmma_m8n8k4(double (&d)[2], double a, double b) 
 template <int ESIZE, int LMAX> struct ExpandShape {
     static constexpr int L = (LMAX + 1) * (LMAX + 1);
     static constexpr int passes = (L + 31) / 32;
-    // per warp: Y image [16][L] in the I/O type + radial image [16][n_rad][LMAX+1] in double, the
-    // latter followed by nrad_max rows of padding (the unrolled contraction reads nrad_max rows per
-    // point whatever n_rad is; what it reads past n_rad only feeds accumulators that are dropped)
+    // per warp: Y image [16][L] + TWO radial images [16][n_rad][LMAX+1], all in the I/O type (the
+    // next tile's radial values arrive by cp.async while this tile is evaluated and contracted),
+    // each radial image followed by nrad_max rows of padding (the unrolled contraction reads
+    // nrad_max rows per point whatever n_rad is; what it reads past n_rad only reaches rows of C
+    // that are dropped), + the warp's segment offsets
     static constexpr int y_bytes = (TPB_PTS * L * ESIZE + 15) & ~15;
     __host__ __device__ static constexpr int r_bytes(int n_rad, int nrad_max) {
-        return (TPB_PTS * n_rad + nrad_max) * (LMAX + 1) * 8;
+        return ((TPB_PTS * n_rad + nrad_max) * (LMAX + 1) * ESIZE + 15) & ~15;
     }
-    __host__ __device__ static constexpr int warp_bytes(int n_rad, int nrad_max) { return y_bytes + r_bytes(n_rad, nrad_max); }
+    __host__ __device__ static constexpr int warp_bytes(int n_rad, int nrad_max) {
+        return y_bytes + 2 * r_bytes(n_rad, nrad_max) + (EXP_SPW + 1) * 8 + 8;
+    }
 };
 
 template <typename T, typename R, int LMAX, int NRAD_MAX>
@@ -82,18 +87,26 @@ __global__ void __launch_bounds__(128) sph_expand_kernel(const ExpandParams prm)
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
     const int n_rad = prm.n_rad;
-    const int64_t seg = (int64_t)blockIdx.x * prm.warps_per_cta + warp;
-    if (seg >= prm.n_seg) return;
+    const int64_t seg0 = ((int64_t)blockIdx.x * prm.warps_per_cta + warp) * EXP_SPW;
+    if (seg0 >= prm.n_seg) return;
     unsigned char* my = smem + (size_t)warp * Shape::warp_bytes(n_rad, NRAD_MAX);
     T* Ys = reinterpret_cast<T*>(my);
-    double* Rs = reinterpret_cast<double*>(my + Shape::y_bytes);
+    T* Rbuf[2] = {reinterpret_cast<T*>(my + Shape::y_bytes),
+                  reinterpret_cast<T*>(my + Shape::y_bytes + Shape::r_bytes(n_rad, NRAD_MAX))};
+    int64_t* sp = reinterpret_cast<int64_t*>(my + Shape::y_bytes + 2 * Shape::r_bytes(n_rad, NRAD_MAX));
     const int pl = lane & (TPB_PTS - 1);   // point inside the tile
     const bool sinb = lane >= TPB_PTS;     // branch
     const T* __restrict__ xyz = static_cast<const T*>(prm.xyz);
     const T* __restrict__ radial = static_cast<const T*>(prm.radial);
     T* __restrict__ coeff = static_cast<T*>(prm.coeff);
-    const int64_t k_begin = prm.seg_ptr[seg], k_end = prm.seg_ptr[seg + 1];
     const int rstride = n_rad * (LMAX + 1);   // radial values per point
+    // this warp's segments j = 0 .. EXP_SPW-1 are the points sp[j] .. sp[j+1]-1 (segments past the
+    // end are empty)
+    if (lane <= EXP_SPW) {
+        const int64_t sidx = seg0 + lane < prm.n_seg ? seg0 + lane : prm.n_seg;
+        sp[lane] = prm.seg_ptr[sidx];
+    }
+    __syncwarp();
 
     using Tiles = ExpandTiles<LMAX>;
     constexpr int MT = NRAD_MAX / 8;   // M-tiles
@@ -105,19 +118,81 @@ __global__ void __launch_bounds__(128) sph_expand_kernel(const ExpandParams prm)
 #pragma unroll
         for (int t = 0; t < NT; ++t) acc[mt][t][0] = acc[mt][t][1] = 0.0;
 
-    for (int64_t k0 = k_begin; k0 < k_end; k0 += TPB_PTS) {
-        const int np = (int)((k_end - k0 < TPB_PTS) ? k_end - k0 : TPB_PTS);
-        __syncwarp();   // the previous tile's accumulation is done with both images
-        // ---- radial values of the tile: one contiguous range -----------------------------------
-        for (int i = lane; i < np * rstride; i += 32) Rs[i] = static_cast<double>(__ldg(radial + k0 * rstride + i));
-        for (int i = np * rstride + lane; i < TPB_PTS * rstride; i += 32) Rs[i] = 0.0;   // absent points contribute 0
-        // ---- harmonics of the tile: two lanes per point ----------------------------------------
-        double x = 0.0, y = 0.0, z = 1.0;  // lanes past the end compute a harmless point
-        if (pl < np) {
-            x = static_cast<double>(__ldg(xyz + 3 * (k0 + pl) + 0));
-            y = static_cast<double>(__ldg(xyz + 3 * (k0 + pl) + 1));
-            z = static_cast<double>(__ldg(xyz + 3 * (k0 + pl) + 2));
+    auto zero_acc = [&]() {
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+            for (int t = 0; t < NT; ++t) acc[mt][t][0] = acc[mt][t][1] = 0.0;
+    };
+    // c[seg, n, lm] of segment j: lane holds C[n = fr + 8 mt][m-index 8 t + 2 fk + {0, 1}] of every tile
+    auto flush = [&](int j) {
+        const int64_t seg = seg0 + j;
+        static_for<0, LMAX + 1>([&](auto lc) {
+            constexpr int l = decltype(lc)::value;
+            constexpr int NTL = Tiles::of(l), T0 = Tiles::first(l);
+            static_for<0, NTL>([&](auto tc) {
+                constexpr int t = decltype(tc)::value;
+#pragma unroll
+                for (int mt = 0; mt < MT; ++mt) {
+                    const int n = fr + 8 * mt;
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        const int jm = 8 * t + 2 * fk + e;
+                        if (n < n_rad && jm < 2 * l + 1)
+                            coeff[(seg * n_rad + n) * L + l * l + jm] = static_cast<T>(acc[mt][T0 + t][e]);
+                    }
+                }
+            });
+        });
+    };
+    // the tiles of this warp in order: (segment j, first point k0); advance() steps to the next one
+    // (j == EXP_SPW: none left).  Empty segments are skipped here and zero-filled at the end.
+    auto settle = [&](int& j, int64_t& k0) {
+        while (j < EXP_SPW && k0 >= sp[j + 1]) {
+            ++j;
+            if (j < EXP_SPW) k0 = sp[j];
         }
+    };
+    // inputs of a tile: radial values by cp.async into image b (absent points' rows zeroed: they
+    // contribute 0), xyz into registers
+    auto fetch = [&](int j, int64_t k0, int b, T& xa, T& ya, T& za) {
+        const int np = (int)((sp[j + 1] - k0 < TPB_PTS) ? sp[j + 1] - k0 : TPB_PTS);
+        T* dst = Rbuf[b];
+        for (int i = lane; i < np * rstride; i += 32) cp_async_elem(dst + i, radial + k0 * rstride + i);
+        cp_async_commit();
+        for (int i = np * rstride + lane; i < TPB_PTS * rstride; i += 32) dst[i] = T(0);
+        xa = T(0), ya = T(0), za = T(1);   // lanes past the end compute a harmless point
+        if (pl < np) {
+            xa = __ldg(xyz + 3 * (k0 + pl) + 0);
+            ya = __ldg(xyz + 3 * (k0 + pl) + 1);
+            za = __ldg(xyz + 3 * (k0 + pl) + 2);
+        }
+    };
+
+    int j = 0;
+    int64_t k0 = sp[0];
+    settle(j, k0);
+    T xn = T(0), yn = T(0), zn = T(1);
+    int buf = 0;
+    if (j < EXP_SPW) fetch(j, k0, 0, xn, yn, zn);
+    zero_acc();
+    while (j < EXP_SPW) {
+        const int np = (int)((sp[j + 1] - k0 < TPB_PTS) ? sp[j + 1] - k0 : TPB_PTS);
+        const double x = static_cast<double>(xn), y = static_cast<double>(yn), z = static_cast<double>(zn);
+        const T* Rs = Rbuf[buf];
+        // the next tile (of this segment or of the warp's next non-empty one): its inputs are in
+        // flight while this tile is evaluated and contracted
+        int jn = j;
+        int64_t kn = k0 + TPB_PTS;
+        settle(jn, kn);
+        __syncwarp();   // the previous tile's contraction is done with the Y image and the other R image
+        if (jn < EXP_SPW) {
+            fetch(jn, kn, buf ^ 1, xn, yn, zn);
+            cp_async_wait_but_one();
+        } else {
+            cp_async_wait_all();
+        }
+        // ---- harmonics of the tile: two lanes per point ----------------------------------------
         R X, Y, Z;
         double rinv;
         RT::normalize(x, y, z, X, Y, Z, rinv);
@@ -170,7 +245,7 @@ __global__ void __launch_bounds__(128) sph_expand_kernel(const ExpandParams prm)
                     constexpr int l = decltype(lc)::value;
                     double a[MT];
 #pragma unroll
-                    for (int mt = 0; mt < MT; ++mt) a[mt] = Rs[p * rstride + (fr + 8 * mt) * (LMAX + 1) + l];
+                    for (int mt = 0; mt < MT; ++mt) a[mt] = static_cast<double>(Rs[p * rstride + (fr + 8 * mt) * (LMAX + 1) + l]);
                     constexpr int NTL = Tiles::of(l), T0 = Tiles::first(l);
                     static_for<0, NTL>([&](auto tc) {
                         constexpr int t = decltype(tc)::value;
@@ -181,25 +256,19 @@ __global__ void __launch_bounds__(128) sph_expand_kernel(const ExpandParams prm)
                 });
             }
         }
+            if (jn != j) {   // the segment is complete
+            flush(j);
+            zero_acc();
+        }
+        j = jn;
+        k0 = kn;
+        buf ^= 1;
     }
-    // ---- c[seg, n, lm]: lane holds C[n = fr + 8 mt][m-index 8 t + 2 fk + {0, 1}] of every tile ------
-    static_for<0, LMAX + 1>([&](auto lc) {
-        constexpr int l = decltype(lc)::value;
-        constexpr int NTL = Tiles::of(l), T0 = Tiles::first(l);
-        static_for<0, NTL>([&](auto tc) {
-            constexpr int t = decltype(tc)::value;
-#pragma unroll
-            for (int mt = 0; mt < MT; ++mt) {
-                const int n = fr + 8 * mt;
-#pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    const int j = 8 * t + 2 * fk + e;
-                    if (n < n_rad && j < 2 * l + 1)
-                        coeff[(seg * n_rad + n) * L + l * l + j] = static_cast<T>(acc[mt][T0 + t][e]);
-                }
-            }
-        });
-    });
+    // empty segments: zeros
+    for (int je = 0; je < EXP_SPW; ++je) {
+        if (seg0 + je < prm.n_seg && sp[je] == sp[je + 1])
+            for (int i = lane; i < n_rad * L; i += 32) coeff[(seg0 + je) * n_rad * L + i] = T(0);
+    }
 }
 
 }  // namespace sphb200
