@@ -23,8 +23,8 @@ OBJ_DIR = PKG / "build"
 
 # (object name, source, extra defines)
 UNITS = [("api", CSRC / "api.cu", []), ("tables", CSRC / "tables.cpp", [])] + [
-    (f"tpb_f{64 if f64 else 32}_{'g' if deriv else 'v'}", CSRC / "tpb_inst.cu", [f"-DTPB_F64={f64}", f"-DTPB_DERIV={deriv}"])
-    for f64 in (0, 1) for deriv in (0, 1)] + [
+    (f"tpb_f{64 if f64 else 32}_{'vgh'[deriv]}", CSRC / "tpb_inst.cu", [f"-DTPB_F64={f64}", f"-DTPB_DERIV={deriv}"])
+    for f64 in (0, 1) for deriv in (0, 1, 2)] + [
     (f"vjpr_f{64 if f64 else 32}", CSRC / "vjpr_inst.cu", [f"-DVJPR_F64={f64}"]) for f64 in (0, 1)] + [
     (f"expand_f{64 if f64 else 32}", CSRC / "expand_inst.cu", [f"-DEXPAND_F64={f64}"]) for f64 in (0, 1)]
 

@@ -71,6 +71,7 @@ static int device_state(DeviceState** out) {
         CUDA_TRY(cudaMemcpyToSymbol(c_tables, &g_host_tables, sizeof(SphTables)));
         if (sph_tpb_upload_f32_v(&g_host_tables) || sph_tpb_upload_f32_g(&g_host_tables) ||
             sph_tpb_upload_f64_v(&g_host_tables) || sph_tpb_upload_f64_g(&g_host_tables) ||
+            sph_tpb_upload_f32_h(&g_host_tables) || sph_tpb_upload_f64_h(&g_host_tables) ||
             sph_vjpr_upload_f32(&g_host_tables) || sph_vjpr_upload_f64(&g_host_tables) ||
             sph_expand_upload_f32(&g_host_tables) || sph_expand_upload_f64(&g_host_tables))
             return fail(SPHERICART_CUDA_ECUDA, "table upload failed: %s", cudaGetErrorString(cudaGetLastError()));
@@ -180,7 +181,7 @@ static int launch_w(const DeviceState& st, const void* xyz, int64_t n, int l_max
     if (!(force && force[0] == 'w' && force[1] == '1')) {
         // long rows: the warps of a CTA share one point, chunks of half a row, ~4 KB bulk stores
         WcLaunch lc{};
-        if (wc_plan(st.smem_optin, n, l_max, normalized, dtype, sph, dsph, ddsph, xyz, st.d_tables, &lc) == 0) {
+        if (wc_plan(st.sm_count, st.smem_optin, n, l_max, normalized, dtype, sph, dsph, ddsph, xyz, st.d_tables, &lc) == 0) {
             int rc = allow_smem(lc.func, (int)lc.smem);
             if (rc) return rc;
             wc_launch(lc, stream);
@@ -231,13 +232,13 @@ static int compute_device(const void* xyz, int64_t n, int l_max, int normalized,
     const bool force_w = force && force[0] == 'w';
     const bool force_tp = force && force[0] == 't' && force[1] == 'p' && force[2] == '\0';
     const bool force_tpg = force && force[0] == 't' && force[1] == 'p' && force[2] == 'g';
-    if (!ddsph && !force_w && !force_tp && !force_tpg) {
+    if (!force_w && !force_tp && !force_tpg) {
         // compile-time-l_max kernels (two threads per point): every l_max that has an instantiation
         const bool f32 = dtype == SPHERICART_CUDA_F32;
-        int r = dsph ? (f32 ? sph_tpb_launch_f32_g : sph_tpb_launch_f64_g)(st->sm_count, xyz, n, l_max, normalized,
-                                                                            sph, dsph, stream)
-                     : (f32 ? sph_tpb_launch_f32_v : sph_tpb_launch_f64_v)(st->sm_count, xyz, n, l_max, normalized,
-                                                                            sph, nullptr, stream);
+        auto launch = ddsph ? (f32 ? sph_tpb_launch_f32_h : sph_tpb_launch_f64_h)
+                            : dsph ? (f32 ? sph_tpb_launch_f32_g : sph_tpb_launch_f64_g)
+                                   : (f32 ? sph_tpb_launch_f32_v : sph_tpb_launch_f64_v);
+        int r = launch(st->sm_count, xyz, n, l_max, normalized, sph, dsph, ddsph, stream);
         if (r < 0) return fail(SPHERICART_CUDA_ECUDA, "tpb launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         if (r == 0) {
             g_launches.fetch_add(1, std::memory_order_relaxed);

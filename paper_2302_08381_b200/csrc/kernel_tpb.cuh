@@ -40,6 +40,7 @@ struct TpbParams {
     const void* xyz;
     void* sph;
     void* dsph;
+    void* ddsph;
     int64_t n;
     int tiles_per_cta;   // consecutive tiles one CTA works through
     int pdl;             // launched as a programmatic dependent launch (tpb_inst.cu)
@@ -90,7 +91,10 @@ template <int ESIZE, int DERIV, int LMAX, int SPLIT> struct TpbShape {
     static constexpr int pitch_s = L + pad_elems;          // elements between the points' rows of sph
     static constexpr int pitch_g = 3 * L + pad_elems;      // ... of dsph
     static constexpr int s_bytes = TPB_PTS * pitch_s * ESIZE;
-    static constexpr int tile_bytes = s_bytes + (DERIV ? TPB_PTS * pitch_g * ESIZE : 0);
+    static constexpr int pitch_h = 9 * L + pad_elems;      // ... of ddsph
+    static constexpr int g_bytes = DERIV >= 1 ? TPB_PTS * pitch_g * ESIZE : 0;
+    static constexpr int h_bytes = DERIV >= 2 ? TPB_PTS * pitch_h * ESIZE : 0;
+    static constexpr int tile_bytes = s_bytes + g_bytes + h_bytes;
     static constexpr int fit = TPB_SMEM_PER_SM / (tile_bytes + 1024);   // resident CTAs per SM by shared memory
     static constexpr int cap = 16 / SPLIT;                              // ... and by registers (<= 128 each)
     static constexpr int min_ctas = fit < 1 ? 1 : (fit < cap ? fit : cap);
@@ -105,7 +109,8 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
     constexpr int L = Shape::L;
     constexpr int CUT = Shape::cut;
     constexpr uint32_t S_BYTES = Shape::s_bytes;
-    constexpr int PS = Shape::pitch_s, PG = Shape::pitch_g;
+    constexpr int PS = Shape::pitch_s, PG = Shape::pitch_g, PH = Shape::pitch_h;
+    constexpr uint32_t G_BYTES = Shape::g_bytes;
     const SphTables& TB = c_tables_tpb;
     extern __shared__ __align__(128) unsigned char smem[];
     const int lane = threadIdx.x & 31;
@@ -117,6 +122,7 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
     const T* __restrict__ xyz = static_cast<const T*>(prm.xyz);
     T* __restrict__ sph = static_cast<T*>(prm.sph);
     T* __restrict__ dsph = static_cast<T*>(prm.dsph);
+    T* __restrict__ ddsph = static_cast<T*>(prm.ddsph);
     const uint64_t policy = policy_evict_first();
     auto cta_sync = [&]() {
         if constexpr (SPLIT == 1) __syncwarp();
@@ -170,9 +176,11 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
         }
         T* S = reinterpret_cast<T*>(smem) + pl * PS;
         T* G = reinterpret_cast<T*>(smem + S_BYTES) + pl * PG;
+        T* H = reinterpret_cast<T*>(smem + S_BYTES + G_BYTES) + pl * PH;
 
         double Qc[LMAX + 1];   // column m:   Qc[l] = Qt_l^m     (0 for l < m)
         double Qn[LMAX + 1];   // column m+1: Qn[l] = Qt_l^{m+1} (0 for l < m+1)
+        double Qnn[DERIV >= 2 ? LMAX + 1 : 1];   // column m+2 (Hessians: Eq. 10 twice needs Qt_{l-2}^{m+2})
         // column M of the folded Eq. 7 into dst[M..LMAX] (static_for: every index is a constant, so
         // the arrays live in registers)
         auto column = [&](auto Mc, double* dst) {
@@ -202,7 +210,10 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
             constexpr int M0 = decltype(M0c)::value, M1 = decltype(M1c)::value;
             R c = RT::make(1.0, 0.0), s = RT::make(0.0, 0.0);
             double c1 = 0.0, s1 = 0.0;  // c_{m-1}, s_{m-1}
+            double c2 = 0.0, s2 = 0.0;  // c_{m-2}, s_{m-2} (Hessians)
             static_for<0, M0>([&](auto) {   // Eq. 9 up to (x + i y)^M0
+                c2 = c1;
+                s2 = s1;
                 c1 = to_double(c);
                 s1 = to_double(s);
                 const R cn = X * c - Y * s;
@@ -211,10 +222,16 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
                 s = sn;
             });
             column(std::integral_constant<int, M0>{}, Qc);
+            if constexpr (DERIV >= 2 && M0 < LMAX) column(std::integral_constant<int, M0 + 1>{}, Qn);
             static_for<M0, M1>([&](auto mc) {
                 constexpr int m = decltype(mc)::value;
                 // column m+1, computed once: Eq. 10 needs Qt_{l-1}^{m+1} now, and it is the next column
-                if constexpr (m < LMAX && (DERIV >= 1 || m + 1 < M1)) column(std::integral_constant<int, m + 1>{}, Qn);
+                // (Hessians: columns m+1 and m+2 are carried, m+2 is the new one)
+                if constexpr (DERIV <= 1) {
+                    if constexpr (m < LMAX && (DERIV >= 1 || m + 1 < M1)) column(std::integral_constant<int, m + 1>{}, Qn);
+                } else {
+                    if constexpr (m + 2 <= LMAX) column(std::integral_constant<int, m + 2>{}, Qnn);
+                }
                 // azimuthal factor of this lane's branch and its x/y derivatives (Eq. 9, Eq. 10)
                 const double cd = to_double(c), sd = to_double(s);
                 const double dm = (double)m;
@@ -222,7 +239,7 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
                 double Ax = dm * (sinb ? s1 : c1);
                 double Ay = dm * (sinb ? c1 : -s1);
                 double xA = xd * A, yA = yd * A, Az = A;
-                if (NORM && DERIV >= 1) {
+                if (NORM && DERIV == 1) {
                     xA *= rinv;
                     yA *= rinv;
                     Az *= rinv;
@@ -235,6 +252,37 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
                     constexpr int kc = l * (l + 1) + m, ks = l * (l + 1) - m;
                     const int k = sinb ? ks : kc;
                     const double Q = Qc[l];
+                    if constexpr (DERIV >= 2) {
+                        constexpr int t = SPH_TRI(l, m);
+                        double q1 = 0.0, qz = 0.0, q2 = 0.0, qxz = 0.0, qzz = 0.0;
+                        if constexpr (l >= m + 2) q1 = TB.G1[t] * Qn[l - 1];     // F_l^m Q_{l-1}^{m+1}
+                        if constexpr (l >= m + 1) qz = TB.Gz[t] * Qc[l - 1];     // F_l^m (l+m) Q_{l-1}^m
+                        if constexpr (l >= m + 4) q2 = TB.H2[t] * Qnn[l - 2];    // F_l^m Q_{l-2}^{m+2}
+                        if constexpr (l >= m + 3) qxz = TB.Hxz[t] * Qn[l - 2];   // F_l^m (l+m) Q_{l-2}^{m+1}
+                        if constexpr (l >= m + 2) qzz = TB.Hzz[t] * Qc[l - 2];   // F_l^m (l+m)(l+m-1) Q_{l-2}^m
+                        const double dmm = dm * (dm - 1.0);
+                        // Eq. 10 twice: cos: A_xx = m(m-1) c_{m-2}, A_xy = -m(m-1) s_{m-2}; sin: s_{m-2}, c_{m-2}
+                        const double Axx = dmm * (sinb ? s2 : c2);
+                        const double Axy = dmm * (sinb ? c2 : -s2);
+                        double o[10];
+                        assemble_scalars<NORM>(l, Q, q1, qz, q2, qxz, qzz, A, Ax, Ay, Axx, Axy, xd, yd, zd, rinv, o);
+                        if (emit) {
+                            S[k] = static_cast<T>(o[0]);
+                            G[k] = static_cast<T>(o[1]);
+                            G[L + k] = static_cast<T>(o[2]);
+                            G[2 * L + k] = static_cast<T>(o[3]);
+                            // o[4..9] = xx xy xz yy yz zz ; rows = xx xy xz yx yy yz zx zy zz
+                            H[k] = static_cast<T>(o[4]);
+                            H[L + k] = static_cast<T>(o[5]);
+                            H[2 * L + k] = static_cast<T>(o[6]);
+                            H[3 * L + k] = static_cast<T>(o[5]);
+                            H[4 * L + k] = static_cast<T>(o[7]);
+                            H[5 * L + k] = static_cast<T>(o[8]);
+                            H[6 * L + k] = static_cast<T>(o[6]);
+                            H[7 * L + k] = static_cast<T>(o[8]);
+                            H[8 * L + k] = static_cast<T>(o[9]);
+                        }
+                    } else {
                     if (emit) S[k] = static_cast<T>(Q * A);
                     if constexpr (DERIV >= 1) {
                         constexpr int t = SPH_TRI(l, m);
@@ -260,10 +308,15 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
                             G[2 * L + k] = static_cast<T>(gz);
                         }
                     }
+                    }
                 });
                 // next column, next power of (x + i y): Eq. 9
                 if constexpr (m + 1 < M1) {
                     static_for<m + 1, LMAX + 1>([&](auto lc) { Qc[decltype(lc)::value] = Qn[decltype(lc)::value]; });
+                    if constexpr (DERIV >= 2)
+                        static_for<m + 2, LMAX + 1>([&](auto lc) { Qn[decltype(lc)::value] = Qnn[decltype(lc)::value]; });
+                    c2 = c1;
+                    s2 = s1;
                     c1 = cd;
                     s1 = sd;
                     const R cn = X * c - Y * s;
@@ -285,6 +338,7 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
         const int64_t p0 = tile * TPB_PTS;
         T* S0 = reinterpret_cast<T*>(smem);
         T* G0 = reinterpret_cast<T*>(smem + S_BYTES);
+        T* H0 = reinterpret_cast<T*>(smem + S_BYTES + G_BYTES);
         if constexpr (Shape::pad) {
             // padded image: rows leave as 16-byte vectors (row lengths are multiples of 16 bytes here)
             constexpr int VE = 16 / (int)sizeof(T);        // elements per vector
@@ -300,11 +354,20 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
                     __stcs(reinterpret_cast<float4*>(dsph + (p0 + r) * 3 * L) + v,
                            reinterpret_cast<const float4*>(G0 + r * PG)[v]);
                 }
+            if (DERIV >= 2) {
+                constexpr int VH = 9 * L / VE;
+                for (int i = threadIdx.x; i < np * VH; i += SPLIT * 32) {
+                    const int r = i / VH, v = i - r * VH;
+                    __stcs(reinterpret_cast<float4*>(ddsph + (p0 + r) * 9 * L) + v,
+                           reinterpret_cast<const float4*>(H0 + r * PH)[v]);
+                }
+            }
             cta_sync();
         } else if (n - p0 >= TPB_PTS) {
             if (threadIdx.x == 0) {
                 bulk_store_hint(sph + p0 * L, S0, S_BYTES, policy);
                 if (DERIV >= 1) bulk_store_hint(dsph + p0 * 3 * L, G0, 3u * S_BYTES, policy);
+                if (DERIV >= 2) bulk_store_hint(ddsph + p0 * 9 * L, H0, 9u * S_BYTES, policy);
                 bulk_commit();
             }
         } else {  // ragged last tile: byte count need not be a multiple of 16 -> plain stores
@@ -312,6 +375,8 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
             for (int i = threadIdx.x; i < np * L; i += SPLIT * 32) st_cs(sph + p0 * L + i, S0[i]);
             if (DERIV >= 1)
                 for (int i = threadIdx.x; i < np * 3 * L; i += SPLIT * 32) st_cs(dsph + p0 * 3 * L + i, G0[i]);
+            if (DERIV >= 2)
+                for (int i = threadIdx.x; i < np * 9 * L; i += SPLIT * 32) st_cs(ddsph + p0 * 9 * L + i, H0[i]);
             cta_sync();
         }
     }

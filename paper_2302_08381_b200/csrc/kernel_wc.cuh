@@ -19,7 +19,7 @@
 //       1/4/13 bulk stores of the image's rows; the stores of one chunk drain while the group
 //       assembles its next chunk into the other image, and the other group works meanwhile.
 //   Slots are handed over with mbarriers (full: A -> B, empty: B -> A).
-// The grid is not persistent: a CTA owns WC_PTS consecutive points.
+// The grid is not persistent: a CTA owns up to WC_PTS consecutive points.
 // Measured on C4 (B200): 6.05 ms with kernel_w.cuh -> 4.88 ms (stores alone: 4.4 ms).
 #pragma once
 #include "kernel_w.cuh"
@@ -33,7 +33,8 @@ constexpr int WC_AW = 4;        // recurrence warps (phase A of a point takes ~4
 constexpr int WC_SLOTS = 6;     // triangles in flight
 constexpr int WC_CH = 368;      // most harmonics in a chunk: l_max = 32 splits into l < 19, 19 <= l < 27, l >= 27
                                 // (361 / 368 / 360 harmonics, 190 / 188 / 183 pairs: one pass each)
-constexpr int WC_PTS = 256;     // points per CTA (the first point's phase A is not overlapped)
+constexpr int WC_PTS = 256;     // most points per CTA (the first point's phase A is not overlapped); fewer for
+                                // small n, so that every SM gets several CTAs
 constexpr int WC_THREADS = (WC_BW + WC_AW) * 32;
 
 // Staging image: as WkStage (kernel_w.cuh), rows of one array a compile-time stride apart and
@@ -81,6 +82,7 @@ struct WcParams {
     int64_t n;
     int l_max;
     int n_chunks;
+    int pts_per_cta;
     unsigned char row0[SPH_MAX_L + 3];   // chunk i = the l-rows [row0[i], row0[i+1])
 };
 
@@ -137,8 +139,8 @@ __global__ void __launch_bounds__(WC_THREADS, 1) sph_wc_kernel(const WcParams pr
     tv.Hxz = tabs + 4 * lay.tsz;
     tv.Hzz = tabs + 5 * lay.tsz;
 
-    const int64_t pt_begin = (int64_t)blockIdx.x * WC_PTS;
-    const int np = (int)((prm.n - pt_begin < WC_PTS) ? prm.n - pt_begin : WC_PTS);
+    const int64_t pt_begin = (int64_t)blockIdx.x * prm.pts_per_cta;
+    const int np = (int)((prm.n - pt_begin < prm.pts_per_cta) ? prm.n - pt_begin : prm.pts_per_cta);
 
     if (warp >= WC_BW) {
         // ================= A-warps: recurrences, lane = m (phase A of kernel_w.cuh) =================
@@ -333,7 +335,7 @@ template <typename T, typename R> static WcKernel wc_pick(int deriv, int norm, b
 
 // returns 0 and fills *out if the cooperative kernel applies (rows long enough to be worth it and
 // the carve-up fits), 1 otherwise
-static inline int wc_plan(int smem_optin, int64_t n, int l_max, int normalized, int dtype, void* sph, void* dsph,
+static inline int wc_plan(int sm_count, int smem_optin, int64_t n, int l_max, int normalized, int dtype, void* sph, void* dsph,
                           void* ddsph, const void* xyz, const SphTables* d_tab, WcLaunch* out) {
     const int deriv = ddsph ? 2 : (dsph ? 1 : 0);
     const int esize = dtype == 0 ? 4 : 8;
@@ -367,7 +369,11 @@ static inline int wc_plan(int smem_optin, int64_t n, int l_max, int normalized, 
     out->prm.row0[nc] = (unsigned char)(l_max + 1);
     for (int e = l_max + 1, i = nc; e > 0; e = from[e]) out->prm.row0[--i] = (unsigned char)from[e];
     out->prm.n_chunks = nc;
-    out->grid = (n + WC_PTS - 1) / WC_PTS;
+    int64_t ppc = n / ((int64_t)sm_count * 4);   // >= 4 CTAs per SM where n allows
+    if (ppc > WC_PTS) ppc = WC_PTS;
+    if (ppc < 16) ppc = 16;
+    out->prm.pts_per_cta = (int)ppc;
+    out->grid = (n + ppc - 1) / ppc;
     if (out->grid > 0x7fffffff) return 1;
     out->smem = lay.total;
     return 0;

@@ -362,4 +362,55 @@ SPH_HD void assemble_pair(int l, int m, int t, const double* Qt, const double* c
 }
 
 
+// All outputs of ONE harmonic from scalars: Q = Qt_l^m, the five Legendre-side neighbours already
+// multiplied by their table ratios (q1 = F Q_{l-1}^{m+1}, qz = F (l+m) Q_{l-1}^m, q2 = F Q_{l-2}^{m+2},
+// qxz = F (l+m) Q_{l-2}^{m+1}, qzz = F (l+m)(l+m-1) Q_{l-2}^m; 0 where the neighbour does not exist),
+// the azimuthal factor A and its derivatives (A_yy = -A_xx).  Same formulas and output order as
+// assemble_element; used by the unrolled Hessian kernels, whose columns live in registers.
+template <bool NORM>
+SPH_HD void assemble_scalars(int l, double Q, double q1, double qz, double q2, double qxz, double qzz, double A,
+                             double Ax, double Ay, double Axx, double Axy, double x, double y, double z,
+                             double rinv, double* out) {
+    out[0] = Q * A;
+    const double q1A = q1 * A;
+    const double gx = SPH_FMA(x, q1A, Q * Ax);
+    const double gy = SPH_FMA(y, q1A, Q * Ay);
+    const double gz = qz * A;
+    const double dl = (double)l;
+    const double lY = dl * out[0];
+    if (NORM) {
+        out[1] = SPH_FMA(-lY, x, gx) * rinv;
+        out[2] = SPH_FMA(-lY, y, gy) * rinv;
+        out[3] = SPH_FMA(-lY, z, gz) * rinv;
+    } else {
+        out[1] = gx;
+        out[2] = gy;
+        out[3] = gz;
+    }
+    const double q2A = q2 * A;
+    const double q1Ax = q1 * Ax, q1Ay = q1 * Ay, QAxx = Q * Axx;
+    // d2Q/dx2 = Q1 + x^2 Q2, d2Q/dxdy = xy Q2, d2Q/dxdz = (l+m) x Qxz, d2Q/dz2 = (l+m)(l+m-1) Qzz
+    double Hxx = SPH_FMA(x * x, q2A, q1A) + SPH_FMA(2.0 * x, q1Ax, QAxx);
+    double Hyy = SPH_FMA(y * y, q2A, q1A) + SPH_FMA(2.0 * y, q1Ay, -QAxx);
+    double Hxy = SPH_FMA(x * y, q2A, Q * Axy) + SPH_FMA(x, q1Ay, y * q1Ax);
+    const double qxzA = qxz * A;
+    double Hxz = SPH_FMA(x, qxzA, qz * Ax);
+    double Hyz = SPH_FMA(y, qxzA, qz * Ay);
+    double Hzz = qzz * A;
+    if (NORM) {
+        // hess Y = (H - l(u g^T + g u^T) + l(l+2) Y u u^T - l Y I) / r^2   with g, H, Y at u
+        const double r2inv = rinv * rinv;
+        const double lgx = dl * gx, lgy = dl * gy, lgz = dl * gz;
+        const double w = (dl + 2.0) * lY;
+        const double wx = w * x, wy = w * y, wz = w * z;
+        Hxx = (SPH_FMA(x, SPH_FMA(-2.0, lgx, wx), Hxx) - lY) * r2inv;
+        Hyy = (SPH_FMA(y, SPH_FMA(-2.0, lgy, wy), Hyy) - lY) * r2inv;
+        Hzz = (SPH_FMA(z, SPH_FMA(-2.0, lgz, wz), Hzz) - lY) * r2inv;
+        Hxy = SPH_FMA(x, wy - lgy, SPH_FMA(-y, lgx, Hxy)) * r2inv;
+        Hxz = SPH_FMA(x, wz - lgz, SPH_FMA(-z, lgx, Hxz)) * r2inv;
+        Hyz = SPH_FMA(y, wz - lgz, SPH_FMA(-z, lgy, Hyz)) * r2inv;
+    }
+    out[4] = Hxx, out[5] = Hxy, out[6] = Hxz, out[7] = Hyy, out[8] = Hyz, out[9] = Hzz;
+}
+
 }  // namespace sphb200

@@ -9,12 +9,14 @@
 namespace sphb200 {
 #define SPH_TPB_DECL(sfx)                                                                                   \
     int sph_tpb_launch_##sfx(int sm_count, const void* xyz, int64_t n, int l_max, int normalized, void* sph, \
-                             void* dsph, cudaStream_t stream);                                              \
+                             void* dsph, void* ddsph, cudaStream_t stream);                                              \
     int sph_tpb_upload_##sfx(const SphTables* host_tables);
 SPH_TPB_DECL(f32_v)
 SPH_TPB_DECL(f32_g)
 SPH_TPB_DECL(f64_v)
 SPH_TPB_DECL(f64_g)
+SPH_TPB_DECL(f32_h)
+SPH_TPB_DECL(f64_h)
 #undef SPH_TPB_DECL
 // recompute-in-backward VJP (vjpr_inst.cu, compiled once per element type); same return codes
 #define SPH_VJPR_DECL(sfx)                                                                              \

@@ -1,5 +1,5 @@
 // One translation unit per (element type, DERIV) of the tpb kernels -- compiled four times by
-// build.py with -DTPB_F64=0|1 -DTPB_DERIV=0|1 so that the instantiations build in parallel.
+// build.py with -DTPB_F64=0|1 -DTPB_DERIV=0|1|2 so that the instantiations build in parallel.
 // Exports (C++ linkage, declared in tpb_api.h):
 //   sph_tpb_upload_<f32|f64>_<v|g>(tables)   copy the coefficient tables into this unit's constant bank
 //   sph_tpb_launch_<f32|f64>_<v|g>(...)      launch if l_max has an instantiation (returns 1 if not)
@@ -22,7 +22,11 @@ typedef float tpb_T;
 typedef double tpb_R;
 #endif
 
-#if TPB_F64 && TPB_DERIV
+#if TPB_F64 && TPB_DERIV == 2
+#define TPB_NAME(f) f##_f64_h
+#elif TPB_DERIV == 2
+#define TPB_NAME(f) f##_f32_h
+#elif TPB_F64 && TPB_DERIV
 #define TPB_NAME(f) f##_f64_g
 #elif TPB_F64
 #define TPB_NAME(f) f##_f64_v
@@ -104,8 +108,8 @@ static int launch_one(int sm_count, const TpbParams& prm, cudaStream_t stream) {
         return normalized ? launch_one<LM, true>(sm_count, prm, stream) : launch_one<LM, false>(sm_count, prm, stream);
 
 int TPB_NAME(sph_tpb_launch)(int sm_count, const void* xyz, int64_t n, int l_max, int normalized, void* sph,
-                             void* dsph, cudaStream_t stream) {
-    TpbParams prm{xyz, sph, dsph, n, 1, 0};
+                             void* dsph, void* ddsph, cudaStream_t stream) {
+    TpbParams prm{xyz, sph, dsph, ddsph, n, 1, 0};
     switch (l_max) {
         TPB_CASE(1)
         TPB_CASE(2)
@@ -113,8 +117,11 @@ int TPB_NAME(sph_tpb_launch)(int sm_count, const void* xyz, int64_t n, int l_max
         TPB_CASE(4)
         TPB_CASE(5)
         TPB_CASE(6)
+#if TPB_DERIV < 2 || !TPB_F64   // Hessians: f32 up to l_max = 8, f64 up to 6 (a 16-point tile must fit)
         TPB_CASE(7)
         TPB_CASE(8)
+#endif
+#if TPB_DERIV < 2
 #if !TPB_F64 || !TPB_DERIV    // f32 (C3 is l_max = 16 values) and f64 values: up to l_max = 16 / 12
         TPB_CASE(9)
         TPB_CASE(10)
@@ -126,6 +133,7 @@ int TPB_NAME(sph_tpb_launch)(int sm_count, const void* xyz, int64_t n, int l_max
         TPB_CASE(14)
         TPB_CASE(15)
         TPB_CASE(16)
+#endif
 #endif
         default:
             return 1;
