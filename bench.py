@@ -288,29 +288,36 @@ def sweep_expand(torch, pkg, device):
 
 def lmax_sweep(torch, pkg, device, peak):
     """`--lmax-sweep`: the metric's own axis -- output GB/s and points/s against l_max, f32 / f64,
-    with and without gradients (normalised harmonics, xyz ~ N(0,1), n sized for ~1.5 GB of output,
-    two rotating output sets).  One JSON object; not part of the default run."""
+    values / + gradients / + Hessians (normalised harmonics, xyz ~ N(0,1), n sized for ~1.5 GB of
+    output but at least 64 points per SM, two rotating output sets where they fit).  One JSON object; not part of the default run."""
     st = torch.cuda.current_stream().cuda_stream
     rows = {}
     for dtype, tdt, es in (("f32", torch.float32, 4), ("f64", torch.float64, 8)):
-        for grads in (False, True):
-            key = f"{dtype}_{'grads' if grads else 'values'}"
+        for deriv, tag in ((0, "values"), (1, "grads"), (2, "hessians")):
+            key = f"{dtype}_{tag}"
             rows[key] = {}
+            mult = (1, 4, 13)[deriv]
             for l_max in (1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12, 13, 14, 15, 16, 20, 24, 28, 32):
                 L = (l_max + 1) ** 2
-                per_pt = L * es * (4 if grads else 1)
+                per_pt = L * es * mult
                 n = int(min(4_000_000, 1.5e9 // per_pt)) // 256 * 256
+                if n < 148 * 64:          # too few points to fill the machine within the byte budget:
+                    n = 148 * 64          # (Hessians at l_max >= 20) take more memory instead
                 x = torch.randn(n, 3, device=device, dtype=tdt)
+                n_sets = 2 if n * per_pt < 3e9 else 1
                 outs = [(torch.empty((n, L), device=device, dtype=tdt),
-                         torch.empty((n, 3, L), device=device, dtype=tdt) if grads else None) for _ in range(2)]
+                         torch.empty((n, 3, L), device=device, dtype=tdt) if deriv >= 1 else None,
+                         torch.empty((n, 3, 3, L), device=device, dtype=tdt) if deriv >= 2 else None)
+                        for _ in range(n_sets)]
                 fn = lambda i: pkg.sphericart_cuda_compute(x, n, l_max, 1, pkg.F32 if dtype == "f32" else pkg.F64,
-                                                           outs[i & 1][0], outs[i & 1][1], None, st)
+                                                           *outs[i % n_sets], st)
                 for i in range(3):
                     fn(i)
                 torch.cuda.synchronize()
-                e0, e1 = time_loop(torch, fn, 10)
+                reps = 10 if n * per_pt < 3e9 else 4
+                e0, e1 = time_loop(torch, fn, reps)
                 torch.cuda.synchronize()
-                sec = e0.elapsed_time(e1) / 10 * 1e-3
+                sec = e0.elapsed_time(e1) / reps * 1e-3
                 rows[key][str(l_max)] = {"n": n, "us": round(sec * 1e6, 1), "points_per_s": n / sec,
                                          "out_gbs": round(n * per_pt / sec / 1e9, 1),
                                          "frac_of_measured_peak": round(n * per_pt / sec / 1e9 / peak, 3)}
