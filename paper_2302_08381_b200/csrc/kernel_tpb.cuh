@@ -179,7 +179,7 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
         T* H = reinterpret_cast<T*>(smem + S_BYTES + G_BYTES) + pl * PH;
 
         double Qc[LMAX + 1];   // column m:   Qc[l] = Qt_l^m     (0 for l < m)
-        double Qn[LMAX + 1];   // column m+1: Qn[l] = Qt_l^{m+1} (0 for l < m+1)
+        double Qn[DERIV >= 1 ? LMAX + 1 : 1];   // column m+1: Qn[l] = Qt_l^{m+1} (0 for l < m+1)
         double Qnn[DERIV >= 2 ? LMAX + 1 : 1];   // column m+2 (Hessians: Eq. 10 twice needs Qt_{l-2}^{m+2})
         // column M of the folded Eq. 7 into dst[M..LMAX] (static_for: every index is a constant, so
         // the arrays live in registers)
@@ -227,9 +227,10 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
                 constexpr int m = decltype(mc)::value;
                 // column m+1, computed once: Eq. 10 needs Qt_{l-1}^{m+1} now, and it is the next column
                 // (Hessians: columns m+1 and m+2 are carried, m+2 is the new one)
-                if constexpr (DERIV <= 1) {
-                    if constexpr (m < LMAX && (DERIV >= 1 || m + 1 < M1)) column(std::integral_constant<int, m + 1>{}, Qn);
-                } else {
+                // (values only: no second column at all, column m+1 is computed in place afterwards)
+                if constexpr (DERIV == 1) {
+                    if constexpr (m < LMAX) column(std::integral_constant<int, m + 1>{}, Qn);
+                } else if constexpr (DERIV >= 2) {
                     if constexpr (m + 2 <= LMAX) column(std::integral_constant<int, m + 2>{}, Qnn);
                 }
                 // azimuthal factor of this lane's branch and its x/y derivatives (Eq. 9, Eq. 10)
@@ -312,7 +313,8 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
                 });
                 // next column, next power of (x + i y): Eq. 9
                 if constexpr (m + 1 < M1) {
-                    static_for<m + 1, LMAX + 1>([&](auto lc) { Qc[decltype(lc)::value] = Qn[decltype(lc)::value]; });
+                    if constexpr (DERIV == 0) column(std::integral_constant<int, m + 1>{}, Qc);
+                    else static_for<m + 1, LMAX + 1>([&](auto lc) { Qc[decltype(lc)::value] = Qn[decltype(lc)::value]; });
                     if constexpr (DERIV >= 2)
                         static_for<m + 2, LMAX + 1>([&](auto lc) { Qn[decltype(lc)::value] = Qnn[decltype(lc)::value]; });
                     c2 = c1;

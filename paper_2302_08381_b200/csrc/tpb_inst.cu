@@ -134,6 +134,15 @@ int TPB_NAME(sph_tpb_launch)(int sm_count, const void* xyz, int64_t n, int l_max
         TPB_CASE(15)
         TPB_CASE(16)
 #endif
+#if !TPB_F64 && !TPB_DERIV     // f32 values: up to l_max = 23 (from 24 on the run-time kernel is as fast)
+        TPB_CASE(17)
+        TPB_CASE(18)
+        TPB_CASE(19)
+        TPB_CASE(20)
+        TPB_CASE(21)
+        TPB_CASE(22)
+        TPB_CASE(23)
+#endif
 #endif
         default:
             return 1;
