@@ -5,10 +5,12 @@
 // flight (kernel_tpb.cuh).  With gradients at l_max = 16 a 16-point f32 tile is already 74 KB; the
 // one-warp-per-point kernels (kernel_w.cuh, kernel_wc.cuh) are built for rows of ~100 KB per point
 // and reach ~1 TB/s here.  So a point is given LP = 2, 4 or 8 lanes:
-//     lane = p + PTS (b + 2 c),   PTS = 32 / LP points per tile,
-//     b = branch of Eq. 5 (0: the m >= 0 / cos outputs, 1: the m < 0 / sin outputs),
+//     lane = p + PTS c,   PTS = 32 / LP points per tile,
 //     c = column class: the lane owns the columns m = c, c + C, c + 2C, ... of the (l,m) triangle,
-//         C = LP / 2.
+//         C = LP, and writes BOTH branches of Eq. 5 (the m >= 0 / cos and the m < 0 / sin outputs)
+//         of its columns: the Legendre recurrences, the bulk of a column's cost, run once for the two
+//         (template flag BB; with BB = false a lane does one branch and C = LP / 2 -- measured
+//         25-55 % slower: f32 values l_max = 24 2.3 -> 3.2 TB/s with BB).
 // A column is run with O(1) state as in eval_point_columns (sph_core.cuh): Qt_l^m by the folded
 // Eq. 7 and, for the gradients, column m+1 one row behind it (Eq. 10 needs Qt_{l-1}^{m+1}); the
 // powers (x + i y)^m of Eq. 9 advance C at a time.  All lanes run the same loops (trip counts
@@ -86,11 +88,11 @@ __host__ __device__ inline int tpg_tab_bytes(int l_max, bool is_dd) {
     return (((is_dd ? 6 : 4) * tsz + (is_dd ? 2 : 1) * ncol) * 8 + 15) & ~15;
 }
 
-template <typename T, typename R, int DERIV, bool NORM, int LP>
+template <typename T, typename R, int DERIV, bool NORM, int LP, bool BB>
 __global__ void __launch_bounds__(128, 4) sph_tpg_kernel(const TpgParams prm) {
     using RT = rec<R>;
     constexpr int PTS = 32 / LP;   // points per tile
-    constexpr int C = LP / 2;      // column classes
+    constexpr int C = BB ? LP : LP / 2;   // column classes (BB: a lane does BOTH branches of its columns)
     extern __shared__ __align__(128) unsigned char smem[];
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
@@ -115,8 +117,8 @@ __global__ void __launch_bounds__(128, 4) sph_tpg_kernel(const TpgParams prm) {
                          (size_t)warp * tpg_tile_bytes(PTS, L, (int)sizeof(T), DERIV);
     const int pl = lane % PTS;          // point inside the tile
     const int role = lane / PTS;
-    const bool sinb = role & 1;         // branch
-    const int cls = role >> 1;          // column class
+    const bool sinb = BB ? false : (role & 1);   // branch (BB: cos here, sin alongside)
+    const int cls = BB ? role : (role >> 1);     // column class
     const T* __restrict__ xyz = static_cast<const T*>(prm.xyz);
     T* __restrict__ sph = static_cast<T*>(prm.sph);
     T* __restrict__ dsph = static_cast<T*>(prm.dsph);
@@ -165,53 +167,55 @@ __global__ void __launch_bounds__(128, 4) sph_tpg_kernel(const TpgParams prm) {
         const double cd = to_double(cm), sd = to_double(sm);
         const double c1 = to_double(cm1), s1 = to_double(sm1);
         const double dm = (double)m;
-        // azimuthal factor of this lane's branch and its x/y derivatives (Eq. 9, Eq. 10)
-        const double A = sinb ? sd : (m == 0 ? SPH_INV_SQRT2 : cd);
-        double Ax = dm * (sinb ? s1 : c1);
-        double Ay = dm * (sinb ? c1 : -s1);
-        double xA = xd * A, yA = yd * A, Az = A;
-        if (NORM && DERIV >= 1) {
-            xA *= rinv;
-            yA *= rinv;
-            Az *= rinv;
-            Ax *= rinv;
-            Ay *= rinv;
-        }
-        const bool emit = (m > 0) || !sinb;   // the sin branch has no m = 0 output
+        const double sc = (NORM && DERIV >= 1) ? rinv : 1.0;   // the chain rule's 1/r, folded into the factors
+        // azimuthal factor of a branch and its x/y derivatives (Eq. 9, Eq. 10): {A, xA, yA, Az, Ax, Ay}
+        // first = this lane's branch (BB: the cos branch), second = the sin branch (BB only)
+        const double A0 = sinb ? sd : (m == 0 ? SPH_INV_SQRT2 : cd);
+        const double Ax0 = dm * (sinb ? s1 : c1) * sc, Ay0 = dm * (sinb ? c1 : -s1) * sc;
+        const double xA0 = xd * A0 * sc, yA0 = yd * A0 * sc, Az0 = A0 * sc;
+        const double A1 = sd;
+        const double Ax1 = dm * s1 * sc, Ay1 = dm * c1 * sc;
+        const double xA1 = xd * A1 * sc, yA1 = yd * A1 * sc, Az1 = A1 * sc;
+        const bool emit0 = (m > 0) || !sinb;   // the sin branch has no m = 0 output
+        const bool emit1 = BB && m > 0;
         R q = TB.d(m);                   // Qt_l^m, starting at Qt_m^m
         R qp = RT::make(0.0, 0.0);       // Qt_{l-1}^m
         R pc = RT::make(0.0, 0.0);       // Qt_{l-1}^{m+1}
         R pp = RT::make(0.0, 0.0);       // Qt_{l-2}^{m+1}
         // running indices: t = TRI(l, m) (so TRI(l+1, m) = t + l + 1 and TRI(l, m+1) = t + 1) and
-        // this lane's output index k = l (l + 1) +- m, which advances by 2 (l + 1)
+        // the output indices k = l (l + 1) +- m, which advance by 2 (l + 1)
         int t = SPH_TRI(m, m);
-        int k = m * (m + 1) + (sinb ? -m : m);
-        T* Sk = S + k;
-        T* Gk = G + k;
+        T* Sk0 = S + m * (m + 1) + (sinb ? -m : m);
+        T* Gk0 = G + m * (m + 1) + (sinb ? -m : m);
+        T* Sk1 = S + m * (m + 1) - m;
+        T* Gk1 = G + m * (m + 1) - m;
 #pragma unroll 2
         for (int l = m; l <= l_max; ++l) {
             const double Q = to_double(q);
-            if (emit) *Sk = static_cast<T>(Q * A);   // Eq. 5
+            double q1 = 0.0, qz = 0.0, lQ = 0.0;
             if (DERIV >= 1) {
-                const double q1 = TB.G1[t] * to_double(pc);   // F_l^m Q_{l-1}^{m+1}
-                const double qz = TB.Gz[t] * to_double(qp);   // F_l^m (l+m) Q_{l-1}^m
-                double gx, gy, gz;
-                if (NORM) {
-                    const double lQ = (double)l * Q;
-                    const double t1 = q1 - lQ;
-                    const double tz = SPH_FMA(-lQ, zd, qz);
-                    gx = SPH_FMA(t1, xA, Q * Ax);
-                    gy = SPH_FMA(t1, yA, Q * Ay);
-                    gz = tz * Az;
-                } else {
-                    gx = SPH_FMA(q1, xA, Q * Ax);
-                    gy = SPH_FMA(q1, yA, Q * Ay);
-                    gz = qz * Az;
+                q1 = TB.G1[t] * to_double(pc);   // F_l^m Q_{l-1}^{m+1}
+                qz = TB.Gz[t] * to_double(qp);   // F_l^m (l+m) Q_{l-1}^m
+                if (NORM) {   // (q1 - l Q) and (qz - l Q z): Eq. 10 + Euler, as in kernel_tpb.cuh
+                    lQ = (double)l * Q;
+                    q1 -= lQ;
+                    qz = SPH_FMA(-lQ, zd, qz);
                 }
-                if (emit) {
-                    Gk[0] = static_cast<T>(gx);
-                    Gk[L] = static_cast<T>(gy);
-                    Gk[2 * L] = static_cast<T>(gz);
+            }
+            if (emit0) {
+                *Sk0 = static_cast<T>(Q * A0);   // Eq. 5
+                if (DERIV >= 1) {
+                    Gk0[0] = static_cast<T>(SPH_FMA(q1, xA0, Q * Ax0));
+                    Gk0[L] = static_cast<T>(SPH_FMA(q1, yA0, Q * Ay0));
+                    Gk0[2 * L] = static_cast<T>(qz * Az0);
+                }
+            }
+            if (emit1) {
+                *Sk1 = static_cast<T>(Q * A1);
+                if (DERIV >= 1) {
+                    Gk1[0] = static_cast<T>(SPH_FMA(q1, xA1, Q * Ax1));
+                    Gk1[L] = static_cast<T>(SPH_FMA(q1, yA1, Q * Ay1));
+                    Gk1[2 * L] = static_cast<T>(qz * Az1);
                 }
             }
             if (l < l_max) {
@@ -240,8 +244,10 @@ __global__ void __launch_bounds__(128, 4) sph_tpg_kernel(const TpgParams prm) {
                 }
             }
             t += l + 1;
-            Sk += 2 * (l + 1);
-            Gk += 2 * (l + 1);
+            Sk0 += 2 * (l + 1);
+            Gk0 += 2 * (l + 1);
+            Sk1 += 2 * (l + 1);
+            Gk1 += 2 * (l + 1);
         }
         // the next column of this class: w^(m+C), w^(m+C-1)
         if (m == 0) {
@@ -304,14 +310,14 @@ struct TpgLaunch {
     size_t smem;
 };
 
-template <typename T, typename R, int LP> static TpgKernel tpg_pick2(int deriv, int norm) {
-    if (deriv == 0) return norm ? sph_tpg_kernel<T, R, 0, true, LP> : sph_tpg_kernel<T, R, 0, false, LP>;
-    return norm ? sph_tpg_kernel<T, R, 1, true, LP> : sph_tpg_kernel<T, R, 1, false, LP>;
+template <typename T, typename R, int LP, bool BB> static TpgKernel tpg_pick2(int deriv, int norm) {
+    if (deriv == 0) return norm ? sph_tpg_kernel<T, R, 0, true, LP, BB> : sph_tpg_kernel<T, R, 0, false, LP, BB>;
+    return norm ? sph_tpg_kernel<T, R, 1, true, LP, BB> : sph_tpg_kernel<T, R, 1, false, LP, BB>;
 }
 template <typename T, typename R> static TpgKernel tpg_pick(int deriv, int norm, int lp) {
-    if (lp == 2) return tpg_pick2<T, R, 2>(deriv, norm);
-    if (lp == 4) return tpg_pick2<T, R, 4>(deriv, norm);
-    return tpg_pick2<T, R, 8>(deriv, norm);
+    if (lp == 2) return tpg_pick2<T, R, 2, true>(deriv, norm);
+    if (lp == 4) return tpg_pick2<T, R, 4, true>(deriv, norm);
+    return tpg_pick2<T, R, 8, true>(deriv, norm);
 }
 
 static inline int tpg_env(const char* name, int dflt) {
@@ -327,15 +333,17 @@ static inline int tpg_plan(int smem_optin, int64_t n, int l_max, int normalized,
     const int esize = dtype == 0 ? 4 : 8;
     const int L = (l_max + 1) * (l_max + 1);
     const int64_t per_pt = (int64_t)L * esize * (deriv ? 4 : 1);
-    // lanes per point: the most points per tile (16, 8, 4) whose image stays under 16 KB (measured:
+    // lanes per point: the most points per tile (16, 8, 4) whose image stays under 12 KB (measured:
     // the kernel is latency-bound, so small tiles = more warps in flight wins almost everywhere)
     int lp = tpg_env("SPHB200_TPG_LP", 0);
     if (lp != 2 && lp != 4 && lp != 8) {
         lp = 2;
-        while (lp < 8 && (32 / lp) * per_pt > 16 * 1024) lp *= 2;
+        while (lp < 8 && (32 / lp) * per_pt > 12 * 1024) lp *= 2;
     }
     const int64_t tile_bytes = tpg_tile_bytes(32 / lp, L, esize, deriv);
-    if (tile_bytes > 48 * 1024) return 1;
+    // longer rows go to the warp-per-point kernels (measured: f64 gradients at l_max = 16, a 37 KB
+    // tile: 1.5 TB/s here, 1.8 there; f32 gradients at l_max = 24, 40 KB: 1.9 here, 1.0 there)
+    if (tile_bytes > (dtype != 0 && deriv ? 32 : 48) * 1024) return 1;
     const int tab_bytes = tpg_tab_bytes(l_max, dtype != 0);
     int warps = 4;
     while (warps > 1 && tab_bytes + warps * tile_bytes > (smem_optin - 1024) / 2) warps >>= 1;   // >= 2 CTAs per SM
