@@ -78,8 +78,11 @@ template <int LMAX, int SPLIT> struct TpbCut {
     }
 };
 
-template <int ESIZE, int DERIV, int LMAX, int SPLIT> struct TpbShape {
+template <int ESIZE, int DERIV, int LMAX, int SPLIT, bool BB = false> struct TpbShape {
     static constexpr int L = (LMAX + 1) * (LMAX + 1);
+    // BB: ONE lane per point does both branches of Eq. 5 (32 points per tile): the Legendre
+    // recurrences run once for the two -- for the kernels that are bound by them (double-double)
+    static constexpr int pts = BB ? 32 : TPB_PTS;
     // Shared-memory banks: lane p writes word p * (row pitch) + k; the lanes of a branch collide 8- or
     // 16-way when the pitch in 32-bit words is 0 or 16 modulo 32, i.e. for l_max = 3 (mod 4)
     // (measured: f32 l_max = 7 ran at 2.0 TB/s where l_max = 6 and 8 reach 6.7 and 6.9).  Those row
@@ -90,10 +93,10 @@ template <int ESIZE, int DERIV, int LMAX, int SPLIT> struct TpbShape {
     static constexpr int pad_elems = pad ? 16 / ESIZE : 0;
     static constexpr int pitch_s = L + pad_elems;          // elements between the points' rows of sph
     static constexpr int pitch_g = 3 * L + pad_elems;      // ... of dsph
-    static constexpr int s_bytes = TPB_PTS * pitch_s * ESIZE;
+    static constexpr int s_bytes = pts * pitch_s * ESIZE;
     static constexpr int pitch_h = 9 * L + pad_elems;      // ... of ddsph
-    static constexpr int g_bytes = DERIV >= 1 ? TPB_PTS * pitch_g * ESIZE : 0;
-    static constexpr int h_bytes = DERIV >= 2 ? TPB_PTS * pitch_h * ESIZE : 0;
+    static constexpr int g_bytes = DERIV >= 1 ? pts * pitch_g * ESIZE : 0;
+    static constexpr int h_bytes = DERIV >= 2 ? pts * pitch_h * ESIZE : 0;
     static constexpr int tile_bytes = s_bytes + g_bytes + h_bytes;
     static constexpr int fit = TPB_SMEM_PER_SM / (tile_bytes + 1024);   // resident CTAs per SM by shared memory
     static constexpr int cap = 16 / SPLIT;                              // ... and by registers (<= 128 each)
@@ -101,11 +104,12 @@ template <int ESIZE, int DERIV, int LMAX, int SPLIT> struct TpbShape {
     static constexpr int cut = TpbCut<LMAX, SPLIT>::cut();
 };
 
-template <typename T, typename R, int DERIV, bool NORM, int LMAX, int SPLIT>
-__global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, SPLIT>::min_ctas)
+template <typename T, typename R, int DERIV, bool NORM, int LMAX, int SPLIT, bool BB = false>
+__global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, SPLIT, BB>::min_ctas)
     sph_tpb_kernel(const TpbParams prm) {
     using RT = rec<R>;
-    using Shape = TpbShape<sizeof(T), DERIV, LMAX, SPLIT>;
+    using Shape = TpbShape<sizeof(T), DERIV, LMAX, SPLIT, BB>;
+    constexpr int PTS = Shape::pts;
     constexpr int L = Shape::L;
     constexpr int CUT = Shape::cut;
     constexpr uint32_t S_BYTES = Shape::s_bytes;
@@ -115,10 +119,10 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
     extern __shared__ __align__(128) unsigned char smem[];
     const int lane = threadIdx.x & 31;
     const int part = threadIdx.x >> 5;     // which share of the columns (warp-uniform)
-    const int pl = lane & (TPB_PTS - 1);   // point inside the tile
-    const bool sinb = lane >= TPB_PTS;     // branch
+    const int pl = lane & (PTS - 1);             // point inside the tile
+    const bool sinb = BB ? false : lane >= PTS;   // branch (BB: cos here, sin alongside)
     const int64_t n = prm.n;
-    const int64_t n_tiles = (n + TPB_PTS - 1) / TPB_PTS;
+    const int64_t n_tiles = (n + PTS - 1) / PTS;
     const T* __restrict__ xyz = static_cast<const T*>(prm.xyz);
     T* __restrict__ sph = static_cast<T*>(prm.sph);
     T* __restrict__ dsph = static_cast<T*>(prm.dsph);
@@ -142,7 +146,7 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
 
     // lanes past the end compute a harmless point
     auto load_xyz = [&](int64_t tile, T& a, T& b, T& c) {
-        const int64_t p = tile * TPB_PTS + pl;
+        const int64_t p = tile * PTS + pl;
         a = T(0), b = T(0), c = T(1);
         if (p < n) {
             a = __ldg(xyz + 3 * p + 0);
@@ -236,81 +240,84 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
                 // azimuthal factor of this lane's branch and its x/y derivatives (Eq. 9, Eq. 10)
                 const double cd = to_double(c), sd = to_double(s);
                 const double dm = (double)m;
-                const double A = sinb ? sd : (m == 0 ? SPH_INV_SQRT2 : cd);
-                double Ax = dm * (sinb ? s1 : c1);
-                double Ay = dm * (sinb ? c1 : -s1);
-                double xA = xd * A, yA = yd * A, Az = A;
-                if (NORM && DERIV == 1) {
-                    xA *= rinv;
-                    yA *= rinv;
-                    Az *= rinv;
-                    Ax *= rinv;
-                    Ay *= rinv;
-                }
-                const bool emit = (m > 0) || !sinb;   // the sin branch has no m = 0 output
-                static_for<m, LMAX + 1>([&](auto lc) {
-                    constexpr int l = decltype(lc)::value;
-                    constexpr int kc = l * (l + 1) + m, ks = l * (l + 1) - m;
-                    const int k = sinb ? ks : kc;
-                    const double Q = Qc[l];
-                    if constexpr (DERIV >= 2) {
-                        constexpr int t = SPH_TRI(l, m);
-                        double q1 = 0.0, qz = 0.0, q2 = 0.0, qxz = 0.0, qzz = 0.0;
-                        if constexpr (l >= m + 2) q1 = TB.G1[t] * Qn[l - 1];     // F_l^m Q_{l-1}^{m+1}
-                        if constexpr (l >= m + 1) qz = TB.Gz[t] * Qc[l - 1];     // F_l^m (l+m) Q_{l-1}^m
-                        if constexpr (l >= m + 4) q2 = TB.H2[t] * Qnn[l - 2];    // F_l^m Q_{l-2}^{m+2}
-                        if constexpr (l >= m + 3) qxz = TB.Hxz[t] * Qn[l - 2];   // F_l^m (l+m) Q_{l-2}^{m+1}
-                        if constexpr (l >= m + 2) qzz = TB.Hzz[t] * Qc[l - 2];   // F_l^m (l+m)(l+m-1) Q_{l-2}^m
-                        const double dmm = dm * (dm - 1.0);
-                        // Eq. 10 twice: cos: A_xx = m(m-1) c_{m-2}, A_xy = -m(m-1) s_{m-2}; sin: s_{m-2}, c_{m-2}
-                        const double Axx = dmm * (sinb ? s2 : c2);
-                        const double Axy = dmm * (sinb ? c2 : -s2);
-                        double o[10];
-                        assemble_scalars<NORM>(l, Q, q1, qz, q2, qxz, qzz, A, Ax, Ay, Axx, Axy, xd, yd, zd, rinv, o);
-                        if (emit) {
-                            S[k] = static_cast<T>(o[0]);
-                            G[k] = static_cast<T>(o[1]);
-                            G[L + k] = static_cast<T>(o[2]);
-                            G[2 * L + k] = static_cast<T>(o[3]);
-                            // o[4..9] = xx xy xz yy yz zz ; rows = xx xy xz yx yy yz zx zy zz
-                            H[k] = static_cast<T>(o[4]);
-                            H[L + k] = static_cast<T>(o[5]);
-                            H[2 * L + k] = static_cast<T>(o[6]);
-                            H[3 * L + k] = static_cast<T>(o[5]);
-                            H[4 * L + k] = static_cast<T>(o[7]);
-                            H[5 * L + k] = static_cast<T>(o[8]);
-                            H[6 * L + k] = static_cast<T>(o[6]);
-                            H[7 * L + k] = static_cast<T>(o[8]);
-                            H[8 * L + k] = static_cast<T>(o[9]);
-                        }
-                    } else {
-                    if (emit) S[k] = static_cast<T>(Q * A);
-                    if constexpr (DERIV >= 1) {
-                        constexpr int t = SPH_TRI(l, m);
-                        double q1 = 0.0, qz = 0.0;
-                        if constexpr (l >= m + 2) q1 = TB.G1[t] * Qn[l - 1];   // F_l^m Q_{l-1}^{m+1}
-                        if constexpr (l >= m + 1) qz = TB.Gz[t] * Qc[l - 1];   // F_l^m (l+m) Q_{l-1}^m
-                        double gx, gy, gz;
-                        if (NORM) {
-                            const double lQ = (double)l * Q;
-                            const double t1 = q1 - lQ;
-                            const double tz = SPH_FMA(-lQ, zd, qz);
-                            gx = SPH_FMA(t1, xA, Q * Ax);
-                            gy = SPH_FMA(t1, yA, Q * Ay);
-                            gz = tz * Az;
+                const double sc = (NORM && DERIV == 1) ? rinv : 1.0;   // gradients only: the chain rule's 1/r, folded in
+                // one branch of Eq. 5 for every l of this column: A = c_m | s_m | 1/sqrt2, its x/y
+                // derivatives, (c,s)_{m-2} for the second derivatives
+                auto branch = [&](bool sin_branch, bool emit) {
+                    const double A = sin_branch ? sd : (m == 0 ? SPH_INV_SQRT2 : cd);
+                    const double Ax = dm * (sin_branch ? s1 : c1) * sc;
+                    const double Ay = dm * (sin_branch ? c1 : -s1) * sc;
+                    const double xA = xd * A * sc, yA = yd * A * sc, Az = A * sc;
+                    static_for<m, LMAX + 1>([&](auto lc) {
+                        constexpr int l = decltype(lc)::value;
+                        constexpr int kc = l * (l + 1) + m, ks = l * (l + 1) - m;
+                        const int k = sin_branch ? ks : kc;
+                        const double Q = Qc[l];
+                        if constexpr (DERIV >= 2) {
+                            constexpr int t = SPH_TRI(l, m);
+                            double q1 = 0.0, qz = 0.0, q2 = 0.0, qxz = 0.0, qzz = 0.0;
+                            if constexpr (l >= m + 2) q1 = TB.G1[t] * Qn[l - 1];     // F_l^m Q_{l-1}^{m+1}
+                            if constexpr (l >= m + 1) qz = TB.Gz[t] * Qc[l - 1];     // F_l^m (l+m) Q_{l-1}^m
+                            if constexpr (l >= m + 4) q2 = TB.H2[t] * Qnn[l - 2];    // F_l^m Q_{l-2}^{m+2}
+                            if constexpr (l >= m + 3) qxz = TB.Hxz[t] * Qn[l - 2];   // F_l^m (l+m) Q_{l-2}^{m+1}
+                            if constexpr (l >= m + 2) qzz = TB.Hzz[t] * Qc[l - 2];   // F_l^m (l+m)(l+m-1) Q_{l-2}^m
+                            const double dmm = dm * (dm - 1.0);
+                            // Eq. 10 twice: cos: A_xx = m(m-1) c_{m-2}, A_xy = -m(m-1) s_{m-2}; sin: s_{m-2}, c_{m-2}
+                            const double Axx = dmm * (sin_branch ? s2 : c2);
+                            const double Axy = dmm * (sin_branch ? c2 : -s2);
+                            double o[10];
+                            assemble_scalars<NORM>(l, Q, q1, qz, q2, qxz, qzz, A, Ax, Ay, Axx, Axy, xd, yd, zd, rinv, o);
+                            if (emit) {
+                                S[k] = static_cast<T>(o[0]);
+                                G[k] = static_cast<T>(o[1]);
+                                G[L + k] = static_cast<T>(o[2]);
+                                G[2 * L + k] = static_cast<T>(o[3]);
+                                // o[4..9] = xx xy xz yy yz zz ; rows = xx xy xz yx yy yz zx zy zz
+                                H[k] = static_cast<T>(o[4]);
+                                H[L + k] = static_cast<T>(o[5]);
+                                H[2 * L + k] = static_cast<T>(o[6]);
+                                H[3 * L + k] = static_cast<T>(o[5]);
+                                H[4 * L + k] = static_cast<T>(o[7]);
+                                H[5 * L + k] = static_cast<T>(o[8]);
+                                H[6 * L + k] = static_cast<T>(o[6]);
+                                H[7 * L + k] = static_cast<T>(o[8]);
+                                H[8 * L + k] = static_cast<T>(o[9]);
+                            }
                         } else {
-                            gx = SPH_FMA(q1, xA, Q * Ax);
-                            gy = SPH_FMA(q1, yA, Q * Ay);
-                            gz = qz * Az;
+                            if (emit) S[k] = static_cast<T>(Q * A);
+                            if constexpr (DERIV >= 1) {
+                                constexpr int t = SPH_TRI(l, m);
+                                double q1 = 0.0, qz = 0.0;
+                                if constexpr (l >= m + 2) q1 = TB.G1[t] * Qn[l - 1];   // F_l^m Q_{l-1}^{m+1}
+                                if constexpr (l >= m + 1) qz = TB.Gz[t] * Qc[l - 1];   // F_l^m (l+m) Q_{l-1}^m
+                                double gx, gy, gz;
+                                if (NORM) {
+                                    const double lQ = (double)l * Q;
+                                    const double t1 = q1 - lQ;
+                                    const double tz = SPH_FMA(-lQ, zd, qz);
+                                    gx = SPH_FMA(t1, xA, Q * Ax);
+                                    gy = SPH_FMA(t1, yA, Q * Ay);
+                                    gz = tz * Az;
+                                } else {
+                                    gx = SPH_FMA(q1, xA, Q * Ax);
+                                    gy = SPH_FMA(q1, yA, Q * Ay);
+                                    gz = qz * Az;
+                                }
+                                if (emit) {
+                                    G[k] = static_cast<T>(gx);
+                                    G[L + k] = static_cast<T>(gy);
+                                    G[2 * L + k] = static_cast<T>(gz);
+                                }
+                            }
                         }
-                        if (emit) {
-                            G[k] = static_cast<T>(gx);
-                            G[L + k] = static_cast<T>(gy);
-                            G[2 * L + k] = static_cast<T>(gz);
-                        }
-                    }
-                    }
-                });
+                    });
+                };
+                if constexpr (BB) {
+                    branch(false, true);
+                    if constexpr (m > 0) branch(true, true);   // the sin branch has no m = 0 output
+                } else {
+                    branch(sinb, (m > 0) || !sinb);
+                }
                 // next column, next power of (x + i y): Eq. 9
                 if constexpr (m + 1 < M1) {
                     if constexpr (DERIV == 0) column(std::integral_constant<int, m + 1>{}, Qc);
@@ -337,14 +344,14 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
 
         fence_proxy_async_smem();
         cta_sync();
-        const int64_t p0 = tile * TPB_PTS;
+        const int64_t p0 = tile * PTS;
         T* S0 = reinterpret_cast<T*>(smem);
         T* G0 = reinterpret_cast<T*>(smem + S_BYTES);
         T* H0 = reinterpret_cast<T*>(smem + S_BYTES + G_BYTES);
         if constexpr (Shape::pad) {
             // padded image: rows leave as 16-byte vectors (row lengths are multiples of 16 bytes here)
             constexpr int VE = 16 / (int)sizeof(T);        // elements per vector
-            const int np = (int)((n - p0 < TPB_PTS) ? n - p0 : TPB_PTS);
+            const int np = (int)((n - p0 < PTS) ? n - p0 : PTS);
             constexpr int VS = L / VE, VG = 3 * L / VE;    // vectors per point
             for (int i = threadIdx.x; i < np * VS; i += SPLIT * 32) {
                 const int r = i / VS, v = i - r * VS;
@@ -365,7 +372,7 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
                 }
             }
             cta_sync();
-        } else if (n - p0 >= TPB_PTS) {
+        } else if (n - p0 >= PTS) {
             if (threadIdx.x == 0) {
                 bulk_store_hint(sph + p0 * L, S0, S_BYTES, policy);
                 if (DERIV >= 1) bulk_store_hint(dsph + p0 * 3 * L, G0, 3u * S_BYTES, policy);

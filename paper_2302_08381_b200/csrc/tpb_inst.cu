@@ -41,11 +41,11 @@ static int env_int(const char* name, int dflt) {
     return (s && *s) ? atoi(s) : dflt;
 }
 
-template <int LMAX, bool NORM, int SPLIT>
+template <int LMAX, bool NORM, int SPLIT, bool BB = false>
 static int launch_split(int sm_count, TpbParams prm, cudaStream_t stream) {
-    using Shape = TpbShape<sizeof(tpb_T), TPB_DERIV, LMAX, SPLIT>;
+    using Shape = TpbShape<sizeof(tpb_T), TPB_DERIV, LMAX, SPLIT, BB>;
     static_assert(Shape::fit >= 1, "tile does not fit in shared memory");
-    auto kern = sph_tpb_kernel<tpb_T, tpb_R, TPB_DERIV, NORM, LMAX, SPLIT>;
+    auto kern = sph_tpb_kernel<tpb_T, tpb_R, TPB_DERIV, NORM, LMAX, SPLIT, BB>;
     static bool attr_done[64] = {false};   // per device; benign race (idempotent call)
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return -1;
@@ -58,7 +58,7 @@ static int launch_split(int sm_count, TpbParams prm, cudaStream_t stream) {
     // gradients: 476 against 508): the CTA launch is cheap next to such a tile.  Small tiles (values
     // only, low l_max) take up to four per CTA, or the launch rate of the block scheduler shows
     // (C5 values only, 3.1 KB tiles: 170 us with one, 147 with two, 136 with four or eight).
-    const int64_t n_tiles = (prm.n + TPB_PTS - 1) / TPB_PTS;
+    const int64_t n_tiles = (prm.n + Shape::pts - 1) / Shape::pts;
     static const int k_env = env_int("SPHB200_TPB_TILES", 0);
     int64_t k = k_env > 0 ? k_env : 12288 / Shape::tile_bytes;
     if (k < 1) k = 1;
@@ -94,13 +94,27 @@ static int launch_split(int sm_count, TpbParams prm, cudaStream_t stream) {
 template <int LMAX, bool NORM>
 static int launch_one(int sm_count, const TpbParams& prm, cudaStream_t stream) {
     static const int split_env = env_int("SPHB200_TPB_SPLIT", 0);
-    constexpr bool can_split = LMAX >= 4;
-    if constexpr (can_split) {
-        constexpr bool dflt = TpbShape<sizeof(tpb_T), TPB_DERIV, LMAX, 1>::fit <= 12;
-        const bool want = split_env ? split_env == 2 : dflt;
-        if (want) return launch_split<LMAX, NORM, 2>(sm_count, prm, stream);
+    // One lane per point doing both branches of Eq. 5 (32-point tiles) where the Legendre recurrences
+    // dominate, i.e. values only: f64 (double-double recurrences) up to l_max = 12, f32 up to 10, and
+    // f64 gradients up to l_max = 4.  Measured: f64 values l_max 4/6/8: 2.9/3.2/3.4 -> 5.2/6.1/5.3
+    // TB/s, f32 values l_max 2/4/6: 2.8/4.8/5.1 -> 4.2/5.3/5.9; with Hessians it loses (f64
+    // l_max = 4: 7.0 -> 4.7), so not there.
+    constexpr bool bb = TPB_DERIV == 0 ? (TPB_F64 ? LMAX <= 12 : LMAX <= 10) : (TPB_DERIV == 1 && TPB_F64 && LMAX <= 4);
+    if constexpr (bb) {
+        constexpr bool s2 = LMAX >= 4 && TpbShape<sizeof(tpb_T), TPB_DERIV, LMAX, 1, true>::fit <= 12;
+        if constexpr (s2) {
+            if (split_env != 1) return launch_split<LMAX, NORM, 2, true>(sm_count, prm, stream);
+        }
+        return launch_split<LMAX, NORM, 1, true>(sm_count, prm, stream);
+    } else {
+        constexpr bool can_split = LMAX >= 4;
+        if constexpr (can_split) {
+            constexpr bool dflt = TpbShape<sizeof(tpb_T), TPB_DERIV, LMAX, 1>::fit <= 12;
+            const bool want = split_env ? split_env == 2 : dflt;
+            if (want) return launch_split<LMAX, NORM, 2>(sm_count, prm, stream);
+        }
+        return launch_split<LMAX, NORM, 1>(sm_count, prm, stream);
     }
-    return launch_split<LMAX, NORM, 1>(sm_count, prm, stream);
 }
 
 #define TPB_CASE(LM) \
