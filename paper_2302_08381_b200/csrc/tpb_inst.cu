@@ -109,7 +109,8 @@ static int launch_one(int sm_count, const TpbParams& prm, cudaStream_t stream) {
     } else {
         constexpr bool can_split = LMAX >= 4;
         if constexpr (can_split) {
-            constexpr bool dflt = TpbShape<sizeof(tpb_T), TPB_DERIV, LMAX, 1>::fit <= 12;
+            // (long value-only rows: one warp per tile would need > 128 registers at 13+ tiles per SM and spills)
+            constexpr bool dflt = TpbShape<sizeof(tpb_T), TPB_DERIV, LMAX, 1>::fit <= 12 || (TPB_DERIV == 0 && LMAX >= 13);
             const bool want = split_env ? split_env == 2 : dflt;
             if (want) return launch_split<LMAX, NORM, 2>(sm_count, prm, stream);
         }
