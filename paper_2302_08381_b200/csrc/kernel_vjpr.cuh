@@ -3,8 +3,9 @@
 // stored derivatives.  Per point it reads 3 + L values and writes 3, against 4 L + 3 for the stored
 // form (C5: 220 B instead of 796 B), and the forward pass no longer has to write dsph at all.
 //
-// Mapping as in kernel_tpb.cuh: two lanes per point (cos | sin branch of Eq. 5), 16 points per
-// warp, l_max a compile-time constant, one tile per single-warp CTA, non-persistent grid.  The
+// Mapping: ONE lane per point doing both branches of Eq. 5 (the Legendre recurrences, half of the
+// work, run once for the two; with two lanes per point as in kernel_tpb.cuh C5 took 216 us), 32
+// points per warp, l_max a compile-time constant, one tile per single-warp CTA, non-persistent grid.  The
 // tile's grad_sph rows are one contiguous range: a 1-D TMA bulk load brings them to shared memory.
 //
 // The gradient of one harmonic (Eq. 10 with the prefactors folded, normalised form as in
@@ -32,17 +33,17 @@ template <typename T, typename R, bool NORM, int LMAX>
 __global__ void __launch_bounds__(32, 16) sph_vjpr_kernel(const VjprParams prm) {
     using RT = rec<R>;
     constexpr int L = (LMAX + 1) * (LMAX + 1);
-    constexpr uint32_t W_BYTES = TPB_PTS * L * sizeof(T);
+    constexpr int PTS = 32;   // points per tile
+    constexpr uint32_t W_BYTES = PTS * L * sizeof(T);
     const SphTables& TB = c_tables_tpb;
     extern __shared__ __align__(128) unsigned char smem[];
-    T* Wt = reinterpret_cast<T*>(smem);                          // [16][L] upstream gradients of the tile
+    T* Wt = reinterpret_cast<T*>(smem);                          // [32][L] upstream gradients of the tile
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem + W_BYTES);
     const int lane = threadIdx.x;
-    const int pl = lane & (TPB_PTS - 1);   // point inside the tile
-    const bool sinb = lane >= TPB_PTS;     // branch
+    const int pl = lane;                   // point inside the tile
     const int64_t n = prm.n;
     const int64_t tile = blockIdx.x;
-    const int64_t p0 = tile * TPB_PTS;
+    const int64_t p0 = tile * PTS;
     const int64_t p = p0 + pl;
     const T* __restrict__ xyz = static_cast<const T*>(prm.xyz);
     const T* __restrict__ gsph = static_cast<const T*>(prm.grad_sph);
@@ -54,7 +55,7 @@ __global__ void __launch_bounds__(32, 16) sph_vjpr_kernel(const VjprParams prm) 
         grid_dependency_wait();
     }
 
-    const bool full = n - p0 >= TPB_PTS;
+    const bool full = n - p0 >= PTS;
     if (full) {
         if (lane == 0) {
             mbar_init(bar, 1);
@@ -64,7 +65,7 @@ __global__ void __launch_bounds__(32, 16) sph_vjpr_kernel(const VjprParams prm) 
         }
     } else {   // ragged last tile: byte count need not be a multiple of 16 -> plain loads
         const int np = (int)(n - p0);
-        for (int i = lane; i < TPB_PTS * L; i += 32) Wt[i] = i < np * L ? gsph[p0 * L + i] : T(0);
+        for (int i = lane; i < PTS * L; i += 32) Wt[i] = i < np * L ? gsph[p0 * L + i] : T(0);
     }
     __syncwarp();
 
@@ -124,28 +125,42 @@ __global__ void __launch_bounds__(32, 16) sph_vjpr_kernel(const VjprParams prm) 
         if constexpr (m < LMAX) column(std::integral_constant<int, m + 1>{}, Qn);
         const double cd = to_double(c), sd = to_double(s);
         const double dm = (double)m;
-        // azimuthal factor of this lane's branch and its x/y derivatives (Eq. 9, Eq. 10); the sin
+        // azimuthal factors of the two branches and their x/y derivatives (Eq. 9, Eq. 10); the sin
         // branch has no m = 0 harmonic
-        const double A = sinb ? (m == 0 ? 0.0 : sd) : (m == 0 ? SPH_INV_SQRT2 : cd);
-        const double Ax = dm * (sinb ? s1 : c1);
-        const double Ay = dm * (sinb ? c1 : -s1);
-        double S1 = 0.0, Sz = 0.0, SQ = 0.0, Sl = 0.0;
+        const double Ac = (m == 0) ? SPH_INV_SQRT2 : cd, As = sd;
+        const double Acx = dm * c1, Acy = -dm * s1, Asx = dm * s1, Asy = dm * c1;
+        double S1c = 0.0, Szc = 0.0, SQc = 0.0, Slc = 0.0;   // the four sums of the cos branch
+        double S1s = 0.0, Szs = 0.0, SQs = 0.0, Sls = 0.0;   // ... of the sin branch
         static_for<m, LMAX + 1>([&](auto lc) {
             constexpr int l = decltype(lc)::value;
             constexpr int kc = l * (l + 1) + m, ks = l * (l + 1) - m;
             constexpr int t = SPH_TRI(l, m);
-            const double w = static_cast<double>(W[sinb ? ks : kc]);
-            const double Qw = Qc[l] * w;
-            SQ += Qw;
-            if (NORM) Sl = SPH_FMA((double)l, Qw, Sl);
-            if constexpr (l >= m + 2) S1 = SPH_FMA(TB.G1[t] * Qn[l - 1], w, S1);   // F_l^m Q_{l-1}^{m+1}
-            if constexpr (l >= m + 1) Sz = SPH_FMA(TB.Gz[t] * Qc[l - 1], w, Sz);   // F_l^m (l+m) Q_{l-1}^m
+            const double wc = static_cast<double>(W[kc]);
+            const double ws = (m > 0) ? static_cast<double>(W[ks]) : 0.0;
+            const double Q = Qc[l];
+            SQc = SPH_FMA(Q, wc, SQc);
+            SQs = SPH_FMA(Q, ws, SQs);
+            if (NORM) {
+                const double lQ = (double)l * Q;
+                Slc = SPH_FMA(lQ, wc, Slc);
+                Sls = SPH_FMA(lQ, ws, Sls);
+            }
+            if constexpr (l >= m + 2) {   // F_l^m Q_{l-1}^{m+1}
+                const double q1 = TB.G1[t] * Qn[l - 1];
+                S1c = SPH_FMA(q1, wc, S1c);
+                S1s = SPH_FMA(q1, ws, S1s);
+            }
+            if constexpr (l >= m + 1) {   // F_l^m (l+m) Q_{l-1}^m
+                const double qz = TB.Gz[t] * Qc[l - 1];
+                Szc = SPH_FMA(qz, wc, Szc);
+                Szs = SPH_FMA(qz, ws, Szs);
+            }
         });
-        const double T1 = NORM ? S1 - Sl : S1;
-        const double Tz = NORM ? SPH_FMA(-zd, Sl, Sz) : Sz;
-        ax += SPH_FMA(xd * A, T1, Ax * SQ);
-        ay += SPH_FMA(yd * A, T1, Ay * SQ);
-        az = SPH_FMA(A, Tz, az);
+        const double T1c = NORM ? S1c - Slc : S1c, T1s = NORM ? S1s - Sls : S1s;
+        const double Tzc = NORM ? SPH_FMA(-zd, Slc, Szc) : Szc, Tzs = NORM ? SPH_FMA(-zd, Sls, Szs) : Szs;
+        ax += SPH_FMA(xd * Ac, T1c, Acx * SQc) + SPH_FMA(xd * As, T1s, Asx * SQs);
+        ay += SPH_FMA(yd * Ac, T1c, Acy * SQc) + SPH_FMA(yd * As, T1s, Asy * SQs);
+        az = SPH_FMA(Ac, Tzc, SPH_FMA(As, Tzs, az));
         if constexpr (m < LMAX) {   // next column, next power of (x + i y): Eq. 9
             static_for<m + 1, LMAX + 1>([&](auto lc) { Qc[decltype(lc)::value] = Qn[decltype(lc)::value]; });
             c1 = cd;
@@ -161,11 +176,7 @@ __global__ void __launch_bounds__(32, 16) sph_vjpr_kernel(const VjprParams prm) 
         ay *= rinv;
         az *= rinv;
     }
-    // the two branches of a point sit 16 lanes apart
-    ax += __shfl_xor_sync(0xffffffffu, ax, TPB_PTS);
-    ay += __shfl_xor_sync(0xffffffffu, ay, TPB_PTS);
-    az += __shfl_xor_sync(0xffffffffu, az, TPB_PTS);
-    if (!sinb && p < n) {
+    if (p < n) {
         gxyz[3 * p + 0] = static_cast<T>(ax);
         gxyz[3 * p + 1] = static_cast<T>(ay);
         gxyz[3 * p + 2] = static_cast<T>(az);

@@ -25,7 +25,7 @@ typedef double vjpr_R;
 
 template <int LMAX, bool NORM> static int launch_one(VjprParams prm, cudaStream_t stream) {
     constexpr int L = (LMAX + 1) * (LMAX + 1);
-    constexpr int smem = TPB_PTS * L * (int)sizeof(vjpr_T) + 16;
+    constexpr int smem = 32 * L * (int)sizeof(vjpr_T) + 16;   // 32 points per tile
     auto kern = sph_vjpr_kernel<vjpr_T, vjpr_R, NORM, LMAX>;
     static bool attr_done[64] = {false};   // per device; benign race (idempotent call)
     int dev = 0;
@@ -34,7 +34,7 @@ template <int LMAX, bool NORM> static int launch_one(VjprParams prm, cudaStream_
         if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return -1;
         attr_done[dev] = true;
     }
-    const int64_t n_tiles = (prm.n + TPB_PTS - 1) / TPB_PTS;
+    const int64_t n_tiles = (prm.n + 31) / 32;
     if (n_tiles > 0x7fffffff) return 1;
     // programmatic dependent launch, as for the forward kernels (tpb_inst.cu)
     cudaLaunchConfig_t cfg = {};
