@@ -179,9 +179,12 @@ static int launch_w(const DeviceState& st, const void* xyz, int64_t n, int l_max
                     void* sph, void* dsph, void* ddsph, cudaStream_t stream) {
     const char* force = getenv("SPHB200_FORCE_KERNEL");  // "w1": the one-warp-per-point kernel even for long rows
     if (!(force && force[0] == 'w' && force[1] == '1')) {
-        // long rows: the warps of a CTA share one point, chunks of half a row, ~4 KB bulk stores
+        // the longest f64 rows: the warps of a CTA share one point, chunks of a third of a row, ~3 KB
+        // bulk stores (kernel_wc.cuh says where it wins); "wc" forces it wherever it can run
+        const bool force_wc = force && force[0] == 'w' && force[1] == 'c';
+        const int min_l = force_wc ? 19 : (dtype == SPHERICART_CUDA_F64 ? 32 : SPHERICART_CUDA_MAX_L + 1);
         WcLaunch lc{};
-        if (wc_plan(st.sm_count, st.smem_optin, n, l_max, normalized, dtype, sph, dsph, ddsph, xyz, st.d_tables, &lc) == 0) {
+        if (wc_plan(min_l, st.sm_count, st.smem_optin, n, l_max, normalized, dtype, sph, dsph, ddsph, xyz, st.d_tables, &lc) == 0) {
             int rc = allow_smem(lc.func, (int)lc.smem);
             if (rc) return rc;
             wc_launch(lc, stream);

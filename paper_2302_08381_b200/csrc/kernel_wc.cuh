@@ -1,6 +1,10 @@
 // "wc" forward kernel: the warps of a CTA work TOGETHER on one point at a time, so that a staged
-// chunk is a third of a row (<= 368 harmonics) and every bulk store is ~3 KB.  Long rows
-// (l_max >= 19), values / +gradients / +Hessians -- config C4.
+// chunk is a third of a row (<= 368 harmonics) and every bulk store is ~3 KB.  Works for
+// l_max >= 19 and any derivative order; used by default where it wins: f64 at l_max = 32 --
+// config C4.  (Measured, Hessians, 131 072-262 144 points: f64 l_max = 32 5.0 TB/s against 4.7 for the
+// one-warp-per-point kernel -- 6.2 against 4.9 at C4's full size with rotating outputs -- but
+// 4.4-4.9 against 4.7-5.1 at l_max 28-31, whose rows split less evenly into chunks and, for even L,
+// are 128-byte aligned anyway; f32: 1.9-2.8 against 2.7-2.9 at every l_max.)
 //
 // Why (profiles/r1b_kernels.md): the one-warp-per-point kernel (kernel_w.cuh) can stage
 // only ~128 harmonics of each of its 13 output rows, so a point leaves as 143 bulk stores of ~1 KB
@@ -335,11 +339,11 @@ template <typename T, typename R> static WcKernel wc_pick(int deriv, int norm, b
 
 // returns 0 and fills *out if the cooperative kernel applies (rows long enough to be worth it and
 // the carve-up fits), 1 otherwise
-static inline int wc_plan(int sm_count, int smem_optin, int64_t n, int l_max, int normalized, int dtype, void* sph, void* dsph,
+static inline int wc_plan(int min_l, int sm_count, int smem_optin, int64_t n, int l_max, int normalized, int dtype, void* sph, void* dsph,
                           void* ddsph, const void* xyz, const SphTables* d_tab, WcLaunch* out) {
     const int deriv = ddsph ? 2 : (dsph ? 1 : 0);
     const int esize = dtype == 0 ? 4 : 8;
-    if (l_max < wk_env("SPHB200_WC_MIN_L", 19)) return 1;
+    if (l_max < wk_env("SPHB200_WC_MIN_L", min_l)) return 1;
     const WcSmem lay(l_max, deriv, esize);
     if ((int64_t)lay.total > smem_optin) return 1;
     const bool lodd = (l_max & 1) == 0;
