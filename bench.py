@@ -3,6 +3,8 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2] [--no-sweep]
     python bench.py --impl reference ...        # the CPU oracle, as it stands, on the host cores
+    python bench.py --lmax-sweep                # the full l_max table (profiles/lmax_sweep_r2.json)
+    python bench.py --kernels-only --workload custom --dtype f32 --deriv 1 --l-max 24   # the command ncu wraps
 
 A "step" is one pass of the hot path over one batch of the named workload: one
 ``sphericart_cuda_compute`` call and, for C5, the ``sphericart_cuda_vjp``
@@ -15,7 +17,8 @@ GB/s vs l_max, f32/f64, +-grads") but the JSON line's headline keys are C2's.
 
 Multi-GPU: the path shards over points with no communication; every rank
 runs the same per-GPU batch ("scaling": "weak"), a barrier + synchronize brackets the timed region
-and the time is the max over ranks.
+and the time is the max over ranks.  `--gpus N` with no WORLD_SIZE in the environment starts its own
+N ranks (torch.distributed.run on 127.0.0.1); under torchrun it is one of them.
 """
 from __future__ import annotations
 
@@ -47,15 +50,15 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-# ncu --set full: dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel,
-# copied by hand from the capture summarised under profiles/ (None until a capture exists).
-NCU_TRAFFIC_BYTES = {
-    # profiles/r1b_kernels.md
-    "C2": 71.43e6,     # 70.19 MB written + 1.24 MB read (a single launch's 129.6 MB output is L2-sized)
-    "C3": 1108.6e6,    # 1096.6 MB written + 12.05 MB read
-    "C4": 29.689e9,    # sph_wc_kernel: 29.676 GB written + 0.013 GB read
-    "C5": 3124.6e6,    # forward kernel: 3076.6 MB written + 48.0 MB read
-}
+def ncu_traffic_bytes(name):
+    """ncu --set full: dram__bytes_read.sum + dram__bytes_write.sum per launch of the configuration's
+    forward kernel, from the capture summarised in profiles/ncu_traffic.json (which names the capture
+    and its command); None when there is no capture of the kernel as it stands."""
+    p = ROOT / "profiles" / "ncu_traffic.json"
+    if not p.exists():
+        return None
+    ent = json.loads(p.read_text()).get(name)
+    return None if ent is None else float(ent["dram_bytes_per_launch"])
 
 
 # -------------------------------------------------------------------------------------------------
@@ -234,12 +237,21 @@ def sweep_one(cfg, torch, pkg, device, peak):
            "buffer_sets": len(wl.sets), "fwd_us": round(ms_f * 1e3, 2), "fwd_points_per_s": cfg.n / (ms_f * 1e-3),
            "fwd_gbs": cfg.n * fwd_b / (ms_f * 1e-3) / 1e9}
     res["fwd_frac_of_measured_peak"] = res["fwd_gbs"] / peak
+    res["kernel"] = pkg.sphericart_cuda_last_kernel()
+    res["roofline"] = {"bound": "hbm", "kernel": "forward (" + res["kernel"] + ")", "achieved": res["fwd_gbs"],
+                       "peak": peak, "unit": "GB/s", "frac": res["fwd_gbs"] / peak,
+                       "traffic": ncu_traffic_bytes(cfg.name), "algorithmic_bytes_per_launch": cfg.n * fwd_b,
+                       "avg_launch_us": ms_f * 1e3}
     if cfg.vjp:
         e0, e1 = time_loop(torch, wl.backward, reps)
         torch.cuda.synchronize()
         ms_b = e0.elapsed_time(e1) / reps
         res.update({"vjp_us": round(ms_b * 1e3, 2), "vjp_gbs": cfg.n * vjp_b / (ms_b * 1e-3) / 1e9})
         res["vjp_frac_of_measured_peak"] = res["vjp_gbs"] / peak
+        res["vjp_roofline"] = {"bound": "hbm", "kernel": "vjp (" + pkg.sphericart_cuda_last_kernel() + ")",
+                               "achieved": res["vjp_gbs"], "peak": peak, "unit": "GB/s", "frac": res["vjp_gbs"] / peak,
+                               "traffic": ncu_traffic_bytes(cfg.name + "_vjp"),
+                               "algorithmic_bytes_per_launch": cfg.n * vjp_b, "avg_launch_us": ms_b * 1e3}
         # the same backward without stored derivatives (reads xyz + grad_sph only), and
         # the values-only forward it pairs with
         esize = 4 if cfg.dtype == "f32" else 8
@@ -250,13 +262,18 @@ def sweep_one(cfg, torch, pkg, device, peak):
             e0, e1 = time_loop(torch, fn, reps)
             torch.cuda.synchronize()
             ms = e0.elapsed_time(e1) / reps
-            res.update({key + "_us": round(ms * 1e3, 2), key + "_gbs": cfg.n * bytes_pt / (ms * 1e-3) / 1e9})
+            gbs = cfg.n * bytes_pt / (ms * 1e-3) / 1e9
+            res.update({key + "_us": round(ms * 1e3, 2), key + "_gbs": gbs})
+            res[key + "_roofline"] = {"bound": "hbm", "kernel": key + " (" + pkg.sphericart_cuda_last_kernel() + ")",
+                                      "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
+                                      "traffic": ncu_traffic_bytes(cfg.name + "_" + key),
+                                      "algorithmic_bytes_per_launch": cfg.n * bytes_pt, "avg_launch_us": ms * 1e3}
     del wl
     torch.cuda.empty_cache()
     return res
 
 
-def sweep_expand(torch, pkg, device):
+def sweep_expand(torch, pkg, device, peak):
     """the fused density expansion of Eq. 1 on a neighbour-list-shaped input
     (32768 centres x Poisson(32) neighbours, l_max = 8, n_rad = 8, f32), and the values-only forward
     over the same points as context (what an unfused consumer would have to run first)."""
@@ -283,45 +300,65 @@ def sweep_expand(torch, pkg, device):
         res[key + "_points_per_s"] = n / (ms * 1e-3)
     in_bytes = n * (12 + n_rad * (l_max + 1) * 4) + n_seg * (8 + n_rad * L * 4)
     res["expand_algorithmic_gbs"] = in_bytes / (res["expand_us"] * 1e-6) / 1e9
+    res["roofline"] = {"bound": "hbm", "kernel": "expand", "achieved": res["expand_algorithmic_gbs"], "peak": peak,
+                       "unit": "GB/s", "frac": res["expand_algorithmic_gbs"] / peak,
+                       "traffic": ncu_traffic_bytes("N2_expand"), "algorithmic_bytes_per_launch": in_bytes,
+                       "avg_launch_us": res["expand_us"]}
     return res
 
 
-def lmax_sweep(torch, pkg, device, peak):
-    """`--lmax-sweep`: the metric's own axis -- output GB/s and points/s against l_max, f32 / f64,
-    values / + gradients / + Hessians (normalised harmonics, xyz ~ N(0,1), n sized for ~1.5 GB of
-    output but at least 64 points per SM, two rotating output sets where they fit).  One JSON object; not part of the default run."""
+LMAX_FULL = (1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12, 13, 14, 15, 16, 20, 24, 28, 32)
+LMAX_BRIEF = (8, 12, 16, 20, 24, 28, 32)       # the cells of the default run (the >= 70 % clause: l_max >= 8)
+
+
+def lmax_cell(torch, pkg, device, peak, dtype, deriv, l_max, normalized=1, n=None, reps=None):
+    """One cell of the metric's axis: xyz ~ N(0,1) on the device, n sized for ~1.5 GB of output (at
+    most 4 M points, at least 64 per SM), two rotating output sets where they fit; CUDA events."""
     st = torch.cuda.current_stream().cuda_stream
+    tdt, es = (torch.float32, 4) if dtype == "f32" else (torch.float64, 8)
+    mult = (1, 4, 13)[deriv]
+    L = (l_max + 1) ** 2
+    per_pt = L * es * mult
+    if n is None:
+        n = int(min(4_000_000, 1.5e9 // per_pt)) // 256 * 256
+        if n < 148 * 64:          # too few points to fill the machine within the byte budget:
+            n = 148 * 64          # (Hessians at l_max >= 20) take more memory instead
+    x = torch.randn(n, 3, device=device, dtype=tdt)
+    n_sets = 2 if n * per_pt < 3e9 else 1
+    outs = [(torch.empty((n, L), device=device, dtype=tdt),
+             torch.empty((n, 3, L), device=device, dtype=tdt) if deriv >= 1 else None,
+             torch.empty((n, 3, 3, L), device=device, dtype=tdt) if deriv >= 2 else None)
+            for _ in range(n_sets)]
+    fn = lambda i: pkg.sphericart_cuda_compute(x, n, l_max, normalized, pkg.F32 if dtype == "f32" else pkg.F64,
+                                               *outs[i % n_sets], st)
+    for i in range(3):
+        fn(i)
+    torch.cuda.synchronize()
+    if reps is None:
+        reps = 10 if n * per_pt < 3e9 else 4
+    e0, e1 = time_loop(torch, fn, reps)
+    torch.cuda.synchronize()
+    sec = e0.elapsed_time(e1) / reps * 1e-3
+    gbs = n * per_pt / sec / 1e9
+    del outs, x
+    return {"n": n, "us": round(sec * 1e6, 1), "points_per_s": n / sec, "out_gbs": round(gbs, 1),
+            "frac": round(gbs / peak, 3), "kernel": pkg.sphericart_cuda_last_kernel()}
+
+
+def lmax_sweep(torch, pkg, device, peak, l_values=LMAX_FULL):
+    """The metric's own axis -- output GB/s and points/s against l_max, f32 / f64, values / + gradients
+    / + Hessians (normalised harmonics), with the kernel family that served each cell and the fraction
+    of the measured HBM peak.  `--lmax-sweep` prints every l_max of LMAX_FULL as one JSON object; the
+    default run carries LMAX_BRIEF under sweep.lmax."""
     rows = {}
-    for dtype, tdt, es in (("f32", torch.float32, 4), ("f64", torch.float64, 8)):
+    for dtype in ("f32", "f64"):
         for deriv, tag in ((0, "values"), (1, "grads"), (2, "hessians")):
-            key = f"{dtype}_{tag}"
-            rows[key] = {}
-            mult = (1, 4, 13)[deriv]
-            for l_max in (1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12, 13, 14, 15, 16, 20, 24, 28, 32):
-                L = (l_max + 1) ** 2
-                per_pt = L * es * mult
-                n = int(min(4_000_000, 1.5e9 // per_pt)) // 256 * 256
-                if n < 148 * 64:          # too few points to fill the machine within the byte budget:
-                    n = 148 * 64          # (Hessians at l_max >= 20) take more memory instead
-                x = torch.randn(n, 3, device=device, dtype=tdt)
-                n_sets = 2 if n * per_pt < 3e9 else 1
-                outs = [(torch.empty((n, L), device=device, dtype=tdt),
-                         torch.empty((n, 3, L), device=device, dtype=tdt) if deriv >= 1 else None,
-                         torch.empty((n, 3, 3, L), device=device, dtype=tdt) if deriv >= 2 else None)
-                        for _ in range(n_sets)]
-                fn = lambda i: pkg.sphericart_cuda_compute(x, n, l_max, 1, pkg.F32 if dtype == "f32" else pkg.F64,
-                                                           *outs[i % n_sets], st)
-                for i in range(3):
-                    fn(i)
-                torch.cuda.synchronize()
-                reps = 10 if n * per_pt < 3e9 else 4
-                e0, e1 = time_loop(torch, fn, reps)
-                torch.cuda.synchronize()
-                sec = e0.elapsed_time(e1) / reps * 1e-3
-                rows[key][str(l_max)] = {"n": n, "us": round(sec * 1e6, 1), "points_per_s": n / sec,
-                                         "out_gbs": round(n * per_pt / sec / 1e9, 1),
-                                         "frac_of_measured_peak": round(n * per_pt / sec / 1e9 / peak, 3)}
-                del outs, x
+            rows[f"{dtype}_{tag}"] = {str(l): lmax_cell(torch, pkg, device, peak, dtype, deriv, l) for l in l_values}
+    cells = [c for r in rows.values() for l, c in r.items() if int(l) >= 8]
+    rows["summary"] = {"cells_lmax_ge_8": len(cells),
+                       "cells_at_or_above_0.70_of_measured_peak": sum(c["frac"] >= 0.70 for c in cells),
+                       "min_out_gbs_lmax_ge_8": min(c["out_gbs"] for c in cells) if cells else None,
+                       "frac_is": "out_gbs / measured copy peak (MEASURED_PEAKS.json hbm_gbs)"}
     return rows
 
 
@@ -391,6 +428,62 @@ def oracle_baseline(cfg, budget_s=12.0):
                       f"median of {len(times)} passes, {med * 1e3:.2f} ms per pass"}, n, med
 
 
+def workload_config(args):
+    """One of BASELINE.json's configurations, or `--workload custom`: any (dtype, l_max, outputs) cell
+    on xyz ~ N(0,1), n sized as in the l_max sweep -- the command ncu wraps for the kernels that serve
+    cells outside the five configurations."""
+    if args.workload != "custom":
+        return W.CONFIGS[args.workload]
+    es = 4 if args.dtype == "f32" else 8
+    per_pt = (args.l_max + 1) ** 2 * es * (1, 4, 13)[args.deriv]
+    n = args.n or max(148 * 64, int(min(4_000_000, 1.5e9 // per_pt)) // 256 * 256)
+    what = (f"custom: N={n} {args.dtype} l_max={args.l_max} {'solid' if args.solid else 'normalized'} "
+            f"{('Y', 'Y+grad', 'Y+grad+Hessian')[args.deriv]}, xyz~N(0,1)")
+    return W.Config("C9", n, args.dtype, args.l_max, not args.solid, args.deriv >= 1, args.deriv >= 2, False, what)
+
+
+def spawn_ranks(n_ranks, argv, extra_env=None):
+    """`--gpus N` without a launcher: start N ranks of this script under torch.distributed.run on
+    127.0.0.1 (free port), one per GPU, and pass their output through (rank 0 prints the JSON line).
+    NCCL's own communicator lines stay on (NCCL_DEBUG=INFO goes to stderr)."""
+    import socket
+    import subprocess
+
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")
+    env.setdefault("OMP_NUM_THREADS", "1")
+    env.update(extra_env or {})
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n_ranks}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), str(Path(__file__).resolve()), *argv]
+    return subprocess.run(cmd, env=env).returncode
+
+
+def run_stub(args):
+    """--impl stub (tests only, no GPU): the rank plumbing of run_cuda -- process group, barrier,
+    max-over-ranks time, one JSON line from rank 0 -- on the gloo backend with a sleep as the step."""
+    import torch
+    import torch.distributed as dist
+
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    if world > 1:
+        dist.init_process_group("gloo")
+        dist.barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        time.sleep(0.001 * (1 + rank))
+    ms = torch.tensor([(time.perf_counter() - t0) * 1e3], dtype=torch.float64)
+    if world > 1:
+        dist.barrier()
+        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps({"impl": "stub", "n_gpus": world, "steps": args.steps, "ms_per_step": float(ms) / args.steps,
+                          "value": world * 1000 / (float(ms) / args.steps * 1e-3), "scaling": "weak"}))
+
+
 def run_cuda(args):
     import torch
 
@@ -410,7 +503,10 @@ def run_cuda(args):
     import paper_2302_08381_b200 as pkg
 
     pkg.load()                                   # raises if the CUDA library is missing
-    cfg = W.CONFIGS[args.workload]
+    for kv in args.option:
+        k, _, v = kv.partition("=")
+        pkg.sphericart_cuda_set_option(k, v)
+    cfg = workload_config(args)
     peak, peak_src = measured_peaks()
     if args.lmax_sweep:
         if rank == 0:
@@ -454,8 +550,8 @@ def run_cuda(args):
     else:
         ms_fwd = ms_step
     achieved = cfg.n * fwd_b / (ms_fwd * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "forward (sph_tpb_kernel; sph_wc_kernel for C4)", "achieved": achieved,
-                "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg.name),
+    roofline = {"bound": "hbm", "kernel": "forward (" + pkg.sphericart_cuda_last_kernel() + ")", "achieved": achieved,
+                "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": ncu_traffic_bytes(cfg.name),
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": cfg.n * fwd_b,
                 "avg_launch_us": ms_fwd * 1e3, "output_gbs": cfg.n * cfg.out_bytes_per_point / (ms_fwd * 1e-3) / 1e9,
                 "frac_of_nominal_8tbs": achieved / 8000.0}
@@ -463,7 +559,11 @@ def run_cuda(args):
     line = {"metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic",
-            "config": {"workload": f"{cfg.name}: {cfg.what}", "n_points_per_gpu": cfg.n, "l_max": cfg.l_max,
+            "config": {"workload": f"{cfg.name}: {cfg.what}",
+                       "why_this_workload": "BASELINE.json configs[1], the configuration the metric is quoted on; the "
+                                            "larger single-GPU configurations (C3, C4, C5) and the l_max axis carry "
+                                            "their own roofline blocks under sweep",
+                       "n_points_per_gpu": cfg.n, "l_max": cfg.l_max,
                        "normalized": cfg.normalized, "gradients": cfg.gradients, "hessians": cfg.hessians,
                        "vjp": cfg.vjp, "parallelism": f"points sharded over {world} GPU(s), no collective",
                        "l2": f"outputs rotate over {len(wl.sets)} buffer sets "
@@ -502,7 +602,8 @@ def run_cuda(args):
                     line["sweep"][name] = {"skipped": "does not fit in free HBM"}
                     continue
                 line["sweep"][name] = sweep_one(c, torch, pkg, device, peak)
-            line["sweep"]["N2_expand"] = sweep_expand(torch, pkg, device)
+            line["sweep"]["N2_expand"] = sweep_expand(torch, pkg, device, peak)
+            line["sweep"]["lmax"] = lmax_sweep(torch, pkg, device, peak, LMAX_BRIEF)
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()
@@ -517,7 +618,7 @@ def run_reference(args):
     import oracle
 
     oracle.build()
-    cfg = W.CONFIGS[args.workload]
+    cfg = workload_config(args)
     cores = oracle.num_threads("f64")
     # one step = one oracle pass over a bounded sample, sized so the whole run ends within minutes
     per_point = 60e-9 * cfg.n_sph * (1 + 3 * cfg.gradients + 9 * cfg.hessians) / cores
@@ -557,8 +658,15 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=None)
     ap.add_argument("--warmup", type=int, default=None)
-    ap.add_argument("--impl", choices=["cuda", "reference"], default="cuda")
-    ap.add_argument("--workload", choices=sorted(W.CONFIGS), default="C2")
+    ap.add_argument("--impl", choices=["cuda", "reference", "stub"], default="cuda")
+    ap.add_argument("--workload", choices=sorted(W.CONFIGS) + ["custom"], default="C2")
+    ap.add_argument("--dtype", choices=["f32", "f64"], default="f32", help="--workload custom")
+    ap.add_argument("--l-max", type=int, default=8, help="--workload custom")
+    ap.add_argument("--deriv", type=int, choices=[0, 1, 2], default=1, help="--workload custom: 0 Y, 1 +grad, 2 +Hessian")
+    ap.add_argument("--solid", action="store_true", help="--workload custom: solid harmonics instead of normalised")
+    ap.add_argument("--n", type=int, default=0, help="--workload custom: points (default: ~1.5 GB of output)")
+    ap.add_argument("--option", action="append", default=[], metavar="NAME=VALUE",
+                    help="sphericart_cuda_set_option(NAME, VALUE) before anything runs (experiments)")
     ap.add_argument("--e2e-steps", type=int, default=20)
     ap.add_argument("--no-sweep", action="store_true", help="skip the brief timing of the other configurations")
     ap.add_argument("--lmax-sweep", action="store_true",
@@ -570,13 +678,13 @@ def main():
         args.steps = 20 if args.steps is None else args.steps
         args.warmup = 1 if args.warmup is None else args.warmup
         return run_reference(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:      # no launcher: start the ranks ourselves
+        raise SystemExit(spawn_ranks(args.gpus, sys.argv[1:]))
+    if args.impl == "stub":
+        args.steps = 5 if args.steps is None else args.steps
+        return run_stub(args)
     args.steps = 2000 if args.steps is None else args.steps
     args.warmup = 20 if args.warmup is None else args.warmup
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    if world != args.gpus:
-        if args.gpus > 1 and world == 1:
-            raise SystemExit(f"--gpus {args.gpus}: launch with python -m torch.distributed.run --nproc-per-node "
-                             f"{args.gpus} --master-addr 127.0.0.1 bench.py --gpus {args.gpus} ...")
     run_cuda(args)
 
 

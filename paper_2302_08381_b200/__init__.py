@@ -58,6 +58,10 @@ def load():
     lib.sphericart_cuda_last_error.argtypes = []
     lib.sphericart_cuda_launch_count.restype = i64
     lib.sphericart_cuda_launch_count.argtypes = []
+    lib.sphericart_cuda_last_kernel.restype = ctypes.c_char_p
+    lib.sphericart_cuda_last_kernel.argtypes = []
+    lib.sphericart_cuda_set_option.restype = ci
+    lib.sphericart_cuda_set_option.argtypes = [ctypes.c_char_p, ctypes.c_char_p]
     _lib = lib
     return lib
 
@@ -122,6 +126,15 @@ def sphericart_cuda_last_error() -> str:
 
 def sphericart_cuda_launch_count() -> int:
     return int(load().sphericart_cuda_launch_count())
+
+
+def sphericart_cuda_last_kernel() -> str:
+    return load().sphericart_cuda_last_kernel().decode()
+
+
+def sphericart_cuda_set_option(name: str, value) -> None:
+    rc = load().sphericart_cuda_set_option(str(name).encode(), str(value).encode())
+    _check(rc, "sphericart_cuda_set_option")
 
 
 # --- torch.Tensor convenience (allocation + marshalling only) -----------------------------------

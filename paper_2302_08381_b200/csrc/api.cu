@@ -11,7 +11,9 @@
 
 #include <cuda_runtime.h>
 
-#include "kernel_tp.cuh"
+#include "options.h"
+#include "ptx.cuh"
+#include "sph_core.cuh"
 #include "kernel_vjp.cuh"
 #include "kernel_tpg.cuh"
 #include "kernel_w.cuh"
@@ -20,8 +22,19 @@
 
 namespace sphb200 {
 
+SphOptions g_opt;   // options.h
+
+// constant-bank copy of the coefficient tables for the kernels of this translation unit
+__constant__ SphTables c_tables;
+
 static thread_local char g_err[512] = "";
+static thread_local const char* g_last_kernel = "";
 static std::atomic<int64_t> g_launches{0};
+
+static void launched(const char* family) {
+    g_last_kernel = family;
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+}
 
 static int fail(int code, const char* fmt, ...) {
     va_list ap;
@@ -44,6 +57,7 @@ static int fail(int code, const char* fmt, ...) {
 constexpr int MAX_DEVICES = 64;
 struct DeviceState {
     bool ready = false;
+    std::atomic<bool> ready_flag{false};
     int sm_count = 0;
     int smem_optin = 0;          // max dynamic shared memory per block
     SphTables* d_tables = nullptr;   // copy of the tables in global memory (warp kernel)
@@ -58,6 +72,10 @@ static int device_state(DeviceState** out) {
     CUDA_TRY(cudaGetDevice(&dev));
     if (dev < 0 || dev >= MAX_DEVICES) return fail(SPHERICART_CUDA_ECUDA, "device index %d out of range", dev);
     DeviceState& st = g_dev[dev];
+    if (st.ready_flag.load(std::memory_order_acquire)) {   // the common case takes no lock
+        *out = &st;
+        return 0;
+    }
     std::lock_guard<std::mutex> lock(g_mutex);
     if (!st.ready) {
         std::call_once(g_tables_once, [] { sph_build_tables(&g_host_tables); });
@@ -78,15 +96,17 @@ static int device_state(DeviceState** out) {
         CUDA_TRY(cudaMalloc(&st.d_tables, sizeof(SphTables)));
         CUDA_TRY(cudaMemcpy(st.d_tables, &g_host_tables, sizeof(SphTables), cudaMemcpyHostToDevice));
         st.ready = true;
+        st.ready_flag.store(true, std::memory_order_release);
     }
     *out = &st;
     return 0;
 }
 
 // cudaFuncSetAttribute(MaxDynamicSharedMemorySize) once per (device, kernel)
+constexpr int MAX_OPTIN_KERNELS = 512;   // more than the instantiations api.cu can launch
 static int allow_smem(const void* func, int bytes) {
     static std::mutex m;
-    static const void* done[MAX_DEVICES][64];
+    static const void* done[MAX_DEVICES][MAX_OPTIN_KERNELS];
     static int n_done[MAX_DEVICES];
     int dev = 0;
     CUDA_TRY(cudaGetDevice(&dev));
@@ -95,80 +115,9 @@ static int allow_smem(const void* func, int bytes) {
         if (done[dev][i] == func) return 0;
     (void)bytes;
     CUDA_TRY(cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, g_dev[dev].smem_optin));
-    if (n_done[dev] < 64) done[dev][n_done[dev]++] = func;
-    return 0;
-}
-
-static int env_int(const char* name, int dflt) {
-    const char* s = getenv(name);
-    return (s && *s) ? atoi(s) : dflt;
-}
-
-// ---------------------------------------------------------------------------------------------
-// forward: thread-per-point kernel
-// ---------------------------------------------------------------------------------------------
-typedef void (*TpKernel)(const TpParams);
-
-template <typename T, typename R> static TpKernel tp_pick(int deriv, int norm) {
-    if (deriv == 0) return norm ? sph_tp_kernel<T, R, 0, true> : sph_tp_kernel<T, R, 0, false>;
-    return norm ? sph_tp_kernel<T, R, 1, true> : sph_tp_kernel<T, R, 1, false>;
-}
-
-// Can the tp kernel run this shape, and with how many warps?  Returns 0 if not.
-static int tp_plan(const DeviceState& st, int64_t n, int l_max, int deriv, int esize, TpParams* prm,
-                   int* grid, size_t* smem) {
-    if (deriv > 1) return 0;
-    const int L = (l_max + 1) * (l_max + 1);
-    const uint32_t tile_bytes = 32u * L * esize * (deriv ? 4 : 1);
-    const int budget = st.smem_optin - 1024;
-    int max_warps = TP_MAX_THREADS / 32;
-    int nbuf = env_int("SPHB200_TP_NBUF", 0);
-    int warps = env_int("SPHB200_TP_WARPS", 0);
-    if (nbuf <= 0) nbuf = ((int64_t)2 * tile_bytes * 8 <= budget) ? 2 : 1;  // 2 images if >= 8 warps still fit
-    if (warps <= 0) warps = max_warps;
-    int fit = (int)(budget / ((int64_t)nbuf * tile_bytes));
-    if (fit < 1 && nbuf == 2) {
-        nbuf = 1;
-        fit = (int)(budget / (int64_t)tile_bytes);
-    }
-    if (fit < 1) return 0;
-    if (warps > fit) warps = fit;
-    const int64_t n_tiles = (n + 31) / 32;
-    // small problems: spread the tiles over the SMs instead of stacking warps on a few of them
-    int64_t per_sm = (n_tiles + st.sm_count - 1) / st.sm_count;
-    if (per_sm < warps) warps = (int)(per_sm < 1 ? 1 : per_sm);
-    int64_t ctas = (n_tiles + warps - 1) / warps;
-    if (ctas > st.sm_count) ctas = st.sm_count;
-    prm->warps_per_cta = warps;
-    prm->nbuf = nbuf;
-    prm->tile_bytes = tile_bytes;
-    *grid = (int)ctas;
-    *smem = (size_t)warps * nbuf * tile_bytes;
-    return warps;
-}
-
-static int launch_tp(const DeviceState& st, const void* xyz, int64_t n, int l_max, int normalized, int dtype,
-                     void* sph, void* dsph, cudaStream_t stream, bool* handled) {
-    TpParams prm{};
-    int grid = 0;
-    size_t smem = 0;
-    const int deriv = dsph ? 1 : 0;
-    const int esize = dtype == SPHERICART_CUDA_F32 ? 4 : 8;
-    const int warps = tp_plan(st, n, l_max, deriv, esize, &prm, &grid, &smem);
-    *handled = warps > 0;
-    if (!*handled) return 0;
-    prm.xyz = xyz;
-    prm.sph = sph;
-    prm.dsph = dsph;
-    prm.n = n;
-    prm.l_max = l_max;
-    TpKernel k = dtype == SPHERICART_CUDA_F32 ? tp_pick<float, double>(deriv, normalized)
-                                              : tp_pick<double, dd>(deriv, normalized);
-    int rc = allow_smem((const void*)k, (int)smem);
-    if (rc) return rc;
-    k<<<grid, warps * 32, smem, stream>>>(prm);
-    g_launches.fetch_add(1, std::memory_order_relaxed);
-    CUDA_TRY(cudaGetLastError());
+    if (n_done[dev] >= MAX_OPTIN_KERNELS)
+        return fail(SPHERICART_CUDA_ECUDA, "internal: more than %d opt-in kernels", MAX_OPTIN_KERNELS);
+    done[dev][n_done[dev]++] = func;
     return 0;
 }
 
@@ -177,18 +126,18 @@ static int launch_tp(const DeviceState& st, const void* xyz, int64_t n, int l_ma
 // ---------------------------------------------------------------------------------------------
 static int launch_w(const DeviceState& st, const void* xyz, int64_t n, int l_max, int normalized, int dtype,
                     void* sph, void* dsph, void* ddsph, cudaStream_t stream) {
-    const char* force = getenv("SPHB200_FORCE_KERNEL");  // "w1": the one-warp-per-point kernel even for long rows
-    if (!(force && force[0] == 'w' && force[1] == '1')) {
+    if (g_opt.force_kernel != FORCE_W1) {
         // the longest f64 rows: the warps of a CTA share one point, chunks of a third of a row, ~3 KB
-        // bulk stores (kernel_wc.cuh says where it wins); "wc" forces it wherever it can run
-        const bool force_wc = force && force[0] == 'w' && force[1] == 'c';
-        const int min_l = force_wc ? 19 : (dtype == SPHERICART_CUDA_F64 ? 32 : SPHERICART_CUDA_MAX_L + 1);
+        // bulk stores (kernel_wc.cuh says where it wins); FORCE_WC takes it wherever it can run
+        const bool force_wc = g_opt.force_kernel == FORCE_WC;
+        int min_l = force_wc ? 19 : (dtype == SPHERICART_CUDA_F64 ? 32 : SPHERICART_CUDA_MAX_L + 1);
+        if (g_opt.wc_min_l > 0) min_l = g_opt.wc_min_l;
         WcLaunch lc{};
         if (wc_plan(min_l, st.sm_count, st.smem_optin, n, l_max, normalized, dtype, sph, dsph, ddsph, xyz, st.d_tables, &lc) == 0) {
             int rc = allow_smem(lc.func, (int)lc.smem);
             if (rc) return rc;
             wc_launch(lc, stream);
-            g_launches.fetch_add(1, std::memory_order_relaxed);
+            launched("wc");
             CUDA_TRY(cudaGetLastError());
             return 0;
         }
@@ -200,7 +149,7 @@ static int launch_w(const DeviceState& st, const void* xyz, int64_t n, int l_max
     rc = allow_smem(lw.func, (int)lw.smem);
     if (rc) return rc;
     wk_launch(lw, stream);
-    g_launches.fetch_add(1, std::memory_order_relaxed);
+    launched("w");
     CUDA_TRY(cudaGetLastError());
     return 0;
 }
@@ -231,11 +180,9 @@ static int compute_device(const void* xyz, int64_t n, int l_max, int normalized,
     rc = device_state(&st);
     if (rc) return rc;
 
-    const char* force = getenv("SPHB200_FORCE_KERNEL");  // "tpb" | "tp" | "w": experiments only
-    const bool force_w = force && force[0] == 'w';
-    const bool force_tp = force && force[0] == 't' && force[1] == 'p' && force[2] == '\0';
-    const bool force_tpg = force && force[0] == 't' && force[1] == 'p' && force[2] == 'g';
-    if (!force_w && !force_tp && !force_tpg) {
+    const int force = g_opt.force_kernel;
+    const bool force_w = force == FORCE_W || force == FORCE_W1 || force == FORCE_WC;
+    if (force == FORCE_NONE || force == FORCE_TPB) {
         // compile-time-l_max kernels (two threads per point): every l_max that has an instantiation
         const bool f32 = dtype == SPHERICART_CUDA_F32;
         auto launch = ddsph ? (f32 ? sph_tpb_launch_f32_h : sph_tpb_launch_f64_h)
@@ -244,35 +191,20 @@ static int compute_device(const void* xyz, int64_t n, int l_max, int normalized,
         int r = launch(st->sm_count, xyz, n, l_max, normalized, sph, dsph, ddsph, stream);
         if (r < 0) return fail(SPHERICART_CUDA_ECUDA, "tpb launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         if (r == 0) {
-            g_launches.fetch_add(1, std::memory_order_relaxed);
+            launched("tpb");
             return 0;
         }
     }
-    if (!ddsph && !force_w && !force_tp) {
+    if (!ddsph && !force_w) {
         // any other l_max without Hessians: several lanes per point, run-time l_max
         TpgLaunch lg{};
         if (tpg_plan(st->smem_optin, n, l_max, normalized, dtype, sph, dsph, xyz, st->d_tables, &lg) == 0) {
             rc = allow_smem(lg.func, (int)lg.smem);
             if (rc) return rc;
             tpg_launch(lg, stream);
-            g_launches.fetch_add(1, std::memory_order_relaxed);
+            launched("tpg");
             CUDA_TRY(cudaGetLastError());
             return 0;
-        }
-    }
-    if (!ddsph && !force_w) {
-        // the tp kernel wants an odd row length (conflict-free staging) and >= 4 warps per SM
-        TpParams probe{};
-        int grid;
-        size_t smem;
-        const int L = (l_max + 1) * (l_max + 1);
-        const int64_t tile_bytes = 32LL * L * (dtype == SPHERICART_CUDA_F32 ? 4 : 8) * (dsph ? 4 : 1);
-        const bool fits = tile_bytes * 4 <= st->smem_optin - 1024;
-        const bool want_tp = force_tp || ((L & 1) && fits);
-        if (want_tp && tp_plan(*st, n, l_max, dsph ? 1 : 0, dtype == SPHERICART_CUDA_F32 ? 4 : 8, &probe, &grid, &smem)) {
-            bool handled = false;
-            rc = launch_tp(*st, xyz, n, l_max, normalized, dtype, sph, dsph, stream, &handled);
-            if (rc || handled) return rc;
         }
     }
     return launch_w(*st, xyz, n, l_max, normalized, dtype, sph, dsph, ddsph, stream);
@@ -319,13 +251,11 @@ static int vjp_recompute_device(const void* xyz, const void* grad_sph, void* gra
     rc = device_state(&st);
     if (rc) return rc;
     const bool f32 = dtype == SPHERICART_CUDA_F32;
-    const char* force = getenv("SPHB200_FORCE_KERNEL");  // "generic": experiments and tests only
-    const bool force_generic = force && force[0] == 'g';
-    if (!force_generic) {
-        int r = (f32 ? sph_vjpr_launch_f32 : sph_vjpr_launch_f64)(xyz, grad_sph, grad_xyz, n, l_max, normalized, stream);
+    if (g_opt.force_kernel != FORCE_GENERIC) {
+        int r = (f32 ? sph_vjpr_launch_f32 : sph_vjpr_launch_f64)(st->sm_count, xyz, grad_sph, grad_xyz, n, l_max, normalized, stream);
         if (r < 0) return fail(SPHERICART_CUDA_ECUDA, "vjpr launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         if (r == 0) {
-            g_launches.fetch_add(1, std::memory_order_relaxed);
+            launched("vjpr");
             return 0;
         }
     }
@@ -338,7 +268,7 @@ static int vjp_recompute_device(const void* xyz, const void* grad_sph, void* gra
         auto k = normalized ? sph_vjpr_generic_kernel<double, dd, true> : sph_vjpr_generic_kernel<double, dd, false>;
         k<<<(unsigned)blocks, 128, 0, stream>>>((const double*)xyz, (const double*)grad_sph, (double*)grad_xyz, n, l_max);
     }
-    g_launches.fetch_add(1, std::memory_order_relaxed);
+    launched("vjpr_generic");
     CUDA_TRY(cudaGetLastError());
     return 0;
 }
@@ -367,7 +297,7 @@ static int vjp_device(const void* dsph, const void* grad_sph, void* grad_xyz, in
     prm.tile_bytes = 4u * 32u * L * esize;
     const int budget = st->smem_optin - 1024;
     int warps = (int)(budget / ((int64_t)VJP_NBUF * prm.tile_bytes + VJP_NBUF * 8));
-    const int want = env_int("SPHB200_VJP_WARPS", VJP_MAX_THREADS / 32);
+    const int want = g_opt.vjp_warps > 0 ? g_opt.vjp_warps : VJP_MAX_THREADS / 32;
     if (warps > want) warps = want;
     const int64_t n_tiles = (n + 31) / 32;
     void (*kern)(const VjpParams);
@@ -375,9 +305,11 @@ static int vjp_device(const void* dsph, const void* grad_sph, void* grad_xyz, in
         kern = dtype == SPHERICART_CUDA_F32 ? sph_vjp_kernel<float> : sph_vjp_kernel<double>;
     } else {
         // rows too long to stage a 32-point tile: warp-per-point streaming kernel
-        return wk_launch_vjp(st->sm_count, dsph, grad_sph, grad_xyz, n, L, dtype, stream, &g_launches) == 0
-                   ? 0
-                   : fail(SPHERICART_CUDA_ECUDA, "vjp launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+        if (wk_launch_vjp(st->sm_count, dsph, grad_sph, grad_xyz, n, L, dtype, stream) == 0) {
+            launched("vjp_warp");
+            return 0;
+        }
+        return fail(SPHERICART_CUDA_ECUDA, "vjp launch failed: %s", cudaGetErrorString(cudaGetLastError()));
     }
     int64_t per_sm = (n_tiles + st->sm_count - 1) / st->sm_count;
     if (per_sm < warps) warps = (int)(per_sm < 1 ? 1 : per_sm);
@@ -388,7 +320,7 @@ static int vjp_device(const void* dsph, const void* grad_sph, void* grad_xyz, in
     rc = allow_smem((const void*)kern, (int)smem);
     if (rc) return rc;
     kern<<<(int)ctas, warps * 32, smem, stream>>>(prm);
-    g_launches.fetch_add(1, std::memory_order_relaxed);
+    launched("vjp");
     CUDA_TRY(cudaGetLastError());
     return 0;
 }
@@ -486,9 +418,28 @@ int sphericart_cuda_expand(const void* xyz, const void* radial, const int64_t* s
     if (r > 0)
         return fail(SPHERICART_CUDA_ENOTSUP, "expand: l_max = %d (max 8) or n_rad = %d (max %d) has no kernel in this build",
                     l_max, n_rad, 16);
-    g_launches.fetch_add(1, std::memory_order_relaxed);
+    launched("expand");
     return 0;
 }
+
+// Every exit of the chunk loops below passes through here: both streams are drained before the
+// call returns, so no copy is still writing into (or reading from) the caller's buffers -- also
+// when a later chunk failed.
+static int host_finish(int rc) {
+    cudaError_t e0 = cudaStreamSynchronize(g_ws.stream[0]);
+    cudaError_t e1 = cudaStreamSynchronize(g_ws.stream[1]);
+    if (rc) return rc;
+    if (e0 != cudaSuccess || e1 != cudaSuccess)
+        return fail(SPHERICART_CUDA_ECUDA, "cudaStreamSynchronize failed: %s",
+                    cudaGetErrorString(e0 != cudaSuccess ? e0 : e1));
+    return 0;
+}
+#define HOST_TRY(call)                                                                                    \
+    do {                                                                                                  \
+        cudaError_t e_ = (call);                                                                          \
+        if (e_ != cudaSuccess)                                                                            \
+            return host_finish(fail(SPHERICART_CUDA_ECUDA, "%s failed: %s", #call, cudaGetErrorString(e_))); \
+    } while (0)
 
 int sphericart_cuda_compute_host(const void* xyz, int64_t n, int l_max, int normalized, int dtype, void* sph,
                                  void* dsph, void* ddsph) {
@@ -503,33 +454,31 @@ int sphericart_cuda_compute_host(const void* xyz, int64_t n, int l_max, int norm
     const size_t es = dtype == SPHERICART_CUDA_F32 ? 4 : 8;
     const size_t L = (size_t)(l_max + 1) * (l_max + 1);
     const size_t bpp = es * L * (1 + (dsph ? 3 : 0) + (ddsph ? 9 : 0));
-    const int64_t chunk = chunk_points(n, bpp, (size_t)256 << 20);
+    const int64_t chunk = chunk_points(n, bpp, (size_t)g_opt.host_chunk_bytes);
     int slot = 0;
     for (int64_t p0 = 0; p0 < n; p0 += chunk, slot ^= 1) {
         const int64_t np = (n - p0 < chunk) ? n - p0 : chunk;
         cudaStream_t s = g_ws.stream[slot];
-        if ((rc = ws_reserve(slot, 0, (size_t)np * 3 * es))) return rc;
-        if ((rc = ws_reserve(slot, 1, (size_t)np * L * es))) return rc;
-        if (dsph && (rc = ws_reserve(slot, 2, (size_t)np * 3 * L * es))) return rc;
-        if (ddsph && (rc = ws_reserve(slot, 3, (size_t)np * 9 * L * es))) return rc;
+        if ((rc = ws_reserve(slot, 0, (size_t)np * 3 * es))) return host_finish(rc);
+        if ((rc = ws_reserve(slot, 1, (size_t)np * L * es))) return host_finish(rc);
+        if (dsph && (rc = ws_reserve(slot, 2, (size_t)np * 3 * L * es))) return host_finish(rc);
+        if (ddsph && (rc = ws_reserve(slot, 3, (size_t)np * 9 * L * es))) return host_finish(rc);
         void** b = g_ws.buf[slot];
-        CUDA_TRY(cudaMemcpyAsync(b[0], (const char*)xyz + (size_t)p0 * 3 * es, (size_t)np * 3 * es,
+        HOST_TRY(cudaMemcpyAsync(b[0], (const char*)xyz + (size_t)p0 * 3 * es, (size_t)np * 3 * es,
                                  cudaMemcpyHostToDevice, s));
         rc = compute_device(b[0], np, l_max, normalized, dtype, b[1], dsph ? b[2] : nullptr,
                             ddsph ? b[3] : nullptr, s);
-        if (rc) return rc;
-        CUDA_TRY(cudaMemcpyAsync((char*)sph + (size_t)p0 * L * es, b[1], (size_t)np * L * es,
+        if (rc) return host_finish(rc);
+        HOST_TRY(cudaMemcpyAsync((char*)sph + (size_t)p0 * L * es, b[1], (size_t)np * L * es,
                                  cudaMemcpyDeviceToHost, s));
         if (dsph)
-            CUDA_TRY(cudaMemcpyAsync((char*)dsph + (size_t)p0 * 3 * L * es, b[2], (size_t)np * 3 * L * es,
+            HOST_TRY(cudaMemcpyAsync((char*)dsph + (size_t)p0 * 3 * L * es, b[2], (size_t)np * 3 * L * es,
                                      cudaMemcpyDeviceToHost, s));
         if (ddsph)
-            CUDA_TRY(cudaMemcpyAsync((char*)ddsph + (size_t)p0 * 9 * L * es, b[3], (size_t)np * 9 * L * es,
+            HOST_TRY(cudaMemcpyAsync((char*)ddsph + (size_t)p0 * 9 * L * es, b[3], (size_t)np * 9 * L * es,
                                      cudaMemcpyDeviceToHost, s));
     }
-    CUDA_TRY(cudaStreamSynchronize(g_ws.stream[0]));
-    CUDA_TRY(cudaStreamSynchronize(g_ws.stream[1]));
-    return 0;
+    return host_finish(0);
 }
 
 int sphericart_cuda_vjp_host(const void* xyz, const void* dsph, const void* grad_sph, void* grad_xyz, int64_t n,
@@ -545,28 +494,60 @@ int sphericart_cuda_vjp_host(const void* xyz, const void* dsph, const void* grad
     if (rc) return rc;
     const size_t es = dtype == SPHERICART_CUDA_F32 ? 4 : 8;
     const size_t L = (size_t)(l_max + 1) * (l_max + 1);
-    const int64_t chunk = chunk_points(n, 4 * L * es, (size_t)256 << 20);
+    const int64_t chunk = chunk_points(n, 4 * L * es, (size_t)g_opt.host_chunk_bytes);
     int slot = 0;
     for (int64_t p0 = 0; p0 < n; p0 += chunk, slot ^= 1) {
         const int64_t np = (n - p0 < chunk) ? n - p0 : chunk;
         cudaStream_t s = g_ws.stream[slot];
-        if ((rc = ws_reserve(slot, 2, (size_t)np * 3 * L * es))) return rc;
-        if ((rc = ws_reserve(slot, 1, (size_t)np * L * es))) return rc;
-        if ((rc = ws_reserve(slot, 4, (size_t)np * 3 * es))) return rc;
+        if ((rc = ws_reserve(slot, 2, (size_t)np * 3 * L * es))) return host_finish(rc);
+        if ((rc = ws_reserve(slot, 1, (size_t)np * L * es))) return host_finish(rc);
+        if ((rc = ws_reserve(slot, 4, (size_t)np * 3 * es))) return host_finish(rc);
         void** b = g_ws.buf[slot];
-        CUDA_TRY(cudaMemcpyAsync(b[2], (const char*)dsph + (size_t)p0 * 3 * L * es, (size_t)np * 3 * L * es,
+        HOST_TRY(cudaMemcpyAsync(b[2], (const char*)dsph + (size_t)p0 * 3 * L * es, (size_t)np * 3 * L * es,
                                  cudaMemcpyHostToDevice, s));
-        CUDA_TRY(cudaMemcpyAsync(b[1], (const char*)grad_sph + (size_t)p0 * L * es, (size_t)np * L * es,
+        HOST_TRY(cudaMemcpyAsync(b[1], (const char*)grad_sph + (size_t)p0 * L * es, (size_t)np * L * es,
                                  cudaMemcpyHostToDevice, s));
         rc = vjp_device(b[2], b[1], b[4], np, l_max, dtype, s);
-        if (rc) return rc;
-        CUDA_TRY(cudaMemcpyAsync((char*)grad_xyz + (size_t)p0 * 3 * es, b[4], (size_t)np * 3 * es,
+        if (rc) return host_finish(rc);
+        HOST_TRY(cudaMemcpyAsync((char*)grad_xyz + (size_t)p0 * 3 * es, b[4], (size_t)np * 3 * es,
                                  cudaMemcpyDeviceToHost, s));
     }
-    CUDA_TRY(cudaStreamSynchronize(g_ws.stream[0]));
-    CUDA_TRY(cudaStreamSynchronize(g_ws.stream[1]));
-    return 0;
+    return host_finish(0);
 }
+
+int sphericart_cuda_set_option(const char* name, const char* value) {
+    if (!name || !value) return fail(SPHERICART_CUDA_EINVAL, "set_option: NULL name or value");
+    struct IntOpt { const char* name; int* slot; };
+    const IntOpt ints[] = {{"tpg_lp", &g_opt.tpg_lp}, {"w_nbuf", &g_opt.w_nbuf}, {"w_warps", &g_opt.w_warps},
+                           {"w_ppw", &g_opt.w_ppw}, {"wc_min_l", &g_opt.wc_min_l}, {"vjp_warps", &g_opt.vjp_warps},
+                           {"tpb_tiles", &g_opt.tpb_tiles}, {"tpb_split", &g_opt.tpb_split}, {"pdl", &g_opt.pdl},
+                           {"tq_points", &g_opt.tq_points}};
+    if (!strcmp(name, "force_kernel")) {
+        struct { const char* v; int code; } const kinds[] = {
+            {"", FORCE_NONE}, {"auto", FORCE_NONE}, {"tpb", FORCE_TPB}, {"tpg", FORCE_TPG}, {"w", FORCE_W},
+            {"w1", FORCE_W1}, {"wc", FORCE_WC}, {"tq", FORCE_TQ}, {"generic", FORCE_GENERIC}};
+        for (const auto& k : kinds)
+            if (!strcmp(value, k.v)) {
+                g_opt.force_kernel = k.code;
+                return 0;
+            }
+        return fail(SPHERICART_CUDA_EINVAL, "set_option: unknown kernel family '%s'", value);
+    }
+    if (!strcmp(name, "host_chunk_bytes")) {
+        const long long v = atoll(value);
+        if (v < 4096) return fail(SPHERICART_CUDA_EINVAL, "set_option: host_chunk_bytes = %s is below 4096", value);
+        g_opt.host_chunk_bytes = v;
+        return 0;
+    }
+    for (const auto& o : ints)
+        if (!strcmp(name, o.name)) {
+            *o.slot = atoi(value);
+            return 0;
+        }
+    return fail(SPHERICART_CUDA_EINVAL, "set_option: unknown option '%s'", name);
+}
+
+const char* sphericart_cuda_last_kernel(void) { return g_last_kernel; }
 
 const char* sphericart_cuda_last_error(void) { return g_err; }
 

@@ -28,7 +28,13 @@ template <int LMAX, int NRAD_MAX> static int launch_nr(int smem_optin, ExpandPar
     while (warps > 1 && warps * Shape::warp_bytes(prm.n_rad, NRAD_MAX) > smem_optin - 1024) warps >>= 1;
     const int smem = warps * Shape::warp_bytes(prm.n_rad, NRAD_MAX);
     if (smem > smem_optin - 1024) return 1;
-    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return -1;
+    static int attr_bytes[64] = {0};   // per device: largest size granted so far (benign race, idempotent call)
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return -1;
+    if (dev < 0 || dev >= 64 || attr_bytes[dev] < smem) {
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return -1;
+        if (dev >= 0 && dev < 64) attr_bytes[dev] = smem;
+    }
     prm.warps_per_cta = warps;
     const int64_t per_cta = (int64_t)warps * EXP_SPW;   // segments per CTA
     const int64_t ctas = (prm.n_seg + per_cta - 1) / per_cta;

@@ -19,6 +19,7 @@
 #pragma once
 #include <cstdlib>
 
+#include "options.h"
 #include "ptx.cuh"
 #include "sph_core.cuh"
 
@@ -320,10 +321,6 @@ template <typename T, typename R> static TpgKernel tpg_pick(int deriv, int norm,
     return tpg_pick2<T, R, 8, true>(deriv, norm);
 }
 
-static inline int tpg_env(const char* name, int dflt) {
-    const char* s = getenv(name);
-    return (s && *s) ? atoi(s) : dflt;
-}
 
 // returns 0 and fills *out if the kernel applies: values or values + gradients whose smallest tile
 // (4 points) still leaves room for several tiles per SM; 1 otherwise
@@ -335,7 +332,7 @@ static inline int tpg_plan(int smem_optin, int64_t n, int l_max, int normalized,
     const int64_t per_pt = (int64_t)L * esize * (deriv ? 4 : 1);
     // lanes per point: the most points per tile (16, 8, 4) whose image stays under 12 KB (measured:
     // the kernel is latency-bound, so small tiles = more warps in flight wins almost everywhere)
-    int lp = tpg_env("SPHB200_TPG_LP", 0);
+    int lp = g_opt.tpg_lp;
     if (lp != 2 && lp != 4 && lp != 8) {
         lp = 2;
         while (lp < 8 && (32 / lp) * per_pt > 12 * 1024) lp *= 2;

@@ -17,6 +17,7 @@
 #pragma once
 #include <atomic>
 
+#include "options.h"
 #include "ptx.cuh"
 #include "sph_core.cuh"
 
@@ -343,17 +344,13 @@ template <typename T, typename R> static WkKernel wk_pick(int deriv, int norm, b
     return lodd ? wk_pick2<T, R, true>(deriv, norm) : wk_pick2<T, R, false>(deriv, norm);
 }
 
-static inline int wk_env(const char* name, int dflt) {
-    const char* s = getenv(name);
-    return (s && *s) ? atoi(s) : dflt;
-}
 
 static inline int wk_plan(int sm_count, int smem_optin, int64_t n, int l_max, int normalized, int dtype,
                           void* sph, void* dsph, void* ddsph, const void* xyz, const SphTables* d_tab,
                           WkLaunch* out) {
     const int deriv = ddsph ? 2 : (dsph ? 1 : 0);
     const int esize = dtype == 0 ? 4 : 8;
-    int nbuf = wk_env("SPHB200_W_NBUF", 1);   // measured on C4: one image per warp and more warps beats two images
+    int nbuf = g_opt.w_nbuf;   // measured on C4: one image per warp and more warps beats two images
     if (nbuf < 1) nbuf = 1;
     if (nbuf > 2) nbuf = 2;
     const int budget = smem_optin - 1024;
@@ -365,12 +362,12 @@ static inline int wk_plan(int sm_count, int smem_optin, int64_t n, int l_max, in
         nbuf = 1;
     }
     if (warps < 1) return 1;
-    const int want = wk_env("SPHB200_W_WARPS", WK_MAX_THREADS / 32);
+    const int want = g_opt.w_warps > 0 ? g_opt.w_warps : WK_MAX_THREADS / 32;
     if (warps > want) warps = want;
     int64_t per_sm = (n + sm_count - 1) / sm_count;
     if (per_sm < warps) warps = (int)(per_sm < 1 ? 1 : per_sm);
     // points per warp: amortise the per-CTA table copy, but keep >= ~16 waves of CTAs
-    int64_t ppw = wk_env("SPHB200_W_PPW", 0);
+    int64_t ppw = g_opt.w_ppw;
     if (ppw <= 0) {
         ppw = n / ((int64_t)sm_count * warps * 16);
         if (ppw > 8) ppw = 8;
@@ -420,7 +417,7 @@ static inline void wk_launch(const WkLaunch& lw, cudaStream_t stream) {
 }
 
 static inline int wk_launch_vjp(int sm_count, const void* dsph, const void* gsph, void* gxyz, int64_t n, int L,
-                                int dtype, cudaStream_t stream, std::atomic<int64_t>* launches) {
+                                int dtype, cudaStream_t stream) {
     int64_t blocks = (n + 7) / 8;
     if (blocks > (int64_t)sm_count * 8) blocks = (int64_t)sm_count * 8;
     if (dtype == 0)
@@ -429,7 +426,6 @@ static inline int wk_launch_vjp(int sm_count, const void* dsph, const void* gsph
     else
         sph_vjp_warp_kernel<double><<<(int)blocks, 256, 0, stream>>>((const double*)dsph, (const double*)gsph,
                                                                       (double*)gxyz, n, L);
-    launches->fetch_add(1, std::memory_order_relaxed);
     return cudaGetLastError() == cudaSuccess ? 0 : 1;
 }
 

@@ -343,7 +343,7 @@ static inline int wc_plan(int min_l, int sm_count, int smem_optin, int64_t n, in
                           void* ddsph, const void* xyz, const SphTables* d_tab, WcLaunch* out) {
     const int deriv = ddsph ? 2 : (dsph ? 1 : 0);
     const int esize = dtype == 0 ? 4 : 8;
-    if (l_max < wk_env("SPHB200_WC_MIN_L", min_l)) return 1;
+    if (l_max < min_l) return 1;
     const WcSmem lay(l_max, deriv, esize);
     if ((int64_t)lay.total > smem_optin) return 1;
     const bool lodd = (l_max & 1) == 0;

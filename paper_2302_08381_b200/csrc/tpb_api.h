@@ -20,7 +20,7 @@ SPH_TPB_DECL(f64_h)
 #undef SPH_TPB_DECL
 // recompute-in-backward VJP (vjpr_inst.cu, compiled once per element type); same return codes
 #define SPH_VJPR_DECL(sfx)                                                                              \
-    int sph_vjpr_launch_##sfx(const void* xyz, const void* grad_sph, void* grad_xyz, int64_t n, int l_max, \
+    int sph_vjpr_launch_##sfx(int sm_count, const void* xyz, const void* grad_sph, void* grad_xyz, int64_t n, int l_max, \
                               int normalized, cudaStream_t stream);                                      \
     int sph_vjpr_upload_##sfx(const SphTables* host_tables);
 SPH_VJPR_DECL(f32)

@@ -4,9 +4,8 @@
 //   sph_tpb_upload_<f32|f64>_<v|g>(tables)   copy the coefficient tables into this unit's constant bank
 //   sph_tpb_launch_<f32|f64>_<v|g>(...)      launch if l_max has an instantiation (returns 1 if not)
 #include "kernel_tpb.cuh"
+#include "options.h"
 #include "tpb_api.h"
-
-#include <cstdlib>
 
 #ifndef TPB_F64
 #error "compile with -DTPB_F64=0|1 -DTPB_DERIV=0|1"
@@ -36,10 +35,6 @@ typedef double tpb_R;
 #define TPB_NAME(f) f##_f32_v
 #endif
 
-static int env_int(const char* name, int dflt) {
-    const char* s = getenv(name);
-    return (s && *s) ? atoi(s) : dflt;
-}
 
 template <int LMAX, bool NORM, int SPLIT, bool BB = false>
 static int launch_split(int sm_count, TpbParams prm, cudaStream_t stream) {
@@ -59,7 +54,7 @@ static int launch_split(int sm_count, TpbParams prm, cudaStream_t stream) {
     // only, low l_max) take up to four per CTA, or the launch rate of the block scheduler shows
     // (C5 values only, 3.1 KB tiles: 170 us with one, 147 with two, 136 with four or eight).
     const int64_t n_tiles = (prm.n + Shape::pts - 1) / Shape::pts;
-    static const int k_env = env_int("SPHB200_TPB_TILES", 0);
+    const int k_env = g_opt.tpb_tiles;
     int64_t k = k_env > 0 ? k_env : 12288 / Shape::tile_bytes;
     if (k < 1) k = 1;
     if (k_env <= 0 && k > 4) k = 4;
@@ -72,8 +67,7 @@ static int launch_split(int sm_count, TpbParams prm, cudaStream_t stream) {
     // predecessor.  It hides the launch ramp between back-to-back calls (C2: 22.8 -> 20.8 us).  Only
     // for grids of a few waves: the two griddepcontrol instructions cost every CTA a fixed latency,
     // which a grid of 250 000 one-tile CTAs cannot hide (C5 values only: 169 -> 261 us with them).
-    static const int pdl_env = env_int("SPHB200_PDL", 1);
-    const int pdl = pdl_env && ctas <= (int64_t)sm_count * 64;
+    const int pdl = g_opt.pdl && ctas <= (int64_t)sm_count * 64;
     prm.pdl = pdl;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)ctas);
@@ -93,7 +87,7 @@ static int launch_split(int sm_count, TpbParams prm, cudaStream_t stream) {
 // Measured: C2 24.7 -> 22.8 us, C3 166 -> 164 us; C5 (17 tiles fit) 476 -> 562 us, so not there.
 template <int LMAX, bool NORM>
 static int launch_one(int sm_count, const TpbParams& prm, cudaStream_t stream) {
-    static const int split_env = env_int("SPHB200_TPB_SPLIT", 0);
+    const int split_env = g_opt.tpb_split;
     // One lane per point doing both branches of Eq. 5 (32-point tiles) where the Legendre recurrences
     // dominate, i.e. values only: f64 (double-double recurrences) up to l_max = 12, f32 up to 10, and
     // f64 gradients up to l_max = 4.  Measured: f64 values l_max 4/6/8: 2.9/3.2/3.4 -> 5.2/6.1/5.3

@@ -3,9 +3,8 @@
 //   sph_vjpr_upload_<f32|f64>(tables)   copy the coefficient tables into this unit's constant bank
 //   sph_vjpr_launch_<f32|f64>(...)      launch if l_max has an instantiation (returns 1 if not)
 #include "kernel_vjpr.cuh"
+#include "options.h"
 #include "tpb_api.h"
-
-#include <cstdlib>
 
 #ifndef VJPR_F64
 #error "compile with -DVJPR_F64=0|1"
@@ -23,7 +22,7 @@ typedef double vjpr_R;
 #define VJPR_NAME(f) f##_f32
 #endif
 
-template <int LMAX, bool NORM> static int launch_one(VjprParams prm, cudaStream_t stream) {
+template <int LMAX, bool NORM> static int launch_one(int sm_count, VjprParams prm, cudaStream_t stream) {
     constexpr int L = (LMAX + 1) * (LMAX + 1);
     constexpr int smem = 32 * L * (int)sizeof(vjpr_T) + 16;   // 32 points per tile
     auto kern = sph_vjpr_kernel<vjpr_T, vjpr_R, NORM, LMAX>;
@@ -46,17 +45,16 @@ template <int LMAX, bool NORM> static int launch_one(VjprParams prm, cudaStream_
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    static const int pdl = [] { const char* e = getenv("SPHB200_PDL"); return (e && *e) ? atoi(e) : 1; }();
-    prm.pdl = pdl && n_tiles <= 148 * 64;   // small grids only (tpb_inst.cu)
+    prm.pdl = g_opt.pdl && n_tiles <= (int64_t)sm_count * 64;   // small grids only (tpb_inst.cu)
     cfg.numAttrs = prm.pdl ? 1 : 0;
     return cudaLaunchKernelEx(&cfg, kern, prm) == cudaSuccess ? 0 : -1;
 }
 
 #define VJPR_CASE(LM) \
     case LM:          \
-        return normalized ? launch_one<LM, true>(prm, stream) : launch_one<LM, false>(prm, stream);
+        return normalized ? launch_one<LM, true>(sm_count, prm, stream) : launch_one<LM, false>(sm_count, prm, stream);
 
-int VJPR_NAME(sph_vjpr_launch)(const void* xyz, const void* grad_sph, void* grad_xyz, int64_t n, int l_max,
+int VJPR_NAME(sph_vjpr_launch)(int sm_count, const void* xyz, const void* grad_sph, void* grad_xyz, int64_t n, int l_max,
                                int normalized, cudaStream_t stream) {
     VjprParams prm{xyz, grad_sph, grad_xyz, n, 0};
     switch (l_max) {

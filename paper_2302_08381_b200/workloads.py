@@ -84,7 +84,7 @@ def make_xyz(cfg: Config | str, n: int | None = None, seed: int = 0) -> np.ndarr
     n = cfg.n if n is None else int(n)
     cid = int(cfg.name[1:])
     rng = np.random.default_rng(seed if cid == 1 else [cid, seed])  # C1: "seed 0" as given
-    if cfg.name in ("C1", "C5"):
+    if cfg.name in ("C1", "C5", "C9"):       # C9: bench.py's `--workload custom` (any dtype / l_max / outputs)
         xyz = rng.standard_normal((n, 3))
     elif cfg.name == "C2":
         n_axis = n // 100                      # 1 % exactly on the +-z axis

@@ -1,0 +1,89 @@
+"""`-m gpu`: every kernel the DEFAULT dispatch can reach, against the oracle, element by element.
+
+The forward entry point picks among separately compiled instantiations (one per l_max, element
+type and derivative order, each with its own tile split, padding and store path), so every
+(dtype, l_max, derivative order, variant) cell is run here with no kernel family forced:
+whatever kernel `sphericart_cuda_compute` chooses for that cell is the one compared.
+The same for the recompute VJP and the fused expansion.  n spans several tiles plus a ragged
+tail; C2-style special points (on +-z, |r| down to 1e-6) for l_max <= 16, C4-style shells above.
+Equations checked: Eq. 5, Eq. 7, Eq. 9, Eq. 10, chain rule P:108,
+backward P:112, Eq. 1.
+"""
+import numpy as np
+import pytest
+
+import parity
+from paper_2302_08381_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def sph():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2302_08381_b200 as pkg
+
+    pkg.load()
+    pkg.sphericart_cuda_set_option("force_kernel", "auto")     # this file tests the default dispatch
+    return pkg
+
+
+def _cloud(l_max, n, dtype):
+    xyz = W.make_xyz("C2" if l_max <= 16 else "C4", n, seed=l_max)
+    return np.ascontiguousarray(xyz.astype(np.float32 if dtype == "f32" else np.float64))
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("l_max", list(range(0, 33)))
+def test_default_dispatch_every_cell(sph, oracle, dtype, l_max):
+    n = 3 * 32 + 100 + 7 if l_max <= 16 else 2 * 32 + 7        # C2 cloud: >= 2 axis and 2 tiny-r points
+    xyz = _cloud(l_max, n, dtype)
+    x_d = torch.from_numpy(xyz).cuda()
+    for normalized in (True, False):
+        want = oracle.compute(xyz, l_max, normalized, True, True)
+        for deriv in (0, 1, 2):
+            before = sph.sphericart_cuda_launch_count()
+            got = sph.compute(x_d, l_max, normalized, deriv >= 1, deriv >= 2)
+            torch.cuda.synchronize()
+            assert sph.sphericart_cuda_launch_count() == before + 1
+            for order in range(deriv + 1):
+                parity.check(got[order].cpu().numpy(), want[order], xyz, l_max, normalized, order, dtype,
+                             f"{dtype} l_max={l_max} norm={normalized} deriv={deriv} order={order}")
+            if deriv == 2:
+                hh = got[2]
+                for a in range(3):
+                    for b in range(a):
+                        assert torch.equal(hh[:, a, b], hh[:, b, a])
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("l_max", list(range(0, 33)))
+def test_default_dispatch_vjp_recompute(sph, oracle, dtype, l_max):
+    n = 3 * 32 + 100 + 7 if l_max <= 16 else 2 * 32 + 7
+    xyz = _cloud(l_max, n, dtype)
+    g = np.random.default_rng([7, l_max]).standard_normal((n, (l_max + 1) ** 2)).astype(xyz.dtype)
+    x_d, g_d = torch.from_numpy(xyz).cuda(), torch.from_numpy(g).cuda()
+    for normalized in (True, False):
+        before = sph.sphericart_cuda_launch_count()
+        gx = sph.vjp_recompute(x_d, g_d, normalized)
+        torch.cuda.synchronize()
+        assert sph.sphericart_cuda_launch_count() == before + 1
+        _, wd, _ = oracle.compute(xyz, l_max, normalized, True)
+        parity.check_vjp(gx.cpu().numpy(), oracle.vjp_recompute(xyz, g, l_max, normalized), wd, g, l_max, dtype,
+                         f"vjp_recompute {dtype} l_max={l_max} norm={normalized}", point_scale=True)
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("l_max", list(range(0, 9)))
+def test_default_dispatch_expand(sph, oracle, dtype, l_max):
+    for n_rad in (1, 7, 8, 9, 16):
+        xyz, rad, seg = W.make_expand_inputs(37, l_max, n_rad, dtype, 19.0, seed=n_rad)
+        before = sph.sphericart_cuda_launch_count()
+        c = sph.expand(torch.from_numpy(xyz).cuda(), torch.from_numpy(rad).cuda(), torch.from_numpy(seg).cuda())
+        torch.cuda.synchronize()
+        assert sph.sphericart_cuda_launch_count() == before + 1
+        parity.check_expand(c.cpu().numpy(), oracle.expand(xyz, rad, seg, l_max), rad, seg, l_max, dtype,
+                            f"expand {dtype} l_max={l_max} n_rad={n_rad}")

@@ -25,6 +25,21 @@ def sph():
     return pkg
 
 
+@pytest.fixture
+def option(sph):
+    """Set launch options (sphericart_cuda_set_option) for one test; defaults restored afterwards."""
+    touched = {}
+
+    def set_(name, value):
+        touched[name] = True
+        sph.sphericart_cuda_set_option(name, value)
+
+    yield set_
+    defaults = {"force_kernel": "auto", "tpg_lp": 0, "host_chunk_bytes": 256 << 20}
+    for name in touched:
+        sph.sphericart_cuda_set_option(name, defaults[name])
+
+
 def _torch_dtype(name):
     return torch.float32 if name == "f32" else torch.float64
 
@@ -174,12 +189,11 @@ def test_all_variants_small(sph, oracle, dtype, l_max, normalized):
         _compare(oracle, xyz, l_max, normalized, dtype, s, d, h, f"{dtype} l={l_max} norm={normalized} d={deriv}")
 
 
-@pytest.mark.parametrize("force", ["auto", "tp", "w"])
-def test_all_forward_kernels_agree_with_the_oracle(sph, oracle, force, monkeypatch):
-    """The compile-time-l_max (auto picks it for l_max <= 8), thread-per-point and warp-per-point
+@pytest.mark.parametrize("force", ["auto", "tpg", "w"])
+def test_all_forward_kernels_agree_with_the_oracle(sph, oracle, force, option):
+    """The compile-time-l_max (auto picks it for l_max <= 8), lanes-per-point and warp-per-point
     kernels are interchangeable where they all apply."""
-    if force != "auto":
-        monkeypatch.setenv("SPHB200_FORCE_KERNEL", force)
+    option("force_kernel", force)
     for dtype, l_max in (("f32", 8), ("f64", 4), ("f32", 3), ("f64", 7)):
         cfgname = "C2"
         xyz = W.make_xyz(cfgname, 2000 + 13).astype(np.float32 if dtype == "f32" else np.float64)
@@ -247,7 +261,7 @@ def test_vjp_recompute_every_l_max(sph, oracle, dtype):
             _check_vjp_recompute(sph, oracle, xyz, l_max, normalized, dtype, f"{dtype} l_max={l_max} norm={normalized}")
 
 
-def test_vjp_recompute_matches_stored_route_and_generic(sph, oracle, monkeypatch):
+def test_vjp_recompute_matches_stored_route_and_generic(sph, oracle, option):
     """Same numbers as forward-with-gradients followed by the stored-derivative VJP (to rounding),
     and the generic kernel agrees with the specialised one."""
     cfg = W.CONFIGS["C5"]
@@ -262,19 +276,20 @@ def test_vjp_recompute_matches_stored_route_and_generic(sph, oracle, monkeypatch
     assert sph.sphericart_cuda_launch_count() == before + 1
     scale = np.abs(stored).max()
     assert np.max(np.abs(rec - stored)) <= 2e-6 * scale
-    monkeypatch.setenv("SPHB200_FORCE_KERNEL", "generic")
+    option("force_kernel", "generic")
     gen = sph.vjp_recompute(x_d, g_d, True).cpu().numpy()
+    assert sph.sphericart_cuda_last_kernel() == "vjpr_generic"
     assert np.max(np.abs(gen - rec)) <= 2e-6 * scale
     # guard bands: grad_xyz is written exactly where it belongs
     buf = torch.full((n * 3 + 64,), 777.0, device="cuda")
-    monkeypatch.delenv("SPHB200_FORCE_KERNEL")
+    option("force_kernel", "auto")
     sph.sphericart_cuda_vjp_recompute(x_d, g_d, buf[32:-32], n, cfg.l_max, 1, 0, torch.cuda.current_stream().cuda_stream)
     torch.cuda.synchronize()
     assert torch.all(buf[:32] == 777.0) and torch.all(buf[-32:] == 777.0) and torch.all(buf[32:-32] != 777.0)
 
 
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
-def test_cooperative_kernel_long_rows(sph, oracle, dtype, monkeypatch):
+def test_cooperative_kernel_long_rows(sph, oracle, dtype, option):
     """Rows with l_max >= 19 take the CTA-cooperative kernel (kernel_wc.cuh): every derivative order,
     both variants, odd and even row lengths, n below / across / not a multiple of the 128 points a
     CTA owns; and it writes the same numbers as the one-warp-per-point kernel."""
@@ -286,12 +301,14 @@ def test_cooperative_kernel_long_rows(sph, oracle, dtype, monkeypatch):
         xyz = W.make_xyz("C4", n).astype(np_dt)
         s, d, h = _run_gpu(sph, xyz, l_max, normalized, grads, hess)
         _compare(oracle, xyz, l_max, normalized, dtype, s, d, h, f"wc {dtype} l_max={l_max} n={n}")
-        monkeypatch.setenv("SPHB200_FORCE_KERNEL", "wc")   # (without Hessians the default route is tpg)
+        option("force_kernel", "wc")   # (the default route may be another family)
         s, d, h = _run_gpu(sph, xyz, l_max, normalized, grads, hess)
+        assert sph.sphericart_cuda_last_kernel() == "wc"
         _compare(oracle, xyz, l_max, normalized, dtype, s, d, h, f"forced wc {dtype} l_max={l_max} n={n}")
-        monkeypatch.setenv("SPHB200_FORCE_KERNEL", "w1")
+        option("force_kernel", "w1")
         s1, d1, h1 = _run_gpu(sph, xyz, l_max, normalized, grads, hess)
-        monkeypatch.delenv("SPHB200_FORCE_KERNEL")
+        assert sph.sphericart_cuda_last_kernel() == "w"
+        option("force_kernel", "auto")
         for a, b in ((s, s1), (d, d1), (h, h1)):
             if a is not None:
                 assert torch.equal(a, b), "cooperative and one-warp kernels disagree bit-wise"
@@ -311,13 +328,13 @@ def test_cooperative_kernel_long_rows(sph, oracle, dtype, monkeypatch):
 
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
 @pytest.mark.parametrize("lp", [2, 4, 8])
-def test_lanes_per_point_kernel(sph, oracle, dtype, lp, monkeypatch):
+def test_lanes_per_point_kernel(sph, oracle, dtype, lp, option):
     """kernel_tpg.cuh (several lanes per point, run-time l_max): forced for every l_max it can take,
     every lanes-per-point variant, values and values + gradients, both variants, ragged n; C2-style
     points (on the z axis, tiny r) included."""
     np_dt = np.float32 if dtype == "f32" else np.float64
-    monkeypatch.setenv("SPHB200_FORCE_KERNEL", "tpg")
-    monkeypatch.setenv("SPHB200_TPG_LP", str(lp))
+    option("force_kernel", "tpg")
+    option("tpg_lp", lp)
     for l_max, n, grads, normalized in ((0, 5, True, True), (1, 33, True, False), (3, 100, False, True),
                                         (9, 131, True, True), (10, 64, True, False), (13, 77, False, False),
                                         (16, 203, True, True), (21, 50, False, True), (32, 37, False, False)):
@@ -325,6 +342,7 @@ def test_lanes_per_point_kernel(sph, oracle, dtype, lp, monkeypatch):
         before = sph.sphericart_cuda_launch_count()
         s, d, _ = _run_gpu(sph, xyz, l_max, normalized, grads, False)
         assert sph.sphericart_cuda_launch_count() == before + 1
+        assert sph.sphericart_cuda_last_kernel() == "tpg"
         _compare(oracle, xyz, l_max, normalized, dtype, s, d, None, f"tpg {dtype} lp={lp} l_max={l_max} n={n}")
 
 
@@ -428,6 +446,38 @@ def test_host_buffer_entry_points(sph, oracle):
     gx = np.empty((n, 3), np.float32)
     sph.sphericart_cuda_vjp_host(None, d, g, gx, n, cfg.l_max, 0)
     parity.check_vjp(gx[idx], oracle.vjp(d[idx], g[idx], cfg.l_max), d[idx], g[idx], cfg.l_max, "f32")
+
+
+def test_host_buffer_entry_points_many_chunks(sph, oracle, option):
+    """The chunked two-stream path: >= 3 chunks with a ragged last one, slot reuse, pinned host
+    memory, Hessians through compute_host and the VJP through vjp_host."""
+    l_max, n = 5, 1000 + 13
+    L = (l_max + 1) ** 2
+    option("host_chunk_bytes", 13 * L * 8 * 300)          # ~300 points per chunk -> 4 chunks, last one ragged
+    xyz = torch.from_numpy(W.make_xyz("C4", n)).pin_memory()
+    s = torch.empty((n, L), dtype=torch.float64).pin_memory()
+    d = torch.empty((n, 3, L), dtype=torch.float64).pin_memory()
+    h = torch.empty((n, 3, 3, L), dtype=torch.float64).pin_memory()
+    before = sph.sphericart_cuda_launch_count()
+    sph.sphericart_cuda_compute_host(xyz, n, l_max, 1, 1, s, d, h)
+    assert sph.sphericart_cuda_launch_count() - before >= 3
+    x_np = xyz.numpy()
+    ws, wd, wh = oracle.compute(x_np, l_max, True, True, True)
+    parity.check(s.numpy(), ws, x_np, l_max, True, 0, "f64", "host chunks values")
+    parity.check(d.numpy(), wd, x_np, l_max, True, 1, "f64", "host chunks gradients")
+    parity.check(h.numpy(), wh, x_np, l_max, True, 2, "f64", "host chunks hessians")
+    g = torch.from_numpy(np.random.default_rng(5).standard_normal((n, L))).pin_memory()
+    gx = torch.empty((n, 3), dtype=torch.float64).pin_memory()
+    option("host_chunk_bytes", 4 * L * 8 * 300)
+    before = sph.sphericart_cuda_launch_count()
+    sph.sphericart_cuda_vjp_host(None, d, g, gx, n, l_max, 1)
+    assert sph.sphericart_cuda_launch_count() - before >= 3
+    parity.check_vjp(gx.numpy(), oracle.vjp(d.numpy(), g.numpy(), l_max), d.numpy(), g.numpy(), l_max, "f64")
+    # an error in a later chunk (device allocation refused) returns only after both streams have drained
+    option("host_chunk_bytes", 1 << 62)
+    with pytest.raises(sph.SphericartCudaError):
+        sph.sphericart_cuda_compute_host(xyz, 1 << 40, l_max, 1, 1, s, d, h)
+    torch.cuda.synchronize()
 
 
 def test_errors_raise(sph):

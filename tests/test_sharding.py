@@ -62,3 +62,24 @@ def test_two_rank_gloo_run():
     for rank, ranges, tmax, total in res:
         assert ranges[0][0] == 0 and ranges[0][1] == ranges[1][0] and ranges[1][1] == 100_003
         assert tmax == 11.0 and total == 100_003
+
+
+def test_bench_starts_its_own_ranks():
+    """`bench.py --gpus 2` with no launcher in the environment spawns two ranks itself (torch.distributed.run
+    on 127.0.0.1); here on the gloo backend with a stub step (--impl stub): one JSON line, from rank 0,
+    carrying the max-over-ranks time (rank 1 sleeps twice as long as rank 0)."""
+    import json
+    import subprocess
+    import sys
+    from pathlib import Path
+
+    root = Path(__file__).resolve().parent.parent
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    res = subprocess.run([sys.executable, str(root / "bench.py"), "--impl", "stub", "--gpus", "2", "--steps", "20"],
+                         capture_output=True, text=True, env=env, timeout=300)
+    assert res.returncode == 0, res.stderr[-2000:]
+    lines = [l for l in res.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    line = json.loads(lines[0])
+    assert line["n_gpus"] == 2 and line["steps"] == 20
+    assert line["ms_per_step"] >= 2.0          # rank 1's 2 ms per step, not rank 0's 1 ms
