@@ -123,6 +123,62 @@ def vjp_recompute(xyz, grad_sph, l_max: int, normalized: bool, kind: str = "ld")
     return vjp(dsph, grad_sph, l_max, kind=kind)
 
 
+def vjp2(xyz, grad_sph, v, l_max: int, normalized: bool, kind: str = "ld"):
+    """Oracle for ``sphericart_cuda_vjp2`` (SURVEY 8(f) N4: "second-order VJP for double backward";
+    backward pass P:112, derivatives "of any order" P:94).  The backward pass is the map
+    ``g(xyz, w)[n,a] = sum_k dsph[n,a,k](xyz) w[n,k]`` with ``w = grad_sph``; given an upstream
+    gradient ``v [n,3]`` on its output, its own backward returns
+
+        out_xyz[n,b] = sum_{a,k} ddsph[n,a,b,k] v[n,a] w[n,k]       (gradient w.r.t. xyz)
+        out_w[n,k]   = sum_a     dsph[n,a,k]    v[n,a]              (gradient w.r.t. grad_sph)
+
+    Nothing but ``compute(..., hessians=True)`` followed by two plain contractions in the oracle's
+    precision."""
+    dt = _DTYPE[kind]
+    _, dsph, ddsph = compute(xyz, l_max, normalized, gradients=True, hessians=True, kind=kind)
+    w = np.asarray(grad_sph).astype(dt)
+    v = np.asarray(v).astype(dt)
+    n, L = w.shape
+    out_xyz = np.zeros((n, 3), dt)
+    for a in range(3):
+        for b in range(3):
+            out_xyz[:, b] += v[:, a] * (ddsph[:, a, b, :] * w).sum(axis=1)
+    out_w = np.zeros((n, L), dt)
+    for a in range(3):
+        out_w += dsph[:, a, :] * v[:, a:a + 1]
+    return out_xyz, out_w
+
+
+# Conventions other than the paper's own (SURVEY 8(f) N4, P:168: the paper compares with e3nn).
+# AXES_E3NN: the harmonics are those of the paper evaluated at the cyclically permuted point
+# (x', y', z') = (z, x, y), so that the l = 1 row is proportional to (x, y, z) in that order instead
+# of (y, z, x) (DESIGN.md reading S1).  SCALE_*: what the per-l row norm sum_m Y_lm^2 is on the
+# unit sphere: (2l+1)/4pi ("integral": orthonormal, the paper's), 2l+1 ("component"), 1 ("norm").
+AXES_STANDARD, AXES_E3NN = 0, 1
+SCALE_INTEGRAL, SCALE_COMPONENT, SCALE_NORM = 0, 1, 2
+
+
+def compute_convention(xyz, l_max: int, normalized: bool, axes: int, scale: int, gradients: bool = False,
+                       hessians: bool = False, kind: str = "ld"):
+    """Oracle for ``sphericart_cuda_compute_ex``: ``compute`` at the permuted point, every l-row
+    multiplied by its scale, derivative axes mapped back to the caller's (x, y, z)."""
+    dt = _DTYPE[kind]
+    xyz = np.ascontiguousarray(np.asarray(xyz), dtype=np.float64).reshape(-1, 3)
+    perm = [2, 0, 1] if axes == AXES_E3NN else [0, 1, 2]       # ours[i] = caller's[perm[i]]
+    sph, dsph, ddsph = compute(xyz[:, perm], l_max, normalized, gradients, hessians, kind=kind)
+    l = np.concatenate([[ll] * (2 * ll + 1) for ll in range(l_max + 1)]).astype(dt)
+    four_pi = 16 * np.arctan(dt(1))
+    sc = {SCALE_INTEGRAL: np.ones_like(l), SCALE_COMPONENT: np.sqrt(four_pi) * np.ones_like(l),
+          SCALE_NORM: np.sqrt(four_pi / (2 * l + 1))}[scale]
+    sph = sph * sc
+    inv = np.argsort(perm)                                     # d/d caller's[j] = d/d ours[inv[j]]
+    if dsph is not None:
+        dsph = dsph[:, inv, :] * sc
+    if ddsph is not None:
+        ddsph = ddsph[:, inv][:, :, inv] * sc
+    return sph, dsph, ddsph
+
+
 def expand(xyz, radial, seg_ptr, l_max: int):
     """Oracle for ``sphericart_cuda_expand`` (Eq. 1):
 

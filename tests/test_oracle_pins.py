@@ -626,6 +626,86 @@ def test_vjp_recompute_is_gradient_of_weighted_sum(oracle, normalized):
     assert np.array_equal(got, oracle.vjp(d, w, l_max))
 
 
+@pytest.mark.parametrize("normalized", [False, True])
+def test_vjp2_is_the_backward_of_the_backward(oracle, normalized):
+    """N4 pin (double backward): with f(x, w) = sum_a v_a * vjp_recompute(x, w)[a],
+    vjp2's out_xyz is the Cartesian gradient of f in x -- checked against 4th-order central
+    differences of oracle.vjp_recompute (the Hessians under test never enter the reference) --
+    and out_w is its gradient in w, which by linearity in w is f evaluated at one-hot w."""
+    l_max = 10
+    L = (l_max + 1) ** 2
+    pts = random_points(30, 21)
+    pts = np.concatenate([pts, [[0, 0, 1.25], [0, 0, -0.5]]])
+    rng = np.random.default_rng(22)
+    w = rng.standard_normal((len(pts), L)).astype(LD)
+    v = rng.standard_normal((len(pts), 3)).astype(LD)
+    out_xyz, out_w = oracle.vjp2(pts, w, v, l_max, normalized)
+    assert out_xyz.shape == (len(pts), 3) and out_w.shape == (len(pts), L) and out_xyz.dtype == LD
+    f = lambda x: (oracle.vjp_recompute(x, w, l_max, normalized) * v).sum(axis=1)
+    h = 2.0 ** -22
+    r = np.linalg.norm(pts, axis=1)
+    scale = np.zeros(len(pts), LD)
+    for l in range(l_max + 1):
+        rho = r ** l if not normalized else np.ones_like(r)
+        scale += row_scale(l) * rho * (max(l, 1) / r) ** 2 * np.abs(w[:, l * l:(l + 1) ** 2]).max(axis=1)
+    scale *= np.abs(v).max(axis=1)
+    for b in range(3):
+        e = np.zeros(3)
+        e[b] = h
+        fd = (8 * (f(pts + e) - f(pts - e)) - (f(pts + 2 * e) - f(pts - 2 * e))) / (12 * LD(h))
+        assert float(np.max(np.abs(fd - out_xyz[:, b]) / scale)) < 1e-10, b
+    for k in (0, 1, 3, 17, L - 1):
+        onehot = np.zeros((len(pts), L), LD)
+        onehot[:, k] = 1
+        fk = (oracle.vjp_recompute(pts, onehot, l_max, normalized) * v).sum(axis=1)
+        assert np.max(np.abs(fk - out_w[:, k])) <= 8 * EPS_LD * np.max(np.abs(fk) + 1)
+    # symmetric Hessians: swapping the roles of v's axis and the output axis gives the same contraction
+    _, _, H = oracle.compute(pts, l_max, normalized, True, True)
+    alt = np.einsum("nbak,na,nk->nb", H, v, w)
+    assert float(np.max(np.abs(alt - out_xyz) / scale[:, None])) < 1e-15
+
+
+def test_conventions_closed_forms_and_row_norms(oracle):
+    """N4 pin (conventions): with the e3nn axes the l = 1 row is proportional to (x, y, z) in
+    that order; 'integral' rows have norm^2 (2l+1)/4pi, 'component' 2l+1, 'norm' 1 on the unit
+    sphere; gradients against finite differences of the converted values; the standard axes with
+    the integral scale are `compute` itself."""
+    l_max = 9
+    pts = random_points(25, 31)
+    r = np.sqrt((pts.astype(LD) ** 2).sum(axis=1))
+    u = pts.astype(LD) / r[:, None]
+    want_norm2 = {oracle.SCALE_INTEGRAL: lambda l: (2 * l + 1) / (16 * np.arctan(LD(1))), oracle.SCALE_COMPONENT: lambda l: LD(2 * l + 1),
+                  oracle.SCALE_NORM: lambda l: LD(1)}
+    for scale, norm2 in want_norm2.items():
+        y, g, H = oracle.compute_convention(pts, l_max, True, oracle.AXES_E3NN, scale, True, True)
+        c1 = np.sqrt(norm2(1))                       # |Y_1|^2 = norm2 and Y_1 = c1 * (x, y, z)/r
+        assert np.max(np.abs(y[:, 1:4] - c1 * u)) < 8 * EPS_LD * float(c1)
+        for l in range(l_max + 1):
+            n2 = (y[:, l * l:(l + 1) ** 2] ** 2).sum(axis=1)
+            assert np.max(np.abs(n2 / norm2(l) - 1)) < 64 * (l + 1) * EPS_LD
+        h = 2.0 ** -22
+        val = lambda x: oracle.compute_convention(x, l_max, True, oracle.AXES_E3NN, scale, True)
+        for a in range(3):
+            e = np.zeros(3)
+            e[a] = h
+            (yp1, gp1, _), (ym1, gm1, _), (yp2, gp2, _), (ym2, gm2, _) = (val(pts + e), val(pts - e), val(pts + 2 * e),
+                                                                            val(pts - 2 * e))
+            fd_g = (8 * (yp1 - ym1) - (yp2 - ym2)) / (12 * LD(h))
+            fd_H = (8 * (gp1 - gm1) - (gp2 - gm2)) / (12 * LD(h))
+            for l in range(l_max + 1):
+                sl = slice(l * l, (l + 1) ** 2)
+                S = np.sqrt(norm2(l))
+                assert float(np.max(np.abs(fd_g[:, sl] - g[:, a, sl]) / (S * max(l, 1) / r)[:, None])) < 1e-11
+                assert float(np.max(np.abs(fd_H[:, :, sl] - H[:, :, a, sl]) / (S * (max(l, 1) / r) ** 2)[:, None, None])) < 1e-11
+    # solid harmonics, e3nn axes: l = 1 row is c1 * (x, y, z) itself
+    y, _, _ = oracle.compute_convention(pts, 2, False, oracle.AXES_E3NN, oracle.SCALE_COMPONENT)
+    assert np.max(np.abs(y[:, 1:4] - np.sqrt(LD(3)) * pts.astype(LD))) < 16 * EPS_LD * 4
+    # the paper's own convention is untouched
+    a = oracle.compute_convention(pts, l_max, True, oracle.AXES_STANDARD, oracle.SCALE_INTEGRAL, True, True)
+    b = oracle.compute(pts, l_max, True, True, True)
+    assert all(np.array_equal(x, z) for x, z in zip(a, b))
+
+
 def test_expand_eq1(oracle):
     """N2 pins for the density expansion of Eq. 1: one-point segments, brute force, order
     independence, parity of antipodal pairs, rotation invariance of the power spectrum."""
