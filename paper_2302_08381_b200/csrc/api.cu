@@ -14,8 +14,15 @@
 #include "options.h"
 #include "ptx.cuh"
 #include "sph_core.cuh"
+#include "tables.h"
+namespace sphb200 {
+// constant-bank copy of the coefficient tables for the kernels of this translation unit
+__constant__ SphTables c_tables;
+}  // namespace sphb200
+
 #include "kernel_vjp.cuh"
 #include "kernel_tpg.cuh"
+#include "kernel_tq.cuh"
 #include "kernel_w.cuh"
 #include "kernel_wc.cuh"
 #include "tpb_api.h"
@@ -23,9 +30,6 @@
 namespace sphb200 {
 
 SphOptions g_opt;   // options.h
-
-// constant-bank copy of the coefficient tables for the kernels of this translation unit
-__constant__ SphTables c_tables;
 
 static thread_local char g_err[512] = "";
 static thread_local const char* g_last_kernel = "";
@@ -61,6 +65,7 @@ struct DeviceState {
     int sm_count = 0;
     int smem_optin = 0;          // max dynamic shared memory per block
     SphTables* d_tables = nullptr;   // copy of the tables in global memory (warp kernel)
+    unsigned short* d_lm = nullptr;  // (l | m << 8) of every triangle index (tq kernel)
 };
 static DeviceState g_dev[MAX_DEVICES];
 static std::mutex g_mutex;
@@ -95,6 +100,11 @@ static int device_state(DeviceState** out) {
             return fail(SPHERICART_CUDA_ECUDA, "table upload failed: %s", cudaGetErrorString(cudaGetLastError()));
         CUDA_TRY(cudaMalloc(&st.d_tables, sizeof(SphTables)));
         CUDA_TRY(cudaMemcpy(st.d_tables, &g_host_tables, sizeof(SphTables), cudaMemcpyHostToDevice));
+        static unsigned short lm[SPH_TRI_SIZE];
+        for (int l = 0; l <= SPH_MAX_L; ++l)
+            for (int m = 0; m <= l; ++m) lm[SPH_TRI(l, m)] = (unsigned short)(l | (m << 8));
+        CUDA_TRY(cudaMalloc(&st.d_lm, sizeof(lm)));
+        CUDA_TRY(cudaMemcpy(st.d_lm, lm, sizeof(lm), cudaMemcpyHostToDevice));
         st.ready = true;
         st.ready_flag.store(true, std::memory_order_release);
     }
@@ -192,6 +202,19 @@ static int compute_device(const void* xyz, int64_t n, int l_max, int normalized,
         if (r < 0) return fail(SPHERICART_CUDA_ECUDA, "tpb launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         if (r == 0) {
             launched("tpb");
+            return 0;
+        }
+    }
+    if (force == FORCE_TQ) {
+        // two-phase kernel: recurrences lane = point, assembly lane = (l, m) pair, small full-row tiles
+        TqLaunch lq{};
+        if (tq_plan(st->sm_count, st->smem_optin, n, l_max, normalized, dtype, sph, dsph, ddsph, xyz, st->d_tables,
+                    st->d_lm, &lq) == 0) {
+            rc = allow_smem(lq.func, (int)lq.smem);
+            if (rc) return rc;
+            tq_launch(lq, stream);
+            launched("tq");
+            CUDA_TRY(cudaGetLastError());
             return 0;
         }
     }

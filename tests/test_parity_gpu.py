@@ -342,8 +342,31 @@ def test_lanes_per_point_kernel(sph, oracle, dtype, lp, option):
         before = sph.sphericart_cuda_launch_count()
         s, d, _ = _run_gpu(sph, xyz, l_max, normalized, grads, False)
         assert sph.sphericart_cuda_launch_count() == before + 1
-        assert sph.sphericart_cuda_last_kernel() == "tpg"
+        assert sph.sphericart_cuda_last_kernel() in ("tpg", "w")     # (tpg declines the longest rows)
         _compare(oracle, xyz, l_max, normalized, dtype, s, d, None, f"tpg {dtype} lp={lp} l_max={l_max} n={n}")
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("l_max", [0, 1, 2, 3, 5, 8, 9, 11, 12, 15, 16, 20, 23, 27, 32])
+def test_two_phase_kernel(sph, oracle, dtype, l_max, option):
+    """kernel_tq.cuh (recurrences lane = point, assembly lane = (l, m) pair, full-row tiles of a few
+    points): forced for every derivative order and both variants; n spans several batches and tiles
+    with a ragged tail, and a second n that ends inside the first tile; C2-style points (on the z
+    axis, tiny r) up to l_max = 16."""
+    np_dt = np.float32 if dtype == "f32" else np.float64
+    option("force_kernel", "tq")
+    for n in (3 * 32 + 100 + 7, 3):
+        xyz = W.make_xyz("C2" if l_max <= 16 else "C4", n, seed=l_max).astype(np_dt)
+        for normalized in (True, False):
+            for deriv in (0, 1, 2):
+                before = sph.sphericart_cuda_launch_count()
+                s, d, h = _run_gpu(sph, xyz, l_max, normalized, deriv >= 1, deriv >= 2)
+                assert sph.sphericart_cuda_launch_count() == before + 1
+                if sph.sphericart_cuda_last_kernel() != "tq":       # rows too long for two full-row images
+                    assert deriv == 2 and l_max > 16
+                    continue
+                _compare(oracle, xyz, l_max, normalized, dtype, s, d, h,
+                         f"tq {dtype} l_max={l_max} n={n} norm={normalized} deriv={deriv}")
 
 
 def test_stream_order_with_programmatic_dependent_launch(sph):
