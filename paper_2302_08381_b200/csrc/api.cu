@@ -192,6 +192,19 @@ static int compute_device(const void* xyz, int64_t n, int l_max, int normalized,
 
     const int force = g_opt.force_kernel;
     const bool force_w = force == FORCE_W || force == FORCE_W1 || force == FORCE_WC;
+    if (force == FORCE_TQ || (force == FORCE_NONE && TQ_SHAPE[dtype != 0][ddsph ? 2 : (dsph ? 1 : 0)][l_max][0])) {
+        // two-phase kernel: recurrences lane = point, assembly lane = (l, m) pair, small full-row tiles
+        TqLaunch lq{};
+        if (tq_plan(st->sm_count, st->smem_optin, n, l_max, normalized, dtype, sph, dsph, ddsph, xyz, st->d_tables,
+                    st->d_lm, &lq) == 0) {
+            rc = allow_smem(lq.func, (int)lq.smem);
+            if (rc) return rc;
+            tq_launch(lq, stream);
+            launched("tq");
+            CUDA_TRY(cudaGetLastError());
+            return 0;
+        }
+    }
     if (force == FORCE_NONE || force == FORCE_TPB) {
         // compile-time-l_max kernels (two threads per point): every l_max that has an instantiation
         const bool f32 = dtype == SPHERICART_CUDA_F32;
@@ -202,19 +215,6 @@ static int compute_device(const void* xyz, int64_t n, int l_max, int normalized,
         if (r < 0) return fail(SPHERICART_CUDA_ECUDA, "tpb launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         if (r == 0) {
             launched("tpb");
-            return 0;
-        }
-    }
-    if (force == FORCE_TQ) {
-        // two-phase kernel: recurrences lane = point, assembly lane = (l, m) pair, small full-row tiles
-        TqLaunch lq{};
-        if (tq_plan(st->sm_count, st->smem_optin, n, l_max, normalized, dtype, sph, dsph, ddsph, xyz, st->d_tables,
-                    st->d_lm, &lq) == 0) {
-            rc = allow_smem(lq.func, (int)lq.smem);
-            if (rc) return rc;
-            tq_launch(lq, stream);
-            launched("tq");
-            CUDA_TRY(cudaGetLastError());
             return 0;
         }
     }
@@ -544,7 +544,7 @@ int sphericart_cuda_set_option(const char* name, const char* value) {
     const IntOpt ints[] = {{"tpg_lp", &g_opt.tpg_lp}, {"w_nbuf", &g_opt.w_nbuf}, {"w_warps", &g_opt.w_warps},
                            {"w_ppw", &g_opt.w_ppw}, {"wc_min_l", &g_opt.wc_min_l}, {"vjp_warps", &g_opt.vjp_warps},
                            {"tpb_tiles", &g_opt.tpb_tiles}, {"tpb_split", &g_opt.tpb_split}, {"pdl", &g_opt.pdl},
-                           {"tq_points", &g_opt.tq_points}};
+                           {"tq_points", &g_opt.tq_points}, {"tq_warps", &g_opt.tq_warps}, {"tq_batch", &g_opt.tq_batch}, {"tq_images", &g_opt.tq_images}};
     if (!strcmp(name, "force_kernel")) {
         struct { const char* v; int code; } const kinds[] = {
             {"", FORCE_NONE}, {"auto", FORCE_NONE}, {"tpb", FORCE_TPB}, {"tpg", FORCE_TPG}, {"w", FORCE_W},

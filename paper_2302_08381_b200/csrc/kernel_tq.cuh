@@ -39,9 +39,12 @@
 // which is Eq. 10 once / twice for the solid harmonics and the Euler-simplified chain rule of
 // sph_core.cuh for the normalised ones, regrouped by the azimuthal factor they multiply.
 #pragma once
+#include <cmath>
+
 #include "options.h"
 #include "ptx.cuh"
 #include "sph_core.cuh"
+#include "tq_table.h"
 
 namespace sphb200 {
 
@@ -57,6 +60,7 @@ struct TqParams {
     int batch;                   // points per phase-A batch: 32, 16 or 8
     int pts_tile;                // points per image; divides batch
     int batches_per_cta;         // consecutive batches one CTA works through
+    int n_images;                // 2: a tile drains while the next is assembled; 1: the longest rows
 };
 
 constexpr int TQ_MAX_WARPS = 8;
@@ -64,21 +68,72 @@ constexpr int TQ_MAX_WARPS = 8;
 // shared-memory carve-up (bytes), identical on host and device
 struct TqSmem {
     int T, TP, CP;
-    size_t q_bytes, cs_bytes, pt_bytes, img_bytes, total;
-    __host__ __device__ TqSmem(int l_max, int deriv, int esize, int batch, int pts_tile) {
+    size_t gt_off, ht_off, lm_off, q_off, cs_off, pt_off, img_off, img_bytes, total;
+    size_t reg_g, reg_h;   // offsets of the dsph / ddsph regions inside an image
+    __host__ __device__ TqSmem(int l_max, int deriv, int esize, int batch, int pts_tile, int n_images) {
         T = (l_max + 1) * (l_max + 2) / 2;
         TP = (T + 3) | 1;          // doubles per point: three finite pad entries, odd pitch (conflict-free lane = point stores)
-        CP = (l_max + 1) | 1;      // (c, s) pairs per point, odd pitch
-        q_bytes = (size_t)batch * TP * 8;
-        cs_bytes = (size_t)batch * CP * 16;
-        pt_bytes = (size_t)batch * 32;
+        CP = (l_max + 3) | 1;      // (c, s) pairs per point behind two zero pad entries ((c,s)_{-1}, (c,s)_{-2}), odd pitch
+        size_t o = 0;
+        gt_off = o;                // {G1, Gz}[t]
+        o += deriv >= 1 ? (size_t)T * 16 : 0;
+        ht_off = o;                // {H2, Hxz, Hzz, -}[t]
+        o += deriv >= 2 ? (size_t)T * 32 : 0;
+        lm_off = o;                // l | m << 8
+        o += ((size_t)T * 2 + 15) & ~(size_t)15;
+        q_off = o;
+        o += (size_t)batch * TP * 8;
+        o = (o + 15) & ~(size_t)15;
+        cs_off = o;
+        o += (size_t)batch * CP * 16;
+        pt_off = o;
+        o += (size_t)batch * 32;
+        img_off = (o + 127) & ~(size_t)127;
         const int rows = deriv == 0 ? 1 : (deriv == 1 ? 4 : 13);
         const size_t L = (size_t)(l_max + 1) * (l_max + 1);
-        img_bytes = ((size_t)pts_tile * rows * L * esize + 127) & ~(size_t)127;
-        total = ((q_bytes + cs_bytes + pt_bytes + 127) & ~(size_t)127) + 2 * img_bytes;
+        // one region per output array, each with 16 bytes of slack: a region is staged at the offset
+        // (0..15 bytes) its global address has from a 16-byte boundary, so that the aligned body of
+        // the run can leave as one bulk store whatever the tile's first point is
+        const size_t sb = (size_t)pts_tile * L * esize;
+        reg_g = (sb + 16 + 15) & ~(size_t)15;
+        reg_h = reg_g + ((3 * sb + 16 + 15) & ~(size_t)15);
+        const size_t end = rows == 1 ? reg_g : (rows == 4 ? reg_h : reg_h + ((9 * sb + 16 + 15) & ~(size_t)15));
+        img_bytes = (end + 127) & ~(size_t)127;
+        total = img_off + (size_t)n_images * img_bytes;
     }
-    __host__ __device__ size_t img_offset() const { return (q_bytes + cs_bytes + pt_bytes + 127) & ~(size_t)127; }
 };
+
+// shared-memory accesses through 32-bit shared addresses (one IADD per address instead of the
+// 64-bit generic arithmetic the compiler emits for pointers into a dynamic carve-up).  volatile:
+// they keep their order against the barriers and fences, which are volatile too.
+__device__ __forceinline__ double tq_lds(uint32_t a) {
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ double tq_lds8(uint32_t a) {   // [a + 8]
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1+8];" : "=d"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ double tq_lds16(uint32_t a) {  // [a + 16]
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1+16];" : "=d"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ void tq_lds2(uint32_t a, double& x, double& y) {
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(x), "=d"(y) : "r"(a));
+}
+__device__ __forceinline__ unsigned tq_lds_u16(uint32_t a) {
+    unsigned short v;
+    asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ void tq_sts(uint32_t a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
+__device__ __forceinline__ void tq_sts(uint32_t a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
+__device__ __forceinline__ void tq_sts2(uint32_t a, double x, double y) {
+    asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(a), "d"(x), "d"(y) : "memory");
+}
 
 template <typename T, typename R, int DERIV, bool NORM>
 __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqParams prm) {
@@ -91,12 +146,12 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
     const int l_max = prm.l_max;
     const int L = (l_max + 1) * (l_max + 1);
     const int B = prm.batch, P = prm.pts_tile;
-    const TqSmem lay(l_max, DERIV, ES, B, P);
+    const TqSmem lay(l_max, DERIV, ES, B, P, prm.n_images);
     const int TT = lay.T, TP = lay.TP, CP = lay.CP;
-    double* __restrict__ Qs = reinterpret_cast<double*>(smem);
-    double2* __restrict__ CS = reinterpret_cast<double2*>(smem + lay.q_bytes);
-    double4* __restrict__ PT = reinterpret_cast<double4*>(smem + lay.q_bytes + lay.cs_bytes);
-    unsigned char* img0 = smem + lay.img_offset();
+    const uint32_t s0 = smem_u32(smem);
+    const uint32_t sGT = s0 + (uint32_t)lay.gt_off, sHT = s0 + (uint32_t)lay.ht_off, sLM = s0 + (uint32_t)lay.lm_off;
+    const uint32_t sQ = s0 + (uint32_t)lay.q_off, sCS = s0 + (uint32_t)lay.cs_off, sPT = s0 + (uint32_t)lay.pt_off;
+    unsigned char* img0 = smem + lay.img_off;
     const int64_t n = prm.n;
     const T* __restrict__ xyz = static_cast<const T*>(prm.xyz);
     T* __restrict__ sph = static_cast<T*>(prm.sph);
@@ -105,10 +160,26 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
     const SphTables& TB = c_tables;
     const uint64_t policy = policy_evict_first();
 
-    // pad entries behind every point's triangle: read (times a zero coefficient) by phase B
-    for (int i = threadIdx.x; i < B * 3; i += blockDim.x) Qs[(i / 3) * TP + TT + (i % 3)] = 0.0;
+    // once per CTA: phase B's coefficient tables and the (l, m) of every triangle index -> shared
+    // memory; the pad entries behind every point's triangle and in front of its (c, s) list, which
+    // phase B reads times a zero coefficient
+    for (int t = threadIdx.x; t < TT; t += blockDim.x) {
+        if (DERIV >= 1) tq_sts2(sGT + t * 16, __ldg(&prm.tab->G1[t]), __ldg(&prm.tab->Gz[t]));
+        if (DERIV >= 2) {
+            tq_sts2(sHT + t * 32, __ldg(&prm.tab->H2[t]), __ldg(&prm.tab->Hxz[t]));
+            tq_sts(sHT + t * 32 + 16, __ldg(&prm.tab->Hzz[t]));
+        }
+        reinterpret_cast<unsigned short*>(smem + lay.lm_off)[t] = __ldg(prm.lm + t);
+    }
+    for (int i = threadIdx.x; i < B * 3; i += blockDim.x) tq_sts(sQ + ((i / 3) * TP + TT + (i % 3)) * 8, 0.0);
+    for (int i = threadIdx.x; i < B * 2; i += blockDim.x) tq_sts2(sCS + ((i >> 1) * CP + (i & 1)) * 16, 0.0, 0.0);
 
-    const uint32_t s_bytes = (uint32_t)P * L * ES;
+    const int NCH = (TT + 31) >> 5;                    // 32-pair chunks of one point's triangle
+    const int d_pl = W / NCH, d_ch = W - d_pl * NCH;   // one step of a warp through the (point, chunk) units
+    const int w_pl0 = warp / NCH, w_ch0 = warp - w_pl0 * NCH;
+    const int PP = P >> 1;                             // pairs of points per tile (P is even)
+    const uint32_t row_b = (uint32_t)L * ES;          // bytes of one row of one point
+    const uint32_t s_bytes = (uint32_t)P * row_b;     // bytes of the tile's sph image
     int tile_no = 0;   // tiles this CTA has issued: parity picks the image
     for (int bi = 0; bi < prm.batches_per_cta; ++bi) {
         const int64_t b0 = ((int64_t)blockIdx.x * prm.batches_per_cta + bi) * B;
@@ -136,11 +207,12 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
                 r2 = RT::r2_of(X, Y, Z);
             }
             if (warp == W - 1) {   // Eq. 9 and the point itself: the warp with the shortest columns
-                PT[lane] = make_double4(to_double(X), to_double(Y), to_double(Z), rinv);
+                tq_sts2(sPT + lane * 32, to_double(X), to_double(Y));
+                tq_sts2(sPT + lane * 32 + 16, to_double(Z), rinv);
                 R c = RT::make(1.0, 0.0), s = RT::make(0.0, 0.0);
-                double2* cs = CS + lane * CP;
-                for (int m = 0; m <= l_max; ++m) {
-                    cs[m] = make_double2(to_double(c), to_double(s));
+                uint32_t a = sCS + (lane * CP + 2) * 16;
+                for (int m = 0; m <= l_max; ++m, a += 16) {
+                    tq_sts2(a, to_double(c), to_double(s));
                     const R cn = X * c - Y * s;
                     const R sn = X * s + Y * c;
                     c = cn;
@@ -148,13 +220,13 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
                 }
             }
             // columns of the folded Eq. 7, dealt to the warps in snake order: m = w, 2W-1-w, 2W+w, ...
-            double* q_out = Qs + lane * TP;
+            const uint32_t q_out = sQ + lane * TP * 8;
             for (int i = 0; i * W <= l_max; ++i) {
                 const int m = (i & 1) ? (i + 1) * W - 1 - warp : i * W + warp;
                 if (m > l_max) continue;
                 int t = SPH_TRI(m, m);
                 R q = RT::make(TB.D_hi[m], TB.D_lo[m]), qp = RT::make(0.0, 0.0);
-                q_out[t] = to_double(q);
+                tq_sts(q_out + t * 8, to_double(q));
                 for (int l = m + 1; l <= l_max; ++l) {
                     t += l;   // SPH_TRI(l, m) - SPH_TRI(l-1, m) = l
                     const R a = RT::make(TB.A_hi[t], TB.A_lo[t]);
@@ -167,7 +239,7 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
                     }
                     qp = q;
                     q = qn;
-                    q_out[t] = to_double(q);
+                    tq_sts(q_out + t * 8, to_double(q));
                 }
             }
         }
@@ -178,119 +250,161 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
         for (int ti = 0; ti < n_tiles; ++ti) {
             const int64_t p0 = b0 + (int64_t)ti * P;
             if (p0 >= n) break;
-            unsigned char* img = img0 + (size_t)(tile_no & 1) * lay.img_bytes;
-            T* __restrict__ S0 = reinterpret_cast<T*>(img);
-            T* __restrict__ G0 = reinterpret_cast<T*>(img + s_bytes);
-            T* __restrict__ H0 = reinterpret_cast<T*>(img + 4u * s_bytes);
-            const int items = P * TT;
-            for (int e0 = warp * 32; e0 < items; e0 += W * 32) {
-                const int e = e0 + lane;
-                if (e >= items) break;
-                int pi = e0 / TT;           // warp-uniform division, then at most a few steps
-                int t = e - pi * TT;
-                while (t >= TT) {
-                    t -= TT;
-                    ++pi;
-                }
-                const int pb = ti * P + pi;   // point inside the batch
-                const double4 pt = PT[pb];
-                const double x = pt.x, y = pt.y, z = pt.z, ri = pt.w;
-                const unsigned lmv = __ldg(prm.lm + t);
-                const int l = (int)(lmv & 0xffu), m = (int)(lmv >> 8);
-                const double* __restrict__ Qp = Qs + pb * TP;
-                const double2* __restrict__ cs = CS + pb * CP;
-                const double Q = Qp[t];
-                const double2 cs0 = cs[m];
-                const double Ac = (m == 0) ? SPH_INV_SQRT2 : cs0.x, As = cs0.y;
-                const int kc = l * (l + 1) + m, ks = kc - 2 * m;
-                T* __restrict__ S = S0 + pi * L;
-                S[kc] = static_cast<T>(Q * Ac);
-                if (m > 0) S[ks] = static_cast<T>(Q * As);
-                if constexpr (DERIV >= 1) {
+            unsigned char* img = img0 + (size_t)(tile_no & (prm.n_images - 1)) * lay.img_bytes;
+            // each array's run is staged at the offset its global address has from a 16-byte boundary
+            const uint32_t tile_b = (uint32_t)(p0 & 15) * row_b;   // (p0 L ES) mod 16, in 32 bits
+            const uint32_t dS = tile_b & 15u, dG = (3u * tile_b) & 15u, dH = (9u * tile_b) & 15u;
+            unsigned char* iS = img + dS;
+            unsigned char* iG = img + lay.reg_g + dG;
+            unsigned char* iH = img + lay.reg_h + dH;
+            const uint32_t sS = smem_u32(iS), sG = smem_u32(iG), sH = smem_u32(iH);
+            if (prm.n_images == 1 && tile_no > 0) {   // the one image: its last stores must have read it
+                if (threadIdx.x == 0) bulk_wait_read<0>();
+                __syncthreads();
+            }
+            // work units = (two points of the tile, 32 consecutive pairs of the triangle), dealt to the warps
+            // round-robin; (pl, ch) of this warp's unit advances incrementally (warp-uniform, no division),
+            // so everything that depends on the point only is computed per unit, not per lane
+            int pp = w_pl0, ch = w_ch0;   // pp: PAIR of points of the tile (a lane does the same (l, m) for both)
+            while (pp < PP) {
+                const int t = ch * 32 + lane;
+                if (t < TT) {
+                    // ---- per (l, m): shared by the two points ----
+                    const unsigned lmv = tq_lds_u16(sLM + t * 2);
+                    const int l = (int)(lmv & 0xffu), m = (int)(lmv >> 8);
                     const double dl = (double)l, dm = (double)m;
-                    const int t1 = t - l;
-                    const double q1 = __ldg(&prm.tab->G1[t]) * Qp[t1 + 1];   // F_l^m Q_{l-1}^{m+1}
-                    const double qz = __ldg(&prm.tab->Gz[t]) * Qp[t1];       // F_l^m (l+m) Q_{l-1}^m
-                    const double2 cs1 = cs[m >= 1 ? m - 1 : 0];
-                    // Eq. 10: cos: A_x = m c_{m-1}, A_y = -m s_{m-1}; sin: A_x = m s_{m-1}, A_y = m c_{m-1}
-                    const double mc1 = dm * cs1.x, ms1 = dm * cs1.y;
-                    const double lQ = dl * Q;
-                    const double E1 = NORM ? q1 - lQ : q1;
-                    const double EZ = NORM ? SPH_FMA(-lQ, z, qz) : qz;
-                    const double sg = NORM ? ri : 1.0;
-                    const double E1g = E1 * sg;
-                    const double ax = x * E1g, ay = y * E1g, az = EZ * sg, Qg = Q * sg;
-                    T* __restrict__ G = G0 + pi * 3 * L;
-                    G[kc] = static_cast<T>(SPH_FMA(ax, Ac, Qg * mc1));
-                    G[L + kc] = static_cast<T>(SPH_FMA(ay, Ac, -(Qg * ms1)));
-                    G[2 * L + kc] = static_cast<T>(az * Ac);
-                    if (m > 0) {
-                        G[ks] = static_cast<T>(SPH_FMA(ax, As, Qg * ms1));
-                        G[L + ks] = static_cast<T>(SPH_FMA(ay, As, Qg * mc1));
-                        G[2 * L + ks] = static_cast<T>(az * As);
-                    }
+                    // the (l, -m) outputs are stored FIRST and unconditionally: for m = 0 they land on the
+                    // (l, 0) slot and the cos-branch store that follows overwrites them (no branch)
+                    const uint32_t kc_b = (uint32_t)(l * (l + 1) + m) * ES, m2_b = (uint32_t)(2 * m) * ES;
+                    const uint32_t l8 = (uint32_t)l * 8;
+                    double G1 = 0.0, Gz = 0.0, H2 = 0.0, Hxz = 0.0, Hzz = 0.0;
+                    if constexpr (DERIV >= 1) tq_lds2(sGT + t * 16, G1, Gz);
                     if constexpr (DERIV >= 2) {
-                        const int t2 = t1 - l + 1;
-                        const double q2 = __ldg(&prm.tab->H2[t]) * Qp[t2 + 2];    // F_l^m Q_{l-2}^{m+2}
-                        const double qxz = __ldg(&prm.tab->Hxz[t]) * Qp[t2 + 1];  // F_l^m (l+m) Q_{l-2}^{m+1}
-                        const double qzz = __ldg(&prm.tab->Hzz[t]) * Qp[t2];      // F_l^m (l+m)(l+m-1) Q_{l-2}^m
-                        const double2 cs2 = cs[m >= 2 ? m - 2 : 0];
-                        const double dmm = dm * (dm - 1.0);
-                        // Eq. 10 twice: cos: A_xx = m(m-1) c_{m-2}, A_xy = -m(m-1) s_{m-2}; sin: s_{m-2}, c_{m-2}
-                        const double mmc2 = dmm * cs2.x, mms2 = dmm * cs2.y;
-                        double F2 = q2, FXZ = qxz, FZZ = qzz;
-                        if (NORM) {
-                            const double w = (dl + 2.0) * lQ;
-                            F2 = SPH_FMA(-2.0 * dl, q1, q2 + w);
-                            FXZ = SPH_FMA(z, SPH_FMA(-dl, q1, w), SPH_FMA(-dl, qz, qxz));
-                            FZZ = SPH_FMA(z, SPH_FMA(w, z, -2.0 * dl * qz), qzz) - lQ;
-                        }
-                        const double sh = NORM ? ri * ri : 1.0;
-                        const double E1h = E1 * sh, F2h = F2 * sh, Qh = Q * sh;
-                        const double cxx = SPH_FMA(x * x, F2h, E1h), cyy = SPH_FMA(y * y, F2h, E1h), cxy = (x * y) * F2h;
-                        const double bx = x * E1h, by = y * E1h, bx2 = bx + bx, by2 = by + by;
-                        const double FXZh = FXZ * sh;
-                        const double cxz = x * FXZh, cyz = y * FXZh, ezh = EZ * sh, czz = FZZ * sh;
-                        T* __restrict__ H = H0 + pi * 9 * L;
-                        auto put = [&](int k, double A, double Ax, double Ay, double Axx, double Axy) {
-                            const double QAxx = Qh * Axx;
-                            const T hxx = static_cast<T>(SPH_FMA(cxx, A, SPH_FMA(bx2, Ax, QAxx)));
-                            const T hyy = static_cast<T>(SPH_FMA(cyy, A, SPH_FMA(by2, Ay, -QAxx)));
-                            const T hxy = static_cast<T>(SPH_FMA(cxy, A, SPH_FMA(bx, Ay, SPH_FMA(by, Ax, Qh * Axy))));
-                            const T hxz = static_cast<T>(SPH_FMA(cxz, A, ezh * Ax));
-                            const T hyz = static_cast<T>(SPH_FMA(cyz, A, ezh * Ay));
-                            const T hzz = static_cast<T>(czz * A);
-                            // rows = xx xy xz yx yy yz zx zy zz (both triangles stored, exactly equal)
-                            H[k] = hxx;
-                            H[L + k] = hxy;
-                            H[2 * L + k] = hxz;
-                            H[3 * L + k] = hxy;
-                            H[4 * L + k] = hyy;
-                            H[5 * L + k] = hyz;
-                            H[6 * L + k] = hxz;
-                            H[7 * L + k] = hyz;
-                            H[8 * L + k] = hzz;
-                        };
-                        put(kc, Ac, mc1, -ms1, mmc2, -mms2);
-                        if (m > 0) put(ks, As, ms1, mc1, mms2, mmc2);
+                        tq_lds2(sHT + t * 32, H2, Hxz);
+                        Hzz = tq_lds16(sHT + t * 32);
                     }
+                    const double dmm = dm * (dm - 1.0);
+#pragma unroll
+                    for (int j = 0; j < 2; ++j) {
+                        const int pl = 2 * pp + j;    // point inside the tile
+                        const int pb = ti * P + pl;   // ... inside the batch
+                        double x, y, z, ri;
+                        tq_lds2(sPT + pb * 32, x, y);
+                        tq_lds2(sPT + pb * 32 + 16, z, ri);
+                        const uint32_t aQ = sQ + (pb * TP + t) * 8;
+                        const uint32_t aC = sCS + (pb * CP + m + 2) * 16;
+                        const double Q = tq_lds(aQ);
+                        double c0, As;
+                        tq_lds2(aC, c0, As);
+                        const double Ac = (m == 0) ? SPH_INV_SQRT2 : c0;
+                        const uint32_t aS = sS + pl * row_b + kc_b;
+                        tq_sts(aS - m2_b, static_cast<T>(Q * As));
+                        tq_sts(aS, static_cast<T>(Q * Ac));
+                        if constexpr (DERIV >= 1) {
+                            const uint32_t aQ1 = aQ - l8;   // Qt_{l-1}^m; Qt_{l-1}^{m+1} behind it
+                            const double q1 = G1 * tq_lds8(aQ1);   // F_l^m Q_{l-1}^{m+1}
+                            const double qz = Gz * tq_lds(aQ1);    // F_l^m (l+m) Q_{l-1}^m
+                            double c1, s1;
+                            tq_lds2(aC - 16, c1, s1);
+                            // Eq. 10: cos: A_x = m c_{m-1}, A_y = -m s_{m-1}; sin: A_x = m s_{m-1}, A_y = m c_{m-1}
+                            const double mc1 = dm * c1, ms1 = dm * s1;
+                            const double lQ = dl * Q;
+                            const double E1 = NORM ? q1 - lQ : q1;
+                            const double EZ = NORM ? SPH_FMA(-lQ, z, qz) : qz;
+                            const double sg = NORM ? ri : 1.0;
+                            const double E1g = E1 * sg;
+                            const double ax = x * E1g, ay = y * E1g, az = EZ * sg, Qg = Q * sg;
+                            const double Qc = Qg * mc1, Qs_ = Qg * ms1;
+                            const uint32_t aG = sG + pl * 3 * row_b + kc_b;
+                            const uint32_t aGs = aG - m2_b;
+                            tq_sts(aGs, static_cast<T>(SPH_FMA(ax, As, Qs_)));
+                            tq_sts(aGs + row_b, static_cast<T>(SPH_FMA(ay, As, Qc)));
+                            tq_sts(aGs + 2 * row_b, static_cast<T>(az * As));
+                            tq_sts(aG, static_cast<T>(SPH_FMA(ax, Ac, Qc)));
+                            tq_sts(aG + row_b, static_cast<T>(SPH_FMA(ay, Ac, -Qs_)));
+                            tq_sts(aG + 2 * row_b, static_cast<T>(az * Ac));
+                            if constexpr (DERIV >= 2) {
+                                const uint32_t aQ2 = aQ1 - l8 + 8;   // Qt_{l-2}^m, then m+1, m+2
+                                const double q2 = H2 * tq_lds16(aQ2);    // F_l^m Q_{l-2}^{m+2}
+                                const double qxz = Hxz * tq_lds8(aQ2);   // F_l^m (l+m) Q_{l-2}^{m+1}
+                                const double qzz = Hzz * tq_lds(aQ2);    // F_l^m (l+m)(l+m-1) Q_{l-2}^m
+                                double c2, s2;
+                                tq_lds2(aC - 32, c2, s2);
+                                // Eq. 10 twice: cos: A_xx = m(m-1) c_{m-2}, A_xy = -m(m-1) s_{m-2}; sin: s_{m-2}, c_{m-2}
+                                const double mmc2 = dmm * c2, mms2 = dmm * s2;
+                                double F2 = q2, FXZ = qxz, FZZ = qzz;
+                                if (NORM) {
+                                    const double w = (dl + 2.0) * lQ;
+                                    F2 = SPH_FMA(-2.0 * dl, q1, q2 + w);
+                                    FXZ = SPH_FMA(z, SPH_FMA(-dl, q1, w), SPH_FMA(-dl, qz, qxz));
+                                    FZZ = SPH_FMA(z, SPH_FMA(w, z, -2.0 * dl * qz), qzz) - lQ;
+                                }
+                                const double sh = NORM ? ri * ri : 1.0;
+                                const double E1h = E1 * sh, F2h = F2 * sh, Qh = Q * sh;
+                                const double cxx = SPH_FMA(x * x, F2h, E1h), cyy = SPH_FMA(y * y, F2h, E1h), cxy = (x * y) * F2h;
+                                const double bx = x * E1h, by = y * E1h, bx2 = bx + bx, by2 = by + by;
+                                const double FXZh = FXZ * sh;
+                                const double cxz = x * FXZh, cyz = y * FXZh, ezh = EZ * sh, czz = FZZ * sh;
+                                const uint32_t aH = sH + pl * 9 * row_b + kc_b;
+                                auto put = [&](uint32_t a, double A, double Ax, double Ay, double Axx, double Axy) {
+                                    const double QAxx = Qh * Axx;
+                                    const T hxx = static_cast<T>(SPH_FMA(cxx, A, SPH_FMA(bx2, Ax, QAxx)));
+                                    const T hyy = static_cast<T>(SPH_FMA(cyy, A, SPH_FMA(by2, Ay, -QAxx)));
+                                    const T hxy = static_cast<T>(SPH_FMA(cxy, A, SPH_FMA(bx, Ay, SPH_FMA(by, Ax, Qh * Axy))));
+                                    const T hxz = static_cast<T>(SPH_FMA(cxz, A, ezh * Ax));
+                                    const T hyz = static_cast<T>(SPH_FMA(cyz, A, ezh * Ay));
+                                    const T hzz = static_cast<T>(czz * A);
+                                    // rows = xx xy xz yx yy yz zx zy zz (both triangles stored, exactly equal)
+                                    tq_sts(a, hxx);
+                                    tq_sts(a += row_b, hxy);
+                                    tq_sts(a += row_b, hxz);
+                                    tq_sts(a += row_b, hxy);
+                                    tq_sts(a += row_b, hyy);
+                                    tq_sts(a += row_b, hyz);
+                                    tq_sts(a += row_b, hxz);
+                                    tq_sts(a += row_b, hyz);
+                                    tq_sts(a += row_b, hzz);
+                                };
+                                put(aH - m2_b, As, ms1, mc1, mms2, mmc2);
+                                put(aH, Ac, mc1, -ms1, mmc2, -mms2);
+                            }
+                        }
+                    }
+                }
+                ch += d_ch;
+                pp += d_pl;
+                if (ch >= NCH) {
+                    ch -= NCH;
+                    ++pp;
                 }
             }
-            // the other image's stores (issued one tile ago) must have read it before anyone writes
-            // there again; this tile's image must be visible to the async proxy
+            // this tile's image must be visible to the async proxy; with two images, the other one's
+            // stores (issued one tile ago) must have read it before anyone writes there again
             fence_proxy_async_smem();
-            if (threadIdx.x == 0) bulk_wait_read<0>();
+            if (prm.n_images == 2 && threadIdx.x == 0) bulk_wait_read<0>();
             __syncthreads();
-            const bool full = n - p0 >= P;
-            if (full && ((s_bytes & 15u) == 0)) {
+            T* S0 = reinterpret_cast<T*>(iS);
+            T* G0 = reinterpret_cast<T*>(iG);
+            T* H0 = reinterpret_cast<T*>(iH);
+            if (n - p0 >= P) {
+                // a run = the tile's rows of one array: contiguous in global memory and in its region; the
+                // 16-byte-aligned body by TMA, the few elements before and behind it by plain stores
                 if (threadIdx.x == 0) {
-                    bulk_store_hint(sph + p0 * L, S0, s_bytes, policy);
-                    if (DERIV >= 1) bulk_store_hint(dsph + p0 * 3 * L, G0, 3u * s_bytes, policy);
-                    if (DERIV >= 2) bulk_store_hint(ddsph + p0 * 9 * L, H0, 9u * s_bytes, policy);
+                    auto run = [&](T* g, const T* src, uint32_t d, uint32_t bytes) {
+                        uint32_t head = (16u - d) & 15u;
+                        if (head > bytes) head = bytes;
+                        const uint32_t body = (bytes - head) & ~15u;
+                        for (uint32_t i = 0; i < head / ES; ++i) st_cs(g + i, src[i]);
+                        if (body) bulk_store_hint(g + head / ES, src + head / ES, body, policy);
+                        for (uint32_t i = (head + body) / ES; i < bytes / ES; ++i) st_cs(g + i, src[i]);
+                    };
+                    run(sph + p0 * L, S0, dS, s_bytes);
+                    if (DERIV >= 1) run(dsph + p0 * 3 * L, G0, dG, 3u * s_bytes);
+                    if (DERIV >= 2) run(ddsph + p0 * 9 * L, H0, dH, 9u * s_bytes);
                     bulk_commit();
                 }
-            } else {   // ragged last tile (or a row length that is not a 16-byte multiple per tile): plain stores
-                const int np = (int)(full ? P : n - p0);
+            } else {   // ragged last tile: plain stores
+                const int np = (int)(n - p0);
                 for (int i = threadIdx.x; i < np * L; i += blockDim.x) st_cs(sph + p0 * L + i, S0[i]);
                 if (DERIV >= 1)
                     for (int i = threadIdx.x; i < np * 3 * L; i += blockDim.x) st_cs(dsph + p0 * 3 * L + i, G0[i]);
@@ -325,37 +439,36 @@ template <typename T, typename R> static TqKernel tq_pick(int deriv, int norm) {
     return norm ? sph_tq_kernel<T, R, 2, true> : sph_tq_kernel<T, R, 2, false>;
 }
 
-// returns 0 and fills *out if a launch shape fits: the smallest tile whose arrays are 16-byte
-// multiples (4 points f32, 2 f64; 1 when the row itself is one), doubled while the image stays
-// under ~20 KB; the largest batch (32, 16, 8 points) that leaves room for two CTAs per SM, or for
-// one if that is all that fits; 1 otherwise (rows too long for two full-row images)
+// Launch shape: points per phase-A batch B (32, 16), points per tile P (even), warps per CTA W,
+// images per CTA.
+// Returns 0 and fills *out, or 1 when the shape does not fit (rows too long for two full-row
+// images: the warp-per-point kernels take those).
 static inline int tq_plan(int sm_count, int smem_optin, int64_t n, int l_max, int normalized, int dtype, void* sph,
                           void* dsph, void* ddsph, const void* xyz, const SphTables* d_tab, const unsigned short* d_lm,
                           TqLaunch* out) {
     const int deriv = ddsph ? 2 : (dsph ? 1 : 0);
     const int esize = dtype == 0 ? 4 : 8;
-    const int rows = deriv == 0 ? 1 : (deriv == 1 ? 4 : 13);
     const int64_t L = (int64_t)(l_max + 1) * (l_max + 1);
-    const int64_t row_bytes = L * esize;
-    int pts = 16 / esize;
-    if (row_bytes % 16 == 0) pts = 1;
-    else if ((2 * row_bytes) % 16 == 0) pts = 2;
-    while (pts < 32 && 2 * pts * rows * row_bytes <= 20 * 1024) pts *= 2;
-    if (g_opt.tq_points > 0) pts = g_opt.tq_points;
-    if (pts > 32 || 32 % pts != 0) return 1;
+    const int T = (l_max + 1) * (l_max + 2) / 2;
     const int budget = smem_optin - 1024;
-    int batch = 0;
-    for (int want_ctas = 2; want_ctas >= 1 && !batch; --want_ctas)
-        for (int b = 32; b >= 8 && b >= pts; b >>= 1) {
-            TqSmem lay(l_max, deriv, esize, b, pts);
-            if ((int64_t)lay.total * want_ctas + 1024 * want_ctas <= (want_ctas == 1 ? budget : 227 * 1024)) {
-                if ((int64_t)lay.total > budget) continue;
-                batch = b;
-                break;
-            }
-        }
-    if (!batch) return 1;
-    TqSmem lay(l_max, deriv, esize, batch, pts);
+    // Measured on B200 over (B, P, W, N) (tq_table.h): small tiles win almost everywhere (more CTAs
+    // per SM, shorter barrier intervals); a lane does two points at a time, so P = 2, or 4 while that
+    // keeps the image small; 32-point batches unless they push a CTA over ~110 KB; one image
+    const int rows = deriv == 0 ? 1 : (deriv == 1 ? 4 : 13);
+    // (the measured table first; these rules serve the cells it leaves to other kernels when tq is forced)
+    const unsigned char* shape = TQ_SHAPE[dtype != 0][deriv][l_max];
+    const bool tab = shape[0] != 0;
+    int bP = g_opt.tq_points > 0 ? g_opt.tq_points : (tab ? shape[1] : ((int64_t)4 * rows * L * esize <= 24 * 1024 ? 4 : 2));
+    int bB = g_opt.tq_batch > 0 ? g_opt.tq_batch : (tab ? shape[0] : 32);
+    int bN = g_opt.tq_images > 0 ? g_opt.tq_images : (tab ? shape[3] : 1);
+    if (g_opt.tq_batch <= 0 && !tab && TqSmem(l_max, deriv, esize, 32, bP, bN).total > 110 * 1024) bB = 16;
+    if (bP > bB || (bP & 1) || bB % bP != 0 || (bN != 1 && bN != 2)) return 1;
+    if ((int64_t)TqSmem(l_max, deriv, esize, bB, bP, bN).total > budget) return 1;
+    const int units = (bP / 2) * ((T + 31) / 32);
+    int bW = g_opt.tq_warps > 0 ? g_opt.tq_warps : (tab ? shape[2] : (units >= 8 ? 8 : 6));
+    if (bW > TQ_MAX_WARPS) bW = TQ_MAX_WARPS;
+    TqSmem lay(l_max, deriv, esize, bB, bP, bN);
+    out->prm.n_images = bN;
     out->kern = dtype == 0 ? tq_pick<float, double>(deriv, normalized) : tq_pick<double, dd>(deriv, normalized);
     out->func = (const void*)out->kern;
     out->prm.xyz = xyz;
@@ -366,17 +479,17 @@ static inline int tq_plan(int sm_count, int smem_optin, int64_t n, int l_max, in
     out->prm.lm = d_lm;
     out->prm.n = n;
     out->prm.l_max = l_max;
-    out->prm.batch = batch;
-    out->prm.pts_tile = pts;
-    const int64_t n_batches = (n + batch - 1) / batch;
-    // a few batches per CTA amortise the pad initialisation and the launch; keep >= ~8 CTAs per SM
+    out->prm.batch = bB;
+    out->prm.pts_tile = bP;
+    const int64_t n_batches = (n + bB - 1) / bB;
+    // a few batches per CTA amortise the table copy; keep >= ~16 CTAs per SM for the block scheduler
     int64_t bpc = n_batches / ((int64_t)sm_count * 16);
     if (bpc > 4) bpc = 4;
     if (bpc < 1) bpc = 1;
     out->prm.batches_per_cta = (int)bpc;
     out->grid = (n_batches + bpc - 1) / bpc;
     if (out->grid > 0x7fffffff) return 1;
-    out->threads = TQ_MAX_WARPS * 32;
+    out->threads = bW * 32;
     out->smem = lay.total;
     return 0;
 }

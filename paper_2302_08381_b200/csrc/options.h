@@ -28,7 +28,10 @@ struct SphOptions {
     int tpb_tiles = 0;       // tiles per CTA of the tpb kernels (0: from the tile size)
     int tpb_split = 0;       // warps per tile of the tpb kernels (0: the dispatch's own rule)
     int pdl = 1;             // programmatic dependent launch for small grids
-    int tq_points = 0;       // points per CTA round of the tq kernel (0: from the row length)
+    int tq_points = 0;       // points per tile of the tq kernel (0: the planner's choice)
+    int tq_warps = 0;        // warps per CTA of the tq kernel (0: the planner's choice)
+    int tq_images = 0;       // staging images per CTA of the tq kernel (0: two unless only one fits)
+    int tq_batch = 0;        // points per phase-A batch of the tq kernel (0: the planner's choice)
     int64_t host_chunk_bytes = (int64_t)256 << 20;   // _host entry points: bytes per chunk and stream
 };
 

@@ -362,8 +362,8 @@ def test_two_phase_kernel(sph, oracle, dtype, l_max, option):
                 before = sph.sphericart_cuda_launch_count()
                 s, d, h = _run_gpu(sph, xyz, l_max, normalized, deriv >= 1, deriv >= 2)
                 assert sph.sphericart_cuda_launch_count() == before + 1
-                if sph.sphericart_cuda_last_kernel() != "tq":       # rows too long for two full-row images
-                    assert deriv == 2 and l_max > 16
+                if sph.sphericart_cuda_last_kernel() != "tq":       # rows too long for one two-point image
+                    assert deriv == 2 and l_max >= 24
                     continue
                 _compare(oracle, xyz, l_max, normalized, dtype, s, d, h,
                          f"tq {dtype} l_max={l_max} n={n} norm={normalized} deriv={deriv}")
