@@ -342,7 +342,7 @@ def test_lanes_per_point_kernel(sph, oracle, dtype, lp, option):
         before = sph.sphericart_cuda_launch_count()
         s, d, _ = _run_gpu(sph, xyz, l_max, normalized, grads, False)
         assert sph.sphericart_cuda_launch_count() == before + 1
-        assert sph.sphericart_cuda_last_kernel() in ("tpg", "w")     # (tpg declines the longest rows)
+        assert sph.sphericart_cuda_last_kernel() in ("tpg", "w", "wc")     # (tpg declines the longest rows)
         _compare(oracle, xyz, l_max, normalized, dtype, s, d, None, f"tpg {dtype} lp={lp} l_max={l_max} n={n}")
 
 
