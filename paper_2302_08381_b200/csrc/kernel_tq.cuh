@@ -9,10 +9,11 @@
 // are separate phases with their own mapping, and the image is sized by the store engine's needs
 // (a contiguous byte range per output array, 16-byte aligned), not by the warp width:
 //
-//   phase A  lane = POINT.  The batch's points (32, 16 for the longest rows) run Eq. 9 and
-//            the folded Eq. 7 (tables.h) -- double for f32 I/O, double-double for f64 I/O --
-//            with warp-uniform coefficient loads from the constant bank; the columns m of the
-//            triangle are dealt to the CTA's warps in snake order (balanced lengths).  Qt_l^m, (c_m, s_m)
+//   phase A  lane = POINT (32-point batches; 2 / 4 lanes per point for batches of 16 / 8, which the
+//            long rows need to fit shared memory).  The batch's points run Eq. 9 and the
+//            folded Eq. 7 (tables.h) -- double for f32 I/O, double-double for f64 I/O -- with
+//            coefficient loads from the constant bank; the columns m of the triangle are dealt to
+//            the CTA's warps (and lane classes) in snake order (balanced lengths).  Qt_l^m, (c_m, s_m)
 //            and (u, 1/r) of every point go to a scratch in shared memory as f64.
 //   phase B  lane = one (l, m >= 0) PAIR of one point of the current tile (tile = the fewest points
 //            whose rows are a 16-byte multiple: 4 f32 / 2 f64, or more while the image stays
@@ -57,7 +58,7 @@ struct TqParams {
     const unsigned short* lm;    // [(l_max+1)(l_max+2)/2]: l | m << 8 of triangle index t
     int64_t n;
     int l_max;
-    int batch;                   // points per phase-A batch: 32, 16 or 8
+    int batch;                   // points per phase-A batch: 32, 16 or 8 (1, 2 or 4 lanes per point)
     int pts_tile;                // points per image; divides batch
     int batches_per_cta;         // consecutive batches one CTA works through
     int n_images;                // 2: a tile drains while the next is assembled; 1: the longest rows
@@ -180,6 +181,137 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
     const int PP = P >> 1;                             // pairs of points per tile (P is even)
     const uint32_t row_b = (uint32_t)L * ES;          // bytes of one row of one point
     const uint32_t s_bytes = (uint32_t)P * row_b;     // bytes of the tile's sph image
+    // Phase B for ONE (l, m >= 0) pair (triangle index t) and TWO points: the points pbb, pbb + 1 of the
+    // batch, staged as points plb, plb + 1 of the image whose regions start at sS / sG / sH.
+    auto assemble = [&](int t, int plb, int pbb, uint32_t sS, uint32_t sG, uint32_t sH) {
+            // ---- per (l, m): shared by the two points ----
+            const unsigned lmv = tq_lds_u16(sLM + t * 2);
+            const int l = (int)(lmv & 0xffu), m = (int)(lmv >> 8);
+            const double dl = (double)l, dm = (double)m;
+            // the (l, -m) outputs are stored FIRST and unconditionally: for m = 0 they land on the
+            // (l, 0) slot and the cos-branch store that follows overwrites them (no branch)
+            const uint32_t kc_b = (uint32_t)(l * (l + 1) + m) * ES, m2_b = (uint32_t)(2 * m) * ES;
+            const uint32_t l8 = (uint32_t)l * 8;
+            double G1 = 0.0, Gz = 0.0, H2 = 0.0, Hxz = 0.0, Hzz = 0.0;
+            if constexpr (DERIV >= 1) tq_lds2(sGT + t * 16, G1, Gz);
+            if constexpr (DERIV >= 2) {
+                tq_lds2(sHT + t * 32, H2, Hxz);
+                Hzz = tq_lds16(sHT + t * 32);
+            }
+            const double dmm = dm * (dm - 1.0);
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                const int pl = plb + j;   // point inside the image
+                const int pb = pbb + j;   // ... inside the batch
+                double x, y, z, ri;
+                tq_lds2(sPT + pb * 32, x, y);
+                tq_lds2(sPT + pb * 32 + 16, z, ri);
+                const uint32_t aQ = sQ + (pb * TP + t) * 8;
+                const uint32_t aC = sCS + (pb * CP + m + 2) * 16;
+                const double Q = tq_lds(aQ);
+                double c0, As;
+                tq_lds2(aC, c0, As);
+                const double Ac = (m == 0) ? SPH_INV_SQRT2 : c0;
+                const uint32_t aS = sS + pl * row_b + kc_b;
+                tq_sts(aS - m2_b, static_cast<T>(Q * As));
+                tq_sts(aS, static_cast<T>(Q * Ac));
+                if constexpr (DERIV >= 1) {
+                    const uint32_t aQ1 = aQ - l8;   // Qt_{l-1}^m; Qt_{l-1}^{m+1} behind it
+                    const double q1 = G1 * tq_lds8(aQ1);   // F_l^m Q_{l-1}^{m+1}
+                    const double qz = Gz * tq_lds(aQ1);    // F_l^m (l+m) Q_{l-1}^m
+                    double c1, s1;
+                    tq_lds2(aC - 16, c1, s1);
+                    // Eq. 10: cos: A_x = m c_{m-1}, A_y = -m s_{m-1}; sin: A_x = m s_{m-1}, A_y = m c_{m-1}
+                    const double mc1 = dm * c1, ms1 = dm * s1;
+                    const double lQ = dl * Q;
+                    const double E1 = NORM ? q1 - lQ : q1;
+                    const double EZ = NORM ? SPH_FMA(-lQ, z, qz) : qz;
+                    const double sg = NORM ? ri : 1.0;
+                    const double E1g = E1 * sg;
+                    const double ax = x * E1g, ay = y * E1g, az = EZ * sg, Qg = Q * sg;
+                    const double Qc = Qg * mc1, Qs_ = Qg * ms1;
+                    const uint32_t aG = sG + pl * 3 * row_b + kc_b;
+                    const uint32_t aGs = aG - m2_b;
+                    tq_sts(aGs, static_cast<T>(SPH_FMA(ax, As, Qs_)));
+                    tq_sts(aGs + row_b, static_cast<T>(SPH_FMA(ay, As, Qc)));
+                    tq_sts(aGs + 2 * row_b, static_cast<T>(az * As));
+                    tq_sts(aG, static_cast<T>(SPH_FMA(ax, Ac, Qc)));
+                    tq_sts(aG + row_b, static_cast<T>(SPH_FMA(ay, Ac, -Qs_)));
+                    tq_sts(aG + 2 * row_b, static_cast<T>(az * Ac));
+                    if constexpr (DERIV >= 2) {
+                        const uint32_t aQ2 = aQ1 - l8 + 8;   // Qt_{l-2}^m, then m+1, m+2
+                        const double q2 = H2 * tq_lds16(aQ2);    // F_l^m Q_{l-2}^{m+2}
+                        const double qxz = Hxz * tq_lds8(aQ2);   // F_l^m (l+m) Q_{l-2}^{m+1}
+                        const double qzz = Hzz * tq_lds(aQ2);    // F_l^m (l+m)(l+m-1) Q_{l-2}^m
+                        double c2, s2;
+                        tq_lds2(aC - 32, c2, s2);
+                        // Eq. 10 twice: cos: A_xx = m(m-1) c_{m-2}, A_xy = -m(m-1) s_{m-2}; sin: s_{m-2}, c_{m-2}
+                        const double mmc2 = dmm * c2, mms2 = dmm * s2;
+                        double F2 = q2, FXZ = qxz, FZZ = qzz;
+                        if (NORM) {
+                            const double w = (dl + 2.0) * lQ;
+                            F2 = SPH_FMA(-2.0 * dl, q1, q2 + w);
+                            FXZ = SPH_FMA(z, SPH_FMA(-dl, q1, w), SPH_FMA(-dl, qz, qxz));
+                            FZZ = SPH_FMA(z, SPH_FMA(w, z, -2.0 * dl * qz), qzz) - lQ;
+                        }
+                        const double sh = NORM ? ri * ri : 1.0;
+                        const double E1h = E1 * sh, F2h = F2 * sh, Qh = Q * sh;
+                        const double cxx = SPH_FMA(x * x, F2h, E1h), cyy = SPH_FMA(y * y, F2h, E1h), cxy = (x * y) * F2h;
+                        const double bx = x * E1h, by = y * E1h, bx2 = bx + bx, by2 = by + by;
+                        const double FXZh = FXZ * sh;
+                        const double cxz = x * FXZh, cyz = y * FXZh, ezh = EZ * sh, czz = FZZ * sh;
+                        const uint32_t aH = sH + pl * 9 * row_b + kc_b;
+                        auto put = [&](uint32_t a, double A, double Ax, double Ay, double Axx, double Axy) {
+                            const double QAxx = Qh * Axx;
+                            const T hxx = static_cast<T>(SPH_FMA(cxx, A, SPH_FMA(bx2, Ax, QAxx)));
+                            const T hyy = static_cast<T>(SPH_FMA(cyy, A, SPH_FMA(by2, Ay, -QAxx)));
+                            const T hxy = static_cast<T>(SPH_FMA(cxy, A, SPH_FMA(bx, Ay, SPH_FMA(by, Ax, Qh * Axy))));
+                            const T hxz = static_cast<T>(SPH_FMA(cxz, A, ezh * Ax));
+                            const T hyz = static_cast<T>(SPH_FMA(cyz, A, ezh * Ay));
+                            const T hzz = static_cast<T>(czz * A);
+                            // rows = xx xy xz yx yy yz zx zy zz (both triangles stored, exactly equal)
+                            tq_sts(a, hxx);
+                            tq_sts(a += row_b, hxy);
+                            tq_sts(a += row_b, hxz);
+                            tq_sts(a += row_b, hxy);
+                            tq_sts(a += row_b, hyy);
+                            tq_sts(a += row_b, hyz);
+                            tq_sts(a += row_b, hxz);
+                            tq_sts(a += row_b, hyz);
+                            tq_sts(a += row_b, hzz);
+                        };
+                        put(aH - m2_b, As, ms1, mc1, mms2, mmc2);
+                        put(aH, Ac, mc1, -ms1, mmc2, -mms2);
+                    }
+                }
+            }
+    };
+    // The image's runs (one per output array: np points' rows, contiguous in global memory) leave: the
+    // 16-byte-aligned body by TMA, the few elements before and behind it by plain stores.  One thread.
+    auto emit_runs = [&](int64_t p0, int np, const T* S0, const T* G0, const T* H0, uint32_t dS, uint32_t dG, uint32_t dH) {
+        auto run = [&](T* g, const T* src, uint32_t d, uint32_t bytes) {
+            uint32_t head = (16u - d) & 15u;
+            if (head > bytes) head = bytes;
+            const uint32_t body = (bytes - head) & ~15u;
+            for (uint32_t i = 0; i < head / ES; ++i) st_cs(g + i, src[i]);
+            if (body) bulk_store_hint(g + head / ES, src + head / ES, body, policy);
+            for (uint32_t i = (head + body) / ES; i < bytes / ES; ++i) st_cs(g + i, src[i]);
+        };
+        const uint32_t sb = (uint32_t)np * row_b;
+        run(sph + p0 * L, S0, dS, sb);
+        if (DERIV >= 1) run(dsph + p0 * 3 * L, G0, dG, 3u * sb);
+        if (DERIV >= 2) run(ddsph + p0 * 9 * L, H0, dH, 9u * sb);
+        bulk_commit();
+    };
+    // ragged end of the batch: np (< the image's points) points by plain stores, threads tid of nthr
+    auto emit_plain = [&](int64_t p0, int np, const T* S0, const T* G0, const T* H0, int tid, int nthr) {
+        for (int i = tid; i < np * L; i += nthr) st_cs(sph + p0 * L + i, S0[i]);
+        if (DERIV >= 1)
+            for (int i = tid; i < np * 3 * L; i += nthr) st_cs(dsph + p0 * 3 * L + i, G0[i]);
+        if (DERIV >= 2)
+            for (int i = tid; i < np * 9 * L; i += nthr) st_cs(ddsph + p0 * 9 * L + i, H0[i]);
+    };
+
     int tile_no = 0;   // tiles this CTA has issued: parity picks the image
     for (int bi = 0; bi < prm.batches_per_cta; ++bi) {
         const int64_t b0 = ((int64_t)blockIdx.x * prm.batches_per_cta + bi) * B;
@@ -187,8 +319,11 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
 
         // ---- phase A: lane = point --------------------------------------------------------------
         __syncthreads();   // the previous batch's phase B has finished reading the scratch
-        if (lane < B) {
-            const int64_t p = b0 + lane;
+        {
+            // B = 32: lane = point.  B = 16 / 8: 2 / 4 lanes per point, each its own share of the
+            // columns (class `cls`), so that every lane of the warp works whatever the batch size
+            const int pt_l = lane & (B - 1), cls = lane / B, NC = 32 / B;
+            const int64_t p = b0 + pt_l;
             double x = 0.0, y = 0.0, z = 1.0;   // lanes past the end compute a harmless point
             if (p < n) {
                 x = static_cast<double>(__ldg(xyz + 3 * p + 0));
@@ -206,11 +341,11 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
                 Z = RT::make(z, 0.0);
                 r2 = RT::r2_of(X, Y, Z);
             }
-            if (warp == W - 1) {   // Eq. 9 and the point itself: the warp with the shortest columns
-                tq_sts2(sPT + lane * 32, to_double(X), to_double(Y));
-                tq_sts2(sPT + lane * 32 + 16, to_double(Z), rinv);
+            if (warp == W - 1 && cls == NC - 1) {   // Eq. 9 and the point itself: the lanes with the shortest columns
+                tq_sts2(sPT + pt_l * 32, to_double(X), to_double(Y));
+                tq_sts2(sPT + pt_l * 32 + 16, to_double(Z), rinv);
                 R c = RT::make(1.0, 0.0), s = RT::make(0.0, 0.0);
-                uint32_t a = sCS + (lane * CP + 2) * 16;
+                uint32_t a = sCS + (pt_l * CP + 2) * 16;
                 for (int m = 0; m <= l_max; ++m, a += 16) {
                     tq_sts2(a, to_double(c), to_double(s));
                     const R cn = X * c - Y * s;
@@ -219,10 +354,13 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
                     s = sn;
                 }
             }
-            // columns of the folded Eq. 7, dealt to the warps in snake order: m = w, 2W-1-w, 2W+w, ...
-            const uint32_t q_out = sQ + lane * TP * 8;
-            for (int i = 0; i * W <= l_max; ++i) {
-                const int m = (i & 1) ? (i + 1) * W - 1 - warp : i * W + warp;
+            // columns of the folded Eq. 7, dealt to the W * NC column classes in snake order
+            // (class v takes m = v, 2V-1-v, 2V+v, ...: balanced lengths; the classes of one warp sit
+            // on neighbouring columns, so their loops run nearly in step)
+            const uint32_t q_out = sQ + pt_l * TP * 8;
+            const int V = W * NC, v = warp * NC + cls;
+            for (int i = 0; i * V <= l_max; ++i) {
+                const int m = (i & 1) ? (i + 1) * V - 1 - v : i * V + v;
                 if (m > l_max) continue;
                 int t = SPH_TRI(m, m);
                 R q = RT::make(TB.D_hi[m], TB.D_lo[m]), qp = RT::make(0.0, 0.0);
@@ -268,109 +406,7 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
             int pp = w_pl0, ch = w_ch0;   // pp: PAIR of points of the tile (a lane does the same (l, m) for both)
             while (pp < PP) {
                 const int t = ch * 32 + lane;
-                if (t < TT) {
-                    // ---- per (l, m): shared by the two points ----
-                    const unsigned lmv = tq_lds_u16(sLM + t * 2);
-                    const int l = (int)(lmv & 0xffu), m = (int)(lmv >> 8);
-                    const double dl = (double)l, dm = (double)m;
-                    // the (l, -m) outputs are stored FIRST and unconditionally: for m = 0 they land on the
-                    // (l, 0) slot and the cos-branch store that follows overwrites them (no branch)
-                    const uint32_t kc_b = (uint32_t)(l * (l + 1) + m) * ES, m2_b = (uint32_t)(2 * m) * ES;
-                    const uint32_t l8 = (uint32_t)l * 8;
-                    double G1 = 0.0, Gz = 0.0, H2 = 0.0, Hxz = 0.0, Hzz = 0.0;
-                    if constexpr (DERIV >= 1) tq_lds2(sGT + t * 16, G1, Gz);
-                    if constexpr (DERIV >= 2) {
-                        tq_lds2(sHT + t * 32, H2, Hxz);
-                        Hzz = tq_lds16(sHT + t * 32);
-                    }
-                    const double dmm = dm * (dm - 1.0);
-#pragma unroll
-                    for (int j = 0; j < 2; ++j) {
-                        const int pl = 2 * pp + j;    // point inside the tile
-                        const int pb = ti * P + pl;   // ... inside the batch
-                        double x, y, z, ri;
-                        tq_lds2(sPT + pb * 32, x, y);
-                        tq_lds2(sPT + pb * 32 + 16, z, ri);
-                        const uint32_t aQ = sQ + (pb * TP + t) * 8;
-                        const uint32_t aC = sCS + (pb * CP + m + 2) * 16;
-                        const double Q = tq_lds(aQ);
-                        double c0, As;
-                        tq_lds2(aC, c0, As);
-                        const double Ac = (m == 0) ? SPH_INV_SQRT2 : c0;
-                        const uint32_t aS = sS + pl * row_b + kc_b;
-                        tq_sts(aS - m2_b, static_cast<T>(Q * As));
-                        tq_sts(aS, static_cast<T>(Q * Ac));
-                        if constexpr (DERIV >= 1) {
-                            const uint32_t aQ1 = aQ - l8;   // Qt_{l-1}^m; Qt_{l-1}^{m+1} behind it
-                            const double q1 = G1 * tq_lds8(aQ1);   // F_l^m Q_{l-1}^{m+1}
-                            const double qz = Gz * tq_lds(aQ1);    // F_l^m (l+m) Q_{l-1}^m
-                            double c1, s1;
-                            tq_lds2(aC - 16, c1, s1);
-                            // Eq. 10: cos: A_x = m c_{m-1}, A_y = -m s_{m-1}; sin: A_x = m s_{m-1}, A_y = m c_{m-1}
-                            const double mc1 = dm * c1, ms1 = dm * s1;
-                            const double lQ = dl * Q;
-                            const double E1 = NORM ? q1 - lQ : q1;
-                            const double EZ = NORM ? SPH_FMA(-lQ, z, qz) : qz;
-                            const double sg = NORM ? ri : 1.0;
-                            const double E1g = E1 * sg;
-                            const double ax = x * E1g, ay = y * E1g, az = EZ * sg, Qg = Q * sg;
-                            const double Qc = Qg * mc1, Qs_ = Qg * ms1;
-                            const uint32_t aG = sG + pl * 3 * row_b + kc_b;
-                            const uint32_t aGs = aG - m2_b;
-                            tq_sts(aGs, static_cast<T>(SPH_FMA(ax, As, Qs_)));
-                            tq_sts(aGs + row_b, static_cast<T>(SPH_FMA(ay, As, Qc)));
-                            tq_sts(aGs + 2 * row_b, static_cast<T>(az * As));
-                            tq_sts(aG, static_cast<T>(SPH_FMA(ax, Ac, Qc)));
-                            tq_sts(aG + row_b, static_cast<T>(SPH_FMA(ay, Ac, -Qs_)));
-                            tq_sts(aG + 2 * row_b, static_cast<T>(az * Ac));
-                            if constexpr (DERIV >= 2) {
-                                const uint32_t aQ2 = aQ1 - l8 + 8;   // Qt_{l-2}^m, then m+1, m+2
-                                const double q2 = H2 * tq_lds16(aQ2);    // F_l^m Q_{l-2}^{m+2}
-                                const double qxz = Hxz * tq_lds8(aQ2);   // F_l^m (l+m) Q_{l-2}^{m+1}
-                                const double qzz = Hzz * tq_lds(aQ2);    // F_l^m (l+m)(l+m-1) Q_{l-2}^m
-                                double c2, s2;
-                                tq_lds2(aC - 32, c2, s2);
-                                // Eq. 10 twice: cos: A_xx = m(m-1) c_{m-2}, A_xy = -m(m-1) s_{m-2}; sin: s_{m-2}, c_{m-2}
-                                const double mmc2 = dmm * c2, mms2 = dmm * s2;
-                                double F2 = q2, FXZ = qxz, FZZ = qzz;
-                                if (NORM) {
-                                    const double w = (dl + 2.0) * lQ;
-                                    F2 = SPH_FMA(-2.0 * dl, q1, q2 + w);
-                                    FXZ = SPH_FMA(z, SPH_FMA(-dl, q1, w), SPH_FMA(-dl, qz, qxz));
-                                    FZZ = SPH_FMA(z, SPH_FMA(w, z, -2.0 * dl * qz), qzz) - lQ;
-                                }
-                                const double sh = NORM ? ri * ri : 1.0;
-                                const double E1h = E1 * sh, F2h = F2 * sh, Qh = Q * sh;
-                                const double cxx = SPH_FMA(x * x, F2h, E1h), cyy = SPH_FMA(y * y, F2h, E1h), cxy = (x * y) * F2h;
-                                const double bx = x * E1h, by = y * E1h, bx2 = bx + bx, by2 = by + by;
-                                const double FXZh = FXZ * sh;
-                                const double cxz = x * FXZh, cyz = y * FXZh, ezh = EZ * sh, czz = FZZ * sh;
-                                const uint32_t aH = sH + pl * 9 * row_b + kc_b;
-                                auto put = [&](uint32_t a, double A, double Ax, double Ay, double Axx, double Axy) {
-                                    const double QAxx = Qh * Axx;
-                                    const T hxx = static_cast<T>(SPH_FMA(cxx, A, SPH_FMA(bx2, Ax, QAxx)));
-                                    const T hyy = static_cast<T>(SPH_FMA(cyy, A, SPH_FMA(by2, Ay, -QAxx)));
-                                    const T hxy = static_cast<T>(SPH_FMA(cxy, A, SPH_FMA(bx, Ay, SPH_FMA(by, Ax, Qh * Axy))));
-                                    const T hxz = static_cast<T>(SPH_FMA(cxz, A, ezh * Ax));
-                                    const T hyz = static_cast<T>(SPH_FMA(cyz, A, ezh * Ay));
-                                    const T hzz = static_cast<T>(czz * A);
-                                    // rows = xx xy xz yx yy yz zx zy zz (both triangles stored, exactly equal)
-                                    tq_sts(a, hxx);
-                                    tq_sts(a += row_b, hxy);
-                                    tq_sts(a += row_b, hxz);
-                                    tq_sts(a += row_b, hxy);
-                                    tq_sts(a += row_b, hyy);
-                                    tq_sts(a += row_b, hyz);
-                                    tq_sts(a += row_b, hxz);
-                                    tq_sts(a += row_b, hyz);
-                                    tq_sts(a += row_b, hzz);
-                                };
-                                put(aH - m2_b, As, ms1, mc1, mms2, mmc2);
-                                put(aH, Ac, mc1, -ms1, mmc2, -mms2);
-                            }
-                        }
-                    }
-                }
+                if (t < TT) assemble(t, 2 * pp, ti * P + 2 * pp, sS, sG, sH);
                 ch += d_ch;
                 pp += d_pl;
                 if (ch >= NCH) {
@@ -387,29 +423,9 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
             T* G0 = reinterpret_cast<T*>(iG);
             T* H0 = reinterpret_cast<T*>(iH);
             if (n - p0 >= P) {
-                // a run = the tile's rows of one array: contiguous in global memory and in its region; the
-                // 16-byte-aligned body by TMA, the few elements before and behind it by plain stores
-                if (threadIdx.x == 0) {
-                    auto run = [&](T* g, const T* src, uint32_t d, uint32_t bytes) {
-                        uint32_t head = (16u - d) & 15u;
-                        if (head > bytes) head = bytes;
-                        const uint32_t body = (bytes - head) & ~15u;
-                        for (uint32_t i = 0; i < head / ES; ++i) st_cs(g + i, src[i]);
-                        if (body) bulk_store_hint(g + head / ES, src + head / ES, body, policy);
-                        for (uint32_t i = (head + body) / ES; i < bytes / ES; ++i) st_cs(g + i, src[i]);
-                    };
-                    run(sph + p0 * L, S0, dS, s_bytes);
-                    if (DERIV >= 1) run(dsph + p0 * 3 * L, G0, dG, 3u * s_bytes);
-                    if (DERIV >= 2) run(ddsph + p0 * 9 * L, H0, dH, 9u * s_bytes);
-                    bulk_commit();
-                }
+                if (threadIdx.x == 0) emit_runs(p0, P, S0, G0, H0, dS, dG, dH);
             } else {   // ragged last tile: plain stores
-                const int np = (int)(n - p0);
-                for (int i = threadIdx.x; i < np * L; i += blockDim.x) st_cs(sph + p0 * L + i, S0[i]);
-                if (DERIV >= 1)
-                    for (int i = threadIdx.x; i < np * 3 * L; i += blockDim.x) st_cs(dsph + p0 * 3 * L + i, G0[i]);
-                if (DERIV >= 2)
-                    for (int i = threadIdx.x; i < np * 9 * L; i += blockDim.x) st_cs(ddsph + p0 * 9 * L + i, H0[i]);
+                emit_plain(p0, (int)(n - p0), S0, G0, H0, threadIdx.x, blockDim.x);
                 __syncthreads();   // the image is free again only when every thread has copied its share
             }
             ++tile_no;
@@ -455,18 +471,23 @@ static inline int tq_plan(int sm_count, int smem_optin, int64_t n, int l_max, in
     // per SM, shorter barrier intervals); a lane does two points at a time, so P = 2, or 4 while that
     // keeps the image small; 32-point batches unless they push a CTA over ~110 KB; one image
     const int rows = deriv == 0 ? 1 : (deriv == 1 ? 4 : 13);
-    // (the measured table first; these rules serve the cells it leaves to other kernels when tq is forced)
+    // (the measured table first; the rules behind it serve the cells the table leaves to other kernels
+    // when tq is forced; the tq_* options override both)
     const unsigned char* shape = TQ_SHAPE[dtype != 0][deriv][l_max];
     const bool tab = shape[0] != 0;
-    int bP = g_opt.tq_points > 0 ? g_opt.tq_points : (tab ? shape[1] : ((int64_t)4 * rows * L * esize <= 24 * 1024 ? 4 : 2));
-    int bB = g_opt.tq_batch > 0 ? g_opt.tq_batch : (tab ? shape[0] : 32);
-    int bN = g_opt.tq_images > 0 ? g_opt.tq_images : (tab ? shape[3] : 1);
-    if (g_opt.tq_batch <= 0 && !tab && TqSmem(l_max, deriv, esize, 32, bP, bN).total > 110 * 1024) bB = 16;
-    if (bP > bB || (bP & 1) || bB % bP != 0 || (bN != 1 && bN != 2)) return 1;
+    int bB = tab ? shape[0] : 32;
+    int bP = tab ? shape[1] : ((int64_t)4 * rows * L * esize <= 24 * 1024 ? 4 : 2);
+    int bW = tab ? shape[2] : 8;
+    int bN = tab ? shape[3] : 1;
+    if (g_opt.tq_batch > 0) bB = g_opt.tq_batch;
+    if (g_opt.tq_points > 0) bP = g_opt.tq_points;
+    if (g_opt.tq_warps > 0) bW = g_opt.tq_warps;
+    if (g_opt.tq_images > 0) bN = g_opt.tq_images;
+    if (bW < 1 || bW > TQ_MAX_WARPS || bN < 1 || bN > 2) return 1;
+    if (!tab && g_opt.tq_batch <= 0)
+        while (bB > 8 && TqSmem(l_max, deriv, esize, bB, bP, bN).total > 110 * 1024) bB >>= 1;
+    if ((bB != 32 && bB != 16 && bB != 8) || bP > bB || (bP & 1) || bB % bP != 0) return 1;
     if ((int64_t)TqSmem(l_max, deriv, esize, bB, bP, bN).total > budget) return 1;
-    const int units = (bP / 2) * ((T + 31) / 32);
-    int bW = g_opt.tq_warps > 0 ? g_opt.tq_warps : (tab ? shape[2] : (units >= 8 ? 8 : 6));
-    if (bW > TQ_MAX_WARPS) bW = TQ_MAX_WARPS;
     TqSmem lay(l_max, deriv, esize, bB, bP, bN);
     out->prm.n_images = bN;
     out->kern = dtype == 0 ? tq_pick<float, double>(deriv, normalized) : tq_pick<double, dd>(deriv, normalized);
