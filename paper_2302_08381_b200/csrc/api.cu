@@ -66,6 +66,7 @@ struct DeviceState {
     int smem_optin = 0;          // max dynamic shared memory per block
     SphTables* d_tables = nullptr;   // copy of the tables in global memory (warp kernel)
     unsigned short* d_lm = nullptr;  // (l | m << 8) of every triangle index (tq kernel)
+    double2* d_ab = nullptr;         // {A_hi, B_hi}[t], then {A_lo, B_lo}[t] (tq kernel)
 };
 static DeviceState g_dev[MAX_DEVICES];
 static std::mutex g_mutex;
@@ -105,6 +106,13 @@ static int device_state(DeviceState** out) {
             for (int m = 0; m <= l; ++m) lm[SPH_TRI(l, m)] = (unsigned short)(l | (m << 8));
         CUDA_TRY(cudaMalloc(&st.d_lm, sizeof(lm)));
         CUDA_TRY(cudaMemcpy(st.d_lm, lm, sizeof(lm), cudaMemcpyHostToDevice));
+        static double2 ab[2 * SPH_TRI_SIZE];
+        for (int t = 0; t < SPH_TRI_SIZE; ++t) {
+            ab[t] = make_double2(g_host_tables.A_hi[t], g_host_tables.B_hi[t]);
+            ab[SPH_TRI_SIZE + t] = make_double2(g_host_tables.A_lo[t], g_host_tables.B_lo[t]);
+        }
+        CUDA_TRY(cudaMalloc(&st.d_ab, sizeof(ab)));
+        CUDA_TRY(cudaMemcpy(st.d_ab, ab, sizeof(ab), cudaMemcpyHostToDevice));
         st.ready = true;
         st.ready_flag.store(true, std::memory_order_release);
     }
@@ -196,7 +204,7 @@ static int compute_device(const void* xyz, int64_t n, int l_max, int normalized,
         // two-phase kernel: recurrences lane = point, assembly lane = (l, m) pair, small full-row tiles
         TqLaunch lq{};
         if (tq_plan(st->sm_count, st->smem_optin, n, l_max, normalized, dtype, sph, dsph, ddsph, xyz, st->d_tables,
-                    st->d_lm, &lq) == 0) {
+                    st->d_lm, st->d_ab, &lq) == 0) {
             rc = allow_smem(lq.func, (int)lq.smem);
             if (rc) return rc;
             tq_launch(lq, stream);

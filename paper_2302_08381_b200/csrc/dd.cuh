@@ -117,6 +117,31 @@ template <> struct rec<dd> {
     SPH_HD static dd r2_of(dd x, dd y, dd z) { return x * x + y * y + z * z; }
 };
 
+// One step of the folded Eq. 7 (tables.h): a (Z q) - b w.
+// Double-double form: the three products keep their error terms unnormalised ((hi, e) with
+// |e| ~ 2^-53 |hi|: first-order terms only, the dropped ones are ~2^-106), the difference of the
+// high parts is an exact two_sum, and the result is normalised once: 23 operations instead of the
+// 32 of  a * (Z * q) - b * w  with normalised intermediates, same ~2^-100 relative accuracy.
+SPH_HD double rec_step(double a_hi, double, double b_hi, double, double Z, double q, double w) {
+    return SPH_FMA(a_hi * Z, q, -(b_hi * w));
+}
+SPH_HD dd rec_step(double a_hi, double a_lo, double b_hi, double b_lo, dd Z, dd q, dd w) {
+    const double p = SPH_MUL(Z.hi, q.hi);
+    double e = SPH_FMA(Z.hi, q.hi, -p);
+    e = SPH_FMA(Z.hi, q.lo, e);
+    e = SPH_FMA(Z.lo, q.hi, e);
+    const double th = SPH_MUL(a_hi, p);
+    double te = SPH_FMA(a_hi, p, -th);
+    te = SPH_FMA(a_hi, e, te);
+    te = SPH_FMA(a_lo, p, te);
+    const double uh = SPH_MUL(b_hi, w.hi);
+    double ue = SPH_FMA(b_hi, w.hi, -uh);
+    ue = SPH_FMA(b_hi, w.lo, ue);
+    ue = SPH_FMA(b_lo, w.hi, ue);
+    const dd s = two_sum(th, -uh);
+    return quick_two_sum(s.hi, SPH_ADD(s.lo, SPH_SUB(te, ue)));
+}
+
 SPH_HD double to_double(double a) { return a; }
 SPH_HD double to_double(dd a) { return a.hi; }
 

@@ -56,6 +56,8 @@ struct TqParams {
     void* ddsph;
     const SphTables* tab;        // global-memory copy of the tables (phase B: G1, Gz, H2, Hxz, Hzz)
     const unsigned short* lm;    // [(l_max+1)(l_max+2)/2]: l | m << 8 of triangle index t
+    const double2* ab_hi;        // {A, B}[t] of the folded Eq. 7 (tables.h), high parts
+    const double2* ab_lo;        // ... low parts (double-double recurrences)
     int64_t n;
     int l_max;
     int batch;                   // points per phase-A batch: 32, 16 or 8 (1, 2 or 4 lanes per point)
@@ -356,28 +358,63 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
             }
             // columns of the folded Eq. 7, dealt to the W * NC column classes in snake order
             // (class v takes m = v, 2V-1-v, 2V+v, ...: balanced lengths; the classes of one warp sit
-            // on neighbouring columns, so their loops run nearly in step)
+            // on neighbouring columns, so their loops run nearly in step).  A lane runs TWO columns at
+            // a time (a long one and the short one that follows it in the snake): the recurrence is one
+            // dependent chain per column -- ~30 double-double operations per step for f64 I/O -- and
+            // two independent chains per lane hide its latency.  Coefficients {A, B} come from a packed
+            // global table through the read-only path (indexed constant-bank loads were the top stall).
             const uint32_t q_out = sQ + pt_l * TP * 8;
             const int V = W * NC, v = warp * NC + cls;
-            for (int i = 0; i * V <= l_max; ++i) {
-                const int m = (i & 1) ? (i + 1) * V - 1 - v : i * V + v;
-                if (m > l_max) continue;
-                int t = SPH_TRI(m, m);
-                R q = RT::make(TB.D_hi[m], TB.D_lo[m]), qp = RT::make(0.0, 0.0);
+            auto step = [&](int t, R& q, R& qp) {   // (q, qp) = (Qt_{l-1}^m, Qt_{l-2}^m) -> (Qt_l^m, Qt_{l-1}^m), t = TRI(l, m)
+                const double2 hi = __ldg(prm.ab_hi + t);
+                double2 lo = make_double2(0.0, 0.0);
+                if constexpr (sizeof(R) > sizeof(double)) lo = __ldg(prm.ab_lo + t);
+                const R w = NORM ? qp : r2 * qp;
+                const R qn = rec_step(hi.x, lo.x, hi.y, lo.y, Z, q, w);   // (B_{m+1}^m = 0)
+                qp = q;
+                q = qn;
                 tq_sts(q_out + t * 8, to_double(q));
-                for (int l = m + 1; l <= l_max; ++l) {
-                    t += l;   // SPH_TRI(l, m) - SPH_TRI(l-1, m) = l
-                    const R a = RT::make(TB.A_hi[t], TB.A_lo[t]);
-                    R qn;
-                    if (l == m + 1) {
-                        qn = a * (Z * q);
-                    } else {
-                        const R w = NORM ? qp : r2 * qp;
-                        qn = a * (Z * q) - RT::make(TB.B_hi[t], TB.B_lo[t]) * w;
+            };
+            if constexpr (sizeof(R) > sizeof(double)) {
+                for (int i = 0; i * V <= l_max; i += 2) {
+                    const int ma = i * V + v;
+                    if (ma > l_max) continue;
+                    int mb = (i + 2) * V - 1 - v;            // > ma; past the triangle: no second column
+                    if (mb > l_max) mb = 0x7fff;
+                    int ta = SPH_TRI(ma, ma), tb = 0;
+                    R qa = RT::make(TB.D_hi[ma], TB.D_lo[ma]), qpa = RT::make(0.0, 0.0);
+                    R qb = RT::make(0.0, 0.0), qpb = RT::make(0.0, 0.0);
+                    tq_sts(q_out + ta * 8, to_double(qa));
+                    for (int l = ma + 1; l <= l_max; ++l) {
+                        ta += l;   // SPH_TRI(l, m) - SPH_TRI(l-1, m) = l
+                        step(ta, qa, qpa);
+                        if (l == mb) {
+                            tb = SPH_TRI(mb, mb);
+                            qb = RT::make(TB.D_hi[mb], TB.D_lo[mb]);
+                            tq_sts(q_out + tb * 8, to_double(qb));
+                        } else if (l > mb) {
+                            tb += l;
+                            step(tb, qb, qpb);
+                        }
                     }
-                    qp = q;
-                    q = qn;
+                }
+            } else {
+                // f32 I/O (recurrences in plain double, 3 operations per step): one column at a time,
+                // coefficients from the constant bank (measured faster than the two-column form here)
+                for (int i = 0; i * V <= l_max; ++i) {
+                    const int m = (i & 1) ? (i + 1) * V - 1 - v : i * V + v;
+                    if (m > l_max) continue;
+                    int t = SPH_TRI(m, m);
+                    R q = RT::make(TB.D_hi[m], TB.D_lo[m]), qp = RT::make(0.0, 0.0);
                     tq_sts(q_out + t * 8, to_double(q));
+                    for (int l = m + 1; l <= l_max; ++l) {
+                        t += l;   // SPH_TRI(l, m) - SPH_TRI(l-1, m) = l
+                        const R w = NORM ? qp : r2 * qp;
+                        const R qn = RT::make(TB.A_hi[t], 0.0) * (Z * q) - RT::make(TB.B_hi[t], 0.0) * w;   // (B_{m+1}^m = 0)
+                        qp = q;
+                        q = qn;
+                        tq_sts(q_out + t * 8, to_double(q));
+                    }
                 }
             }
         }
@@ -461,7 +498,7 @@ template <typename T, typename R> static TqKernel tq_pick(int deriv, int norm) {
 // images: the warp-per-point kernels take those).
 static inline int tq_plan(int sm_count, int smem_optin, int64_t n, int l_max, int normalized, int dtype, void* sph,
                           void* dsph, void* ddsph, const void* xyz, const SphTables* d_tab, const unsigned short* d_lm,
-                          TqLaunch* out) {
+                          const double2* d_ab, TqLaunch* out) {
     const int deriv = ddsph ? 2 : (dsph ? 1 : 0);
     const int esize = dtype == 0 ? 4 : 8;
     const int64_t L = (int64_t)(l_max + 1) * (l_max + 1);
@@ -498,6 +535,8 @@ static inline int tq_plan(int sm_count, int smem_optin, int64_t n, int l_max, in
     out->prm.ddsph = ddsph;
     out->prm.tab = d_tab;
     out->prm.lm = d_lm;
+    out->prm.ab_hi = d_ab;
+    out->prm.ab_lo = d_ab + SPH_TRI_SIZE;
     out->prm.n = n;
     out->prm.l_max = l_max;
     out->prm.batch = bB;
