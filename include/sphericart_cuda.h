@@ -93,11 +93,55 @@ int sphericart_cuda_vjp(const void* xyz, const void* dsph, const void* grad_sph,
  *   xyz       [n,3]    in
  *   grad_sph  [n,L]    in
  *   grad_xyz  [n,3]    out
- * Any 0 <= l_max <= SPHERICART_CUDA_MAX_L (compile-time-specialised kernels for l_max <= 8, f32 <= 12).
+ * Any 0 <= l_max <= SPHERICART_CUDA_MAX_L (compile-time-specialised kernels for l_max <= 8, f32 <= 12;
+ * the two-phase kernel above that).
  * Errors as for sphericart_cuda_compute; normalized = 1 at r = 0 gives NaN for that point only.
  */
 int sphericart_cuda_vjp_recompute(const void* xyz, const void* grad_sph, void* grad_xyz, int64_t n,
                                   int l_max, int normalized, int dtype, void* stream);
+
+/*
+ * Forward pass in another convention (the paper compares with e3nn).
+ *   axes   SPHERICART_CUDA_AXES_STANDARD  the paper's: the l = 1 row is proportional to (y, z, x)
+ *          SPHERICART_CUDA_AXES_E3NN      the harmonics of the paper evaluated at the cyclically permuted
+ *                                         point (x', y', z') = (z, x, y): the l = 1 row is proportional to
+ *                                         (x, y, z); dsph / ddsph are derivatives w.r.t. the caller's x, y, z
+ *   scale  what sum_m Y_lm^2 is on the unit sphere:
+ *          SPHERICART_CUDA_SCALE_INTEGRAL   (2l+1)/4pi  (orthonormal; the paper's)
+ *          SPHERICART_CUDA_SCALE_COMPONENT  2l+1        (every degree-l output times sqrt(4pi))
+ *          SPHERICART_CUDA_SCALE_NORM       1           (... times sqrt(4pi/(2l+1)))
+ * Everything else as sphericart_cuda_compute, which (axes, scale) = (0, 0) is.  The permutation is
+ * applied where the point is loaded and where a derivative row is staged, the scale is folded into
+ * the coefficient tables: no extra pass over the outputs.
+ */
+#define SPHERICART_CUDA_AXES_STANDARD 0
+#define SPHERICART_CUDA_AXES_E3NN 1
+#define SPHERICART_CUDA_SCALE_INTEGRAL 0
+#define SPHERICART_CUDA_SCALE_COMPONENT 1
+#define SPHERICART_CUDA_SCALE_NORM 2
+int sphericart_cuda_compute_ex(const void* xyz, int64_t n, int l_max, int normalized, int dtype, int axes,
+                               int scale, void* sph, void* dsph, void* ddsph, void* stream);
+
+/*
+ * Second-order VJP: the backward pass of the backward pass ("double backward";
+ * P:112 for the backward pass, P:94 for derivatives beyond the first).  The backward pass is the map
+ *     g(xyz, w)[i,a] = sum_k (d sph[i,k] / d xyz[i,a]) w[i,k],     w = grad_sph;
+ * given an upstream gradient v [n,3] on its output, its own backward is
+ *     grad_grad_xyz[i,b] = sum_{a,k} (d2 sph[i,k] / d xyz[i,a] d xyz[i,b]) v[i,a] w[i,k]
+ *     grad_grad_sph[i,k] = sum_a     (d sph[i,k] / d xyz[i,a]) v[i,a]
+ * Both derivative orders are evaluated from xyz inside the kernel (Eq. 10 once and twice, through
+ * x/r for normalized = 1) and contracted as they are assembled: neither dsph nor ddsph is read or
+ * written.
+ *   xyz            [n,3]  in
+ *   grad_sph       [n,L]  in
+ *   v              [n,3]  in
+ *   grad_grad_xyz  [n,3]  out
+ *   grad_grad_sph  [n,L]  out, or NULL: not wanted
+ * Device pointers, caller-owned, 16-byte aligned; asynchronous on `stream`; any l_max up to
+ * SPHERICART_CUDA_MAX_L.  Errors as for sphericart_cuda_compute.
+ */
+int sphericart_cuda_vjp2(const void* xyz, const void* grad_sph, const void* v, void* grad_grad_xyz,
+                         void* grad_grad_sph, int64_t n, int l_max, int normalized, int dtype, void* stream);
 
 /*
  * Fused density expansion (the use the paper motivates, Eq. 1):
@@ -135,7 +179,7 @@ const char* sphericart_cuda_last_error(void);
 int64_t sphericart_cuda_launch_count(void);
 
 /* Name of the kernel family the calling thread's last launch used ("tpb", "tq", "tpg", "w", "wc",
- * "vjp", "vjp_warp", "vjpr", "vjpr_generic", "expand", ...; "" before the first launch).  Static
+ * "vjp", "vjp_warp", "vjpr", "tq_vjpr", "tq_vjp2", "vjpr_generic", "expand", ...; "" before the first launch).  Static
  * storage, never NULL.  For harnesses: bench.py records which kernel served each cell of its sweep. */
 const char* sphericart_cuda_last_kernel(void);
 

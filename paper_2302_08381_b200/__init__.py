@@ -21,6 +21,8 @@ _lib = None
 
 F32, F64 = 0, 1
 MAX_L = 32
+AXES_STANDARD, AXES_E3NN = 0, 1
+SCALE_INTEGRAL, SCALE_COMPONENT, SCALE_NORM = 0, 1, 2
 
 
 class SphericartCudaError(RuntimeError):
@@ -50,6 +52,10 @@ def load():
     lib.sphericart_cuda_compute_host.argtypes = [vp, i64, ci, ci, ci, vp, vp, vp]
     lib.sphericart_cuda_vjp_recompute.restype = ci
     lib.sphericart_cuda_vjp_recompute.argtypes = [vp, vp, vp, i64, ci, ci, ci, vp]
+    lib.sphericart_cuda_compute_ex.restype = ci
+    lib.sphericart_cuda_compute_ex.argtypes = [vp, i64, ci, ci, ci, ci, ci, vp, vp, vp, vp]
+    lib.sphericart_cuda_vjp2.restype = ci
+    lib.sphericart_cuda_vjp2.argtypes = [vp, vp, vp, vp, vp, i64, ci, ci, ci, vp]
     lib.sphericart_cuda_expand.restype = ci
     lib.sphericart_cuda_expand.argtypes = [vp, vp, vp, i64, ci, ci, ci, vp, vp]
     lib.sphericart_cuda_vjp_host.restype = ci
@@ -108,6 +114,18 @@ def sphericart_cuda_vjp_recompute(xyz, grad_sph, grad_xyz, n, l_max, normalized,
     _check(rc, "sphericart_cuda_vjp_recompute")
 
 
+def sphericart_cuda_compute_ex(xyz, n, l_max, normalized, dtype, axes, scale, sph, dsph, ddsph, stream):
+    rc = load().sphericart_cuda_compute_ex(_ptr(xyz), n, l_max, int(normalized), dtype, int(axes), int(scale),
+                                           _ptr(sph), _ptr(dsph), _ptr(ddsph), _ptr(stream))
+    _check(rc, "sphericart_cuda_compute_ex")
+
+
+def sphericart_cuda_vjp2(xyz, grad_sph, v, grad_grad_xyz, grad_grad_sph, n, l_max, normalized, dtype, stream):
+    rc = load().sphericart_cuda_vjp2(_ptr(xyz), _ptr(grad_sph), _ptr(v), _ptr(grad_grad_xyz), _ptr(grad_grad_sph), n,
+                                     l_max, int(bool(normalized)), dtype, _ptr(stream))
+    _check(rc, "sphericart_cuda_vjp2")
+
+
 def sphericart_cuda_expand(xyz, radial, seg_ptr, n_seg, l_max, n_rad, dtype, coeff, stream):
     rc = load().sphericart_cuda_expand(_ptr(xyz), _ptr(radial), _ptr(seg_ptr), n_seg, l_max, n_rad, dtype,
                                        _ptr(coeff), _ptr(stream))
@@ -149,10 +167,11 @@ def _dtype_code(t):
 
 
 def compute(xyz, l_max: int, normalized: bool = True, gradients: bool = False, hessians: bool = False,
-            out=None):
+            out=None, axes: int = AXES_STANDARD, scale: int = SCALE_INTEGRAL):
     """``xyz`` [n,3] CUDA tensor -> ``(sph [n,L], dsph [n,3,L] | None, ddsph [n,3,3,L] | None)``.
 
     Enqueued on torch's current stream.  ``out`` may hold preallocated ``(sph, dsph, ddsph)``.
+    ``axes`` / ``scale``: another convention (``sphericart_cuda_compute_ex``).
     """
     import torch
 
@@ -170,7 +189,7 @@ def compute(xyz, l_max: int, normalized: bool = True, gradients: bool = False, h
         sph, dsph, ddsph = out
     with torch.cuda.device(xyz.device):
         stream = torch.cuda.current_stream().cuda_stream
-        sphericart_cuda_compute(xyz, n, l_max, normalized, _dtype_code(xyz), sph, dsph, ddsph, stream)
+        sphericart_cuda_compute_ex(xyz, n, l_max, normalized, _dtype_code(xyz), axes, scale, sph, dsph, ddsph, stream)
     return sph, dsph, ddsph
 
 
@@ -209,6 +228,26 @@ def vjp_recompute(xyz, grad_sph, normalized: bool, out=None):
         stream = torch.cuda.current_stream().cuda_stream
         sphericart_cuda_vjp_recompute(xyz, grad_sph, gx, n, l_max, normalized, _dtype_code(xyz), stream)
     return gx
+
+
+def vjp2(xyz, grad_sph, v, normalized: bool, want_grad_grad_sph: bool = True):
+    """Double backward from ``xyz``: ``(grad_grad_xyz [n,3], grad_grad_sph [n,L] | None)`` for the upstream
+    gradient ``v`` [n,3] on ``vjp_recompute(xyz, grad_sph)`` (``sphericart_cuda_vjp2``)."""
+    import torch
+
+    if not xyz.is_cuda:
+        raise SphericartCudaError("xyz must be a CUDA tensor (no CPU fallback)")
+    xyz, grad_sph, v = xyz.contiguous(), grad_sph.contiguous(), v.contiguous()
+    n, L = grad_sph.shape
+    l_max = int(round(L ** 0.5)) - 1
+    if (l_max + 1) ** 2 != L or xyz.shape != (n, 3) or v.shape != (n, 3) or not (xyz.dtype == grad_sph.dtype == v.dtype):
+        raise ValueError("shapes: xyz [n,3], grad_sph [n,L], v [n,3], L a perfect square, same dtype")
+    ggx = torch.empty((n, 3), dtype=xyz.dtype, device=xyz.device)
+    ggs = torch.empty((n, L), dtype=xyz.dtype, device=xyz.device) if want_grad_grad_sph else None
+    with torch.cuda.device(xyz.device):
+        stream = torch.cuda.current_stream().cuda_stream
+        sphericart_cuda_vjp2(xyz, grad_sph, v, ggx, ggs, n, l_max, normalized, _dtype_code(xyz), stream)
+    return ggx, ggs
 
 
 def expand(xyz, radial, seg_ptr, out=None):

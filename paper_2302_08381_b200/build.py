@@ -2,7 +2,7 @@
 
 sm_100a only, ``-lineinfo`` so ncu's source page maps to the .cuh files.  The translation units
 (``api.cu``, ``tables.cpp``, ``tpb_inst.cu`` once per element type and derivative order, ``vjpr_inst.cu`` and
-``expand_inst.cu`` once per element type) are
+``expand_inst.cu`` and ``tq_inst.cu`` once per element type) are
 compiled in parallel and linked into one shared library.
 The result, ``paper_2302_08381_b200/libsphericart_cuda.so``, is git-ignored but travels to the
 GPU box with the repository snapshot.
@@ -17,7 +17,8 @@ from pathlib import Path
 PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libsphericart_cuda.so"
-SOURCES = [CSRC / "api.cu", CSRC / "tables.cpp", CSRC / "tpb_inst.cu", CSRC / "vjpr_inst.cu", CSRC / "expand_inst.cu"]
+SOURCES = [CSRC / "api.cu", CSRC / "tables.cpp", CSRC / "tpb_inst.cu", CSRC / "vjpr_inst.cu", CSRC / "expand_inst.cu",
+           CSRC / "tq_inst.cu"]
 HEADERS = sorted(CSRC.glob("*.cuh")) + sorted(CSRC.glob("*.h")) + [PKG.parent / "include" / "sphericart_cuda.h"]
 OBJ_DIR = PKG / "build"
 
@@ -26,7 +27,8 @@ UNITS = [("api", CSRC / "api.cu", []), ("tables", CSRC / "tables.cpp", [])] + [
     (f"tpb_f{64 if f64 else 32}_{'vgh'[deriv]}", CSRC / "tpb_inst.cu", [f"-DTPB_F64={f64}", f"-DTPB_DERIV={deriv}"])
     for f64 in (0, 1) for deriv in (0, 1, 2)] + [
     (f"vjpr_f{64 if f64 else 32}", CSRC / "vjpr_inst.cu", [f"-DVJPR_F64={f64}"]) for f64 in (0, 1)] + [
-    (f"expand_f{64 if f64 else 32}", CSRC / "expand_inst.cu", [f"-DEXPAND_F64={f64}"]) for f64 in (0, 1)]
+    (f"expand_f{64 if f64 else 32}", CSRC / "expand_inst.cu", [f"-DEXPAND_F64={f64}"]) for f64 in (0, 1)] + [
+    (f"tq_f{64 if f64 else 32}", CSRC / "tq_inst.cu", [f"-DTQ_F64={f64}"]) for f64 in (0, 1)]
 
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC"]

@@ -22,7 +22,7 @@ __constant__ SphTables c_tables;
 
 #include "kernel_vjp.cuh"
 #include "kernel_tpg.cuh"
-#include "kernel_tq.cuh"
+#include "tq_table.h"
 #include "kernel_w.cuh"
 #include "kernel_wc.cuh"
 #include "tpb_api.h"
@@ -97,7 +97,8 @@ static int device_state(DeviceState** out) {
             sph_tpb_upload_f64_v(&g_host_tables) || sph_tpb_upload_f64_g(&g_host_tables) ||
             sph_tpb_upload_f32_h(&g_host_tables) || sph_tpb_upload_f64_h(&g_host_tables) ||
             sph_vjpr_upload_f32(&g_host_tables) || sph_vjpr_upload_f64(&g_host_tables) ||
-            sph_expand_upload_f32(&g_host_tables) || sph_expand_upload_f64(&g_host_tables))
+            sph_expand_upload_f32(&g_host_tables) || sph_expand_upload_f64(&g_host_tables) ||
+            sph_tq_upload_f32(&g_host_tables) || sph_tq_upload_f64(&g_host_tables))
             return fail(SPHERICART_CUDA_ECUDA, "table upload failed: %s", cudaGetErrorString(cudaGetLastError()));
         CUDA_TRY(cudaMalloc(&st.d_tables, sizeof(SphTables)));
         CUDA_TRY(cudaMemcpy(st.d_tables, &g_host_tables, sizeof(SphTables), cudaMemcpyHostToDevice));
@@ -172,6 +173,44 @@ static int launch_w(const DeviceState& st, const void* xyz, int64_t n, int l_max
     return 0;
 }
 
+// ---------------------------------------------------------------------------------------------
+// two-phase kernel (tq_inst.cu): forward (optionally in another convention), second-order VJP,
+// recompute VJP.  Returns 0 launched, 1 no shape fits, -1 CUDA error.
+// ---------------------------------------------------------------------------------------------
+struct TqConv {
+    int src[3], row[3];
+    double lscale[SPH_MAX_L + 1];
+};
+static int launch_tq(const DeviceState& st, int mode, int normalized, int dtype, const TqConv* conv, const void* xyz,
+                     void* sph, void* dsph, void* ddsph, const void* gsph, const void* vvec, void* gxyz, int64_t n,
+                     int l_max, cudaStream_t stream) {
+    TqArgs a{};
+    a.sm_count = st.sm_count;
+    a.smem_optin = st.smem_optin;
+    a.mode = mode;
+    a.deriv = ddsph ? 2 : (dsph ? 1 : 0);
+    a.normalized = normalized;
+    a.conv = conv != nullptr;
+    a.xyz = xyz;
+    a.sph = sph;
+    a.dsph = dsph;
+    a.ddsph = ddsph;
+    a.gsph = gsph;
+    a.vvec = vvec;
+    a.gxyz = gxyz;
+    a.n = n;
+    a.l_max = l_max;
+    a.d_tab = st.d_tables;
+    a.d_lm = st.d_lm;
+    a.d_ab = st.d_ab;
+    for (int i = 0; i < 3; ++i) a.src[i] = conv ? conv->src[i] : i, a.row[i] = conv ? conv->row[i] : i;
+    a.lscale = conv ? conv->lscale : nullptr;
+    a.stream = stream;
+    const int r = dtype == SPHERICART_CUDA_F32 ? sph_tq_launch_f32(a) : sph_tq_launch_f64(a);
+    if (r == 0) launched(mode == 0 ? "tq" : (mode == 1 ? "tq_vjp2" : "tq_vjpr"));
+    return r;
+}
+
 static bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
 
 static int check_common(int64_t n, int l_max, int dtype) {
@@ -202,16 +241,10 @@ static int compute_device(const void* xyz, int64_t n, int l_max, int normalized,
     const bool force_w = force == FORCE_W || force == FORCE_W1 || force == FORCE_WC;
     if (force == FORCE_TQ || (force == FORCE_NONE && TQ_SHAPE[dtype != 0][ddsph ? 2 : (dsph ? 1 : 0)][l_max][0])) {
         // two-phase kernel: recurrences lane = point, assembly lane = (l, m) pair, small full-row tiles
-        TqLaunch lq{};
-        if (tq_plan(st->sm_count, st->smem_optin, n, l_max, normalized, dtype, sph, dsph, ddsph, xyz, st->d_tables,
-                    st->d_lm, st->d_ab, &lq) == 0) {
-            rc = allow_smem(lq.func, (int)lq.smem);
-            if (rc) return rc;
-            tq_launch(lq, stream);
-            launched("tq");
-            CUDA_TRY(cudaGetLastError());
-            return 0;
-        }
+        const int r = launch_tq(*st, 0, normalized, dtype, nullptr, xyz, sph, dsph, ddsph, nullptr, nullptr, nullptr, n, l_max,
+                                stream);
+        if (r < 0) return fail(SPHERICART_CUDA_ECUDA, "tq launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+        if (r == 0) return 0;
     }
     if (force == FORCE_NONE || force == FORCE_TPB) {
         // compile-time-l_max kernels (two threads per point): every l_max that has an instantiation
@@ -289,6 +322,13 @@ static int vjp_recompute_device(const void* xyz, const void* grad_sph, void* gra
             launched("vjpr");
             return 0;
         }
+    }
+    if (g_opt.force_kernel != FORCE_GENERIC) {
+        // every other l_max: the two-phase kernel, gradients contracted with grad_sph as they are assembled
+        const int r = launch_tq(*st, 2, normalized, dtype, nullptr, xyz, nullptr, nullptr, nullptr, grad_sph, nullptr, grad_xyz,
+                                n, l_max, stream);
+        if (r < 0) return fail(SPHERICART_CUDA_ECUDA, "tq launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+        if (r == 0) return 0;
     }
     const int64_t blocks = (n + 127) / 128;
     if (blocks > 0x7fffffff) return fail(SPHERICART_CUDA_EINVAL, "n = %lld is too large", (long long)n);
@@ -428,6 +468,64 @@ int sphericart_cuda_vjp_recompute(const void* xyz, const void* grad_sph, void* g
                                   int normalized, int dtype, void* stream) {
     return vjp_recompute_device(xyz, grad_sph, grad_xyz, n, l_max, normalized, dtype,
                                 static_cast<cudaStream_t>(stream));
+}
+
+int sphericart_cuda_compute_ex(const void* xyz, int64_t n, int l_max, int normalized, int dtype, int axes, int scale,
+                               void* sph, void* dsph, void* ddsph, void* stream) {
+    if (axes != SPHERICART_CUDA_AXES_STANDARD && axes != SPHERICART_CUDA_AXES_E3NN)
+        return fail(SPHERICART_CUDA_EINVAL, "axes = %d is neither 0 (standard) nor 1 (e3nn)", axes);
+    if (scale < SPHERICART_CUDA_SCALE_INTEGRAL || scale > SPHERICART_CUDA_SCALE_NORM)
+        return fail(SPHERICART_CUDA_EINVAL, "scale = %d is not 0 (integral), 1 (component) or 2 (norm)", scale);
+    if (axes == SPHERICART_CUDA_AXES_STANDARD && scale == SPHERICART_CUDA_SCALE_INTEGRAL)
+        return compute_device(xyz, n, l_max, normalized, dtype, sph, dsph, ddsph, static_cast<cudaStream_t>(stream));
+    int rc = check_common(n, l_max, dtype);
+    if (rc) return rc;
+    if (normalized != 0 && normalized != 1)
+        return fail(SPHERICART_CUDA_EINVAL, "normalized = %d is neither 0 nor 1", normalized);
+    if (ddsph && !dsph) return fail(SPHERICART_CUDA_EINVAL, "ddsph given without dsph");
+    if (n == 0) return 0;
+    if (!xyz || !sph) return fail(SPHERICART_CUDA_EINVAL, "xyz and sph must not be NULL when n > 0");
+    if (misaligned(xyz) || misaligned(sph) || misaligned(dsph) || misaligned(ddsph))
+        return fail(SPHERICART_CUDA_EALIGN, "device pointers must be 16-byte aligned");
+    DeviceState* st = nullptr;
+    rc = device_state(&st);
+    if (rc) return rc;
+    TqConv conv;
+    const bool e3nn = axes == SPHERICART_CUDA_AXES_E3NN;
+    // e3nn axes: the evaluation frame is (x', y', z') = (z, x, y) of the caller's point, so axis a of
+    // the evaluation frame is the caller's axis src[a]
+    const int src[3] = {e3nn ? 2 : 0, e3nn ? 0 : 1, e3nn ? 1 : 2};
+    for (int i = 0; i < 3; ++i) conv.src[i] = conv.row[i] = src[i];
+    const double four_pi = 12.566370614359172953850573533118;
+    for (int l = 0; l <= SPH_MAX_L; ++l)
+        conv.lscale[l] = scale == SPHERICART_CUDA_SCALE_INTEGRAL ? 1.0
+                       : scale == SPHERICART_CUDA_SCALE_COMPONENT ? sqrt(four_pi) : sqrt(four_pi / (2 * l + 1));
+    const int r = launch_tq(*st, 0, normalized, dtype, &conv, xyz, sph, dsph, ddsph, nullptr, nullptr, nullptr, n, l_max,
+                            static_cast<cudaStream_t>(stream));
+    if (r < 0) return fail(SPHERICART_CUDA_ECUDA, "tq launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    if (r > 0) return fail(SPHERICART_CUDA_ENOTSUP, "compute_ex: rows of l_max = %d with these outputs do not fit the kernel", l_max);
+    return 0;
+}
+
+int sphericart_cuda_vjp2(const void* xyz, const void* grad_sph, const void* v, void* grad_grad_xyz, void* grad_grad_sph,
+                         int64_t n, int l_max, int normalized, int dtype, void* stream) {
+    int rc = check_common(n, l_max, dtype);
+    if (rc) return rc;
+    if (normalized != 0 && normalized != 1)
+        return fail(SPHERICART_CUDA_EINVAL, "normalized = %d is neither 0 nor 1", normalized);
+    if (n == 0) return 0;
+    if (!xyz || !grad_sph || !v || !grad_grad_xyz)
+        return fail(SPHERICART_CUDA_EINVAL, "xyz, grad_sph, v and grad_grad_xyz must not be NULL when n > 0");
+    if (misaligned(xyz) || misaligned(grad_sph) || misaligned(v) || misaligned(grad_grad_xyz) || misaligned(grad_grad_sph))
+        return fail(SPHERICART_CUDA_EALIGN, "device pointers must be 16-byte aligned");
+    DeviceState* st = nullptr;
+    rc = device_state(&st);
+    if (rc) return rc;
+    const int r = launch_tq(*st, 1, normalized, dtype, nullptr, xyz, grad_grad_sph, nullptr, nullptr, grad_sph, v, grad_grad_xyz,
+                            n, l_max, static_cast<cudaStream_t>(stream));
+    if (r < 0) return fail(SPHERICART_CUDA_ECUDA, "tq launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    if (r > 0) return fail(SPHERICART_CUDA_ENOTSUP, "vjp2: l_max = %d does not fit the kernel", l_max);
+    return 0;
 }
 
 int sphericart_cuda_expand(const void* xyz, const void* radial, const int64_t* seg_ptr, int64_t n_seg, int l_max,

@@ -1,5 +1,10 @@
-// "tq" forward kernel: two phases per batch of points, the whole CTA on both.  Any l_max, values /
-// + gradients / + Hessians, run-time l_max (12 instantiations in all).
+// "tq" kernel: two phases per batch of points, the whole CTA on both.  Any l_max, run-time l_max.
+//   MODE 0  forward: values / + gradients / + Hessians (optionally in another axis / scale
+//           convention, CONV: SURVEY 8(f) N4)
+//   MODE 1  second-order VJP (double backward): the Hessians are
+//           assembled as in MODE 0 and contracted on the fly, nothing but grad_grad rows is stored
+//   MODE 2  recompute-in-backward VJP: the gradients are assembled as in
+//           MODE 0 and contracted with grad_sph on the fly, nothing is staged at all
 //
 // Why (profiles/r2_*): the unrolled tpb kernels keep a point's whole Legendre
 // column in registers and stage 16 points per warp, so from l_max ~ 11 (gradients) / 6 (Hessians)
@@ -40,8 +45,6 @@
 // which is Eq. 10 once / twice for the solid harmonics and the Euler-simplified chain rule of
 // sph_core.cuh for the normalised ones, regrouped by the azimuthal factor they multiply.
 #pragma once
-#include <cmath>
-
 #include "options.h"
 #include "ptx.cuh"
 #include "sph_core.cuh"
@@ -49,11 +52,17 @@
 
 namespace sphb200 {
 
+// every translation unit that instantiates these kernels carries its own copy of the tables
+static __constant__ SphTables c_tables_tq;
+
 struct TqParams {
     const void* xyz;
-    void* sph;
+    void* sph;                   // MODE 0: sph [n,L];  MODE 1: grad_grad_sph [n,L] (may be NULL)
     void* dsph;
     void* ddsph;
+    const void* gsph;            // MODE 1, 2: grad_sph [n,L] (the upstream gradient w)
+    const void* vvec;            // MODE 1: v [n,3] (the upstream gradient on grad_xyz)
+    void* gxyz;                  // MODE 1: grad_grad_xyz [n,3];  MODE 2: grad_xyz [n,3]
     const SphTables* tab;        // global-memory copy of the tables (phase B: G1, Gz, H2, Hxz, Hzz)
     const unsigned short* lm;    // [(l_max+1)(l_max+2)/2]: l | m << 8 of triangle index t
     const double2* ab_hi;        // {A, B}[t] of the folded Eq. 7 (tables.h), high parts
@@ -64,24 +73,36 @@ struct TqParams {
     int pts_tile;                // points per image; divides batch
     int batches_per_cta;         // consecutive batches one CTA works through
     int n_images;                // 2: a tile drains while the next is assembled; 1: the longest rows
+    // CONV: the harmonics are evaluated at (x', y', z') = xyz[src[0..2]] and derivative axis a of the
+    // evaluation frame is the caller's axis row[a]; every degree-l output is multiplied by lscale[l]
+    int src[3], row[3];
+    double lscale[SPH_MAX_L + 1];
 };
 
 constexpr int TQ_MAX_WARPS = 8;
 
 // shared-memory carve-up (bytes), identical on host and device
 struct TqSmem {
-    int T, TP, CP;
-    size_t gt_off, ht_off, lm_off, q_off, cs_off, pt_off, img_off, img_bytes, total;
+    int T, TP, CP, PTB;
+    size_t gt_off, ht_off, lm_off, sl_off, red_off, q_off, cs_off, pt_off, img_off, img_bytes, total;
     size_t reg_g, reg_h;   // offsets of the dsph / ddsph regions inside an image
-    __host__ __device__ TqSmem(int l_max, int deriv, int esize, int batch, int pts_tile, int n_images) {
+    // deriv: derivative order assembled; img_rows: rows per point staged (1 / 4 / 13 forward, 1 or 0
+    // for the contracting modes); pt_bytes: per-point record (x, y, z, 1/r [, v])
+    __host__ __device__ TqSmem(int l_max, int deriv, int img_rows, int pt_bytes, int esize, int batch, int pts_tile,
+                               int n_images) {
         T = (l_max + 1) * (l_max + 2) / 2;
         TP = (T + 3) | 1;          // doubles per point: three finite pad entries, odd pitch (conflict-free lane = point stores)
         CP = (l_max + 3) | 1;      // (c, s) pairs per point behind two zero pad entries ((c,s)_{-1}, (c,s)_{-2}), odd pitch
+        PTB = pt_bytes;
         size_t o = 0;
         gt_off = o;                // {G1, Gz}[t]
         o += deriv >= 1 ? (size_t)T * 16 : 0;
         ht_off = o;                // {H2, Hxz, Hzz, -}[t]
         o += deriv >= 2 ? (size_t)T * 32 : 0;
+        sl_off = o;                // lscale[l] (CONV)
+        o += (size_t)(SPH_MAX_L + 1) * 8 + 8;
+        red_off = o;               // [warps][2 points][3] partial sums of the contracting modes
+        o += 8 * 48;
         lm_off = o;                // l | m << 8
         o += ((size_t)T * 2 + 15) & ~(size_t)15;
         q_off = o;
@@ -90,21 +111,22 @@ struct TqSmem {
         cs_off = o;
         o += (size_t)batch * CP * 16;
         pt_off = o;
-        o += (size_t)batch * 32;
+        o += (size_t)batch * pt_bytes;
         img_off = (o + 127) & ~(size_t)127;
-        const int rows = deriv == 0 ? 1 : (deriv == 1 ? 4 : 13);
-        const size_t L = (size_t)(l_max + 1) * (l_max + 1);
         // one region per output array, each with 16 bytes of slack: a region is staged at the offset
         // (0..15 bytes) its global address has from a 16-byte boundary, so that the aligned body of
         // the run can leave as one bulk store whatever the tile's first point is
+        const size_t L = (size_t)(l_max + 1) * (l_max + 1);
         const size_t sb = (size_t)pts_tile * L * esize;
         reg_g = (sb + 16 + 15) & ~(size_t)15;
         reg_h = reg_g + ((3 * sb + 16 + 15) & ~(size_t)15);
-        const size_t end = rows == 1 ? reg_g : (rows == 4 ? reg_h : reg_h + ((9 * sb + 16 + 15) & ~(size_t)15));
+        const size_t end = img_rows == 0 ? 0 : (img_rows == 1 ? reg_g : (img_rows == 4 ? reg_h : reg_h + ((9 * sb + 16 + 15) & ~(size_t)15)));
         img_bytes = (end + 127) & ~(size_t)127;
         total = img_off + (size_t)n_images * img_bytes;
     }
 };
+__host__ __device__ constexpr int tq_img_rows(int mode, int deriv) { return mode == 2 ? 0 : (mode == 1 ? 1 : (deriv == 0 ? 1 : (deriv == 1 ? 4 : 13))); }
+__host__ __device__ constexpr int tq_pt_bytes(int mode) { return mode == 1 ? 64 : 32; }
 
 // shared-memory accesses through 32-bit shared addresses (one IADD per address instead of the
 // 64-bit generic arithmetic the compiler emits for pointers into a dynamic carve-up).  volatile:
@@ -138,10 +160,12 @@ __device__ __forceinline__ void tq_sts2(uint32_t a, double x, double y) {
     asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(a), "d"(x), "d"(y) : "memory");
 }
 
-template <typename T, typename R, int DERIV, bool NORM>
+template <typename T, typename R, int DERIV, bool NORM, int MODE, bool CONV>
 __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqParams prm) {
     using RT = rec<R>;
     constexpr int ES = (int)sizeof(T);
+    constexpr int PTB = tq_pt_bytes(MODE);
+    static_assert(MODE == 0 || (MODE == 1 && DERIV == 2) || (MODE == 2 && DERIV == 1), "mode / derivative order");
     extern __shared__ __align__(128) unsigned char smem[];
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
@@ -149,10 +173,11 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
     const int l_max = prm.l_max;
     const int L = (l_max + 1) * (l_max + 1);
     const int B = prm.batch, P = prm.pts_tile;
-    const TqSmem lay(l_max, DERIV, ES, B, P, prm.n_images);
+    const TqSmem lay(l_max, DERIV, tq_img_rows(MODE, DERIV), PTB, ES, B, P, prm.n_images);
     const int TT = lay.T, TP = lay.TP, CP = lay.CP;
     const uint32_t s0 = smem_u32(smem);
     const uint32_t sGT = s0 + (uint32_t)lay.gt_off, sHT = s0 + (uint32_t)lay.ht_off, sLM = s0 + (uint32_t)lay.lm_off;
+    const uint32_t sSL = s0 + (uint32_t)lay.sl_off;
     const uint32_t sQ = s0 + (uint32_t)lay.q_off, sCS = s0 + (uint32_t)lay.cs_off, sPT = s0 + (uint32_t)lay.pt_off;
     unsigned char* img0 = smem + lay.img_off;
     const int64_t n = prm.n;
@@ -160,133 +185,182 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
     T* __restrict__ sph = static_cast<T*>(prm.sph);
     T* __restrict__ dsph = static_cast<T*>(prm.dsph);
     T* __restrict__ ddsph = static_cast<T*>(prm.ddsph);
-    const SphTables& TB = c_tables;
+    const T* __restrict__ gsph = static_cast<const T*>(prm.gsph);
+    T* __restrict__ gxyz = static_cast<T*>(prm.gxyz);
+    const SphTables& TB = c_tables_tq;
     const uint64_t policy = policy_evict_first();
 
-    // once per CTA: phase B's coefficient tables and the (l, m) of every triangle index -> shared
-    // memory; the pad entries behind every point's triangle and in front of its (c, s) list, which
-    // phase B reads times a zero coefficient
+    // once per CTA: phase B's coefficient tables (times the degree's scale for CONV: every output of
+    // degree l is linear in them and in Qt_l^m, which phase B scales as it reads it) and the (l, m)
+    // of every triangle index -> shared memory; the pad entries behind every point's triangle and
+    // in front of its (c, s) list, which phase B reads times a zero coefficient
     for (int t = threadIdx.x; t < TT; t += blockDim.x) {
-        if (DERIV >= 1) tq_sts2(sGT + t * 16, __ldg(&prm.tab->G1[t]), __ldg(&prm.tab->Gz[t]));
+        const unsigned short lmv = __ldg(prm.lm + t);
+        const double sl = CONV ? prm.lscale[lmv & 0xff] : 1.0;
+        if (DERIV >= 1) tq_sts2(sGT + t * 16, sl * __ldg(&prm.tab->G1[t]), sl * __ldg(&prm.tab->Gz[t]));
         if (DERIV >= 2) {
-            tq_sts2(sHT + t * 32, __ldg(&prm.tab->H2[t]), __ldg(&prm.tab->Hxz[t]));
-            tq_sts(sHT + t * 32 + 16, __ldg(&prm.tab->Hzz[t]));
+            tq_sts2(sHT + t * 32, sl * __ldg(&prm.tab->H2[t]), sl * __ldg(&prm.tab->Hxz[t]));
+            tq_sts(sHT + t * 32 + 16, sl * __ldg(&prm.tab->Hzz[t]));
         }
-        reinterpret_cast<unsigned short*>(smem + lay.lm_off)[t] = __ldg(prm.lm + t);
+        reinterpret_cast<unsigned short*>(smem + lay.lm_off)[t] = lmv;
     }
+    if (CONV)
+        for (int l = threadIdx.x; l <= l_max; l += blockDim.x) tq_sts(sSL + l * 8, prm.lscale[l]);
     for (int i = threadIdx.x; i < B * 3; i += blockDim.x) tq_sts(sQ + ((i / 3) * TP + TT + (i % 3)) * 8, 0.0);
     for (int i = threadIdx.x; i < B * 2; i += blockDim.x) tq_sts2(sCS + ((i >> 1) * CP + (i & 1)) * 16, 0.0, 0.0);
 
     const int NCH = (TT + 31) >> 5;                    // 32-pair chunks of one point's triangle
-    const int d_pl = W / NCH, d_ch = W - d_pl * NCH;   // one step of a warp through the (point, chunk) units
+    const int d_pl = W / NCH, d_ch = W - d_pl * NCH;   // one step of a warp through the (point pair, chunk) units
     const int w_pl0 = warp / NCH, w_ch0 = warp - w_pl0 * NCH;
-    const int PP = P >> 1;                             // pairs of points per tile (P is even)
+    const int PP = (P + 1) >> 1;                       // pairs of points per tile (the last one may hold one point)
     const uint32_t row_b = (uint32_t)L * ES;          // bytes of one row of one point
     const uint32_t s_bytes = (uint32_t)P * row_b;     // bytes of the tile's sph image
-    // Phase B for ONE (l, m >= 0) pair (triangle index t) and TWO points: the points pbb, pbb + 1 of the
-    // batch, staged as points plb, plb + 1 of the image whose regions start at sS / sG / sH.
-    auto assemble = [&](int t, int plb, int pbb, uint32_t sS, uint32_t sG, uint32_t sH) {
-            // ---- per (l, m): shared by the two points ----
-            const unsigned lmv = tq_lds_u16(sLM + t * 2);
-            const int l = (int)(lmv & 0xffu), m = (int)(lmv >> 8);
-            const double dl = (double)l, dm = (double)m;
-            // the (l, -m) outputs are stored FIRST and unconditionally: for m = 0 they land on the
-            // (l, 0) slot and the cos-branch store that follows overwrites them (no branch)
-            const uint32_t kc_b = (uint32_t)(l * (l + 1) + m) * ES, m2_b = (uint32_t)(2 * m) * ES;
-            const uint32_t l8 = (uint32_t)l * 8;
-            double G1 = 0.0, Gz = 0.0, H2 = 0.0, Hxz = 0.0, Hzz = 0.0;
-            if constexpr (DERIV >= 1) tq_lds2(sGT + t * 16, G1, Gz);
-            if constexpr (DERIV >= 2) {
-                tq_lds2(sHT + t * 32, H2, Hxz);
-                Hzz = tq_lds16(sHT + t * 32);
-            }
-            const double dmm = dm * (dm - 1.0);
+    // derivative axis a of the evaluation frame is row `row[a]` of the caller's arrays
+    const uint32_t rx = (CONV ? prm.row[0] : 0) * row_b, ry = (CONV ? prm.row[1] : 1) * row_b, rz = (CONV ? prm.row[2] : 2) * row_b;
+    // Phase B for ONE (l, m >= 0) pair (triangle index t) and up to TWO points: the points pbb, pbb + 1
+    // of the batch (global index pg0, pg0 + 1), staged as points plb, plb + 1 of the image whose
+    // regions start at sS / sG / sH.  acc: this lane's partial sums of the contracting modes.
+    auto assemble = [&](int t, int plb, int pbb, int npt, int64_t pg0, uint32_t sS, uint32_t sG, uint32_t sH, double* acc) {
+        // ---- per (l, m): shared by the two points ----
+        const unsigned lmv = tq_lds_u16(sLM + t * 2);
+        const int l = (int)(lmv & 0xffu), m = (int)(lmv >> 8);
+        const double dl = (double)l, dm = (double)m;
+        // the (l, -m) outputs are stored FIRST and unconditionally: for m = 0 they land on the
+        // (l, 0) slot and the cos-branch store that follows overwrites them (no branch)
+        const int kc = l * (l + 1) + m;
+        const uint32_t kc_b = (uint32_t)kc * ES, m2_b = (uint32_t)(2 * m) * ES;
+        const uint32_t l8 = (uint32_t)l * 8;
+        double G1 = 0.0, Gz = 0.0, H2 = 0.0, Hxz = 0.0, Hzz = 0.0, sl = 1.0;
+        if constexpr (DERIV >= 1) tq_lds2(sGT + t * 16, G1, Gz);
+        if constexpr (DERIV >= 2) {
+            tq_lds2(sHT + t * 32, H2, Hxz);
+            Hzz = tq_lds16(sHT + t * 32);
+        }
+        if constexpr (CONV) sl = tq_lds(sSL + l * 8);
+        const double dmm = dm * (dm - 1.0);
 #pragma unroll
-            for (int j = 0; j < 2; ++j) {
-                const int pl = plb + j;   // point inside the image
-                const int pb = pbb + j;   // ... inside the batch
-                double x, y, z, ri;
-                tq_lds2(sPT + pb * 32, x, y);
-                tq_lds2(sPT + pb * 32 + 16, z, ri);
-                const uint32_t aQ = sQ + (pb * TP + t) * 8;
-                const uint32_t aC = sCS + (pb * CP + m + 2) * 16;
-                const double Q = tq_lds(aQ);
-                double c0, As;
-                tq_lds2(aC, c0, As);
-                const double Ac = (m == 0) ? SPH_INV_SQRT2 : c0;
-                const uint32_t aS = sS + pl * row_b + kc_b;
+        for (int j = 0; j < 2; ++j) {
+            if (j >= npt) break;
+            const int pl = plb + j;   // point inside the image
+            const int pb = pbb + j;   // ... inside the batch
+            double x, y, z, ri;
+            tq_lds2(sPT + pb * PTB, x, y);
+            tq_lds2(sPT + pb * PTB + 16, z, ri);
+            const uint32_t aQ = sQ + (pb * TP + t) * 8;
+            const uint32_t aC = sCS + (pb * CP + m + 2) * 16;
+            const double Q = CONV ? sl * tq_lds(aQ) : tq_lds(aQ);
+            double c0, As;
+            tq_lds2(aC, c0, As);
+            const double Ac = (m == 0) ? SPH_INV_SQRT2 : c0;
+            const uint32_t aS = sS + pl * row_b + kc_b;
+            if constexpr (MODE == 0) {
                 tq_sts(aS - m2_b, static_cast<T>(Q * As));
                 tq_sts(aS, static_cast<T>(Q * Ac));
-                if constexpr (DERIV >= 1) {
-                    const uint32_t aQ1 = aQ - l8;   // Qt_{l-1}^m; Qt_{l-1}^{m+1} behind it
-                    const double q1 = G1 * tq_lds8(aQ1);   // F_l^m Q_{l-1}^{m+1}
-                    const double qz = Gz * tq_lds(aQ1);    // F_l^m (l+m) Q_{l-1}^m
-                    double c1, s1;
-                    tq_lds2(aC - 16, c1, s1);
-                    // Eq. 10: cos: A_x = m c_{m-1}, A_y = -m s_{m-1}; sin: A_x = m s_{m-1}, A_y = m c_{m-1}
-                    const double mc1 = dm * c1, ms1 = dm * s1;
-                    const double lQ = dl * Q;
-                    const double E1 = NORM ? q1 - lQ : q1;
-                    const double EZ = NORM ? SPH_FMA(-lQ, z, qz) : qz;
-                    const double sg = NORM ? ri : 1.0;
-                    const double E1g = E1 * sg;
-                    const double ax = x * E1g, ay = y * E1g, az = EZ * sg, Qg = Q * sg;
-                    const double Qc = Qg * mc1, Qs_ = Qg * ms1;
-                    const uint32_t aG = sG + pl * 3 * row_b + kc_b;
-                    const uint32_t aGs = aG - m2_b;
-                    tq_sts(aGs, static_cast<T>(SPH_FMA(ax, As, Qs_)));
-                    tq_sts(aGs + row_b, static_cast<T>(SPH_FMA(ay, As, Qc)));
-                    tq_sts(aGs + 2 * row_b, static_cast<T>(az * As));
-                    tq_sts(aG, static_cast<T>(SPH_FMA(ax, Ac, Qc)));
-                    tq_sts(aG + row_b, static_cast<T>(SPH_FMA(ay, Ac, -Qs_)));
-                    tq_sts(aG + 2 * row_b, static_cast<T>(az * Ac));
-                    if constexpr (DERIV >= 2) {
-                        const uint32_t aQ2 = aQ1 - l8 + 8;   // Qt_{l-2}^m, then m+1, m+2
-                        const double q2 = H2 * tq_lds16(aQ2);    // F_l^m Q_{l-2}^{m+2}
-                        const double qxz = Hxz * tq_lds8(aQ2);   // F_l^m (l+m) Q_{l-2}^{m+1}
-                        const double qzz = Hzz * tq_lds(aQ2);    // F_l^m (l+m)(l+m-1) Q_{l-2}^m
-                        double c2, s2;
-                        tq_lds2(aC - 32, c2, s2);
-                        // Eq. 10 twice: cos: A_xx = m(m-1) c_{m-2}, A_xy = -m(m-1) s_{m-2}; sin: s_{m-2}, c_{m-2}
-                        const double mmc2 = dmm * c2, mms2 = dmm * s2;
-                        double F2 = q2, FXZ = qxz, FZZ = qzz;
-                        if (NORM) {
-                            const double w = (dl + 2.0) * lQ;
-                            F2 = SPH_FMA(-2.0 * dl, q1, q2 + w);
-                            FXZ = SPH_FMA(z, SPH_FMA(-dl, q1, w), SPH_FMA(-dl, qz, qxz));
-                            FZZ = SPH_FMA(z, SPH_FMA(w, z, -2.0 * dl * qz), qzz) - lQ;
-                        }
-                        const double sh = NORM ? ri * ri : 1.0;
-                        const double E1h = E1 * sh, F2h = F2 * sh, Qh = Q * sh;
-                        const double cxx = SPH_FMA(x * x, F2h, E1h), cyy = SPH_FMA(y * y, F2h, E1h), cxy = (x * y) * F2h;
-                        const double bx = x * E1h, by = y * E1h, bx2 = bx + bx, by2 = by + by;
-                        const double FXZh = FXZ * sh;
-                        const double cxz = x * FXZh, cyz = y * FXZh, ezh = EZ * sh, czz = FZZ * sh;
-                        const uint32_t aH = sH + pl * 9 * row_b + kc_b;
-                        auto put = [&](uint32_t a, double A, double Ax, double Ay, double Axx, double Axy) {
-                            const double QAxx = Qh * Axx;
-                            const T hxx = static_cast<T>(SPH_FMA(cxx, A, SPH_FMA(bx2, Ax, QAxx)));
-                            const T hyy = static_cast<T>(SPH_FMA(cyy, A, SPH_FMA(by2, Ay, -QAxx)));
-                            const T hxy = static_cast<T>(SPH_FMA(cxy, A, SPH_FMA(bx, Ay, SPH_FMA(by, Ax, Qh * Axy))));
-                            const T hxz = static_cast<T>(SPH_FMA(cxz, A, ezh * Ax));
-                            const T hyz = static_cast<T>(SPH_FMA(cyz, A, ezh * Ay));
-                            const T hzz = static_cast<T>(czz * A);
-                            // rows = xx xy xz yx yy yz zx zy zz (both triangles stored, exactly equal)
-                            tq_sts(a, hxx);
-                            tq_sts(a += row_b, hxy);
-                            tq_sts(a += row_b, hxz);
-                            tq_sts(a += row_b, hxy);
-                            tq_sts(a += row_b, hyy);
-                            tq_sts(a += row_b, hyz);
-                            tq_sts(a += row_b, hxz);
-                            tq_sts(a += row_b, hyz);
-                            tq_sts(a += row_b, hzz);
-                        };
-                        put(aH - m2_b, As, ms1, mc1, mms2, mmc2);
-                        put(aH, Ac, mc1, -ms1, mmc2, -mms2);
-                    }
+            }
+            // the upstream gradient of the two harmonics (contracting modes); 0 for the absent (l, -0)
+            double wc = 0.0, ws = 0.0;
+            if constexpr (MODE != 0) {
+                const int64_t pg = pg0 + j;
+                if (pg < n) {
+                    wc = static_cast<double>(__ldg(gsph + pg * L + kc));
+                    if (m > 0) ws = static_cast<double>(__ldg(gsph + pg * L + kc - 2 * m));
                 }
             }
+            if constexpr (DERIV >= 1) {
+                const uint32_t aQ1 = aQ - l8;   // Qt_{l-1}^m; Qt_{l-1}^{m+1} behind it
+                const double q1 = G1 * tq_lds8(aQ1);   // F_l^m Q_{l-1}^{m+1}
+                const double qz = Gz * tq_lds(aQ1);    // F_l^m (l+m) Q_{l-1}^m
+                double c1, s1;
+                tq_lds2(aC - 16, c1, s1);
+                // Eq. 10: cos: A_x = m c_{m-1}, A_y = -m s_{m-1}; sin: A_x = m s_{m-1}, A_y = m c_{m-1}
+                const double mc1 = dm * c1, ms1 = dm * s1;
+                const double lQ = dl * Q;
+                const double E1 = NORM ? q1 - lQ : q1;
+                const double EZ = NORM ? SPH_FMA(-lQ, z, qz) : qz;
+                const double sg = NORM ? ri : 1.0;
+                const double E1g = E1 * sg;
+                const double ax = x * E1g, ay = y * E1g, az = EZ * sg, Qg = Q * sg;
+                const double Qc = Qg * mc1, Qs_ = Qg * ms1;
+                const double gxs = SPH_FMA(ax, As, Qs_), gys = SPH_FMA(ay, As, Qc), gzs = az * As;
+                const double gxc = SPH_FMA(ax, Ac, Qc), gyc = SPH_FMA(ay, Ac, -Qs_), gzc = az * Ac;
+                if constexpr (MODE == 0) {
+                    const uint32_t aG = sG + pl * 3 * row_b + kc_b;
+                    const uint32_t aGs = aG - m2_b;
+                    tq_sts(aGs + rx, static_cast<T>(gxs));
+                    tq_sts(aGs + ry, static_cast<T>(gys));
+                    tq_sts(aGs + rz, static_cast<T>(gzs));
+                    tq_sts(aG + rx, static_cast<T>(gxc));
+                    tq_sts(aG + ry, static_cast<T>(gyc));
+                    tq_sts(aG + rz, static_cast<T>(gzc));
+                } else if constexpr (MODE == 2) {   // grad_xyz[a] += dY/dx_a * grad_sph, both harmonics
+                    acc[3 * j + 0] = SPH_FMA(gxc, wc, SPH_FMA(gxs, ws, acc[3 * j + 0]));
+                    acc[3 * j + 1] = SPH_FMA(gyc, wc, SPH_FMA(gys, ws, acc[3 * j + 1]));
+                    acc[3 * j + 2] = SPH_FMA(gzc, wc, SPH_FMA(gzs, ws, acc[3 * j + 2]));
+                }
+                if constexpr (DERIV >= 2) {
+                    const uint32_t aQ2 = aQ1 - l8 + 8;   // Qt_{l-2}^m, then m+1, m+2
+                    const double q2 = H2 * tq_lds16(aQ2);    // F_l^m Q_{l-2}^{m+2}
+                    const double qxz = Hxz * tq_lds8(aQ2);   // F_l^m (l+m) Q_{l-2}^{m+1}
+                    const double qzz = Hzz * tq_lds(aQ2);    // F_l^m (l+m)(l+m-1) Q_{l-2}^m
+                    double c2, s2;
+                    tq_lds2(aC - 32, c2, s2);
+                    // Eq. 10 twice: cos: A_xx = m(m-1) c_{m-2}, A_xy = -m(m-1) s_{m-2}; sin: s_{m-2}, c_{m-2}
+                    const double mmc2 = dmm * c2, mms2 = dmm * s2;
+                    double F2 = q2, FXZ = qxz, FZZ = qzz;
+                    if (NORM) {
+                        const double w = (dl + 2.0) * lQ;
+                        F2 = SPH_FMA(-2.0 * dl, q1, q2 + w);
+                        FXZ = SPH_FMA(z, SPH_FMA(-dl, q1, w), SPH_FMA(-dl, qz, qxz));
+                        FZZ = SPH_FMA(z, SPH_FMA(w, z, -2.0 * dl * qz), qzz) - lQ;
+                    }
+                    const double sh = NORM ? ri * ri : 1.0;
+                    const double E1h = E1 * sh, F2h = F2 * sh, Qh = Q * sh;
+                    const double cxx = SPH_FMA(x * x, F2h, E1h), cyy = SPH_FMA(y * y, F2h, E1h), cxy = (x * y) * F2h;
+                    const double bx = x * E1h, by = y * E1h, bx2 = bx + bx, by2 = by + by;
+                    const double FXZh = FXZ * sh;
+                    const double cxz = x * FXZh, cyz = y * FXZh, ezh = EZ * sh, czz = FZZ * sh;
+                    double vx = 0.0, vy = 0.0, vz = 0.0, pad_;
+                    if constexpr (MODE == 1) {
+                        tq_lds2(sPT + pb * PTB + 32, vx, vy);
+                        tq_lds2(sPT + pb * PTB + 48, vz, pad_);
+                    }
+                    // one branch: its six second derivatives, stored (MODE 0) or contracted (MODE 1)
+                    auto branch2 = [&](uint32_t a, double A, double Ax, double Ay, double Axx, double Axy, double wk,
+                                       double gx, double gy, double gz) {
+                        const double QAxx = Qh * Axx;
+                        const double hxx = SPH_FMA(cxx, A, SPH_FMA(bx2, Ax, QAxx));
+                        const double hyy = SPH_FMA(cyy, A, SPH_FMA(by2, Ay, -QAxx));
+                        const double hxy = SPH_FMA(cxy, A, SPH_FMA(bx, Ay, SPH_FMA(by, Ax, Qh * Axy)));
+                        const double hxz = SPH_FMA(cxz, A, ezh * Ax);
+                        const double hyz = SPH_FMA(cyz, A, ezh * Ay);
+                        const double hzz = czz * A;
+                        if constexpr (MODE == 0) {
+                            const T txx = static_cast<T>(hxx), tyy = static_cast<T>(hyy), tzz = static_cast<T>(hzz);
+                            const T txy = static_cast<T>(hxy), txz = static_cast<T>(hxz), tyz = static_cast<T>(hyz);
+                            // row (a, b) of the caller's [3][3] block; both triangles stored, exactly equal
+                            tq_sts(a + 3 * rx + rx, txx);
+                            tq_sts(a + 3 * rx + ry, txy);
+                            tq_sts(a + 3 * rx + rz, txz);
+                            tq_sts(a + 3 * ry + rx, txy);
+                            tq_sts(a + 3 * ry + ry, tyy);
+                            tq_sts(a + 3 * ry + rz, tyz);
+                            tq_sts(a + 3 * rz + rx, txz);
+                            tq_sts(a + 3 * rz + ry, tyz);
+                            tq_sts(a + 3 * rz + rz, tzz);
+                        } else {
+                            // grad_grad_sph[k] = sum_a dY_k/dx_a v_a;  grad_grad_xyz[b] += w_k sum_a d2Y_k/dx_a dx_b v_a
+                            tq_sts(a, static_cast<T>(SPH_FMA(gx, vx, SPH_FMA(gy, vy, gz * vz))));
+                            acc[3 * j + 0] = SPH_FMA(wk, SPH_FMA(hxx, vx, SPH_FMA(hxy, vy, hxz * vz)), acc[3 * j + 0]);
+                            acc[3 * j + 1] = SPH_FMA(wk, SPH_FMA(hxy, vx, SPH_FMA(hyy, vy, hyz * vz)), acc[3 * j + 1]);
+                            acc[3 * j + 2] = SPH_FMA(wk, SPH_FMA(hxz, vx, SPH_FMA(hyz, vy, hzz * vz)), acc[3 * j + 2]);
+                        }
+                    };
+                    const uint32_t aH = (MODE == 0 ? sH + pl * 9 * row_b : aS - kc_b) + kc_b;
+                    branch2(aH - m2_b, As, ms1, mc1, mms2, mmc2, ws, gxs, gys, gzs);
+                    branch2(aH, Ac, mc1, -ms1, mmc2, -mms2, wc, gxc, gyc, gzc);
+                }
+            }
+        }
     };
     // The image's runs (one per output array: np points' rows, contiguous in global memory) leave: the
     // 16-byte-aligned body by TMA, the few elements before and behind it by plain stores.  One thread.
@@ -301,18 +375,19 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
         };
         const uint32_t sb = (uint32_t)np * row_b;
         run(sph + p0 * L, S0, dS, sb);
-        if (DERIV >= 1) run(dsph + p0 * 3 * L, G0, dG, 3u * sb);
-        if (DERIV >= 2) run(ddsph + p0 * 9 * L, H0, dH, 9u * sb);
+        if (MODE == 0 && DERIV >= 1) run(dsph + p0 * 3 * L, G0, dG, 3u * sb);
+        if (MODE == 0 && DERIV >= 2) run(ddsph + p0 * 9 * L, H0, dH, 9u * sb);
         bulk_commit();
     };
     // ragged end of the batch: np (< the image's points) points by plain stores, threads tid of nthr
     auto emit_plain = [&](int64_t p0, int np, const T* S0, const T* G0, const T* H0, int tid, int nthr) {
         for (int i = tid; i < np * L; i += nthr) st_cs(sph + p0 * L + i, S0[i]);
-        if (DERIV >= 1)
+        if (MODE == 0 && DERIV >= 1)
             for (int i = tid; i < np * 3 * L; i += nthr) st_cs(dsph + p0 * 3 * L + i, G0[i]);
-        if (DERIV >= 2)
+        if (MODE == 0 && DERIV >= 2)
             for (int i = tid; i < np * 9 * L; i += nthr) st_cs(ddsph + p0 * 9 * L + i, H0[i]);
     };
+    constexpr bool HAS_IMG = MODE != 2;
 
     int tile_no = 0;   // tiles this CTA has issued: parity picks the image
     for (int bi = 0; bi < prm.batches_per_cta; ++bi) {
@@ -328,9 +403,9 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
             const int64_t p = b0 + pt_l;
             double x = 0.0, y = 0.0, z = 1.0;   // lanes past the end compute a harmless point
             if (p < n) {
-                x = static_cast<double>(__ldg(xyz + 3 * p + 0));
-                y = static_cast<double>(__ldg(xyz + 3 * p + 1));
-                z = static_cast<double>(__ldg(xyz + 3 * p + 2));
+                x = static_cast<double>(__ldg(xyz + 3 * p + (CONV ? prm.src[0] : 0)));
+                y = static_cast<double>(__ldg(xyz + 3 * p + (CONV ? prm.src[1] : 1)));
+                z = static_cast<double>(__ldg(xyz + 3 * p + (CONV ? prm.src[2] : 2)));
             }
             R X, Y, Z, r2;
             double rinv = 1.0;
@@ -344,8 +419,19 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
                 r2 = RT::r2_of(X, Y, Z);
             }
             if (warp == W - 1 && cls == NC - 1) {   // Eq. 9 and the point itself: the lanes with the shortest columns
-                tq_sts2(sPT + pt_l * 32, to_double(X), to_double(Y));
-                tq_sts2(sPT + pt_l * 32 + 16, to_double(Z), rinv);
+                tq_sts2(sPT + pt_l * PTB, to_double(X), to_double(Y));
+                tq_sts2(sPT + pt_l * PTB + 16, to_double(Z), rinv);
+                if constexpr (MODE == 1) {
+                    const T* __restrict__ vv = static_cast<const T*>(prm.vvec);
+                    double vx = 0.0, vy = 0.0, vz = 0.0;
+                    if (p < n) {
+                        vx = static_cast<double>(__ldg(vv + 3 * p + 0));
+                        vy = static_cast<double>(__ldg(vv + 3 * p + 1));
+                        vz = static_cast<double>(__ldg(vv + 3 * p + 2));
+                    }
+                    tq_sts2(sPT + pt_l * PTB + 32, vx, vy);
+                    tq_sts2(sPT + pt_l * PTB + 48, vz, 0.0);
+                }
                 R c = RT::make(1.0, 0.0), s = RT::make(0.0, 0.0);
                 uint32_t a = sCS + (pt_l * CP + 2) * 16;
                 for (int m = 0; m <= l_max; ++m, a += 16) {
@@ -420,7 +506,7 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
         }
         __syncthreads();
 
-        // ---- phase B: lane = (point of the tile, pair) --------------------------------------------
+        // ---- phase B: lane = (point pair of the tile, (l, m) pair) ---------------------------------
         const int n_tiles = B / P;
         for (int ti = 0; ti < n_tiles; ++ti) {
             const int64_t p0 = b0 + (int64_t)ti * P;
@@ -433,17 +519,19 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
             unsigned char* iG = img + lay.reg_g + dG;
             unsigned char* iH = img + lay.reg_h + dH;
             const uint32_t sS = smem_u32(iS), sG = smem_u32(iG), sH = smem_u32(iH);
-            if (prm.n_images == 1 && tile_no > 0) {   // the one image: its last stores must have read it
-                if (threadIdx.x == 0) bulk_wait_read<0>();
+            if ((prm.n_images == 1 || MODE != 0) && tile_no > 0) {
+                // the one image: its last stores must have read it (and, in the contracting modes, the
+                // partial sums of the last tile must have been summed and written out)
+                if (HAS_IMG && threadIdx.x == 0) bulk_wait_read<0>();
                 __syncthreads();
             }
             // work units = (two points of the tile, 32 consecutive pairs of the triangle), dealt to the warps
-            // round-robin; (pl, ch) of this warp's unit advances incrementally (warp-uniform, no division),
-            // so everything that depends on the point only is computed per unit, not per lane
+            // round-robin; (pp, ch) of this warp's unit advances incrementally (warp-uniform, no division)
+            double acc[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
             int pp = w_pl0, ch = w_ch0;   // pp: PAIR of points of the tile (a lane does the same (l, m) for both)
             while (pp < PP) {
                 const int t = ch * 32 + lane;
-                if (t < TT) assemble(t, 2 * pp, ti * P + 2 * pp, sS, sG, sH);
+                if (t < TT) assemble(t, 2 * pp, ti * P + 2 * pp, P - 2 * pp, p0 + 2 * pp, sS, sG, sH, acc);
                 ch += d_ch;
                 pp += d_pl;
                 if (ch >= NCH) {
@@ -451,111 +539,46 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
                     ++pp;
                 }
             }
+            if constexpr (MODE != 0) {
+                // this warp's partial sums (P = 2: the tile is one pair of points): over the lanes, then
+                // into the warp's slot; summed over the warps in a fixed order below (deterministic)
+#pragma unroll
+                for (int q = 0; q < 6; ++q) {
+                    double v = acc[q];
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+                    if (lane == 0) reinterpret_cast<double*>(smem + lay.red_off)[warp * 6 + q] = v;
+                }
+            }
             // this tile's image must be visible to the async proxy; with two images, the other one's
             // stores (issued one tile ago) must have read it before anyone writes there again
-            fence_proxy_async_smem();
-            if (prm.n_images == 2 && threadIdx.x == 0) bulk_wait_read<0>();
+            if (HAS_IMG) fence_proxy_async_smem();
+            if (HAS_IMG && MODE == 0 && prm.n_images == 2 && threadIdx.x == 0) bulk_wait_read<0>();
             __syncthreads();
-            T* S0 = reinterpret_cast<T*>(iS);
-            T* G0 = reinterpret_cast<T*>(iG);
-            T* H0 = reinterpret_cast<T*>(iH);
-            if (n - p0 >= P) {
-                if (threadIdx.x == 0) emit_runs(p0, P, S0, G0, H0, dS, dG, dH);
-            } else {   // ragged last tile: plain stores
-                emit_plain(p0, (int)(n - p0), S0, G0, H0, threadIdx.x, blockDim.x);
-                __syncthreads();   // the image is free again only when every thread has copied its share
+            const T* S0 = reinterpret_cast<const T*>(iS);
+            const T* G0 = reinterpret_cast<const T*>(iG);
+            const T* H0 = reinterpret_cast<const T*>(iH);
+            if constexpr (MODE != 0) {   // the tile's two points: 3 sums each
+                if (threadIdx.x < 6 && p0 + threadIdx.x / 3 < n) {
+                    const double* red = reinterpret_cast<const double*>(smem + lay.red_off);
+                    double sum = 0.0;
+                    for (int w = 0; w < W; ++w) sum += red[w * 6 + threadIdx.x];
+                    gxyz[p0 * 3 + threadIdx.x] = static_cast<T>(sum);
+                }
+            }
+            if (HAS_IMG && (MODE == 0 || sph != nullptr)) {
+                if (n - p0 >= P) {
+                    if (threadIdx.x == 0) emit_runs(p0, P, S0, G0, H0, dS, dG, dH);
+                } else {   // ragged last tile: plain stores
+                    emit_plain(p0, (int)(n - p0), S0, G0, H0, threadIdx.x, blockDim.x);
+                    __syncthreads();   // the image is free again only when every thread has copied its share
+                }
             }
             ++tile_no;
         }
     }
     // shared memory must outlive the bulk stores' reads of it
     if (threadIdx.x == 0) bulk_wait_read<0>();
-}
-
-// ---------------------------------------------------------------------------------------------
-// host side
-// ---------------------------------------------------------------------------------------------
-typedef void (*TqKernel)(const TqParams);
-
-struct TqLaunch {
-    const void* func;
-    TqKernel kern;
-    TqParams prm;
-    int64_t grid;
-    int threads;
-    size_t smem;
-};
-
-template <typename T, typename R> static TqKernel tq_pick(int deriv, int norm) {
-    if (deriv == 0) return norm ? sph_tq_kernel<T, R, 0, true> : sph_tq_kernel<T, R, 0, false>;
-    if (deriv == 1) return norm ? sph_tq_kernel<T, R, 1, true> : sph_tq_kernel<T, R, 1, false>;
-    return norm ? sph_tq_kernel<T, R, 2, true> : sph_tq_kernel<T, R, 2, false>;
-}
-
-// Launch shape: points per phase-A batch B (32, 16), points per tile P (even), warps per CTA W,
-// images per CTA.
-// Returns 0 and fills *out, or 1 when the shape does not fit (rows too long for two full-row
-// images: the warp-per-point kernels take those).
-static inline int tq_plan(int sm_count, int smem_optin, int64_t n, int l_max, int normalized, int dtype, void* sph,
-                          void* dsph, void* ddsph, const void* xyz, const SphTables* d_tab, const unsigned short* d_lm,
-                          const double2* d_ab, TqLaunch* out) {
-    const int deriv = ddsph ? 2 : (dsph ? 1 : 0);
-    const int esize = dtype == 0 ? 4 : 8;
-    const int64_t L = (int64_t)(l_max + 1) * (l_max + 1);
-    const int T = (l_max + 1) * (l_max + 2) / 2;
-    const int budget = smem_optin - 1024;
-    // Measured on B200 over (B, P, W, N) (tq_table.h): small tiles win almost everywhere (more CTAs
-    // per SM, shorter barrier intervals); a lane does two points at a time, so P = 2, or 4 while that
-    // keeps the image small; 32-point batches unless they push a CTA over ~110 KB; one image
-    const int rows = deriv == 0 ? 1 : (deriv == 1 ? 4 : 13);
-    // (the measured table first; the rules behind it serve the cells the table leaves to other kernels
-    // when tq is forced; the tq_* options override both)
-    const unsigned char* shape = TQ_SHAPE[dtype != 0][deriv][l_max];
-    const bool tab = shape[0] != 0;
-    int bB = tab ? shape[0] : 32;
-    int bP = tab ? shape[1] : ((int64_t)4 * rows * L * esize <= 24 * 1024 ? 4 : 2);
-    int bW = tab ? shape[2] : 8;
-    int bN = tab ? shape[3] : 1;
-    if (g_opt.tq_batch > 0) bB = g_opt.tq_batch;
-    if (g_opt.tq_points > 0) bP = g_opt.tq_points;
-    if (g_opt.tq_warps > 0) bW = g_opt.tq_warps;
-    if (g_opt.tq_images > 0) bN = g_opt.tq_images;
-    if (bW < 1 || bW > TQ_MAX_WARPS || bN < 1 || bN > 2) return 1;
-    if (!tab && g_opt.tq_batch <= 0)
-        while (bB > 8 && TqSmem(l_max, deriv, esize, bB, bP, bN).total > 110 * 1024) bB >>= 1;
-    if ((bB != 32 && bB != 16 && bB != 8) || bP > bB || (bP & 1) || bB % bP != 0) return 1;
-    if ((int64_t)TqSmem(l_max, deriv, esize, bB, bP, bN).total > budget) return 1;
-    TqSmem lay(l_max, deriv, esize, bB, bP, bN);
-    out->prm.n_images = bN;
-    out->kern = dtype == 0 ? tq_pick<float, double>(deriv, normalized) : tq_pick<double, dd>(deriv, normalized);
-    out->func = (const void*)out->kern;
-    out->prm.xyz = xyz;
-    out->prm.sph = sph;
-    out->prm.dsph = dsph;
-    out->prm.ddsph = ddsph;
-    out->prm.tab = d_tab;
-    out->prm.lm = d_lm;
-    out->prm.ab_hi = d_ab;
-    out->prm.ab_lo = d_ab + SPH_TRI_SIZE;
-    out->prm.n = n;
-    out->prm.l_max = l_max;
-    out->prm.batch = bB;
-    out->prm.pts_tile = bP;
-    const int64_t n_batches = (n + bB - 1) / bB;
-    // a few batches per CTA amortise the table copy; keep >= ~16 CTAs per SM for the block scheduler
-    int64_t bpc = n_batches / ((int64_t)sm_count * 16);
-    if (bpc > 4) bpc = 4;
-    if (bpc < 1) bpc = 1;
-    out->prm.batches_per_cta = (int)bpc;
-    out->grid = (n_batches + bpc - 1) / bpc;
-    if (out->grid > 0x7fffffff) return 1;
-    out->threads = bW * 32;
-    out->smem = lay.total;
-    return 0;
-}
-
-static inline void tq_launch(const TqLaunch& lw, cudaStream_t stream) {
-    lw.kern<<<(unsigned)lw.grid, lw.threads, lw.smem, stream>>>(lw.prm);
 }
 
 }  // namespace sphb200

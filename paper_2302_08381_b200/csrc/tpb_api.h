@@ -34,4 +34,31 @@ SPH_VJPR_DECL(f64)
 SPH_EXPAND_DECL(f32)
 SPH_EXPAND_DECL(f64)
 #undef SPH_EXPAND_DECL
+// two-phase kernel (tq_inst.cu, compiled once per element type); same return codes
+struct TqArgs {
+    int sm_count, smem_optin;
+    int mode;          // 0 forward, 1 second-order VJP, 2 recompute VJP
+    int deriv;         // mode 0: 0 values, 1 + gradients, 2 + Hessians
+    int normalized;
+    int conv;          // mode 0: another axis / scale convention (src, row, lscale)
+    const void* xyz;
+    void* sph;         // mode 0: sph; mode 1: grad_grad_sph (may be NULL)
+    void* dsph;
+    void* ddsph;
+    const void* gsph;  // modes 1, 2
+    const void* vvec;  // mode 1
+    void* gxyz;        // modes 1, 2
+    int64_t n;
+    int l_max;
+    const SphTables* d_tab;
+    const unsigned short* d_lm;
+    const double2* d_ab;
+    int src[3], row[3];
+    const double* lscale;   // [SPH_MAX_L + 1] or NULL
+    cudaStream_t stream;
+};
+int sph_tq_launch_f32(const TqArgs& a);
+int sph_tq_launch_f64(const TqArgs& a);
+int sph_tq_upload_f32(const SphTables* host_tables);
+int sph_tq_upload_f64(const SphTables* host_tables);
 }  // namespace sphb200

@@ -1,0 +1,111 @@
+// One translation unit per element type of the tq kernels (kernel_tq.cuh), compiled twice by
+// build.py with -DTQ_F64=0|1.  Exports (C++ linkage, declared in tpb_api.h):
+//   sph_tq_upload_<f32|f64>(tables)   copy the coefficient tables into this unit's constant bank
+//   sph_tq_launch_<f32|f64>(args)     pick a launch shape and launch; 1 if no shape fits, -1 CUDA error
+#include "kernel_tq.cuh"
+#include "tpb_api.h"
+
+#ifndef TQ_F64
+#error "compile with -DTQ_F64=0|1"
+#endif
+
+namespace sphb200 {
+
+#if TQ_F64
+typedef double tq_T;
+typedef dd tq_R;
+#define TQ_NAME(f) f##_f64
+#else
+typedef float tq_T;
+typedef double tq_R;
+#define TQ_NAME(f) f##_f32
+#endif
+
+typedef void (*TqKernel)(const TqParams);
+
+template <int MODE, bool CONV> static TqKernel pick(int deriv, int norm) {
+    if constexpr (MODE == 1) return norm ? sph_tq_kernel<tq_T, tq_R, 2, true, 1, false> : sph_tq_kernel<tq_T, tq_R, 2, false, 1, false>;
+    else if constexpr (MODE == 2) return norm ? sph_tq_kernel<tq_T, tq_R, 1, true, 2, false> : sph_tq_kernel<tq_T, tq_R, 1, false, 2, false>;
+    else {
+        if (deriv == 0) return norm ? sph_tq_kernel<tq_T, tq_R, 0, true, 0, CONV> : sph_tq_kernel<tq_T, tq_R, 0, false, 0, CONV>;
+        if (deriv == 1) return norm ? sph_tq_kernel<tq_T, tq_R, 1, true, 0, CONV> : sph_tq_kernel<tq_T, tq_R, 1, false, 0, CONV>;
+        return norm ? sph_tq_kernel<tq_T, tq_R, 2, true, 0, CONV> : sph_tq_kernel<tq_T, tq_R, 2, false, 0, CONV>;
+    }
+}
+
+// Launch shape: points per phase-A batch B (32, 16, 8), points per tile P, warps per CTA W, images
+// per CTA N.  The measured table (tq_table.h) first; the rules behind it serve the cells the table
+// leaves to other kernels when tq is asked for anyway (forced, another convention, the contracting
+// modes); the tq_* options override both.  The shape shrinks (N, then B, then P) until it fits.
+int TQ_NAME(sph_tq_launch)(const TqArgs& a) {
+    const int esize = (int)sizeof(tq_T);
+    const int deriv = a.mode == 1 ? 2 : (a.mode == 2 ? 1 : a.deriv);
+    const int rows = tq_img_rows(a.mode, deriv), ptb = tq_pt_bytes(a.mode);
+    const int64_t L = (int64_t)(a.l_max + 1) * (a.l_max + 1);
+    const int budget = a.smem_optin - 1024;
+    const unsigned char* shape = TQ_SHAPE[TQ_F64][deriv][a.l_max];
+    const bool tab = a.mode == 0 && shape[0] != 0;
+    int bB = tab ? shape[0] : 32;
+    int bP = tab ? shape[1] : ((int64_t)4 * rows * L * esize <= 24 * 1024 ? 4 : 2);
+    int bW = tab ? shape[2] : 8;
+    int bN = tab ? shape[3] : 1;
+    if (a.mode != 0) bP = 2, bN = 1;   // (one pair of points per tile: its sums are the tile's)
+    if (g_opt.tq_batch > 0) bB = g_opt.tq_batch;
+    if (g_opt.tq_points > 0 && a.mode == 0) bP = g_opt.tq_points;
+    if (g_opt.tq_warps > 0) bW = g_opt.tq_warps;
+    if (g_opt.tq_images > 0 && a.mode == 0) bN = g_opt.tq_images;
+    if (bW < 1 || bW > TQ_MAX_WARPS || bN < 1 || bN > 2) return 1;
+    if ((bB != 32 && bB != 16 && bB != 8) || bP > bB || bP < 1 || bB % bP != 0) return 1;
+    auto bytes = [&](int B, int P, int N) { return (int64_t)TqSmem(a.l_max, deriv, rows, ptb, esize, B, P, N).total; };
+    const bool fixed = tab || g_opt.tq_batch > 0 || g_opt.tq_points > 0 || g_opt.tq_images > 0;
+    if (!fixed)
+        while (bB > 8 && bytes(bB, bP, bN) > 110 * 1024) bB >>= 1;
+    while (bytes(bB, bP, bN) > budget) {   // shrink until it fits: images, then the batch, then the tile
+        if (bN == 2) bN = 1;
+        else if (bB > 8 && bB / 2 >= bP) bB >>= 1;
+        else if (bP > 1 && a.mode == 0) bP >>= 1;
+        else return 1;
+    }
+    const TqSmem lay(a.l_max, deriv, rows, ptb, esize, bB, bP, bN);
+
+    TqKernel kern = a.mode == 1 ? pick<1, false>(deriv, a.normalized)
+                  : a.mode == 2 ? pick<2, false>(deriv, a.normalized)
+                  : a.conv ? pick<0, true>(deriv, a.normalized) : pick<0, false>(deriv, a.normalized);
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, a.smem_optin) != cudaSuccess) return -1;
+
+    TqParams prm{};
+    prm.xyz = a.xyz;
+    prm.sph = a.sph;
+    prm.dsph = a.dsph;
+    prm.ddsph = a.ddsph;
+    prm.gsph = a.gsph;
+    prm.vvec = a.vvec;
+    prm.gxyz = a.gxyz;
+    prm.tab = a.d_tab;
+    prm.lm = a.d_lm;
+    prm.ab_hi = a.d_ab;
+    prm.ab_lo = a.d_ab + SPH_TRI_SIZE;
+    prm.n = a.n;
+    prm.l_max = a.l_max;
+    prm.batch = bB;
+    prm.pts_tile = bP;
+    prm.n_images = bN;
+    for (int i = 0; i < 3; ++i) prm.src[i] = a.src[i], prm.row[i] = a.row[i];
+    for (int l = 0; l <= SPH_MAX_L; ++l) prm.lscale[l] = a.lscale ? a.lscale[l] : 1.0;
+    const int64_t n_batches = (a.n + bB - 1) / bB;
+    // a few batches per CTA amortise the table copy; keep >= ~16 CTAs per SM for the block scheduler
+    int64_t bpc = n_batches / ((int64_t)a.sm_count * 16);
+    if (bpc > 4) bpc = 4;
+    if (bpc < 1) bpc = 1;
+    prm.batches_per_cta = (int)bpc;
+    const int64_t grid = (n_batches + bpc - 1) / bpc;
+    if (grid > 0x7fffffff) return 1;
+    kern<<<(unsigned)grid, bW * 32, lay.total, a.stream>>>(prm);
+    return cudaGetLastError() == cudaSuccess ? 0 : -1;
+}
+
+int TQ_NAME(sph_tq_upload)(const SphTables* host_tables) {
+    return cudaMemcpyToSymbol(c_tables_tq, host_tables, sizeof(SphTables)) == cudaSuccess ? 0 : -1;
+}
+
+}  // namespace sphb200

@@ -254,7 +254,7 @@ def test_vjp_recompute_configs(sph, oracle, name, n):
 
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
 def test_vjp_recompute_every_l_max(sph, oracle, dtype):
-    """Specialised kernels (l_max <= 8, f32 <= 12), the generic one above that, l_max = 0, ragged n."""
+    """Specialised kernels (l_max <= 8, f32 <= 12), the two-phase kernel above that, l_max = 0, ragged n."""
     for l_max in (0, 1, 2, 3, 5, 7, 8, 9, 12, 13, 20, 32):
         n = 3 * 16 + 5
         xyz = W.make_xyz("C4" if l_max > 12 else "C2", n).astype(np.float32 if dtype == "f32" else np.float64)
