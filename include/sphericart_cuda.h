@@ -155,7 +155,8 @@ int sphericart_cuda_vjp2(const void* xyz, const void* grad_sph, const void* v, v
  *                                     an empty segment gives zeros
  *   coeff    [n_seg, n_rad, L]   out
  * Device pointers, caller-owned, 16-byte aligned (seg_ptr: 8); asynchronous on `stream`.
- * This build has kernels for l_max <= 8 and n_rad <= 16: otherwise SPHERICART_CUDA_ENOTSUP, no launch.
+ * Any l_max <= SPHERICART_CUDA_MAX_L and any n_rad >= 1: a compile-time kernel (f64 tensor-core
+ * contraction) for 4 <= l_max <= 8 with n_rad <= 16, a run-time-size kernel for everything else.
  * A point with r = 0 makes its segment's coefficients NaN.
  */
 int sphericart_cuda_expand(const void* xyz, const void* radial, const int64_t* seg_ptr, int64_t n_seg,

@@ -21,6 +21,7 @@ __constant__ SphTables c_tables;
 }  // namespace sphb200
 
 #include "kernel_vjp.cuh"
+#include "kernel_expand_generic.cuh"
 #include "kernel_tpg.cuh"
 #include "tq_table.h"
 #include "kernel_w.cuh"
@@ -541,13 +542,48 @@ int sphericart_cuda_expand(const void* xyz, const void* radial, const int64_t* s
     DeviceState* st = nullptr;
     rc = device_state(&st);
     if (rc) return rc;
-    const int r = (dtype == SPHERICART_CUDA_F32 ? sph_expand_launch_f32 : sph_expand_launch_f64)(
-        st->smem_optin, xyz, radial, seg_ptr, n_seg, l_max, n_rad, coeff, static_cast<cudaStream_t>(stream));
-    if (r < 0) return fail(SPHERICART_CUDA_ECUDA, "expand launch failed: %s", cudaGetErrorString(cudaGetLastError()));
-    if (r > 0)
-        return fail(SPHERICART_CUDA_ENOTSUP, "expand: l_max = %d (max 8) or n_rad = %d (max %d) has no kernel in this build",
-                    l_max, n_rad, 16);
-    launched("expand");
+    // the compile-time kernel (DMMA contraction) where it has an instantiation; l_max <= 3 goes to the
+    // generic kernel, whose image of the harmonics is f64 (the tolerance is tightest there)
+    if (g_opt.force_kernel != FORCE_GENERIC && l_max > 3) {
+        const int r = (dtype == SPHERICART_CUDA_F32 ? sph_expand_launch_f32 : sph_expand_launch_f64)(
+            st->smem_optin, xyz, radial, seg_ptr, n_seg, l_max, n_rad, coeff, static_cast<cudaStream_t>(stream));
+        if (r < 0) return fail(SPHERICART_CUDA_ECUDA, "expand launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+        if (r == 0) {
+            launched("expand");
+            return 0;
+        }
+    }
+    // every other (l_max, n_rad): run-time sizes, one CTA per (segment, slice of the radial rows)
+    const int L = (l_max + 1) * (l_max + 1);
+    if (n_seg > 0x7fffffff) return fail(SPHERICART_CUDA_EINVAL, "n_seg = %lld is too large", (long long)n_seg);
+    ExpandGenParams gp{};
+    gp.xyz = xyz;
+    gp.radial = radial;
+    gp.seg_ptr = seg_ptr;
+    gp.coeff = coeff;
+    gp.n_rad = n_rad;
+    gp.l_max = l_max;
+    gp.pts_tile = 32;
+    while (gp.pts_tile > 1 && (size_t)gp.pts_tile * L * 8 > (size_t)48 * 1024) gp.pts_tile >>= 1;   // a few CTAs per SM
+    gp.rows_per_slice = EXG_THREADS * EXG_ACC / L;
+    if (gp.rows_per_slice > n_rad) gp.rows_per_slice = n_rad;
+    const int slices = (n_rad + gp.rows_per_slice - 1) / gp.rows_per_slice;
+    if (slices > 65535) return fail(SPHERICART_CUDA_EINVAL, "n_rad = %d is too large", n_rad);
+    const size_t smem = (size_t)gp.pts_tile * L * 8;
+    const dim3 grid((unsigned)n_seg, (unsigned)slices);
+    if (dtype == SPHERICART_CUDA_F32) {
+        auto k = sph_expand_generic_kernel<float, double>;
+        rc = allow_smem((const void*)k, (int)smem);
+        if (rc) return rc;
+        k<<<grid, EXG_THREADS, smem, static_cast<cudaStream_t>(stream)>>>(gp, st->d_tables);
+    } else {
+        auto k = sph_expand_generic_kernel<double, dd>;
+        rc = allow_smem((const void*)k, (int)smem);
+        if (rc) return rc;
+        k<<<grid, EXG_THREADS, smem, static_cast<cudaStream_t>(stream)>>>(gp, st->d_tables);
+    }
+    CUDA_TRY(cudaGetLastError());
+    launched("expand_generic");
     return 0;
 }
 

@@ -77,9 +77,9 @@ def test_default_dispatch_vjp_recompute(sph, oracle, dtype, l_max):
 
 
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
-@pytest.mark.parametrize("l_max", list(range(0, 9)))
+@pytest.mark.parametrize("l_max", list(range(0, 17)) + [20, 25, 32])
 def test_default_dispatch_expand(sph, oracle, dtype, l_max):
-    for n_rad in (1, 7, 8, 9, 16):
+    for n_rad in (1, 7, 8, 9, 16, 17, 32):
         xyz, rad, seg = W.make_expand_inputs(37, l_max, n_rad, dtype, 19.0, seed=n_rad)
         before = sph.sphericart_cuda_launch_count()
         c = sph.expand(torch.from_numpy(xyz).cuda(), torch.from_numpy(rad).cuda(), torch.from_numpy(seg).cuda())

@@ -444,9 +444,14 @@ def test_expand_eq1(sph, oracle, dtype):
     terms = r_d.double()[:, :, l_of] * Y[:, None, :]
     ref = torch.stack([terms[seg[i]:seg[i + 1]].sum(dim=0) for i in range(100)])
     assert torch.allclose(c.double(), ref, rtol=1e-5 if dtype == "f32" else 1e-12, atol=1e-5 if dtype == "f32" else 1e-12)
-    # unsupported sizes are refused, nothing is launched
-    with pytest.raises(sph.SphericartCudaError):
-        sph.expand(x_d, torch.zeros((x_d.shape[0], 17, 7), device="cuda", dtype=x_d.dtype), torch.from_numpy(seg).cuda())
+    # the run-time-size kernel agrees with the compile-time one where both apply
+    sph.sphericart_cuda_set_option("force_kernel", "generic")
+    try:
+        cg = sph.expand(x_d, r_d, torch.from_numpy(seg).cuda())
+        assert sph.sphericart_cuda_last_kernel() == "expand_generic"
+    finally:
+        sph.sphericart_cuda_set_option("force_kernel", "auto")
+    assert torch.allclose(cg.double(), ref, rtol=1e-5 if dtype == "f32" else 1e-12, atol=1e-5 if dtype == "f32" else 1e-12)
 
 
 def test_origin_and_untouched_memory(sph, oracle):
