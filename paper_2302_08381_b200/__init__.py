@@ -166,6 +166,15 @@ def _dtype_code(t):
     raise TypeError(f"unsupported dtype {t.dtype}: float32 or float64")
 
 
+def _check_out(name, t, shape, like):
+    """An output tensor handed in by the caller: right shape, dtype, device, dense."""
+    if t is None:
+        raise ValueError(f"out: {name} is missing")
+    if tuple(t.shape) != tuple(shape) or t.dtype != like.dtype or t.device != like.device or not t.is_contiguous():
+        raise ValueError(f"out: {name} must be a contiguous {like.dtype} tensor of shape {tuple(shape)} on {like.device}")
+    return t
+
+
 def compute(xyz, l_max: int, normalized: bool = True, gradients: bool = False, hessians: bool = False,
             out=None, axes: int = AXES_STANDARD, scale: int = SCALE_INTEGRAL):
     """``xyz`` [n,3] CUDA tensor -> ``(sph [n,L], dsph [n,3,L] | None, ddsph [n,3,3,L] | None)``.
@@ -179,6 +188,10 @@ def compute(xyz, l_max: int, normalized: bool = True, gradients: bool = False, h
         raise SphericartCudaError("xyz must be a CUDA tensor (no CPU fallback)")
     if hessians and not gradients:
         raise ValueError("hessians need gradients")
+    if xyz.dim() != 2 or xyz.shape[1] != 3:
+        raise ValueError("xyz must have shape [n, 3]")
+    if not 0 <= int(l_max) <= MAX_L:
+        raise SphericartCudaError(f"l_max = {l_max} outside [0, {MAX_L}]")
     xyz = xyz.contiguous()
     n, L = xyz.shape[0], (l_max + 1) ** 2
     if out is None:
@@ -187,6 +200,9 @@ def compute(xyz, l_max: int, normalized: bool = True, gradients: bool = False, h
         ddsph = torch.empty((n, 3, 3, L), dtype=xyz.dtype, device=xyz.device) if hessians else None
     else:
         sph, dsph, ddsph = out
+        _check_out("sph", sph, (n, L), xyz)
+        dsph = _check_out("dsph", dsph, (n, 3, L), xyz) if gradients else None
+        ddsph = _check_out("ddsph", ddsph, (n, 3, 3, L), xyz) if hessians else None
     with torch.cuda.device(xyz.device):
         stream = torch.cuda.current_stream().cuda_stream
         sphericart_cuda_compute_ex(xyz, n, l_max, normalized, _dtype_code(xyz), axes, scale, sph, dsph, ddsph, stream)
@@ -204,7 +220,7 @@ def vjp(dsph, grad_sph, out=None):
     l_max = int(round(L ** 0.5)) - 1
     if (l_max + 1) ** 2 != L or dsph.shape != (n, 3, L) or dsph.dtype != grad_sph.dtype:
         raise ValueError("shapes: dsph [n,3,L], grad_sph [n,L], L a perfect square, same dtype")
-    gx = torch.empty((n, 3), dtype=dsph.dtype, device=dsph.device) if out is None else out
+    gx = torch.empty((n, 3), dtype=dsph.dtype, device=dsph.device) if out is None else _check_out("grad_xyz", out, (n, 3), dsph)
     with torch.cuda.device(dsph.device):
         stream = torch.cuda.current_stream().cuda_stream
         sphericart_cuda_vjp(None, dsph, grad_sph, gx, n, l_max, _dtype_code(dsph), stream)
@@ -223,7 +239,7 @@ def vjp_recompute(xyz, grad_sph, normalized: bool, out=None):
     l_max = int(round(L ** 0.5)) - 1
     if (l_max + 1) ** 2 != L or xyz.shape != (n, 3) or xyz.dtype != grad_sph.dtype:
         raise ValueError("shapes: xyz [n,3], grad_sph [n,L], L a perfect square, same dtype")
-    gx = torch.empty((n, 3), dtype=xyz.dtype, device=xyz.device) if out is None else out
+    gx = torch.empty((n, 3), dtype=xyz.dtype, device=xyz.device) if out is None else _check_out("grad_xyz", out, (n, 3), xyz)
     with torch.cuda.device(xyz.device):
         stream = torch.cuda.current_stream().cuda_stream
         sphericart_cuda_vjp_recompute(xyz, grad_sph, gx, n, l_max, normalized, _dtype_code(xyz), stream)
@@ -262,7 +278,10 @@ def expand(xyz, radial, seg_ptr, out=None):
     if xyz.shape != (n, 3) or xyz.dtype != radial.dtype or seg_ptr.dtype != torch.int64:
         raise ValueError("shapes: xyz [n,3], radial [n,n_rad,l_max+1] of the same dtype, seg_ptr int64")
     n_seg, L = seg_ptr.numel() - 1, lp1 * lp1
-    c = torch.empty((n_seg, n_rad, L), dtype=xyz.dtype, device=xyz.device) if out is None else out
+    if n_seg < 0 or (n_seg >= 0 and seg_ptr.numel() and int(seg_ptr[-1]) != n) or (seg_ptr.numel() and int(seg_ptr[0]) != 0):
+        raise ValueError("seg_ptr must run from 0 to the number of points")
+    c = (torch.empty((n_seg, n_rad, L), dtype=xyz.dtype, device=xyz.device) if out is None
+         else _check_out("coeff", out, (n_seg, n_rad, L), xyz))
     with torch.cuda.device(xyz.device):
         stream = torch.cuda.current_stream().cuda_stream
         sphericart_cuda_expand(xyz, radial, seg_ptr, n_seg, lp1 - 1, n_rad, _dtype_code(xyz), c, stream)
