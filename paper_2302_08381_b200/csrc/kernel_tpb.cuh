@@ -248,6 +248,7 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
                     const double Ax = dm * (sin_branch ? s1 : c1) * sc;
                     const double Ay = dm * (sin_branch ? c1 : -s1) * sc;
                     const double xA = xd * A * sc, yA = yd * A * sc, Az = A * sc;
+                    double y_prev = 0.0;   // Ytilde_{l-1}^m of this branch (Eq. 11 shortcut below)
                     static_for<m, LMAX + 1>([&](auto lc) {
                         constexpr int l = decltype(lc)::value;
                         constexpr int kc = l * (l + 1) + m, ks = l * (l + 1) - m;
@@ -284,12 +285,13 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
                                 H[8 * L + k] = static_cast<T>(o[9]);
                             }
                         } else {
-                            if (emit) S[k] = static_cast<T>(Q * A);
+                            const double Yl = Q * A;
+                            if (emit) S[k] = static_cast<T>(Yl);
                             if constexpr (DERIV >= 1) {
                                 constexpr int t = SPH_TRI(l, m);
                                 double q1 = 0.0, qz = 0.0;
                                 if constexpr (l >= m + 2) q1 = TB.G1[t] * Qn[l - 1];   // F_l^m Q_{l-1}^{m+1}
-                                if constexpr (l >= m + 1) qz = TB.Gz[t] * Qc[l - 1];   // F_l^m (l+m) Q_{l-1}^m
+                                if constexpr (NORM && l >= m + 1) qz = TB.Gz[t] * Qc[l - 1];   // F_l^m (l+m) Q_{l-1}^m
                                 double gx, gy, gz;
                                 if (NORM) {
                                     const double lQ = (double)l * Q;
@@ -301,8 +303,12 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
                                 } else {
                                     gx = SPH_FMA(q1, xA, Q * Ax);
                                     gy = SPH_FMA(q1, yA, Q * Ay);
-                                    gz = qz * Az;
+                                    // Eq. 11 (reading E2): d/dz Ytilde_l^m = (F_l^m / F_{l-1}^m)(l+|m|) Ytilde_{l-1}^m,
+                                    // the ratio being the table Gz: the value of the previous degree, already
+                                    // in a register, times one constant (one multiply less than F (l+m) Q_{l-1}^m A)
+                                    gz = TB.Gz[t] * y_prev;
                                 }
+                                y_prev = Yl;
                                 if (emit) {
                                     G[k] = static_cast<T>(gx);
                                     G[L + k] = static_cast<T>(gy);
