@@ -307,6 +307,53 @@ def sweep_expand(torch, pkg, device, peak):
     return res
 
 
+def sweep_backward(torch, pkg, device, peak):
+    """SURVEY 8(f) N1 / N4 against l_max (f32 and f64, normalised, xyz ~ N(0,1), grad_sph ~ N(0,1)): the
+    training step with stored derivatives (forward V+G, then sphericart_cuda_vjp) beside the one without
+    (forward V, then sphericart_cuda_vjp_recompute), the second-order VJP, and the forward pass in the e3nn
+    'component' convention; us per call and the kernel family that served each."""
+    st = torch.cuda.current_stream().cuda_stream
+    out = {}
+    for dtype, tdt, es in (("f32", torch.float32, 4), ("f64", torch.float64, 8)):
+        dc = pkg.F32 if dtype == "f32" else pkg.F64
+        for l_max in (4, 8, 12, 16, 24, 32):
+            L = (l_max + 1) ** 2
+            n = max(148 * 64, int(min(2_000_000, 0.8e9 // (4 * L * es))) // 256 * 256)
+            x = torch.randn(n, 3, device=device, dtype=tdt)
+            w = torch.randn(n, L, device=device, dtype=tdt)
+            v = torch.randn(n, 3, device=device, dtype=tdt)
+            sph = torch.empty((n, L), device=device, dtype=tdt)
+            dsph = torch.empty((n, 3, L), device=device, dtype=tdt)
+            gx = torch.empty((n, 3), device=device, dtype=tdt)
+            ggs = torch.empty((n, L), device=device, dtype=tdt)
+            calls = {
+                "fwd_vg": lambda i: pkg.sphericart_cuda_compute(x, n, l_max, 1, dc, sph, dsph, None, st),
+                "vjp_stored": lambda i: pkg.sphericart_cuda_vjp(None, dsph, w, gx, n, l_max, dc, st),
+                "fwd_v": lambda i: pkg.sphericart_cuda_compute(x, n, l_max, 1, dc, sph, None, None, st),
+                "vjp_recompute": lambda i: pkg.sphericart_cuda_vjp_recompute(x, w, gx, n, l_max, 1, dc, st),
+                "vjp2": lambda i: pkg.sphericart_cuda_vjp2(x, w, v, gx, ggs, n, l_max, 1, dc, st),
+                "fwd_vg_e3nn_component": lambda i: pkg.sphericart_cuda_compute_ex(x, n, l_max, 1, dc, pkg.AXES_E3NN,
+                                                                                 pkg.SCALE_COMPONENT, sph, dsph, None, st),
+            }
+            row = {"n": n}
+            for key, fn in calls.items():
+                for i in range(2):
+                    fn(i)
+                torch.cuda.synchronize()
+                e0, e1 = time_loop(torch, fn, 5)
+                torch.cuda.synchronize()
+                row[key + "_us"] = round(e0.elapsed_time(e1) / 5 * 1e3, 1)
+                row[key + "_kernel"] = pkg.sphericart_cuda_last_kernel()
+            row["step_stored_us"] = round(row["fwd_vg_us"] + row["vjp_stored_us"], 1)
+            row["step_recompute_us"] = round(row["fwd_v_us"] + row["vjp_recompute_us"], 1)
+            # algorithmic bytes of the recompute VJP: xyz + grad_sph read, grad_xyz written
+            row["vjp_recompute_gbs"] = round(n * (L + 6) * es / (row["vjp_recompute_us"] * 1e-6) / 1e9, 1)
+            row["vjp_stored_gbs"] = round(n * (4 * L + 3) * es / (row["vjp_stored_us"] * 1e-6) / 1e9, 1)
+            out[f"{dtype}_l{l_max}"] = row
+            del x, w, v, sph, dsph, gx, ggs
+    return out
+
+
 LMAX_FULL = (1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12, 13, 14, 15, 16, 20, 24, 28, 32)
 LMAX_BRIEF = (8, 12, 16, 20, 24, 28, 32)       # the cells of the default run (the >= 70 % clause: l_max >= 8)
 
@@ -604,6 +651,7 @@ def run_cuda(args):
                 line["sweep"][name] = sweep_one(c, torch, pkg, device, peak)
             line["sweep"]["N2_expand"] = sweep_expand(torch, pkg, device, peak)
             line["sweep"]["lmax"] = lmax_sweep(torch, pkg, device, peak, LMAX_BRIEF)
+            line["sweep"]["backward"] = sweep_backward(torch, pkg, device, peak)
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()

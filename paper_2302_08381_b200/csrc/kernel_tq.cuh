@@ -101,8 +101,9 @@ struct TqSmem {
         o += deriv >= 2 ? (size_t)T * 32 : 0;
         sl_off = o;                // lscale[l] (CONV)
         o += (size_t)(SPH_MAX_L + 1) * 8 + 8;
-        red_off = o;               // [warps][2 points][3] partial sums of the contracting modes
-        o += 8 * 48;
+        red_off = o;               // [warps][pairs of points of a tile][2][3] partial sums of the contracting modes
+        const bool contracting = img_rows == 0 || pt_bytes == 64;   // (modes 1 and 2)
+        o += contracting ? (size_t)2 * 8 * ((pts_tile + 1) / 2) * 48 : 0;
         lm_off = o;                // l | m << 8
         o += ((size_t)T * 2 + 15) & ~(size_t)15;
         q_off = o;
@@ -220,7 +221,8 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
     // Phase B for ONE (l, m >= 0) pair (triangle index t) and up to TWO points: the points pbb, pbb + 1
     // of the batch (global index pg0, pg0 + 1), staged as points plb, plb + 1 of the image whose
     // regions start at sS / sG / sH.  acc: this lane's partial sums of the contracting modes.
-    auto assemble = [&](int t, int plb, int pbb, int npt, int64_t pg0, uint32_t sS, uint32_t sG, uint32_t sH, double* acc) {
+    // wv: the upstream gradient of the four harmonics {(l,+m), (l,-m)} x {point 0, 1} (contracting modes).
+    auto assemble = [&](int t, int plb, int pbb, int npt, const T* wv, uint32_t sS, uint32_t sG, uint32_t sH, double* acc) {
         // ---- per (l, m): shared by the two points ----
         const unsigned lmv = tq_lds_u16(sLM + t * 2);
         const int l = (int)(lmv & 0xffu), m = (int)(lmv >> 8);
@@ -257,14 +259,10 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
                 tq_sts(aS - m2_b, static_cast<T>(Q * As));
                 tq_sts(aS, static_cast<T>(Q * Ac));
             }
-            // the upstream gradient of the two harmonics (contracting modes); 0 for the absent (l, -0)
             double wc = 0.0, ws = 0.0;
             if constexpr (MODE != 0) {
-                const int64_t pg = pg0 + j;
-                if (pg < n) {
-                    wc = static_cast<double>(__ldg(gsph + pg * L + kc));
-                    if (m > 0) ws = static_cast<double>(__ldg(gsph + pg * L + kc - 2 * m));
-                }
+                wc = static_cast<double>(wv[2 * j]);
+                ws = static_cast<double>(wv[2 * j + 1]);
             }
             if constexpr (DERIV >= 1) {
                 const uint32_t aQ1 = aQ - l8;   // Qt_{l-1}^m; Qt_{l-1}^{m+1} behind it
@@ -358,6 +356,25 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
                     const uint32_t aH = (MODE == 0 ? sH + pl * 9 * row_b : aS - kc_b) + kc_b;
                     branch2(aH - m2_b, As, ms1, mc1, mms2, mmc2, ws, gxs, gys, gzs);
                     branch2(aH, Ac, mc1, -ms1, mmc2, -mms2, wc, gxc, gyc, gzc);
+                }
+            }
+        }
+    };
+    // The upstream gradient of pair t for the points pg0, pg0 + 1 (contracting modes), fetched one unit
+    // ahead of its use so that the global-memory latency hides under the previous unit's arithmetic;
+    // 0 for the absent (l, -0), for points past the end and for lanes past the triangle
+    auto load_w = [&](int t, int npt, int64_t pg0, T* wv) {
+        wv[0] = wv[1] = wv[2] = wv[3] = T(0);
+        if (t < TT) {
+            const unsigned lmv = tq_lds_u16(sLM + t * 2);
+            const int l = (int)(lmv & 0xffu), m = (int)(lmv >> 8);
+            const int kc = l * (l + 1) + m;
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                const int64_t pg = pg0 + j;
+                if (j < npt && pg < n) {
+                    wv[2 * j] = __ldg(gsph + pg * L + kc);
+                    if (m > 0) wv[2 * j + 1] = __ldg(gsph + pg * L + kc - 2 * m);
                 }
             }
         }
@@ -519,50 +536,84 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
             unsigned char* iG = img + lay.reg_g + dG;
             unsigned char* iH = img + lay.reg_h + dH;
             const uint32_t sS = smem_u32(iS), sG = smem_u32(iG), sH = smem_u32(iH);
-            if ((prm.n_images == 1 || MODE != 0) && tile_no > 0) {
-                // the one image: its last stores must have read it (and, in the contracting modes, the
-                // partial sums of the last tile must have been summed and written out)
-                if (HAS_IMG && threadIdx.x == 0) bulk_wait_read<0>();
+            if (HAS_IMG && prm.n_images == 1 && tile_no > 0) {   // the one image: its last stores must have read it
+                if (threadIdx.x == 0) bulk_wait_read<0>();
                 __syncthreads();
             }
             // work units = (two points of the tile, 32 consecutive pairs of the triangle), dealt to the warps
             // round-robin; (pp, ch) of this warp's unit advances incrementally (warp-uniform, no division)
             double acc[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
-            int pp = w_pl0, ch = w_ch0;   // pp: PAIR of points of the tile (a lane does the same (l, m) for both)
-            while (pp < PP) {
-                const int t = ch * 32 + lane;
-                if (t < TT) assemble(t, 2 * pp, ti * P + 2 * pp, P - 2 * pp, p0 + 2 * pp, sS, sG, sH, acc);
-                ch += d_ch;
-                pp += d_pl;
-                if (ch >= NCH) {
-                    ch -= NCH;
-                    ++pp;
-                }
-            }
-            if constexpr (MODE != 0) {
-                // this warp's partial sums (P = 2: the tile is one pair of points): over the lanes, then
-                // into the warp's slot; summed over the warps in a fixed order below (deterministic)
+            // (two sets of slots, alternating by tile: the threads that sum one tile's need no barrier
+            // against the warps that fill the next one's)
+            double* red_set = reinterpret_cast<double*>(smem + lay.red_off) + (tile_no & 1) * (TQ_MAX_WARPS * PP * 6);
+            double* red = red_set + warp * PP * 6;   // this warp's slots
+            // contracting modes: a warp's units visit the pairs of points in ascending order, so its partial
+            // sums of one pair are complete when the pair changes: over the lanes, then into the warp's slot
+            auto flush = [&](int pair) {
 #pragma unroll
                 for (int q = 0; q < 6; ++q) {
                     double v = acc[q];
 #pragma unroll
                     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-                    if (lane == 0) reinterpret_cast<double*>(smem + lay.red_off)[warp * 6 + q] = v;
+                    if (lane == 0) red[pair * 6 + q] = v;
+                    acc[q] = 0.0;
                 }
+            };
+            if constexpr (MODE != 0) {
+                for (int i = lane; i < PP * 6; i += 32) red[i] = 0.0;
+                __syncwarp();
+            }
+            if constexpr (MODE == 0) {
+                int pp = w_pl0, ch = w_ch0;   // pp: PAIR of points of the tile (a lane does the same (l, m) for both)
+                while (pp < PP) {
+                    const int t = ch * 32 + lane;
+                    if (t < TT) assemble(t, 2 * pp, ti * P + 2 * pp, P - 2 * pp, nullptr, sS, sG, sH, acc);
+                    ch += d_ch;
+                    pp += d_pl;
+                    if (ch >= NCH) {
+                        ch -= NCH;
+                        ++pp;
+                    }
+                }
+            } else {
+                // contracting modes: the units are dealt in contiguous ranges instead, so that a warp stays
+                // on one pair of points for as long as possible (a change of pair costs a reduction)
+                const int U = PP * NCH, u0 = warp * U / W, u1 = (warp + 1) * U / W;
+                int pp = u0 / NCH, ch = u0 - pp * NCH, cur = pp;
+                T wn[4];
+                if (u0 < u1) load_w(ch * 32 + lane, P - 2 * pp, p0 + 2 * pp, wn);
+                for (int u = u0; u < u1; ++u) {
+                    if (pp != cur) {
+                        flush(cur);
+                        cur = pp;
+                    }
+                    const T wv[4] = {wn[0], wn[1], wn[2], wn[3]};
+                    const int t = ch * 32 + lane, pp_now = pp;
+                    if (++ch == NCH) {
+                        ch = 0;
+                        ++pp;
+                    }
+                    if (u + 1 < u1) load_w(ch * 32 + lane, P - 2 * pp, p0 + 2 * pp, wn);   // the next unit's
+                    if (t < TT) assemble(t, 2 * pp_now, ti * P + 2 * pp_now, P - 2 * pp_now, wv, sS, sG, sH, acc);
+                }
+                if (u1 > u0) flush(cur);
             }
             // this tile's image must be visible to the async proxy; with two images, the other one's
             // stores (issued one tile ago) must have read it before anyone writes there again
             if (HAS_IMG) fence_proxy_async_smem();
-            if (HAS_IMG && MODE == 0 && prm.n_images == 2 && threadIdx.x == 0) bulk_wait_read<0>();
+            if (HAS_IMG && prm.n_images == 2 && threadIdx.x == 0) bulk_wait_read<0>();
             __syncthreads();
             const T* S0 = reinterpret_cast<const T*>(iS);
             const T* G0 = reinterpret_cast<const T*>(iG);
             const T* H0 = reinterpret_cast<const T*>(iH);
-            if constexpr (MODE != 0) {   // the tile's two points: 3 sums each
-                if (threadIdx.x < 6 && p0 + threadIdx.x / 3 < n) {
-                    const double* red = reinterpret_cast<const double*>(smem + lay.red_off);
+            if constexpr (MODE != 0) {
+                // the tile's points: 3 sums each, over the warps in a fixed order (deterministic)
+                if (threadIdx.x < 3 * P && p0 + threadIdx.x / 3 < n) {
+                    const double* all = red_set;
+                    const int point = threadIdx.x / 3, comp = threadIdx.x - 3 * point;
+                    const int slot = (point >> 1) * 6 + (point & 1) * 3 + comp;
                     double sum = 0.0;
-                    for (int w = 0; w < W; ++w) sum += red[w * 6 + threadIdx.x];
+                    for (int w = 0; w < W; ++w) sum += all[w * PP * 6 + slot];
                     gxyz[p0 * 3 + threadIdx.x] = static_cast<T>(sum);
                 }
             }

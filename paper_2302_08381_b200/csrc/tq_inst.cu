@@ -48,22 +48,24 @@ int TQ_NAME(sph_tq_launch)(const TqArgs& a) {
     int bB = tab ? shape[0] : 32;
     int bP = tab ? shape[1] : ((int64_t)4 * rows * L * esize <= 24 * 1024 ? 4 : 2);
     int bW = tab ? shape[2] : 8;
+    if (!tab && (a.l_max + 1) * (a.l_max + 2) / 2 <= 64) bP = 8, bW = 4;   // short triangles: fewer, fuller warps
     int bN = tab ? shape[3] : 1;
-    if (a.mode != 0) bP = 2, bN = 1;   // (one pair of points per tile: its sums are the tile's)
+    // contracting modes: little or nothing staged: tiles of 16 points (8 pairs x chunks divide evenly among 8 warps)
+    if (a.mode != 0) bP = 16, bN = a.mode == 1 ? 2 : 1, bW = 8, bB = 32;
     if (g_opt.tq_batch > 0) bB = g_opt.tq_batch;
-    if (g_opt.tq_points > 0 && a.mode == 0) bP = g_opt.tq_points;
+    if (g_opt.tq_points > 0) bP = g_opt.tq_points;
     if (g_opt.tq_warps > 0) bW = g_opt.tq_warps;
-    if (g_opt.tq_images > 0 && a.mode == 0) bN = g_opt.tq_images;
+    if (g_opt.tq_images > 0 && a.mode != 2) bN = g_opt.tq_images;
     if (bW < 1 || bW > TQ_MAX_WARPS || bN < 1 || bN > 2) return 1;
     if ((bB != 32 && bB != 16 && bB != 8) || bP > bB || bP < 1 || bB % bP != 0) return 1;
     auto bytes = [&](int B, int P, int N) { return (int64_t)TqSmem(a.l_max, deriv, rows, ptb, esize, B, P, N).total; };
     const bool fixed = tab || g_opt.tq_batch > 0 || g_opt.tq_points > 0 || g_opt.tq_images > 0;
     if (!fixed)
-        while (bB > 8 && bytes(bB, bP, bN) > 110 * 1024) bB >>= 1;
+        while (bB > 8 && bB / 2 >= bP && bytes(bB, bP, bN) > 110 * 1024) bB >>= 1;
     while (bytes(bB, bP, bN) > budget) {   // shrink until it fits: images, then the batch, then the tile
         if (bN == 2) bN = 1;
         else if (bB > 8 && bB / 2 >= bP) bB >>= 1;
-        else if (bP > 1 && a.mode == 0) bP >>= 1;
+        else if (bP > 1) bP >>= 1;
         else return 1;
     }
     const TqSmem lay(a.l_max, deriv, rows, ptb, esize, bB, bP, bN);
