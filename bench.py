@@ -177,6 +177,49 @@ class DeviceWorkload:
             self.backward(i)
 
 
+class OpWorkload:
+    """`--workload custom --op vjp_recompute | vjp2 | expand`: one of the other entry points as the step
+    (the command ncu wraps for their kernels); same interface as DeviceWorkload."""
+
+    def __init__(self, cfg, op, torch, pkg, device):
+        self.cfg, self.op, self.pkg = cfg, op, pkg
+        dt = torch.float32 if cfg.dtype == "f32" else torch.float64
+        self.dcode = pkg.F32 if cfg.dtype == "f32" else pkg.F64
+        self.sets = [None]
+        self.stream = torch.cuda.current_stream().cuda_stream
+        n, L = cfg.n, cfg.n_sph
+        if op == "expand":
+            n_rad, n_seg = 8, max(1, cfg.n // 32)
+            xyz, rad, seg = W.make_expand_inputs(n_seg, cfg.l_max, n_rad, cfg.dtype, 32.0)
+            self.x, self.rad, self.seg = (torch.from_numpy(a).to(device) for a in (xyz, rad, seg))
+            self.n_seg, self.n_rad = n_seg, n_rad
+            self.out = [torch.empty((n_seg, n_rad, L), dtype=dt, device=device) for _ in range(2)]
+            self.points = xyz.shape[0]
+            self.bytes = self.points * (3 + n_rad * (cfg.l_max + 1)) * cfg.itemsize + n_seg * (8 + n_rad * L * cfg.itemsize)
+        else:
+            self.x = torch.randn(n, 3, device=device, dtype=dt)
+            self.w = torch.randn(n, L, device=device, dtype=dt)
+            self.v = torch.randn(n, 3, device=device, dtype=dt)
+            self.gx = torch.empty((n, 3), device=device, dtype=dt)
+            self.ggs = torch.empty((n, L), device=device, dtype=dt)
+            self.points = n
+            # xyz + grad_sph read, grad_xyz written (+ v read, grad_grad_sph written for vjp2)
+            self.bytes = n * ((L + 6) * cfg.itemsize + ((L + 3) * cfg.itemsize if op == "vjp2" else 0))
+
+    def step(self, i):
+        c, p = self.cfg, self.pkg
+        if self.op == "expand":
+            p.sphericart_cuda_expand(self.x, self.rad, self.seg, self.n_seg, c.l_max, self.n_rad, self.dcode,
+                                     self.out[i % 2], self.stream)
+        elif self.op == "vjp2":
+            p.sphericart_cuda_vjp2(self.x, self.w, self.v, self.gx, self.ggs, c.n, c.l_max, c.normalized, self.dcode,
+                                   self.stream)
+        else:
+            p.sphericart_cuda_vjp_recompute(self.x, self.w, self.gx, c.n, c.l_max, c.normalized, self.dcode, self.stream)
+
+    forward = step
+
+
 def time_loop(torch, fn, steps):
     """CUDA events on torch's current stream (the stream the library launches on) around `steps` calls."""
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -561,7 +604,12 @@ def run_cuda(args):
                               "peak_source": peak_src}))
         return
     free, _ = torch.cuda.mem_get_info()
-    wl = DeviceWorkload(cfg, torch, pkg, device, n_sets_for(cfg, free), seed=rank)
+    if args.op != "forward":
+        if args.workload != "custom" or not args.kernels_only:
+            raise SystemExit("--op needs --workload custom --kernels-only")
+        wl = OpWorkload(cfg, args.op, torch, pkg, device)
+    else:
+        wl = DeviceWorkload(cfg, torch, pkg, device, n_sets_for(cfg, free), seed=rank)
 
     def barrier():
         if dist is not None:
@@ -590,6 +638,8 @@ def run_cuda(args):
     # dominant kernel: the forward kernel.  One launch per step for forward-only workloads, so its
     # average duration IS the step time; for C5 the forward launches are timed in a pass of their own.
     fwd_b, vjp_b = algorithmic_bytes_per_point(cfg, cfg.vjp)
+    if args.op != "forward":
+        fwd_b = wl.bytes / cfg.n
     if cfg.vjp:
         f0, f1 = time_loop(torch, wl.forward, args.steps)
         torch.cuda.synchronize()
@@ -713,6 +763,8 @@ def main():
     ap.add_argument("--deriv", type=int, choices=[0, 1, 2], default=1, help="--workload custom: 0 Y, 1 +grad, 2 +Hessian")
     ap.add_argument("--solid", action="store_true", help="--workload custom: solid harmonics instead of normalised")
     ap.add_argument("--n", type=int, default=0, help="--workload custom: points (default: ~1.5 GB of output)")
+    ap.add_argument("--op", choices=["forward", "vjp_recompute", "vjp2", "expand"], default="forward",
+                    help="--workload custom --kernels-only: the entry point the step calls")
     ap.add_argument("--option", action="append", default=[], metavar="NAME=VALUE",
                     help="sphericart_cuda_set_option(NAME, VALUE) before anything runs (experiments)")
     ap.add_argument("--e2e-steps", type=int, default=20)
