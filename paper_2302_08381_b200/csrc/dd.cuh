@@ -142,6 +142,9 @@ SPH_HD dd rec_step(double a_hi, double a_lo, double b_hi, double b_lo, dd Z, dd 
     return quick_two_sum(s.hi, SPH_ADD(s.lo, SPH_SUB(te, ue)));
 }
 
+SPH_HD double rec_step2(double a, double b, double Z, double q, double w) { return rec_step(a, 0.0, b, 0.0, Z, q, w); }
+SPH_HD dd rec_step2(dd a, dd b, dd Z, dd q, dd w) { return rec_step(a.hi, a.lo, b.hi, b.lo, Z, q, w); }
+
 SPH_HD double to_double(double a) { return a; }
 SPH_HD double to_double(dd a) { return a.hi; }
 

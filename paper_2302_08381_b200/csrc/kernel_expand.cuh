@@ -212,7 +212,7 @@ __global__ void __launch_bounds__(128) sph_expand_kernel(const ExpandParams prm)
                         const R a = RT::make(TB.A_hi[t1], TB.A_lo[t1]);
                         R qn;
                         if constexpr (l == m) qn = a * (Z * q);
-                        else qn = a * (Z * q) - RT::make(TB.B_hi[t1], TB.B_lo[t1]) * qp;
+                        else qn = rec_step(TB.A_hi[t1], TB.A_lo[t1], TB.B_hi[t1], TB.B_lo[t1], Z, q, qp);   // (dd.cuh)
                         qp = q;
                         q = qn;
                     }

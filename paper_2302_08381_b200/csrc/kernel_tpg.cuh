@@ -226,7 +226,7 @@ __global__ void __launch_bounds__(128, 4) sph_tpg_kernel(const TpgParams prm) {
                     qn = TB.a(t1) * (Z * q);
                 } else {
                     const R w = NORM ? qp : r2 * qp;
-                    qn = TB.a(t1) * (Z * q) - TB.b(t1) * w;
+                    qn = rec_step2(TB.a(t1), TB.b(t1), Z, q, w);   // (dd.cuh)
                 }
                 qp = q;
                 q = qn;
@@ -238,7 +238,7 @@ __global__ void __launch_bounds__(128, 4) sph_tpg_kernel(const TpgParams prm) {
                         pn = TB.d(m + 1);
                     } else {
                         const R w2 = NORM ? pp : r2 * pp;
-                        pn = TB.a(t + 1) * (Z * pc) - TB.b(t + 1) * w2;   // TRI(l, m + 1) = t + 1
+                        pn = rec_step2(TB.a(t + 1), TB.b(t + 1), Z, pc, w2);   // TRI(l, m + 1) = t + 1
                     }
                     pp = pc;
                     pc = pn;

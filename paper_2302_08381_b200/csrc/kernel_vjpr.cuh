@@ -105,7 +105,7 @@ __global__ void __launch_bounds__(32, 16) sph_vjpr_kernel(const VjprParams prm) 
                     qn = a * (Z * q);
                 } else {
                     const R w = NORM ? qp : r2 * qp;
-                    qn = a * (Z * q) - RT::make(TB.B_hi[t1], TB.B_lo[t1]) * w;
+                    qn = rec_step(TB.A_hi[t1], TB.A_lo[t1], TB.B_hi[t1], TB.B_lo[t1], Z, q, w);   // (dd.cuh)
                 }
                 qp = q;
                 q = qn;

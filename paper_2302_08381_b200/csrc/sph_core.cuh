@@ -165,7 +165,7 @@ SPH_HD R column_step(int l, int m, R Z, R r2, R q, R qp, const SphTables& T) {
     const R a = RT::make(T.A_hi[t], T.A_lo[t]);
     const R b = RT::make(T.B_hi[t], T.B_lo[t]);
     const R w = NORM ? qp : r2 * qp;
-    return a * (Z * q) - b * w;
+    return rec_step(T.A_hi[t], T.A_lo[t], T.B_hi[t], T.B_lo[t], Z, q, w);   // (dd.cuh)
 }
 
 // The same column in the integer-coefficient scaling used by the warp kernel (tables.h):
