@@ -188,12 +188,12 @@ const char* sphericart_cuda_last_kernel(void);
  * Launch options, for test harnesses and experiments only: the defaults are compiled in and
  * nothing on the call path reads the environment.  Process-wide, not synchronised with concurrent
  * calls.  Returns 0, or SPHERICART_CUDA_EINVAL for an unknown name or value.
- *   "force_kernel"      "" | "auto" (default dispatch) | "tpb" | "tq" | "tpg" | "w" | "w1" | "wc" | "generic":
+ *   "force_kernel"      "" | "auto" (default dispatch) | "tpb" | "tq" | "tv" | "tpg" | "w" | "w1" | "wc" | "generic":
  *                       restrict the dispatch to one kernel family where it applies (results are
  *                       the same function; the tests compare every family with the oracle)
  *   "host_chunk_bytes"  bytes per chunk and stream of the _host entry points (default 256 MiB)
  *   "tpg_lp", "w_nbuf", "w_warps", "w_ppw", "wc_min_l", "vjp_warps", "tpb_tiles", "tpb_split",
- *   "pdl", "tq_points", "tq_warps", "tq_batch", "tq_images"  integer launch-shape parameters (0 = the library's own rule)
+ *   "pdl", "tq_points", "tq_warps", "tq_batch", "tq_images", "tq_cs_warps"  integer launch-shape parameters (0 = the library's own rule)
  */
 int sphericart_cuda_set_option(const char* name, const char* value);
 

@@ -208,9 +208,12 @@ static int launch_tq(const DeviceState& st, int mode, int normalized, int dtype,
     a.lscale = conv ? conv->lscale : nullptr;
     a.stream = stream;
     const int r = dtype == SPHERICART_CUDA_F32 ? sph_tq_launch_f32(a) : sph_tq_launch_f64(a);
-    if (r == 0) launched(mode == 0 ? "tq" : (mode == 1 ? "tq_vjp2" : "tq_vjpr"));
+    if (r == 0) launched(mode == 0 ? "tq" : (mode == 1 ? "tq_vjp2" : (mode == 2 ? "tq_vjpr" : "tv")));
     return r;
 }
+
+// where the values-only kernel (kernel_tv.cuh) beats the other families (measured: tq_table.h)
+static bool tv_wins(int dtype, int l_max) { return TV_SHAPE[dtype != 0][l_max][0] != 0; }
 
 static bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
 
@@ -240,6 +243,13 @@ static int compute_device(const void* xyz, int64_t n, int l_max, int normalized,
 
     const int force = g_opt.force_kernel;
     const bool force_w = force == FORCE_W || force == FORCE_W1 || force == FORCE_WC;
+    if (!dsph && (force == FORCE_TV || (force == FORCE_NONE && tv_wins(dtype, l_max)))) {
+        // values only: every Legendre entry straight into the image (kernel_tv.cuh)
+        const int r = launch_tq(*st, 3, normalized, dtype, nullptr, xyz, sph, nullptr, nullptr, nullptr, nullptr, nullptr, n, l_max,
+                                stream);
+        if (r < 0) return fail(SPHERICART_CUDA_ECUDA, "tv launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+        if (r == 0) return 0;
+    }
     if (force == FORCE_TQ || (force == FORCE_NONE && TQ_SHAPE[dtype != 0][ddsph ? 2 : (dsph ? 1 : 0)][l_max][0])) {
         // two-phase kernel: recurrences lane = point, assembly lane = (l, m) pair, small full-row tiles
         const int r = launch_tq(*st, 0, normalized, dtype, nullptr, xyz, sph, dsph, ddsph, nullptr, nullptr, nullptr, n, l_max,
@@ -686,11 +696,11 @@ int sphericart_cuda_set_option(const char* name, const char* value) {
     const IntOpt ints[] = {{"tpg_lp", &g_opt.tpg_lp}, {"w_nbuf", &g_opt.w_nbuf}, {"w_warps", &g_opt.w_warps},
                            {"w_ppw", &g_opt.w_ppw}, {"wc_min_l", &g_opt.wc_min_l}, {"vjp_warps", &g_opt.vjp_warps},
                            {"tpb_tiles", &g_opt.tpb_tiles}, {"tpb_split", &g_opt.tpb_split}, {"pdl", &g_opt.pdl},
-                           {"tq_points", &g_opt.tq_points}, {"tq_warps", &g_opt.tq_warps}, {"tq_batch", &g_opt.tq_batch}, {"tq_images", &g_opt.tq_images}};
+                           {"tq_points", &g_opt.tq_points}, {"tq_warps", &g_opt.tq_warps}, {"tq_batch", &g_opt.tq_batch}, {"tq_images", &g_opt.tq_images}, {"tq_cs_warps", &g_opt.tq_cs_warps}};
     if (!strcmp(name, "force_kernel")) {
         struct { const char* v; int code; } const kinds[] = {
             {"", FORCE_NONE}, {"auto", FORCE_NONE}, {"tpb", FORCE_TPB}, {"tpg", FORCE_TPG}, {"w", FORCE_W},
-            {"w1", FORCE_W1}, {"wc", FORCE_WC}, {"tq", FORCE_TQ}, {"generic", FORCE_GENERIC}};
+            {"w1", FORCE_W1}, {"wc", FORCE_WC}, {"tq", FORCE_TQ}, {"tv", FORCE_TV}, {"generic", FORCE_GENERIC}};
         for (const auto& k : kinds)
             if (!strcmp(value, k.v)) {
                 g_opt.force_kernel = k.code;

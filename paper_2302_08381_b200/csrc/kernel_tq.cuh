@@ -73,6 +73,7 @@ struct TqParams {
     int pts_tile;                // points per image; divides batch
     int batches_per_cta;         // consecutive batches one CTA works through
     int n_images;                // 2: a tile drains while the next is assembled; 1: the longest rows
+    int cs_warps;                // f64 I/O: warps of phase A that run Eq. 9 only (1 or 2; the others run the columns)
     // CONV: the harmonics are evaluated at (x', y', z') = xyz[src[0..2]] and derivative axis a of the
     // evaluation frame is the caller's axis row[a]; every degree-l output is multiplied by lscale[l]
     int src[3], row[3];
@@ -435,23 +436,56 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
                 Z = RT::make(z, 0.0);
                 r2 = RT::r2_of(X, Y, Z);
             }
-            if (warp == W - 1 && cls == NC - 1) {   // Eq. 9 and the point itself: the lanes with the shortest columns
-                tq_sts2(sPT + pt_l * PTB, to_double(X), to_double(Y));
-                tq_sts2(sPT + pt_l * PTB + 16, to_double(Z), rinv);
-                if constexpr (MODE == 1) {
-                    const T* __restrict__ vv = static_cast<const T*>(prm.vvec);
-                    double vx = 0.0, vy = 0.0, vz = 0.0;
-                    if (p < n) {
-                        vx = static_cast<double>(__ldg(vv + 3 * p + 0));
-                        vy = static_cast<double>(__ldg(vv + 3 * p + 1));
-                        vz = static_cast<double>(__ldg(vv + 3 * p + 2));
+            // Eq. 9 and the point itself.  f32 I/O (plain double: 4 operations per power): the lanes
+            // with the shortest columns do it on the side.  f64 I/O (double-double: ~50 per power, against
+            // ~23 per Legendre entry): ONE chain over all m would be the critical path of the whole phase, so
+            // `cs_warps` warps do nothing else, each lane class a SEGMENT of the powers, started from
+            // (x + iy)^(segment start) by squarings (segment length a power of two).
+            constexpr bool DD = sizeof(R) > sizeof(double);
+            const int WC = DD ? prm.cs_warps : 0;          // warps that only run Eq. 9
+            const int Wq = W - WC;                          // warps that run the Legendre columns
+            const bool cs_lane = DD ? warp >= Wq : (warp == W - 1 && cls == NC - 1);
+            if (cs_lane) {
+                const int seg = DD ? (warp - Wq) * NC + cls : 0, nseg = DD ? WC * NC : 1;
+                // segments of h = 2^sq powers, the largest power of two <= ceil((l_max + 1) / nseg); the
+                // last segment takes what is left
+                int h = 1, sq = 0;
+                while (2 * h * nseg <= l_max + nseg) h <<= 1, ++sq;
+                if (seg == 0) {
+                    tq_sts2(sPT + pt_l * PTB, to_double(X), to_double(Y));
+                    tq_sts2(sPT + pt_l * PTB + 16, to_double(Z), rinv);
+                    if constexpr (MODE == 1) {
+                        const T* __restrict__ vv = static_cast<const T*>(prm.vvec);
+                        double vx = 0.0, vy = 0.0, vz = 0.0;
+                        if (p < n) {
+                            vx = static_cast<double>(__ldg(vv + 3 * p + 0));
+                            vy = static_cast<double>(__ldg(vv + 3 * p + 1));
+                            vz = static_cast<double>(__ldg(vv + 3 * p + 2));
+                        }
+                        tq_sts2(sPT + pt_l * PTB + 32, vx, vy);
+                        tq_sts2(sPT + pt_l * PTB + 48, vz, 0.0);
                     }
-                    tq_sts2(sPT + pt_l * PTB + 32, vx, vy);
-                    tq_sts2(sPT + pt_l * PTB + 48, vz, 0.0);
                 }
                 R c = RT::make(1.0, 0.0), s = RT::make(0.0, 0.0);
-                uint32_t a = sCS + (pt_l * CP + 2) * 16;
-                for (int m = 0; m <= l_max; ++m, a += 16) {
+                if (seg > 0) {
+                    R pr = X, pi = Y;                       // (x + iy)^h by squarings ...
+                    for (int i = 0; i < sq; ++i) {
+                        const R prn = pr * pr - pi * pi;
+                        const R pin = (pr * pi) * 2.0;
+                        pr = prn;
+                        pi = pin;
+                    }
+                    c = pr, s = pi;                         // ... to the power seg
+                    for (int i = 1; i < seg; ++i) {
+                        const R cn = c * pr - s * pi;
+                        const R sn = c * pi + s * pr;
+                        c = cn;
+                        s = sn;
+                    }
+                }
+                const int m0 = seg * h, m1 = seg == nseg - 1 ? l_max + 1 : min(m0 + h, l_max + 1);
+                uint32_t a = sCS + (pt_l * CP + 2 + m0) * 16;
+                for (int m = m0; m < m1; ++m, a += 16) {
                     tq_sts2(a, to_double(c), to_double(s));
                     const R cn = X * c - Y * s;
                     const R sn = X * s + Y * c;
@@ -467,7 +501,7 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
             // two independent chains per lane hide its latency.  Coefficients {A, B} come from a packed
             // global table through the read-only path (indexed constant-bank loads were the top stall).
             const uint32_t q_out = sQ + pt_l * TP * 8;
-            const int V = W * NC, v = warp * NC + cls;
+            const int V = Wq * NC, v = warp * NC + cls;   // (the cs warps of the double-double path run no columns)
             auto step = [&](int t, R& q, R& qp) {   // (q, qp) = (Qt_{l-1}^m, Qt_{l-2}^m) -> (Qt_l^m, Qt_{l-1}^m), t = TRI(l, m)
                 const double2 hi = __ldg(prm.ab_hi + t);
                 double2 lo = make_double2(0.0, 0.0);
@@ -479,7 +513,7 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
                 tq_sts(q_out + t * 8, to_double(q));
             };
             if constexpr (sizeof(R) > sizeof(double)) {
-                for (int i = 0; i * V <= l_max; i += 2) {
+                for (int i = 0; warp < Wq && i * V <= l_max; i += 2) {
                     const int ma = i * V + v;
                     if (ma > l_max) continue;
                     int mb = (i + 2) * V - 1 - v;            // > ma; past the triangle: no second column

@@ -1,0 +1,218 @@
+// "tv" forward kernel: VALUES only, any l_max, run-time l_max; built for the cells where the values
+// are bound by the recurrences themselves (f64 I/O: double-double, ~23 operations per Legendre entry
+// for two outputs) and the two-phase kernel's second pass over a scratch costs more than it saves.
+//
+//   lane = (point of the batch, column class), as phase A of kernel_tq.cuh (batches of 32 / 16 / 8
+//   points: 1 / 2 / 4 lanes per point), two columns of the folded Eq. 7 at a time per lane.
+//   Every entry Qt_l^m goes STRAIGHT into the image as the two harmonics (l, +-m) = Qt c_m | Qt s_m
+//   (Eq. 5): no scratch for the triangle, no second phase.
+//   The powers (c_m, s_m) (Eq. 9) of batch i+1 are computed WHILE batch i's columns run: by
+//   dedicated warps in segments for f64 I/O (double-double: ~50 operations per power, see
+//   kernel_tq.cuh), on the side by one lane class for f32 I/O; two sets of them in shared memory.
+//   Image: one row per point, rows a pitch apart that keeps lane = point stores conflict-free and
+//   leaves each row 16 bytes of slack, so that it is staged at the offset its global address has
+//   from a 16-byte boundary; every row leaves as one bulk store (TMA) issued by a thread of its own.
+#pragma once
+#include "kernel_tq.cuh"
+
+namespace sphb200 {
+
+struct TvParams {
+    const void* xyz;
+    void* sph;
+    const double2* ab_hi;   // {A, B}[t] of the folded Eq. 7, high parts (tables.h)
+    const double2* ab_lo;   // ... low parts
+    int64_t n;
+    int l_max;
+    int batch;              // 32, 16 or 8 points
+    int cs_warps;           // f64 I/O: warps that run Eq. 9 only
+    int batches_per_cta;
+};
+
+struct TvSmem {
+    int CP;                 // (c, s) pairs per point and set
+    uint32_t pitch;         // bytes between the rows of the image
+    size_t cs_off, img_off, total;
+    __host__ __device__ TvSmem(int l_max, int esize, int batch) {
+        CP = (l_max + 1) | 1;   // odd pitch: conflict-free lane = point stores
+        const uint32_t L = (uint32_t)(l_max + 1) * (l_max + 1);
+        // row + 16 bytes of slack, rounded up to 16, then to an odd number of 16-byte units: lanes of
+        // one class (consecutive points) then fall into different banks for 4- and 8-byte elements alike
+        uint32_t units = (L * esize + 16 + 15) / 16;
+        units |= 1;
+        pitch = units * 16;
+        cs_off = 0;
+        img_off = ((size_t)2 * batch * CP * 16 + 127) & ~(size_t)127;
+        total = img_off + (size_t)batch * pitch;
+    }
+};
+
+template <typename T, typename R, bool NORM>
+__global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tv_kernel(const TvParams prm) {
+    using RT = rec<R>;
+    constexpr int ES = (int)sizeof(T);
+    constexpr bool DD = sizeof(R) > sizeof(double);
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, W = blockDim.x >> 5;
+    const int l_max = prm.l_max, L = (l_max + 1) * (l_max + 1), B = prm.batch;
+    const TvSmem lay(l_max, ES, B);
+    const int CP = lay.CP;
+    const uint32_t s0 = smem_u32(smem), sCS = s0 + (uint32_t)lay.cs_off, sIMG = s0 + (uint32_t)lay.img_off;
+    const int64_t n = prm.n;
+    const T* __restrict__ xyz = static_cast<const T*>(prm.xyz);
+    T* __restrict__ sph = static_cast<T*>(prm.sph);
+    const SphTables& TB = c_tables_tq;
+    const uint64_t policy = policy_evict_first();
+    const int pt_l = lane & (B - 1), cls = lane / B, NC = 32 / B;
+    const int WC = DD ? prm.cs_warps : 0, Wq = W - WC;
+    const bool cs_lane = DD ? warp >= Wq : (warp == W - 1 && cls == NC - 1);
+    const bool col_lane = warp < Wq;
+    const int V = Wq * NC, v = warp * NC + cls;
+    const uint32_t row_b = (uint32_t)L * ES;
+
+    // the point of this lane in batch b0 (lanes past the end: a harmless point)
+    auto load_point = [&](int64_t b0, R& X, R& Y, R& Z, R& r2) {
+        const int64_t p = b0 + pt_l;
+        double x = 0.0, y = 0.0, z = 1.0;
+        if (p < n) {
+            x = static_cast<double>(__ldg(xyz + 3 * p + 0));
+            y = static_cast<double>(__ldg(xyz + 3 * p + 1));
+            z = static_cast<double>(__ldg(xyz + 3 * p + 2));
+        }
+        if (NORM) {
+            double rinv;
+            RT::normalize(x, y, z, X, Y, Z, rinv);
+            r2 = RT::make(1.0, 0.0);
+        } else {
+            X = RT::make(x, 0.0), Y = RT::make(y, 0.0), Z = RT::make(z, 0.0);
+            r2 = RT::r2_of(X, Y, Z);
+        }
+    };
+    // Eq. 9 for batch b0 into set `set`: this lane's segment of the powers (kernel_tq.cuh, phase A)
+    auto powers = [&](int64_t b0, int set) {
+        if (b0 >= n) return;
+        R X, Y, Z, r2;
+        load_point(b0, X, Y, Z, r2);
+        const int seg = DD ? (warp - Wq) * NC + cls : 0, nseg = DD ? WC * NC : 1;
+        // segments of h = 2^sq powers, the largest power of two <= ceil((l_max + 1) / nseg); the last
+        // segment takes what is left
+        int h = 1, sq = 0;
+        while (2 * h * nseg <= l_max + nseg) h <<= 1, ++sq;
+        R c = RT::make(1.0, 0.0), s = RT::make(0.0, 0.0);
+        if (seg > 0) {
+            R pr = X, pi = Y;
+            for (int i = 0; i < sq; ++i) {
+                const R prn = pr * pr - pi * pi;
+                const R pin = (pr * pi) * 2.0;
+                pr = prn, pi = pin;
+            }
+            c = pr, s = pi;
+            for (int i = 1; i < seg; ++i) {
+                const R cn = c * pr - s * pi;
+                const R sn = c * pi + s * pr;
+                c = cn, s = sn;
+            }
+        }
+        const int m0 = seg * h, m1 = seg == nseg - 1 ? l_max + 1 : min(m0 + h, l_max + 1);
+        uint32_t a = sCS + ((set * B + pt_l) * CP + m0) * 16;
+        for (int m = m0; m < m1; ++m, a += 16) {
+            // (the m = 0 slot holds the factor of Eq. 5 for m = 0, 1/sqrt2, instead of c_0 = 1)
+            tq_sts2(a, m == 0 ? SPH_INV_SQRT2 : to_double(c), to_double(s));
+            const R cn = X * c - Y * s;
+            const R sn = X * s + Y * c;
+            c = cn, s = sn;
+        }
+    };
+
+    const int64_t b_first = (int64_t)blockIdx.x * prm.batches_per_cta * B;
+    if (b_first >= n) return;
+    if (cs_lane) powers(b_first, 0);
+    __syncthreads();
+
+    for (int bi = 0; bi < prm.batches_per_cta; ++bi) {
+        const int64_t b0 = b_first + (int64_t)bi * B;
+        if (b0 >= n) break;
+        const int set = bi & 1;
+        if (cs_lane && bi + 1 < prm.batches_per_cta) powers(b0 + B, set ^ 1);   // the next batch's, meanwhile
+        if (col_lane) {
+            R X, Y, Z, r2;
+            load_point(b0, X, Y, Z, r2);
+            // this point's row, staged at the offset its global address has from a 16-byte boundary
+            const uint32_t shift = (uint32_t)(((b0 + pt_l) & 15) * row_b) & 15u;
+            const uint32_t row = sIMG + pt_l * lay.pitch + shift;
+            const uint32_t cs_row = sCS + ((set * B + pt_l) * CP) * 16;
+            // one entry of column m at row l: the harmonics (l, +m) and (l, -m); the sin one first, so that
+            // for m = 0 (s_0 = 0, same slot) the cos store that follows overwrites it
+            auto emit = [&](R q, double Ac, double As, uint32_t ac, uint32_t as) {
+                const double Q = to_double(q);
+                tq_sts(as, static_cast<T>(Q * As));
+                tq_sts(ac, static_cast<T>(Q * Ac));
+            };
+            auto step = [&](int t, R& q, R& qp) {
+                const double2 hi = __ldg(prm.ab_hi + t);
+                double2 lo = make_double2(0.0, 0.0);
+                if constexpr (DD) lo = __ldg(prm.ab_lo + t);
+                const R w = NORM ? qp : r2 * qp;
+                const R qn = rec_step(hi.x, lo.x, hi.y, lo.y, Z, q, w);
+                qp = q;
+                q = qn;
+            };
+            for (int i = 0; i * V <= l_max; i += 2) {
+                const int ma = i * V + v;
+                if (ma > l_max) continue;
+                int mb = (i + 2) * V - 1 - v;            // > ma; past the triangle: no second column
+                if (mb > l_max) mb = 0x7fff;
+                double Aca, Asa, Acb = 0.0, Asb = 0.0;
+                tq_lds2(cs_row + ma * 16, Aca, Asa);
+                if (mb <= l_max) tq_lds2(cs_row + mb * 16, Acb, Asb);
+                int ta = SPH_TRI(ma, ma), tb = 0;
+                R qa = RT::make(TB.D_hi[ma], TB.D_lo[ma]), qpa = RT::make(0.0, 0.0);
+                R qb = RT::make(0.0, 0.0), qpb = RT::make(0.0, 0.0);
+                // byte addresses of (l, +m) and (l, -m) in the row; from row l to l + 1 both move by 2 (l + 1) elements
+                uint32_t aca = row + (uint32_t)(ma * (ma + 1) + ma) * ES, asa = row + (uint32_t)(ma * (ma + 1) - ma) * ES;
+                uint32_t acb = 0, asb = 0;
+                emit(qa, Aca, Asa, aca, asa);
+                for (int l = ma + 1; l <= l_max; ++l) {
+                    ta += l;   // SPH_TRI(l, m) - SPH_TRI(l-1, m) = l
+                    step(ta, qa, qpa);
+                    aca += 2u * l * ES, asa += 2u * l * ES;
+                    emit(qa, Aca, Asa, aca, asa);
+                    if (l == mb) {
+                        tb = SPH_TRI(mb, mb);
+                        qb = RT::make(TB.D_hi[mb], TB.D_lo[mb]);
+                        acb = row + (uint32_t)(mb * (mb + 1) + mb) * ES, asb = row + (uint32_t)(mb * (mb + 1) - mb) * ES;
+                        emit(qb, Acb, Asb, acb, asb);
+                    } else if (l > mb) {
+                        tb += l;
+                        step(tb, qb, qpb);
+                        acb += 2u * l * ES, asb += 2u * l * ES;
+                        emit(qb, Acb, Asb, acb, asb);
+                    }
+                }
+            }
+        }
+        fence_proxy_async_smem();
+        __syncthreads();   // the image is complete; so are the next batch's powers
+        if (threadIdx.x < B) {
+            const int64_t p = b0 + threadIdx.x;
+            if (p < n) {
+                const uint32_t d = (uint32_t)((p & 15) * row_b) & 15u;
+                const T* src = reinterpret_cast<const T*>(smem + lay.img_off + threadIdx.x * lay.pitch + d);
+                T* g = sph + p * L;
+                uint32_t head = (16u - d) & 15u;
+                if (head > row_b) head = row_b;
+                const uint32_t body = (row_b - head) & ~15u;
+                for (uint32_t i = 0; i < head / ES; ++i) st_cs(g + i, src[i]);
+                if (body) bulk_store_hint(g + head / ES, src + head / ES, body, policy);
+                for (uint32_t i = (head + body) / ES; i < row_b / ES; ++i) st_cs(g + i, src[i]);
+                bulk_commit();
+                bulk_wait_read<0>();   // the row has been read: the image may be overwritten
+            }
+        }
+        __syncthreads();
+        // (two images, so that a batch drains while the next is computed, were measured: slower everywhere --
+        // the shared memory they take costs more resident CTAs than the second barrier costs time)
+    }
+}
+
+}  // namespace sphb200

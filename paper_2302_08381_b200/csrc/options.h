@@ -14,6 +14,7 @@ enum ForceKernel {
     FORCE_W1,         // one-warp-per-point kernel even for the longest rows
     FORCE_WC,         // CTA-cooperative kernel wherever it can run (l_max >= 19)
     FORCE_TQ,         // two-phase kernel (kernel_tq.cuh) wherever it can run
+    FORCE_TV,         // values-only kernel (kernel_tv.cuh) wherever it can run
     FORCE_GENERIC,    // recompute VJP / expansion: the run-time-l_max kernels
 };
 
@@ -31,6 +32,7 @@ struct SphOptions {
     int tq_points = 0;       // points per tile of the tq kernel (0: the planner's choice)
     int tq_warps = 0;        // warps per CTA of the tq kernel (0: the planner's choice)
     int tq_images = 0;       // staging images per CTA of the tq kernel (0: two unless only one fits)
+    int tq_cs_warps = 0;     // f64 I/O: warps of the tq kernel's recurrence phase that run Eq. 9 only (0: balanced by the planner)
     int tq_batch = 0;        // points per phase-A batch of the tq kernel (0: the planner's choice)
     int64_t host_chunk_bytes = (int64_t)256 << 20;   // _host entry points: bytes per chunk and stream
 };

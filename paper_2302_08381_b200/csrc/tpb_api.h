@@ -37,7 +37,7 @@ SPH_EXPAND_DECL(f64)
 // two-phase kernel (tq_inst.cu, compiled once per element type); same return codes
 struct TqArgs {
     int sm_count, smem_optin;
-    int mode;          // 0 forward, 1 second-order VJP, 2 recompute VJP
+    int mode;          // 0 forward, 1 second-order VJP, 2 recompute VJP, 3 forward values only (kernel_tv.cuh)
     int deriv;         // mode 0: 0 values, 1 + gradients, 2 + Hessians
     int normalized;
     int conv;          // mode 0: another axis / scale convention (src, row, lscale)

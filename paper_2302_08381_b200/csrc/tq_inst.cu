@@ -2,7 +2,7 @@
 // build.py with -DTQ_F64=0|1.  Exports (C++ linkage, declared in tpb_api.h):
 //   sph_tq_upload_<f32|f64>(tables)   copy the coefficient tables into this unit's constant bank
 //   sph_tq_launch_<f32|f64>(args)     pick a launch shape and launch; 1 if no shape fits, -1 CUDA error
-#include "kernel_tq.cuh"
+#include "kernel_tv.cuh"
 #include "tpb_api.h"
 
 #ifndef TQ_F64
@@ -37,7 +37,57 @@ template <int MODE, bool CONV> static TqKernel pick(int deriv, int norm) {
 // per CTA N.  The measured table (tq_table.h) first; the rules behind it serve the cells the table
 // leaves to other kernels when tq is asked for anyway (forced, another convention, the contracting
 // modes); the tq_* options override both.  The shape shrinks (N, then B, then P) until it fits.
+// values-only kernel (kernel_tv.cuh): the largest batch that leaves room for two CTAs per SM (or fits at all)
+static int tv_launch(const TqArgs& a) {
+    const int esize = (int)sizeof(tq_T);
+    const int budget = a.smem_optin - 1024;
+    const unsigned char* shape = TV_SHAPE[TQ_F64][a.l_max];   // the measured table first (tq_table.h)
+    int bB = g_opt.tq_batch > 0 ? g_opt.tq_batch : (shape[0] ? shape[0] : 32);
+    if (g_opt.tq_batch <= 0 && !shape[0])
+        while (bB > 8 && (int64_t)TvSmem(a.l_max, esize, bB).total > 100 * 1024) bB >>= 1;
+    while (bB > 8 && (int64_t)TvSmem(a.l_max, esize, bB).total > budget) bB >>= 1;
+    if ((bB != 32 && bB != 16 && bB != 8) || (int64_t)TvSmem(a.l_max, esize, bB).total > budget) return 1;
+    const TvSmem lay(a.l_max, esize, bB);
+    const int bW = g_opt.tq_warps > 0 && g_opt.tq_warps <= TQ_MAX_WARPS ? g_opt.tq_warps : (shape[0] ? shape[1] : 8);
+    auto kern = a.normalized ? sph_tv_kernel<tq_T, tq_R, true> : sph_tv_kernel<tq_T, tq_R, false>;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, a.smem_optin) != cudaSuccess) return -1;
+    TvParams prm{};
+    prm.xyz = a.xyz;
+    prm.sph = a.sph;
+    prm.ab_hi = a.d_ab;
+    prm.ab_lo = a.d_ab + SPH_TRI_SIZE;
+    prm.n = a.n;
+    prm.l_max = a.l_max;
+    prm.batch = bB;
+    {   // f64 I/O: warps for Eq. 9 alone, balanced against the column warps (as for the two-phase kernel)
+        const int NC = 32 / bB, T = (a.l_max + 1) * (a.l_max + 2) / 2;
+        int best = 1;
+        double best_t = 1e30;
+        for (int wc = 1; wc <= 2 && wc < bW; ++wc) {
+            const int nseg = wc * NC;
+            int h = 1, sq = 0;
+            while (2 * h * nseg <= a.l_max + nseg) h <<= 1, ++sq;
+            const int last = a.l_max + 1 - (nseg - 1) * h;   // the last segment's length
+            const double t_cs = 50.0 * (last > h ? last : h) + (nseg > 1 ? 40.0 * sq + 50.0 * (nseg - 2) : 0.0);
+            const double t_col = 25.0 * T / ((bW - wc) * NC);
+            const double t = t_cs > t_col ? t_cs : t_col;
+            if (t < best_t) best_t = t, best = wc;
+        }
+        prm.cs_warps = g_opt.tq_cs_warps > 0 && g_opt.tq_cs_warps < bW ? g_opt.tq_cs_warps : (shape[0] ? shape[2] : best);
+    }
+    const int64_t n_batches = (a.n + bB - 1) / bB;
+    int64_t bpc = n_batches / ((int64_t)a.sm_count * 16);   // several batches per CTA: the powers run one batch ahead
+    if (bpc > 8) bpc = 8;
+    if (bpc < 1) bpc = 1;
+    prm.batches_per_cta = (int)bpc;
+    const int64_t grid = (n_batches + bpc - 1) / bpc;
+    if (grid > 0x7fffffff) return 1;
+    kern<<<(unsigned)grid, bW * 32, lay.total, a.stream>>>(prm);
+    return cudaGetLastError() == cudaSuccess ? 0 : -1;
+}
+
 int TQ_NAME(sph_tq_launch)(const TqArgs& a) {
+    if (a.mode == 3) return tv_launch(a);
     const int esize = (int)sizeof(tq_T);
     const int deriv = a.mode == 1 ? 2 : (a.mode == 2 ? 1 : a.deriv);
     const int rows = tq_img_rows(a.mode, deriv), ptb = tq_pt_bytes(a.mode);
@@ -92,6 +142,23 @@ int TQ_NAME(sph_tq_launch)(const TqArgs& a) {
     prm.batch = bB;
     prm.pts_tile = bP;
     prm.n_images = bN;
+    {   // f64 I/O: one or two warps for Eq. 9 alone, whichever balances them against the column warps
+        // (per lane: ~50 operations per power + ~40 per squaring against ~23 per Legendre entry)
+        const int NC = 32 / bB, T = (a.l_max + 1) * (a.l_max + 2) / 2;
+        int best = 1;
+        double best_t = 1e30;
+        for (int wc = 1; wc <= 2 && wc < bW; ++wc) {
+            const int nseg = wc * NC;
+            int h = 1, sq = 0;
+            while (2 * h * nseg <= a.l_max + nseg) h <<= 1, ++sq;
+            const int last = a.l_max + 1 - (nseg - 1) * h;   // the last segment's length
+            const double t_cs = 50.0 * (last > h ? last : h) + (nseg > 1 ? 40.0 * sq + 50.0 * (nseg - 2) : 0.0);
+            const double t_col = 23.0 * T / ((bW - wc) * NC);
+            const double t = t_cs > t_col ? t_cs : t_col;
+            if (t < best_t) best_t = t, best = wc;
+        }
+        prm.cs_warps = g_opt.tq_cs_warps > 0 && g_opt.tq_cs_warps < bW ? g_opt.tq_cs_warps : best;
+    }
     for (int i = 0; i < 3; ++i) prm.src[i] = a.src[i], prm.row[i] = a.row[i];
     for (int l = 0; l <= SPH_MAX_L; ++l) prm.lscale[l] = a.lscale ? a.lscale[l] : 1.0;
     const int64_t n_batches = (a.n + bB - 1) / bB;

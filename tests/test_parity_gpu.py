@@ -389,6 +389,36 @@ def test_two_phase_kernel_shapes(sph, oracle, dtype, shape, option):
                      f"{sph.sphericart_cuda_last_kernel()} shape={shape} {dtype} l_max={l_max} n={n} norm={normalized} deriv={deriv}")
 
 
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("l_max", [0, 1, 2, 3, 4, 7, 8, 11, 12, 15, 16, 19, 24, 25, 31, 32])
+def test_values_only_kernel(sph, oracle, dtype, l_max, option):
+    """kernel_tv.cuh (values only: every Legendre entry straight into a per-point image row, the powers
+    of x + iy one batch ahead): forced, both variants, every batch size, ragged n, n below one batch;
+    C2-style points (on the z axis, tiny r) up to l_max = 16."""
+    np_dt = np.float32 if dtype == "f32" else np.float64
+    option("force_kernel", "tv")
+    for batch in (0, 32, 16, 8):
+        option("tq_batch", batch)
+        for n in (5 * 32 + 100 + 7, 3):
+            xyz = W.make_xyz("C2" if l_max <= 16 else "C4", n, seed=l_max).astype(np_dt)
+            for normalized in (True, False):
+                before = sph.sphericart_cuda_launch_count()
+                s, _, _ = _run_gpu(sph, xyz, l_max, normalized, False, False)
+                assert sph.sphericart_cuda_launch_count() == before + 1
+                assert sph.sphericart_cuda_last_kernel() == "tv"
+                _compare(oracle, xyz, l_max, normalized, dtype, s, None, None,
+                         f"tv {dtype} l_max={l_max} n={n} batch={batch} norm={normalized}")
+    # guard bands: the rows are written exactly where they belong
+    n, L = 77, (l_max + 1) ** 2
+    t_dt = torch.float32 if dtype == "f32" else torch.float64
+    pts = torch.from_numpy(W.make_xyz("C4", n).astype(np_dt)).cuda()
+    buf = torch.full((n * L + 64,), 777.0, device="cuda", dtype=t_dt)
+    sph.sphericart_cuda_compute(pts, n, l_max, 1, 0 if dtype == "f32" else 1, buf[32:-32], None, None,
+                                torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert torch.all(buf[:32] == 777.0) and torch.all(buf[-32:] == 777.0) and torch.all(buf[32:-32] != 777.0)
+
+
 def test_stream_order_with_programmatic_dependent_launch(sph):
     """The small-grid kernels are launched as programmatic dependent launches: their CTAs may become
     resident while the previous kernel in the stream still runs, but must not read or write
