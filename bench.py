@@ -452,6 +452,25 @@ def lmax_sweep(torch, pkg, device, peak, l_values=LMAX_FULL):
     return rows
 
 
+def render_lmax_table(path):
+    """`--render-lmax-table FILE`: the markdown table of DESIGN.md / BASELINE.md from a stored `--lmax-sweep`
+    JSON (profiles/lmax_sweep_r2.json): output GB/s and the kernel family per cell."""
+    d = json.loads(Path(path).read_text())
+    rows, peak = d["lmax_sweep"], d["peak_gbs"]
+    names = {"f32_values": "f32 values", "f32_grads": "f32 grads", "f32_hessians": "f32 hessians",
+             "f64_values": "f64 values", "f64_grads": "f64 grads", "f64_hessians": "f64 hessians"}
+    ls = list(rows["f32_values"].keys())
+    out = ["| variant \\ l_max | " + " | ".join(ls) + " |", "|---" * (len(ls) + 1) + "|"]
+    for key, name in names.items():
+        out.append(f"| {name} | " + " | ".join(f"{rows[key][l]['out_gbs']:.0f} {rows[key][l]['kernel']}" for l in ls) + " |")
+    sm = rows["summary"]
+    out.append("")
+    out.append(f"Measured copy peak {peak:.0f} GB/s; cells with l_max >= 8: {sm['cells_lmax_ge_8']}, of which at or above 0.70 of "
+               f"that peak ({0.7 * peak:.0f} GB/s): {sm['cells_at_or_above_0.70_of_measured_peak']}; slowest: "
+               f"{sm['min_out_gbs_lmax_ge_8']:.0f} GB/s.")
+    print("\n".join(out))
+
+
 def time_e2e(cfg, torch, pkg, steps):
     """The same metric through the host-buffer C-ABI call: pinned host arrays in, pinned host arrays
     out, H2D + kernels + D2H inside the timed region (wall clock around a synchronous call)."""
@@ -771,9 +790,13 @@ def main():
     ap.add_argument("--no-sweep", action="store_true", help="skip the brief timing of the other configurations")
     ap.add_argument("--lmax-sweep", action="store_true",
                     help="print output GB/s against l_max (f32/f64, +-gradients) as one JSON object and exit")
+    ap.add_argument("--render-lmax-table", metavar="FILE", default=None,
+                    help="print the markdown table of a stored --lmax-sweep JSON (no GPU needed) and exit")
     ap.add_argument("--kernels-only", action="store_true",
                     help="time the device-resident step only (no e2e, no oracle, no sweep): the command ncu wraps")
     args = ap.parse_args()
+    if args.render_lmax_table:
+        return render_lmax_table(args.render_lmax_table)
     if args.impl == "reference":
         args.steps = 20 if args.steps is None else args.steps
         args.warmup = 1 if args.warmup is None else args.warmup
