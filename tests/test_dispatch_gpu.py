@@ -87,3 +87,55 @@ def test_default_dispatch_expand(sph, oracle, dtype, l_max):
         assert sph.sphericart_cuda_launch_count() == before + 1
         parity.check_expand(c.cpu().numpy(), oracle.expand(xyz, rad, seg, l_max), rad, seg, l_max, dtype,
                             f"expand {dtype} l_max={l_max} n_rad={n_rad}")
+
+
+@pytest.mark.parametrize("dtype,l_max,deriv", [("f32", 12, 1), ("f32", 16, 1), ("f32", 9, 2), ("f64", 12, 1), ("f64", 10, 2),
+                                               ("f64", 14, 0), ("f32", 28, 0), ("f64", 20, 1), ("f32", 20, 2)])
+def test_sweep_cells_at_bench_size(sph, oracle, dtype, l_max, deriv):
+    """Cells of the l_max sweep at the size and launch configuration bench.py times them in (n sized for
+    ~1.5 GB of output: several batches per CTA, every SM busy), default dispatch: sampled points against the
+    oracle (first / last points and tile edges included) and, on EVERY point, properties that hold at any
+    size: the addition theorem sum_m Y_lm^2 = (2l+1)/4pi, Euler's x . grad Y = 0 for the normalised
+    harmonics, and trace(Hessian) = -l(l+1) Y / r^2."""
+    es = 4 if dtype == "f32" else 8
+    L = (l_max + 1) ** 2
+    per_pt = L * es * (1, 4, 13)[deriv]
+    n = max(148 * 64, int(min(4_000_000, 1.5e9 // per_pt)) // 256 * 256) + 37          # + a ragged tail
+    tdt = torch.float32 if dtype == "f32" else torch.float64
+    g = torch.Generator(device="cuda").manual_seed(1000 + l_max)
+    x_d = torch.randn(n, 3, device="cuda", dtype=tdt, generator=g)
+    before = sph.sphericart_cuda_launch_count()
+    got = sph.compute(x_d, l_max, True, deriv >= 1, deriv >= 2)
+    torch.cuda.synchronize()
+    assert sph.sphericart_cuda_launch_count() == before + 1
+    rng = np.random.default_rng(l_max)
+    idx = np.unique(np.concatenate([rng.integers(0, n, 400 if deriv < 2 else 150),
+                                    [0, 1, 2, 3, 15, 16, 31, 32, 33, n - 38, n - 37, n - 33, n - 2, n - 1]]))
+    it = torch.from_numpy(idx).cuda()
+    xyz = x_d.index_select(0, it).cpu().numpy()
+    want = oracle.compute(xyz, l_max, True, deriv >= 1, deriv >= 2)
+    for order in range(deriv + 1):
+        parity.check(got[order].index_select(0, it).cpu().numpy(), want[order], xyz, l_max, True, order, dtype,
+                     f"bench-size {dtype} l_max={l_max} deriv={deriv} order={order} ({sph.sphericart_cuda_last_kernel()})")
+    # whole-array properties, in f64 on the device, in chunks
+    eps = 1.2e-7 if dtype == "f32" else 2.3e-16
+    lt = torch.from_numpy(parity.l_of_k(l_max)).cuda()
+    lv = torch.arange(l_max + 1, device="cuda", dtype=torch.float64)
+    for a in range(0, n, 65536):
+        sl = slice(a, min(a + 65536, n))
+        Y = got[0][sl].double()
+        rows = torch.zeros((Y.shape[0], l_max + 1), dtype=torch.float64, device="cuda").index_add_(1, lt, Y * Y)
+        rel = (rows / ((2 * lv + 1) / (4 * np.pi)) - 1).abs().max()
+        assert float(rel) < 8 * (l_max + 1) * eps, f"addition theorem off by {float(rel):.3e}"
+        if deriv >= 1:
+            X = x_d[sl].double()
+            r = X.norm(dim=1)
+            G = got[1][sl].double()
+            xg = torch.einsum("na,nak->nk", X, G)                      # = 0; scale: r |grad| ~ l
+            assert float(xg.abs().max()) < 64 * (l_max + 1) ** 1.5 * eps, f"x.grad Y = {float(xg.abs().max()):.3e}"
+        if deriv >= 2:
+            H = got[2][sl].double()
+            tr = H[:, 0, 0] + H[:, 1, 1] + H[:, 2, 2]
+            res = tr + (lt * (lt + 1)).double()[None, :] * Y / (r * r)[:, None]
+            scale = ((l_max + 1) ** 2.5) / (r * r)[:, None]
+            assert float((res.abs() / scale).max()) < 64 * eps, f"trace(H) + l(l+1) Y / r^2: {float((res.abs() / scale).max()):.3e}"

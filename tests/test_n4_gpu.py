@@ -112,3 +112,33 @@ def test_vjp2_matches_finite_differences_of_the_gpu_backward(sph):
         fm = (sph.vjp_recompute(xyz - e, w, True) * v).sum(dim=1)
         fd = (fp - fm) / (2 * h)
         assert float(((fd - ggx[:, b]).abs() / (ggx.abs().max() + 1)).max()) < 1e-6
+
+
+@pytest.mark.parametrize("dtype,l_max", [("f32", 16), ("f64", 13), ("f32", 9)])
+def test_contracting_modes_at_bench_size(sph, dtype, l_max):
+    """The recompute VJP and the second-order VJP at a size that gives every CTA several batches (the launch
+    configuration bench.py's sweep.backward times): EVERY point against the stored derivatives of the forward
+    kernels contracted by torch in f64."""
+    tdt = torch.float32 if dtype == "f32" else torch.float64
+    L = (l_max + 1) ** 2
+    n = 148 * 16 * 32 * 3 // (2 if l_max > 12 else 1) + 21
+    g = torch.Generator(device="cuda").manual_seed(77 + l_max)
+    x = torch.randn(n, 3, device="cuda", dtype=tdt, generator=g)
+    w = torch.randn(n, L, device="cuda", dtype=tdt, generator=g)
+    v = torch.randn(n, 3, device="cuda", dtype=tdt, generator=g)
+    _, d, h = sph.compute(x, l_max, True, True, True)
+    tol = (2e-5 if dtype == "f32" else 1e-11)
+    gx = sph.vjp_recompute(x, w, True)
+    ref = torch.einsum("nak,nk->na", d.double(), w.double())
+    scale = d.double().norm(dim=2).max(dim=1, keepdim=True).values * w.double().norm(dim=1, keepdim=True)
+    assert float(((gx.double() - ref).abs() / scale).max()) < tol
+    ggx, ggs = sph.vjp2(x, w, v, True)
+    assert sph.sphericart_cuda_last_kernel() == "tq_vjp2"
+    ref_s = torch.einsum("nak,na->nk", d.double(), v.double())
+    scale_s = d.double().norm(dim=1).max(dim=1, keepdim=True).values * v.double().norm(dim=1, keepdim=True)
+    assert float(((ggs.double() - ref_s).abs() / scale_s).max()) < tol
+    ref_x = torch.zeros((n, 3), dtype=torch.float64, device="cuda")
+    for a in range(3):                                    # (chunked over a: h is the large tensor)
+        ref_x += torch.einsum("nbk,nk->nb", h[:, a].double(), w.double()) * v[:, a:a + 1].double()
+    scale_x = h.double().norm(dim=3).amax(dim=(1, 2))[:, None] * w.double().norm(dim=1, keepdim=True) * v.double().norm(dim=1, keepdim=True)
+    assert float(((ggx.double() - ref_x).abs() / scale_x).max()) < tol
