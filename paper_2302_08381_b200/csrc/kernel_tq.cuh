@@ -407,6 +407,19 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
     };
     constexpr bool HAS_IMG = MODE != 2;
 
+    // this lane's point of a batch; lanes past the end get a harmless point
+    auto load_xyz = [&](int64_t b0, T& xa, T& ya, T& za) {
+        const int64_t p = b0 + (lane & (B - 1));
+        xa = T(0), ya = T(0), za = T(1);
+        if (p < n) {
+            xa = __ldg(xyz + 3 * p + (CONV ? prm.src[0] : 0));
+            ya = __ldg(xyz + 3 * p + (CONV ? prm.src[1] : 1));
+            za = __ldg(xyz + 3 * p + (CONV ? prm.src[2] : 2));
+        }
+    };
+    T xn, yn, zn;   // the NEXT batch's point: fetched while the current batch is assembled
+    load_xyz((int64_t)blockIdx.x * prm.batches_per_cta * B, xn, yn, zn);
+
     int tile_no = 0;   // tiles this CTA has issued: parity picks the image
     for (int bi = 0; bi < prm.batches_per_cta; ++bi) {
         const int64_t b0 = ((int64_t)blockIdx.x * prm.batches_per_cta + bi) * B;
@@ -419,12 +432,8 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
             // columns (class `cls`), so that every lane of the warp works whatever the batch size
             const int pt_l = lane & (B - 1), cls = lane / B, NC = 32 / B;
             const int64_t p = b0 + pt_l;
-            double x = 0.0, y = 0.0, z = 1.0;   // lanes past the end compute a harmless point
-            if (p < n) {
-                x = static_cast<double>(__ldg(xyz + 3 * p + (CONV ? prm.src[0] : 0)));
-                y = static_cast<double>(__ldg(xyz + 3 * p + (CONV ? prm.src[1] : 1)));
-                z = static_cast<double>(__ldg(xyz + 3 * p + (CONV ? prm.src[2] : 2)));
-            }
+            const double x = static_cast<double>(xn), y = static_cast<double>(yn), z = static_cast<double>(zn);
+            if (bi + 1 < prm.batches_per_cta) load_xyz(b0 + B, xn, yn, zn);   // in flight through this batch
             R X, Y, Z, r2;
             double rinv = 1.0;
             if (NORM) {
