@@ -193,7 +193,7 @@ const char* sphericart_cuda_last_kernel(void);
  *                       the same function; the tests compare every family with the oracle)
  *   "host_chunk_bytes"  bytes per chunk and stream of the _host entry points (default 256 MiB)
  *   "tpg_lp", "w_nbuf", "w_warps", "w_ppw", "wc_min_l", "vjp_warps", "tpb_tiles", "tpb_split",
- *   "pdl", "tq_points", "tq_warps", "tq_batch", "tq_images", "tq_cs_warps"  integer launch-shape parameters (0 = the library's own rule)
+ *   "pdl", "tq_points", "tq_warps", "tq_batch", "tq_images", "tq_cs_warps", "tq_direct"  integer launch-shape parameters (0 = the library's own rule)
  */
 int sphericart_cuda_set_option(const char* name, const char* value);
 

@@ -696,7 +696,7 @@ int sphericart_cuda_set_option(const char* name, const char* value) {
     const IntOpt ints[] = {{"tpg_lp", &g_opt.tpg_lp}, {"w_nbuf", &g_opt.w_nbuf}, {"w_warps", &g_opt.w_warps},
                            {"w_ppw", &g_opt.w_ppw}, {"wc_min_l", &g_opt.wc_min_l}, {"vjp_warps", &g_opt.vjp_warps},
                            {"tpb_tiles", &g_opt.tpb_tiles}, {"tpb_split", &g_opt.tpb_split}, {"pdl", &g_opt.pdl},
-                           {"tq_points", &g_opt.tq_points}, {"tq_warps", &g_opt.tq_warps}, {"tq_batch", &g_opt.tq_batch}, {"tq_images", &g_opt.tq_images}, {"tq_cs_warps", &g_opt.tq_cs_warps}};
+                           {"tq_points", &g_opt.tq_points}, {"tq_warps", &g_opt.tq_warps}, {"tq_batch", &g_opt.tq_batch}, {"tq_images", &g_opt.tq_images}, {"tq_cs_warps", &g_opt.tq_cs_warps}, {"tq_direct", &g_opt.tq_direct}};
     if (!strcmp(name, "force_kernel")) {
         struct { const char* v; int code; } const kinds[] = {
             {"", FORCE_NONE}, {"auto", FORCE_NONE}, {"tpb", FORCE_TPB}, {"tpg", FORCE_TPG}, {"w", FORCE_W},

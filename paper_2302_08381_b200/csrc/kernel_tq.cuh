@@ -80,7 +80,8 @@ struct TqParams {
     double lscale[SPH_MAX_L + 1];
 };
 
-constexpr int TQ_MAX_WARPS = 8;
+constexpr int TQ_MAX_WARPS = 16;   // (one CTA per SM where the staging images leave room for no second one)
+constexpr int TQ_RED_WARPS = 8;    // warps per CTA of the contracting modes (their reduction slots are sized for it)
 
 // shared-memory carve-up (bytes), identical on host and device
 struct TqSmem {
@@ -89,8 +90,10 @@ struct TqSmem {
     size_t reg_g, reg_h;   // offsets of the dsph / ddsph regions inside an image
     // deriv: derivative order assembled; img_rows: rows per point staged (1 / 4 / 13 forward, 1 or 0
     // for the contracting modes); pt_bytes: per-point record (x, y, z, 1/r [, v])
+    // direct: no staging image at all (phase B stores straight to global memory)
     __host__ __device__ TqSmem(int l_max, int deriv, int img_rows, int pt_bytes, int esize, int batch, int pts_tile,
-                               int n_images) {
+                               int n_images, bool direct = false) {
+        if (direct) img_rows = 0, n_images = 0;
         T = (l_max + 1) * (l_max + 2) / 2;
         TP = (T + 3) | 1;          // doubles per point: three finite pad entries, odd pitch (conflict-free lane = point stores)
         CP = (l_max + 3) | 1;      // (c, s) pairs per point behind two zero pad entries ((c,s)_{-1}, (c,s)_{-2}), odd pitch
@@ -103,8 +106,8 @@ struct TqSmem {
         sl_off = o;                // lscale[l] (CONV)
         o += (size_t)(SPH_MAX_L + 1) * 8 + 8;
         red_off = o;               // [warps][pairs of points of a tile][2][3] partial sums of the contracting modes
-        const bool contracting = img_rows == 0 || pt_bytes == 64;   // (modes 1 and 2)
-        o += contracting ? (size_t)2 * 8 * ((pts_tile + 1) / 2) * 48 : 0;
+        const bool contracting = !direct && (img_rows == 0 || pt_bytes == 64);   // (modes 1 and 2)
+        o += contracting ? (size_t)2 * TQ_RED_WARPS * ((pts_tile + 1) / 2) * 48 : 0;
         lm_off = o;                // l | m << 8
         o += ((size_t)T * 2 + 15) & ~(size_t)15;
         q_off = o;
@@ -158,24 +161,32 @@ __device__ __forceinline__ unsigned tq_lds_u16(uint32_t a) {
 }
 __device__ __forceinline__ void tq_sts(uint32_t a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
 __device__ __forceinline__ void tq_sts(uint32_t a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
+// (DIRECT: the same call sites store to global memory, streaming)
+__device__ __forceinline__ void tq_sts(unsigned char* a, float v) { __stcs(reinterpret_cast<float*>(a), v); }
+__device__ __forceinline__ void tq_sts(unsigned char* a, double v) { __stcs(reinterpret_cast<double*>(a), v); }
 __device__ __forceinline__ void tq_sts2(uint32_t a, double x, double y) {
     asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(a), "d"(x), "d"(y) : "memory");
 }
 
-template <typename T, typename R, int DERIV, bool NORM, int MODE, bool CONV>
-__global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqParams prm) {
+// DIRECT (forward mode only): no staging image; phase B stores every harmonic straight to global memory
+// (lanes = consecutive (l, m) of one point: runs of consecutive words for +m, descending ones for -m).
+// Where one tile image leaves room for a single CTA per SM (long rows), the shared memory this frees
+// buys resident warps, and the kernel is latency-bound there.
+template <typename T, typename R, int DERIV, bool NORM, int MODE, bool CONV, bool DIRECT = false>
+__global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 1) sph_tq_kernel(const TqParams prm) {
     using RT = rec<R>;
     constexpr int ES = (int)sizeof(T);
     constexpr int PTB = tq_pt_bytes(MODE);
     static_assert(MODE == 0 || (MODE == 1 && DERIV == 2) || (MODE == 2 && DERIV == 1), "mode / derivative order");
+    static_assert(!DIRECT || MODE == 0, "direct stores: forward mode only");
     extern __shared__ __align__(128) unsigned char smem[];
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
     const int W = blockDim.x >> 5;
     const int l_max = prm.l_max;
     const int L = (l_max + 1) * (l_max + 1);
-    const int B = prm.batch, P = prm.pts_tile;
-    const TqSmem lay(l_max, DERIV, tq_img_rows(MODE, DERIV), PTB, ES, B, P, prm.n_images);
+    const int B = prm.batch, P = DIRECT ? prm.batch : prm.pts_tile;   // (DIRECT: the batch is the one tile)
+    const TqSmem lay(l_max, DERIV, tq_img_rows(MODE, DERIV), PTB, ES, B, P, prm.n_images, DIRECT);
     const int TT = lay.T, TP = lay.TP, CP = lay.CP;
     const uint32_t s0 = smem_u32(smem);
     const uint32_t sGT = s0 + (uint32_t)lay.gt_off, sHT = s0 + (uint32_t)lay.ht_off, sLM = s0 + (uint32_t)lay.lm_off;
@@ -223,7 +234,8 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
     // of the batch (global index pg0, pg0 + 1), staged as points plb, plb + 1 of the image whose
     // regions start at sS / sG / sH.  acc: this lane's partial sums of the contracting modes.
     // wv: the upstream gradient of the four harmonics {(l,+m), (l,-m)} x {point 0, 1} (contracting modes).
-    auto assemble = [&](int t, int plb, int pbb, int npt, const T* wv, uint32_t sS, uint32_t sG, uint32_t sH, double* acc) {
+    // (sS / sG / sH: 32-bit shared addresses, or for DIRECT global byte pointers to the tile's first point)
+    auto assemble = [&](int t, int plb, int pbb, int npt, const T* wv, auto sS, auto sG, auto sH, double* acc) {
         // ---- per (l, m): shared by the two points ----
         const unsigned lmv = tq_lds_u16(sLM + t * 2);
         const int l = (int)(lmv & 0xffu), m = (int)(lmv >> 8);
@@ -255,7 +267,7 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
             double c0, As;
             tq_lds2(aC, c0, As);
             const double Ac = (m == 0) ? SPH_INV_SQRT2 : c0;
-            const uint32_t aS = sS + pl * row_b + kc_b;
+            const auto aS = sS + pl * row_b + kc_b;
             if constexpr (MODE == 0) {
                 tq_sts(aS - m2_b, static_cast<T>(Q * As));
                 tq_sts(aS, static_cast<T>(Q * Ac));
@@ -283,8 +295,8 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
                 const double gxs = SPH_FMA(ax, As, Qs_), gys = SPH_FMA(ay, As, Qc), gzs = az * As;
                 const double gxc = SPH_FMA(ax, Ac, Qc), gyc = SPH_FMA(ay, Ac, -Qs_), gzc = az * Ac;
                 if constexpr (MODE == 0) {
-                    const uint32_t aG = sG + pl * 3 * row_b + kc_b;
-                    const uint32_t aGs = aG - m2_b;
+                    const auto aG = sG + pl * 3 * row_b + kc_b;
+                    const auto aGs = aG - m2_b;
                     tq_sts(aGs + rx, static_cast<T>(gxs));
                     tq_sts(aGs + ry, static_cast<T>(gys));
                     tq_sts(aGs + rz, static_cast<T>(gzs));
@@ -324,7 +336,7 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
                         tq_lds2(sPT + pb * PTB + 48, vz, pad_);
                     }
                     // one branch: its six second derivatives, stored (MODE 0) or contracted (MODE 1)
-                    auto branch2 = [&](uint32_t a, double A, double Ax, double Ay, double Axx, double Axy, double wk,
+                    auto branch2 = [&](auto a, double A, double Ax, double Ay, double Axx, double Axy, double wk,
                                        double gx, double gy, double gz) {
                         const double QAxx = Qh * Axx;
                         const double hxx = SPH_FMA(cxx, A, SPH_FMA(bx2, Ax, QAxx));
@@ -354,7 +366,7 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
                             acc[3 * j + 2] = SPH_FMA(wk, SPH_FMA(hxz, vx, SPH_FMA(hyz, vy, hzz * vz)), acc[3 * j + 2]);
                         }
                     };
-                    const uint32_t aH = (MODE == 0 ? sH + pl * 9 * row_b : aS - kc_b) + kc_b;
+                    const auto aH = (MODE == 0 ? sH + pl * 9 * row_b : aS - kc_b) + kc_b;
                     branch2(aH - m2_b, As, ms1, mc1, mms2, mmc2, ws, gxs, gys, gzs);
                     branch2(aH, Ac, mc1, -ms1, mmc2, -mms2, wc, gxc, gyc, gzc);
                 }
@@ -405,7 +417,7 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
         if (MODE == 0 && DERIV >= 2)
             for (int i = tid; i < np * 9 * L; i += nthr) st_cs(ddsph + p0 * 9 * L + i, H0[i]);
     };
-    constexpr bool HAS_IMG = MODE != 2;
+    constexpr bool HAS_IMG = MODE != 2 && !DIRECT;
 
     // this lane's point of a batch; lanes past the end get a harmless point
     auto load_xyz = [&](int64_t b0, T& xa, T& ya, T& za) {
@@ -588,7 +600,7 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
             double acc[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
             // (two sets of slots, alternating by tile: the threads that sum one tile's need no barrier
             // against the warps that fill the next one's)
-            double* red_set = reinterpret_cast<double*>(smem + lay.red_off) + (tile_no & 1) * (TQ_MAX_WARPS * PP * 6);
+            double* red_set = reinterpret_cast<double*>(smem + lay.red_off) + (tile_no & 1) * (TQ_RED_WARPS * PP * 6);
             double* red = red_set + warp * PP * 6;   // this warp's slots
             // contracting modes: a warp's units visit the pairs of points in ascending order, so its partial
             // sums of one pair are complete when the pair changes: over the lanes, then into the warp's slot
@@ -610,7 +622,13 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
                 int pp = w_pl0, ch = w_ch0;   // pp: PAIR of points of the tile (a lane does the same (l, m) for both)
                 while (pp < PP) {
                     const int t = ch * 32 + lane;
-                    if (t < TT) assemble(t, 2 * pp, ti * P + 2 * pp, P - 2 * pp, nullptr, sS, sG, sH, acc);
+                    if constexpr (DIRECT) {   // straight to the caller's arrays; points past the end are skipped here
+                        const int left = (int)min((int64_t)P, n - p0) - 2 * pp;
+                        if (t < TT && left > 0)
+                            assemble(t, 2 * pp, 2 * pp, left, nullptr, reinterpret_cast<unsigned char*>(sph + p0 * L),
+                                     reinterpret_cast<unsigned char*>(dsph + (DERIV >= 1 ? p0 * 3 * L : 0)),
+                                     reinterpret_cast<unsigned char*>(ddsph + (DERIV >= 2 ? p0 * 9 * L : 0)), acc);
+                    } else if (t < TT) assemble(t, 2 * pp, ti * P + 2 * pp, P - 2 * pp, nullptr, sS, sG, sH, acc);
                     ch += d_ch;
                     pp += d_pl;
                     if (ch >= NCH) {
@@ -645,7 +663,7 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
             // stores (issued one tile ago) must have read it before anyone writes there again
             if (HAS_IMG) fence_proxy_async_smem();
             if (HAS_IMG && prm.n_images == 2 && threadIdx.x == 0) bulk_wait_read<0>();
-            __syncthreads();
+            if constexpr (!DIRECT) __syncthreads();   // (DIRECT: nothing staged; the barrier ahead of phase A orders the scratch)
             const T* S0 = reinterpret_cast<const T*>(iS);
             const T* G0 = reinterpret_cast<const T*>(iG);
             const T* H0 = reinterpret_cast<const T*>(iH);
@@ -672,7 +690,7 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tq_kernel(const TqPa
         }
     }
     // shared memory must outlive the bulk stores' reads of it
-    if (threadIdx.x == 0) bulk_wait_read<0>();
+    if (HAS_IMG && threadIdx.x == 0) bulk_wait_read<0>();
 }
 
 }  // namespace sphb200

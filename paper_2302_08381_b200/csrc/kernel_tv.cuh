@@ -48,7 +48,7 @@ struct TvSmem {
 };
 
 template <typename T, typename R, bool NORM>
-__global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 2) sph_tv_kernel(const TvParams prm) {
+__global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 1) sph_tv_kernel(const TvParams prm) {
     using RT = rec<R>;
     constexpr int ES = (int)sizeof(T);
     constexpr bool DD = sizeof(R) > sizeof(double);

@@ -11,6 +11,7 @@
 #error "compile with -DTPB_F64=0|1 -DTPB_DERIV=0|1"
 #endif
 
+
 namespace sphb200 {
 
 #if TPB_F64
@@ -89,22 +90,31 @@ template <int LMAX, bool NORM>
 static int launch_one(int sm_count, const TpbParams& prm, cudaStream_t stream) {
     const int split_env = g_opt.tpb_split;
     // One lane per point doing both branches of Eq. 5 (32-point tiles) where the Legendre recurrences
-    // dominate, i.e. values only: f64 (double-double recurrences) up to l_max = 12, f32 up to 10, and
+    // dominate, i.e. values only: f64 (double-double recurrences) up to l_max = 13, f32 up to 10, and
     // f64 gradients up to l_max = 4.  Measured: f64 values l_max 4/6/8: 2.9/3.2/3.4 -> 5.2/6.1/5.3
     // TB/s, f32 values l_max 2/4/6: 2.8/4.8/5.1 -> 4.2/5.3/5.9; with Hessians it loses (f64
     // l_max = 4: 7.0 -> 4.7), so not there.
-    constexpr bool bb = TPB_DERIV == 0 ? (TPB_F64 ? LMAX <= 12 : LMAX <= 10) : (TPB_DERIV == 1 && TPB_F64 && LMAX <= 4);
+    constexpr bool bb = TPB_DERIV == 0 ? (TPB_F64 ? LMAX <= 13 : LMAX <= 10) : (TPB_DERIV == 1 && TPB_F64 && LMAX <= 4);
     if constexpr (bb) {
-        constexpr bool s2 = LMAX >= 4 && TpbShape<sizeof(tpb_T), TPB_DERIV, LMAX, 1, true>::fit <= 12;
+        // f64 values, l_max 8-12: ONE warp per tile although few tiles fit (its ~250 registers hold every
+        // column's running pair; two warps at 128 registers each re-load them).  Measured, one / two warps:
+        // l_max 8: 6.2 / 5.9 TB/s, 10: 5.6-6.0 / 4.5-4.9, 12: 3.9-4.3 / 3.5-3.8; l_max 13: 3.3-3.6 either way.
+        constexpr bool one = TPB_F64 && TPB_DERIV == 0 && LMAX >= 8 && LMAX <= 12;
+        constexpr bool s2 = LMAX >= 4 && !one && TpbShape<sizeof(tpb_T), TPB_DERIV, LMAX, 1, true>::fit <= 12;
         if constexpr (s2) {
             if (split_env != 1) return launch_split<LMAX, NORM, 2, true>(sm_count, prm, stream);
+        } else if constexpr (LMAX >= 4) {
+            if (split_env == 2) return launch_split<LMAX, NORM, 2, true>(sm_count, prm, stream);
         }
         return launch_split<LMAX, NORM, 1, true>(sm_count, prm, stream);
     } else {
         constexpr bool can_split = LMAX >= 4;
         if constexpr (can_split) {
             // (long value-only rows: one warp per tile would need > 128 registers at 13+ tiles per SM and spills)
-            constexpr bool dflt = TpbShape<sizeof(tpb_T), TPB_DERIV, LMAX, 1>::fit <= 12 || (TPB_DERIV == 0 && LMAX >= 13);
+            // Two cells measured faster with one warp: f32 values l_max 19 (3.8 against 3.4 TB/s), f32 Hessians
+            // l_max 4 (7.1 against 6.6).
+            constexpr bool one = !TPB_F64 && ((TPB_DERIV == 0 && LMAX == 19) || (TPB_DERIV == 2 && LMAX == 4));
+            constexpr bool dflt = !one && (TpbShape<sizeof(tpb_T), TPB_DERIV, LMAX, 1>::fit <= 12 || (TPB_DERIV == 0 && LMAX >= 13));
             const bool want = split_env ? split_env == 2 : dflt;
             if (want) return launch_split<LMAX, NORM, 2>(sm_count, prm, stream);
         }
@@ -137,8 +147,10 @@ int TPB_NAME(sph_tpb_launch)(int sm_count, const void* xyz, int64_t n, int l_max
         TPB_CASE(11)
         TPB_CASE(12)
 #endif
-#if !TPB_F64
+#if !TPB_F64 || !TPB_DERIV   // (f64 values: up to l_max = 13)
         TPB_CASE(13)
+#endif
+#if !TPB_F64
         TPB_CASE(14)
         TPB_CASE(15)
         TPB_CASE(16)

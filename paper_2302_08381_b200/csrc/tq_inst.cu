@@ -33,6 +33,12 @@ template <int MODE, bool CONV> static TqKernel pick(int deriv, int norm) {
     }
 }
 
+static TqKernel pick_direct(int deriv, int norm) {
+    if (deriv == 0) return norm ? sph_tq_kernel<tq_T, tq_R, 0, true, 0, false, true> : sph_tq_kernel<tq_T, tq_R, 0, false, 0, false, true>;
+    if (deriv == 1) return norm ? sph_tq_kernel<tq_T, tq_R, 1, true, 0, false, true> : sph_tq_kernel<tq_T, tq_R, 1, false, 0, false, true>;
+    return norm ? sph_tq_kernel<tq_T, tq_R, 2, true, 0, false, true> : sph_tq_kernel<tq_T, tq_R, 2, false, 0, false, true>;
+}
+
 // Launch shape: points per phase-A batch B (32, 16, 8), points per tile P, warps per CTA W, images
 // per CTA N.  The measured table (tq_table.h) first; the rules behind it serve the cells the table
 // leaves to other kernels when tq is asked for anyway (forced, another convention, the contracting
@@ -100,29 +106,36 @@ int TQ_NAME(sph_tq_launch)(const TqArgs& a) {
     int bW = tab ? shape[2] : 8;
     if (!tab && (a.l_max + 1) * (a.l_max + 2) / 2 <= 64) bP = 8, bW = 4;   // short triangles: fewer, fuller warps
     int bN = tab ? shape[3] : 1;
+    // direct stores (no staging image): table entries {B, 0, W, 0}, or the tq_direct option (1: on, 2: off)
+    bool direct = a.mode == 0 && !a.conv && ((tab && shape[3] == 0 && g_opt.tq_direct != 2) || g_opt.tq_direct == 1);
+    if (tab && shape[3] == 0) bP = 2, bN = 1;   // (used only when tq_direct = 2 turns the entry's direct stores off)
     // contracting modes: little or nothing staged: tiles of 16 points (8 pairs x chunks divide evenly among 8 warps)
     if (a.mode != 0) bP = 16, bN = a.mode == 1 ? 2 : 1, bW = 8, bB = 32;
     if (g_opt.tq_batch > 0) bB = g_opt.tq_batch;
     if (g_opt.tq_points > 0) bP = g_opt.tq_points;
     if (g_opt.tq_warps > 0) bW = g_opt.tq_warps;
     if (g_opt.tq_images > 0 && a.mode != 2) bN = g_opt.tq_images;
-    if (bW < 1 || bW > TQ_MAX_WARPS || bN < 1 || bN > 2) return 1;
+    if (bW < 1 || bW > TQ_MAX_WARPS || (a.mode != 0 && bW > TQ_RED_WARPS) || bN < 1 || bN > 2) return 1;
+    if (direct) bP = bB, bN = 1;
     if ((bB != 32 && bB != 16 && bB != 8) || bP > bB || bP < 1 || bB % bP != 0) return 1;
-    auto bytes = [&](int B, int P, int N) { return (int64_t)TqSmem(a.l_max, deriv, rows, ptb, esize, B, P, N).total; };
+    auto bytes = [&](int B, int P, int N) { return (int64_t)TqSmem(a.l_max, deriv, rows, ptb, esize, B, P, N, direct).total; };
     const bool fixed = tab || g_opt.tq_batch > 0 || g_opt.tq_points > 0 || g_opt.tq_images > 0;
     if (!fixed)
         while (bB > 8 && bB / 2 >= bP && bytes(bB, bP, bN) > 110 * 1024) bB >>= 1;
     while (bytes(bB, bP, bN) > budget) {   // shrink until it fits: images, then the batch, then the tile
         if (bN == 2) bN = 1;
+        else if (direct && bB > 8) bB >>= 1, bP = bB;
+        else if (direct) return 1;
         else if (bB > 8 && bB / 2 >= bP) bB >>= 1;
         else if (bP > 1) bP >>= 1;
         else return 1;
     }
-    const TqSmem lay(a.l_max, deriv, rows, ptb, esize, bB, bP, bN);
+    const TqSmem lay(a.l_max, deriv, rows, ptb, esize, bB, bP, bN, direct);
 
     TqKernel kern = a.mode == 1 ? pick<1, false>(deriv, a.normalized)
                   : a.mode == 2 ? pick<2, false>(deriv, a.normalized)
-                  : a.conv ? pick<0, true>(deriv, a.normalized) : pick<0, false>(deriv, a.normalized);
+                  : a.conv ? pick<0, true>(deriv, a.normalized)
+                  : direct ? pick_direct(deriv, a.normalized) : pick<0, false>(deriv, a.normalized);
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, a.smem_optin) != cudaSuccess) return -1;
 
     TqParams prm{};

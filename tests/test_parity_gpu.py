@@ -36,7 +36,7 @@ def option(sph):
 
     yield set_
     defaults = {"force_kernel": "auto", "tpg_lp": 0, "host_chunk_bytes": 256 << 20, "tq_images": 0, "tq_batch": 0,
-                "tq_points": 0, "tq_warps": 0}
+                "tq_points": 0, "tq_warps": 0, "tq_direct": 0, "tq_cs_warps": 0, "tpb_split": 0, "tpb_tiles": 0}
     for name in touched:
         sph.sphericart_cuda_set_option(name, defaults[name])
 
@@ -387,6 +387,40 @@ def test_two_phase_kernel_shapes(sph, oracle, dtype, shape, option):
             # (a shape that does not fit these rows falls through to another kernel: compared all the same)
             _compare(oracle, xyz, l_max, normalized, dtype, s, d, h,
                      f"{sph.sphericart_cuda_last_kernel()} shape={shape} {dtype} l_max={l_max} n={n} norm={normalized} deriv={deriv}")
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("shape", [(32, 8), (32, 12), (16, 4), (16, 16), (8, 3), (8, 10)])
+def test_two_phase_kernel_direct_stores(sph, oracle, dtype, shape, option):
+    """The DIRECT variant of kernel_tq.cuh (no staging image: phase B stores every harmonic straight to
+    the caller's arrays; the shape table names it for long rows) and CTAs of up to 16 warps: every
+    derivative order, both variants, ragged n and n below one pair of points; then guard bands around
+    all three output arrays (nothing written outside them, every element inside written)."""
+    np_dt = np.float32 if dtype == "f32" else np.float64
+    option("force_kernel", "tq")
+    option("tq_direct", 1)
+    option("tq_batch", shape[0])
+    option("tq_warps", shape[1])
+    for l_max, n in ((0, 5), (3, 70), (9, 203), (14, 77), (16, 1), (23, 70), (32, 45)):
+        xyz = W.make_xyz("C2" if l_max <= 16 else "C4", n, seed=l_max).astype(np_dt)
+        for normalized, deriv in ((True, 2), (False, 1), (True, 0), (False, 2)):
+            before = sph.sphericart_cuda_launch_count()
+            s, d, h = _run_gpu(sph, xyz, l_max, normalized, deriv >= 1, deriv >= 2)
+            assert sph.sphericart_cuda_launch_count() == before + 1
+            assert sph.sphericart_cuda_last_kernel() == "tq"
+            _compare(oracle, xyz, l_max, normalized, dtype, s, d, h,
+                     f"tq direct shape={shape} {dtype} l_max={l_max} n={n} norm={normalized} deriv={deriv}")
+    l_max, n = 21, 45
+    L = (l_max + 1) ** 2
+    t_dt = torch.float32 if dtype == "f32" else torch.float64
+    pts = torch.from_numpy(W.make_xyz("C4", n).astype(np_dt)).cuda()
+    bufs = [torch.full((n * rows * L + 64,), 777.0, device="cuda", dtype=t_dt) for rows in (1, 3, 9)]
+    sph.sphericart_cuda_compute(pts, n, l_max, 1, 0 if dtype == "f32" else 1, bufs[0][32:-32], bufs[1][32:-32], bufs[2][32:-32],
+                                torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert sph.sphericart_cuda_last_kernel() == "tq"
+    for buf in bufs:
+        assert torch.all(buf[:32] == 777.0) and torch.all(buf[-32:] == 777.0) and torch.all(buf[32:-32] != 777.0)
 
 
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
