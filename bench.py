@@ -619,8 +619,12 @@ def run_cuda(args):
     peak, peak_src = measured_peaks()
     if args.lmax_sweep:
         if rank == 0:
-            print(json.dumps({"lmax_sweep": lmax_sweep(torch, pkg, device, peak), "peak_gbs": peak,
-                              "peak_source": peak_src}))
+            sampler = ClockSampler(local_rank)     # the SM clock the cells were timed at (boxes differ by several %)
+            sampler.start()
+            rows = lmax_sweep(torch, pkg, device, peak)
+            sampler.stop()
+            print(json.dumps({"lmax_sweep": rows, "peak_gbs": peak, "peak_source": peak_src,
+                              "clocks": sampler.summary()}))
         return
     free, _ = torch.cuda.mem_get_info()
     if args.op != "forward":

@@ -514,65 +514,63 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 1) sph_tq_kernel(const TqPa
                     s = sn;
                 }
             }
-            // columns of the folded Eq. 7, dealt to the W * NC column classes in snake order
-            // (class v takes m = v, 2V-1-v, 2V+v, ...: balanced lengths; the classes of one warp sit
-            // on neighbouring columns, so their loops run nearly in step).  A lane runs TWO columns at
-            // a time (a long one and the short one that follows it in the snake): the recurrence is one
-            // dependent chain per column -- ~30 double-double operations per step for f64 I/O -- and
-            // two independent chains per lane hide its latency.  Coefficients {A, B} come from a packed
-            // global table through the read-only path (indexed constant-bank loads were the top stall).
+            // Columns of the folded Eq. 7 in ADJACENT pairs (2k, 2k+1), the pairs dealt to the V column
+            // classes in snake order (class v: k = v, 2V-1-v, 2V+v, ...: balanced step counts; the classes of
+            // one warp sit on neighbouring pairs, so their loops run nearly in step).  Both chains of a pair
+            // run over (nearly) the same rows: a lane has two independent recurrences in flight for its whole
+            // loop -- the recurrence is one dependent chain per column, ~23 double-double operations per step
+            // for f64 I/O.  The row loop is unrolled by two with the roles of (q, qp) exchanged, so that no
+            // register is copied from one step to the next.  Coefficients {A, B}: f64 I/O from a packed
+            // global table through the read-only path (indexed constant-bank loads were the top stall), f32
+            // I/O from the constant bank (measured faster there).
             const uint32_t q_out = sQ + pt_l * TP * 8;
             const int V = Wq * NC, v = warp * NC + cls;   // (the cs warps of the double-double path run no columns)
-            auto step = [&](int t, R& q, R& qp) {   // (q, qp) = (Qt_{l-1}^m, Qt_{l-2}^m) -> (Qt_l^m, Qt_{l-1}^m), t = TRI(l, m)
-                const double2 hi = __ldg(prm.ab_hi + t);
-                double2 lo = make_double2(0.0, 0.0);
-                if constexpr (sizeof(R) > sizeof(double)) lo = __ldg(prm.ab_lo + t);
+            auto next = [&](int t, const R& q, const R& qp) -> R {   // Qt_l^m from (Qt_{l-1}^m, Qt_{l-2}^m), t = TRI(l, m)
                 const R w = NORM ? qp : r2 * qp;
-                const R qn = rec_step(hi.x, lo.x, hi.y, lo.y, Z, q, w);   // (B_{m+1}^m = 0)
-                qp = q;
-                q = qn;
-                tq_sts(q_out + t * 8, to_double(q));
-            };
-            if constexpr (sizeof(R) > sizeof(double)) {
-                for (int i = 0; warp < Wq && i * V <= l_max; i += 2) {
-                    const int ma = i * V + v;
-                    if (ma > l_max) continue;
-                    int mb = (i + 2) * V - 1 - v;            // > ma; past the triangle: no second column
-                    if (mb > l_max) mb = 0x7fff;
-                    int ta = SPH_TRI(ma, ma), tb = 0;
-                    R qa = RT::make(TB.D_hi[ma], TB.D_lo[ma]), qpa = RT::make(0.0, 0.0);
-                    R qb = RT::make(0.0, 0.0), qpb = RT::make(0.0, 0.0);
-                    tq_sts(q_out + ta * 8, to_double(qa));
-                    for (int l = ma + 1; l <= l_max; ++l) {
-                        ta += l;   // SPH_TRI(l, m) - SPH_TRI(l-1, m) = l
-                        step(ta, qa, qpa);
-                        if (l == mb) {
-                            tb = SPH_TRI(mb, mb);
-                            qb = RT::make(TB.D_hi[mb], TB.D_lo[mb]);
-                            tq_sts(q_out + tb * 8, to_double(qb));
-                        } else if (l > mb) {
-                            tb += l;
-                            step(tb, qb, qpb);
-                        }
-                    }
+                R qn;
+                if constexpr (sizeof(R) > sizeof(double)) {
+                    const double2 hi = __ldg(prm.ab_hi + t);
+                    const double2 lo = __ldg(prm.ab_lo + t);
+                    qn = rec_step(hi.x, lo.x, hi.y, lo.y, Z, q, w);   // (B_{m+1}^m = 0)
+                } else {
+                    qn = RT::make(TB.A_hi[t], 0.0) * (Z * q) - RT::make(TB.B_hi[t], 0.0) * w;
                 }
-            } else {
-                // f32 I/O (recurrences in plain double, 3 operations per step): one column at a time,
-                // coefficients from the constant bank (measured faster than the two-column form here)
-                for (int i = 0; i * V <= l_max; ++i) {
-                    const int m = (i & 1) ? (i + 1) * V - 1 - v : i * V + v;
-                    if (m > l_max) continue;
-                    int t = SPH_TRI(m, m);
-                    R q = RT::make(TB.D_hi[m], TB.D_lo[m]), qp = RT::make(0.0, 0.0);
-                    tq_sts(q_out + t * 8, to_double(q));
-                    for (int l = m + 1; l <= l_max; ++l) {
-                        t += l;   // SPH_TRI(l, m) - SPH_TRI(l-1, m) = l
-                        const R w = NORM ? qp : r2 * qp;
-                        const R qn = RT::make(TB.A_hi[t], 0.0) * (Z * q) - RT::make(TB.B_hi[t], 0.0) * w;   // (B_{m+1}^m = 0)
-                        qp = q;
-                        q = qn;
-                        tq_sts(q_out + t * 8, to_double(q));
-                    }
+                tq_sts(q_out + t * 8, to_double(qn));
+                return qn;
+            };
+            const int n_pairs = l_max / 2 + 1;
+            for (int i = 0; warp < Wq && i * V < n_pairs; ++i) {
+                const int k = (i & 1) ? (i + 1) * V - 1 - v : i * V + v;
+                if (k >= n_pairs) continue;
+                const int ma = 2 * k, mb = ma + 1;
+                R qa = RT::make(TB.D_hi[ma], TB.D_lo[ma]), qpa = RT::make(0.0, 0.0);
+                int ta = SPH_TRI(ma, ma);
+                tq_sts(q_out + ta * 8, to_double(qa));
+                if (mb > l_max) continue;
+                ta += mb;   // SPH_TRI(l, m) - SPH_TRI(l-1, m) = l
+                int tb = SPH_TRI(mb, mb);
+                qpa = next(ta, qa, qpa);                           // (column a: newest in qpa)
+                R qb = RT::make(TB.D_hi[mb], TB.D_lo[mb]), qpb = RT::make(0.0, 0.0);
+                tq_sts(q_out + tb * 8, to_double(qb));
+                int l = mb + 1;
+                if (l <= l_max) {   // one single step brings column a back to (newest in qa); b: newest in qpb
+                    ta += l, tb += l;
+                    qa = next(ta, qpa, qa);
+                    qpb = next(tb, qb, qpb);
+                    ++l;
+                }
+                for (; l + 1 <= l_max; l += 2) {
+                    ta += l, tb += l;
+                    qpa = next(ta, qa, qpa);
+                    qb = next(tb, qpb, qb);
+                    ta += l + 1, tb += l + 1;
+                    qa = next(ta, qpa, qa);
+                    qpb = next(tb, qb, qpb);
+                }
+                if (l <= l_max) {
+                    ta += l, tb += l;
+                    next(ta, qa, qpa);
+                    next(tb, qpb, qb);
                 }
             }
         }

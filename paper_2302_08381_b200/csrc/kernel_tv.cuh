@@ -148,46 +148,73 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 1) sph_tv_kernel(const TvPa
                 tq_sts(as, static_cast<T>(Q * As));
                 tq_sts(ac, static_cast<T>(Q * Ac));
             };
-            auto step = [&](int t, R& q, R& qp) {
+            // one step of the folded Eq. 7: Qt_l^m from (q, qp) = (Qt_{l-1}^m, Qt_{l-2}^m), t = TRI(l, m)
+            auto next = [&](int t, const R& q, const R& qp) -> R {
                 const double2 hi = __ldg(prm.ab_hi + t);
                 double2 lo = make_double2(0.0, 0.0);
                 if constexpr (DD) lo = __ldg(prm.ab_lo + t);
                 const R w = NORM ? qp : r2 * qp;
-                const R qn = rec_step(hi.x, lo.x, hi.y, lo.y, Z, q, w);
-                qp = q;
-                q = qn;
+                return rec_step(hi.x, lo.x, hi.y, lo.y, Z, q, w);   // (B_{m+1}^m = 0)
             };
-            for (int i = 0; i * V <= l_max; i += 2) {
-                const int ma = i * V + v;
-                if (ma > l_max) continue;
-                int mb = (i + 2) * V - 1 - v;            // > ma; past the triangle: no second column
-                if (mb > l_max) mb = 0x7fff;
+            // Columns in ADJACENT pairs (2k, 2k+1): both chains of a pair run over (nearly) the same rows, so a
+            // lane has two independent recurrences in flight for the whole of its loop, not only where a long
+            // and a short column happen to overlap.  Pair k takes M - 2k row steps (M = l_max + 1); the pairs
+            // are dealt to the V column classes in snake order (class v: k = v, 2V-1-v, 2V+v, ...), which
+            // balances the classes' step counts where V <= ~M/4.  The row loop is unrolled by two with the
+            // roles of (q, qp) exchanged, so that no register is copied from one step to the next.
+            const int n_pairs = l_max / 2 + 1;
+            for (int i = 0; i * V < n_pairs; ++i) {
+                const int k = (i & 1) ? (i + 1) * V - 1 - v : i * V + v;
+                if (k >= n_pairs) continue;
+                const int ma = 2 * k, mb = ma + 1;
+                const bool has_b = mb <= l_max;
                 double Aca, Asa, Acb = 0.0, Asb = 0.0;
                 tq_lds2(cs_row + ma * 16, Aca, Asa);
-                if (mb <= l_max) tq_lds2(cs_row + mb * 16, Acb, Asb);
-                int ta = SPH_TRI(ma, ma), tb = 0;
+                if (has_b) tq_lds2(cs_row + mb * 16, Acb, Asb);
                 R qa = RT::make(TB.D_hi[ma], TB.D_lo[ma]), qpa = RT::make(0.0, 0.0);
-                R qb = RT::make(0.0, 0.0), qpb = RT::make(0.0, 0.0);
                 // byte addresses of (l, +m) and (l, -m) in the row; from row l to l + 1 both move by 2 (l + 1) elements
                 uint32_t aca = row + (uint32_t)(ma * (ma + 1) + ma) * ES, asa = row + (uint32_t)(ma * (ma + 1) - ma) * ES;
-                uint32_t acb = 0, asb = 0;
                 emit(qa, Aca, Asa, aca, asa);
-                for (int l = ma + 1; l <= l_max; ++l) {
-                    ta += l;   // SPH_TRI(l, m) - SPH_TRI(l-1, m) = l
-                    step(ta, qa, qpa);
-                    aca += 2u * l * ES, asa += 2u * l * ES;
+                if (!has_b) continue;
+                // row l = mb: the second entry of column a, the first of column b
+                int ta = SPH_TRI(ma, ma) + mb, tb = SPH_TRI(mb, mb);
+                qpa = next(ta, qa, qpa);                           // (newest in qpa, the one before in qa)
+                R qb = RT::make(TB.D_hi[mb], TB.D_lo[mb]), qpb = RT::make(0.0, 0.0);
+                aca += 2u * mb * ES, asa += 2u * mb * ES;
+                uint32_t acb = row + (uint32_t)(mb * (mb + 1) + mb) * ES, asb = row + (uint32_t)(mb * (mb + 1) - mb) * ES;
+                emit(qpa, Aca, Asa, aca, asa);
+                emit(qb, Acb, Asb, acb, asb);
+                int l = mb + 1;
+                if (l <= l_max) {   // one single step brings column a back to (newest in qa)
+                    ta += l, tb += l;
+                    qa = next(ta, qpa, qa);
+                    qpb = next(tb, qb, qpb);                       // (column b: newest in qpb)
+                    aca += 2u * l * ES, asa += 2u * l * ES, acb += 2u * l * ES, asb += 2u * l * ES;
                     emit(qa, Aca, Asa, aca, asa);
-                    if (l == mb) {
-                        tb = SPH_TRI(mb, mb);
-                        qb = RT::make(TB.D_hi[mb], TB.D_lo[mb]);
-                        acb = row + (uint32_t)(mb * (mb + 1) + mb) * ES, asb = row + (uint32_t)(mb * (mb + 1) - mb) * ES;
-                        emit(qb, Acb, Asb, acb, asb);
-                    } else if (l > mb) {
-                        tb += l;
-                        step(tb, qb, qpb);
-                        acb += 2u * l * ES, asb += 2u * l * ES;
-                        emit(qb, Acb, Asb, acb, asb);
-                    }
+                    emit(qpb, Acb, Asb, acb, asb);
+                    ++l;
+                }
+                for (; l + 1 <= l_max; l += 2) {   // a: newest in qa; b: newest in qpb
+                    ta += l, tb += l;
+                    qpa = next(ta, qa, qpa);
+                    qb = next(tb, qpb, qb);
+                    aca += 2u * l * ES, asa += 2u * l * ES, acb += 2u * l * ES, asb += 2u * l * ES;
+                    emit(qpa, Aca, Asa, aca, asa);
+                    emit(qb, Acb, Asb, acb, asb);
+                    ta += l + 1, tb += l + 1;
+                    qa = next(ta, qpa, qa);
+                    qpb = next(tb, qb, qpb);
+                    aca += 2u * (l + 1) * ES, asa += 2u * (l + 1) * ES, acb += 2u * (l + 1) * ES, asb += 2u * (l + 1) * ES;
+                    emit(qa, Aca, Asa, aca, asa);
+                    emit(qpb, Acb, Asb, acb, asb);
+                }
+                if (l <= l_max) {   // the last row of an odd count
+                    ta += l, tb += l;
+                    qpa = next(ta, qa, qpa);
+                    qb = next(tb, qpb, qb);
+                    aca += 2u * l * ES, asa += 2u * l * ES, acb += 2u * l * ES, asb += 2u * l * ES;
+                    emit(qpa, Aca, Asa, aca, asa);
+                    emit(qb, Acb, Asb, acb, asb);
                 }
             }
         }
