@@ -142,6 +142,38 @@ SPH_HD dd rec_step(double a_hi, double a_lo, double b_hi, double b_lo, dd Z, dd 
     return quick_two_sum(s.hi, SPH_ADD(s.lo, SPH_SUB(te, ue)));
 }
 
+// The same step WITHOUT the final normalisation: the result is the unevaluated pair (hi, lo) with
+// hi = fl(fl(a_hi fl(Z_hi q_hi)) - fl(b_hi w_hi)) -- the plain f64 recurrence on the high parts -- and
+// lo = the first-order correction (every rounding error of those operations, exact by FMA / two_sum,
+// plus the low parts of a, b, Z, q, w).  |lo| stays ~ l 2^-53 |hi| over a whole column, so the
+// second-order terms dropped are ~2^-94; the value is hi + lo (pair_value).  What this buys is the
+// DEPENDENCY DEPTH from one step to the next: 3 operations for hi, 4 for lo, against 8-10 through the
+// normalisation -- the columns of Eq. 7 are latency-bound chains.  q and w may be such pairs themselves.
+SPH_HD double rec_step_u(double a_hi, double, double b_hi, double, double Z, double q, double w) {
+    return SPH_FMA(a_hi * Z, q, -(b_hi * w));
+}
+SPH_HD dd rec_step_u(double a_hi, double a_lo, double b_hi, double b_lo, dd Z, dd q, dd w) {
+    const double p = SPH_MUL(Z.hi, q.hi);
+    double e = SPH_FMA(Z.hi, q.hi, -p);
+    e = SPH_FMA(Z.lo, q.hi, e);
+    e = SPH_FMA(Z.hi, q.lo, e);              // (the carried low part enters last)
+    const double th = SPH_MUL(a_hi, p);
+    double te = SPH_FMA(a_hi, p, -th);
+    te = SPH_FMA(a_lo, p, te);
+    te = SPH_FMA(a_hi, e, te);
+    const double uh = SPH_MUL(b_hi, w.hi);
+    double ue = SPH_FMA(b_hi, w.hi, -uh);
+    ue = SPH_FMA(b_lo, w.hi, ue);
+    ue = SPH_FMA(b_hi, w.lo, ue);
+    const dd s = two_sum(th, -uh);
+    dd r;
+    r.hi = s.hi;
+    r.lo = SPH_ADD(s.lo, SPH_SUB(te, ue));
+    return r;
+}
+SPH_HD double pair_value(double a) { return a; }
+SPH_HD double pair_value(dd a) { return SPH_ADD(a.hi, a.lo); }
+
 SPH_HD double rec_step2(double a, double b, double Z, double q, double w) { return rec_step(a, 0.0, b, 0.0, Z, q, w); }
 SPH_HD dd rec_step2(dd a, dd b, dd Z, dd q, dd w) { return rec_step(a.hi, a.lo, b.hi, b.lo, Z, q, w); }
 

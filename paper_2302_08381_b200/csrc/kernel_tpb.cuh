@@ -192,7 +192,7 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
             R q = RT::make(TB.D_hi[M], TB.D_lo[M]), qp = RT::make(0.0, 0.0);
             static_for<M, LMAX + 1>([&](auto lc) {
                 constexpr int l = decltype(lc)::value;
-                dst[l] = to_double(q);
+                dst[l] = pair_value(q);   // (q: unnormalised pair from rec_step_u)
                 if constexpr (l < LMAX) {
                     constexpr int t1 = SPH_TRI(l + 1, M);
                     const R a = RT::make(TB.A_hi[t1], TB.A_lo[t1]);
@@ -201,7 +201,7 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
                         qn = a * (Z * q);
                     } else {
                         const R w = NORM ? qp : r2 * qp;
-                        qn = rec_step(TB.A_hi[t1], TB.A_lo[t1], TB.B_hi[t1], TB.B_lo[t1], Z, q, w);   // (dd.cuh)
+                        qn = rec_step_u(TB.A_hi[t1], TB.A_lo[t1], TB.B_hi[t1], TB.B_lo[t1], Z, q, w);   // (dd.cuh: short dependency chain)
                     }
                     qp = q;
                     q = qn;

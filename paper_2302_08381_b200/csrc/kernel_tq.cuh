@@ -531,11 +531,11 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 1) sph_tq_kernel(const TqPa
                 if constexpr (sizeof(R) > sizeof(double)) {
                     const double2 hi = __ldg(prm.ab_hi + t);
                     const double2 lo = __ldg(prm.ab_lo + t);
-                    qn = rec_step(hi.x, lo.x, hi.y, lo.y, Z, q, w);   // (B_{m+1}^m = 0)
+                    qn = rec_step_u(hi.x, lo.x, hi.y, lo.y, Z, q, w);   // (B_{m+1}^m = 0)
                 } else {
                     qn = RT::make(TB.A_hi[t], 0.0) * (Z * q) - RT::make(TB.B_hi[t], 0.0) * w;
                 }
-                tq_sts(q_out + t * 8, to_double(qn));
+                tq_sts(q_out + t * 8, pair_value(qn));   // (unnormalised pair from rec_step_u)
                 return qn;
             };
             const int n_pairs = l_max / 2 + 1;

@@ -144,7 +144,7 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 1) sph_tv_kernel(const TvPa
             // one entry of column m at row l: the harmonics (l, +m) and (l, -m); the sin one first, so that
             // for m = 0 (s_0 = 0, same slot) the cos store that follows overwrites it
             auto emit = [&](R q, double Ac, double As, uint32_t ac, uint32_t as) {
-                const double Q = to_double(q);
+                const double Q = pair_value(q);   // (unnormalised pair from rec_step_u)
                 tq_sts(as, static_cast<T>(Q * As));
                 tq_sts(ac, static_cast<T>(Q * Ac));
             };
@@ -154,7 +154,7 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 1) sph_tv_kernel(const TvPa
                 double2 lo = make_double2(0.0, 0.0);
                 if constexpr (DD) lo = __ldg(prm.ab_lo + t);
                 const R w = NORM ? qp : r2 * qp;
-                return rec_step(hi.x, lo.x, hi.y, lo.y, Z, q, w);   // (B_{m+1}^m = 0)
+                return rec_step_u(hi.x, lo.x, hi.y, lo.y, Z, q, w);   // (B_{m+1}^m = 0)
             };
             // Columns in ADJACENT pairs (2k, 2k+1): both chains of a pair run over (nearly) the same rows, so a
             // lane has two independent recurrences in flight for the whole of its loop, not only where a long
@@ -237,6 +237,8 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 1) sph_tv_kernel(const TvPa
             }
         }
         __syncthreads();
+        // (the points parked in shared memory two batches ahead, so that no lane waits on global memory at the
+        // top of a batch, were measured: 3 % slower -- other CTAs cover that latency already)
         // (two images, so that a batch drains while the next is computed, were measured: slower everywhere --
         // the shared memory they take costs more resident CTAs than the second barrier costs time)
     }
