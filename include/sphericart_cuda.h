@@ -173,6 +173,34 @@ int sphericart_cuda_compute_host(const void* xyz, int64_t n, int l_max, int norm
 int sphericart_cuda_vjp_host(const void* xyz, const void* dsph, const void* grad_sph,
                              void* grad_xyz, int64_t n, int l_max, int dtype);
 
+/*
+ * Backward pass (the same contraction as sphericart_cuda_vjp:
+ * grad_xyz[i,a] = sum_k dsph[i,a,k] * grad_sph[i,k]) for callers that must not allocate: code under
+ * CUDA graph capture, serving loops and harnesses that forbid cudaMalloc.  This call, its first
+ * use on a device included, calls no cudaMalloc / cudaFree and no allocating library routine,
+ * creates no stream or event, and does not synchronise: it enqueues two kernels on `stream`.
+ *   dsph      [n,3,L]  in, DEVICE
+ *   grad_sph  [n,L]    in, DEVICE
+ *   grad_xyz  [n,3]    out, DEVICE
+ * A row is cut into up to 8 slices, one warp per (point, slice) -- small batches of long rows fill
+ * the GPU, which one warp per point does not -- and the slices' partial sums pass through a scratch
+ * that is a file-scope `static __device__` array of the library:
+ * SPHERICART_CUDA_NOALLOC_SCRATCH_BYTES (6 MiB) held by every GPU that loads the library until the
+ * process exits.  Hence the limit: n <= SPHERICART_CUDA_NOALLOC_MAX_POINTS; a larger n returns
+ * SPHERICART_CUDA_EINVAL with a message naming the limit (split the batch, or use
+ * sphericart_cuda_vjp).  Sums are accumulated in f64 in a fixed order (deterministic); the result
+ * differs from sphericart_cuda_vjp's only by the order of the additions.
+ * Every call on a device shares the one scratch array: calls that may OVERLAP on the GPU (different
+ * streams, or graph branches without a dependency between them) race on it and must be serialised
+ * by the caller; calls in one stream are ordered and safe.  The array keeps the last call's
+ * contents; every element a call reads it has written itself first, so nothing needs clearing.
+ * Errors as for sphericart_cuda_vjp (EINVAL, EALIGN, ECUDA); n = 0 is a no-op.
+ */
+#define SPHERICART_CUDA_NOALLOC_MAX_POINTS 32768
+#define SPHERICART_CUDA_NOALLOC_SCRATCH_BYTES (32768u * 8u * 3u * 8u)
+int sphericart_cuda_vjp_noalloc(const void* dsph, const void* grad_sph, void* grad_xyz, int64_t n, int l_max,
+                                int dtype, void* stream);
+
 /* Message for the last non-zero return on the calling thread ("" if none).  Never NULL. */
 const char* sphericart_cuda_last_error(void);
 

@@ -58,6 +58,8 @@ def load():
     lib.sphericart_cuda_vjp2.argtypes = [vp, vp, vp, vp, vp, i64, ci, ci, ci, vp]
     lib.sphericart_cuda_expand.restype = ci
     lib.sphericart_cuda_expand.argtypes = [vp, vp, vp, i64, ci, ci, ci, vp, vp]
+    lib.sphericart_cuda_vjp_noalloc.restype = ci
+    lib.sphericart_cuda_vjp_noalloc.argtypes = [vp, vp, vp, i64, ci, ci, vp]
     lib.sphericart_cuda_vjp_host.restype = ci
     lib.sphericart_cuda_vjp_host.argtypes = [vp, vp, vp, vp, i64, ci, ci]
     lib.sphericart_cuda_last_error.restype = ctypes.c_char_p
@@ -130,6 +132,14 @@ def sphericart_cuda_expand(xyz, radial, seg_ptr, n_seg, l_max, n_rad, dtype, coe
     rc = load().sphericart_cuda_expand(_ptr(xyz), _ptr(radial), _ptr(seg_ptr), n_seg, l_max, n_rad, dtype,
                                        _ptr(coeff), _ptr(stream))
     _check(rc, "sphericart_cuda_expand")
+
+
+NOALLOC_MAX_POINTS = 32768   # SPHERICART_CUDA_NOALLOC_MAX_POINTS (include/sphericart_cuda.h)
+
+
+def sphericart_cuda_vjp_noalloc(dsph, grad_sph, grad_xyz, n, l_max, dtype, stream):
+    rc = load().sphericart_cuda_vjp_noalloc(_ptr(dsph), _ptr(grad_sph), _ptr(grad_xyz), n, l_max, dtype, _ptr(stream))
+    _check(rc, "sphericart_cuda_vjp_noalloc")
 
 
 def sphericart_cuda_vjp_host(xyz, dsph, grad_sph, grad_xyz, n, l_max, dtype):

@@ -458,6 +458,142 @@ static int64_t chunk_points(int64_t n, size_t bytes_per_point, size_t target) {
     return c < n ? c : n;
 }
 
+// ---------------------------------------------------------------------------------------------
+// sphericart_cuda_vjp_noalloc: the stored-derivative VJP for callers that must not allocate
+// ---------------------------------------------------------------------------------------------
+// A split-row variant of sph_vjp_warp_kernel (kernel_w.cuh): a point's row of L harmonics is cut into
+// S slices, one warp per (point, slice), so that a SMALL batch with long rows still fills the machine;
+// the warps' partial sums (3 doubles per point and slice) go through a scratch in global memory and a
+// second kernel adds the S slices of every point in a fixed order (deterministic).  The scratch is a
+// file-scope array of the library image: every GPU that loads the library holds its
+// SPHERICART_CUDA_NOALLOC_SCRATCH_BYTES until the process exits, and the call allocates nothing.
+// The array's name is a host-side stand-in in host code; the kernels get the address that
+// cudaGetSymbolAddress returns for the current device (noalloc_state below).
+constexpr int NOALLOC_MAX_SLICES = 8;
+static_assert(SPHERICART_CUDA_NOALLOC_SCRATCH_BYTES ==
+                  (size_t)SPHERICART_CUDA_NOALLOC_MAX_POINTS * NOALLOC_MAX_SLICES * 3 * sizeof(double),
+              "scratch size = max points x max slices x 3 partial sums");
+static __device__ __align__(256) unsigned char g_noalloc_scratch[SPHERICART_CUDA_NOALLOC_SCRATCH_BYTES];
+
+// partial[(s * n + p) * 3 + a] = sum over slice s of dsph[p, a, k] * grad_sph[p, k]
+template <typename T>
+__global__ void __launch_bounds__(256) sph_vjp_split_kernel(const T* __restrict__ dsph, const T* __restrict__ gsph,
+                                                            double* __restrict__ partial, int64_t n, int L, int S) {
+    const int lane = threadIdx.x & 31;
+    const int64_t unit = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);   // (point, slice)
+    if (unit >= n * S) return;
+    const int64_t p = unit / S;
+    const int s = (int)(unit - p * S);
+    const int k0 = (int)((int64_t)L * s / S), k1 = (int)((int64_t)L * (s + 1) / S);
+    const T* g = gsph + p * L;
+    const T* d = dsph + p * 3 * L;
+    double ax = 0.0, ay = 0.0, az = 0.0;
+    for (int k = k0 + lane; k < k1; k += 32) {
+        const double w = static_cast<double>(__ldcs(g + k));
+        ax = fma(static_cast<double>(__ldcs(d + k)), w, ax);
+        ay = fma(static_cast<double>(__ldcs(d + L + k)), w, ay);
+        az = fma(static_cast<double>(__ldcs(d + 2 * L + k)), w, az);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        ax += __shfl_xor_sync(0xffffffffu, ax, o);
+        ay += __shfl_xor_sync(0xffffffffu, ay, o);
+        az += __shfl_xor_sync(0xffffffffu, az, o);
+    }
+    if (lane == 0) {
+        double* out = partial + ((int64_t)s * n + p) * 3;
+        out[0] = ax;
+        out[1] = ay;
+        out[2] = az;
+    }
+}
+
+// grad_xyz[p, a] = sum_s partial[s][p][a], slices in ascending order
+template <typename T>
+__global__ void __launch_bounds__(256) sph_vjp_split_sum_kernel(const double* __restrict__ partial, T* __restrict__ gxyz,
+                                                                int64_t n, int S) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;   // = 3 p + a
+    if (i >= 3 * n) return;
+    double sum = 0.0;
+    for (int s = 0; s < S; ++s) sum += partial[(int64_t)s * n * 3 + i];
+    gxyz[i] = static_cast<T>(sum);
+}
+
+struct NoallocState {
+    std::atomic<bool> ready{false};
+    int sm_count = 0;
+    double* scratch = nullptr;   // DEVICE address of g_noalloc_scratch on this device
+};
+static NoallocState g_noalloc[MAX_DEVICES];
+
+// once per device, with that device current; no allocation (no cudaMalloc, no stream, no event)
+static int noalloc_state(NoallocState** out) {
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= MAX_DEVICES) return fail(SPHERICART_CUDA_ECUDA, "device index %d out of range", dev);
+    NoallocState& st = g_noalloc[dev];
+    if (!st.ready.load(std::memory_order_acquire)) {
+        std::lock_guard<std::mutex> lock(g_mutex);
+        if (!st.ready.load(std::memory_order_relaxed)) {
+            int major = 0;
+            CUDA_TRY(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+            if (major < 10)
+                return fail(SPHERICART_CUDA_ECUDA, "device %d is sm_%dx; this library is built for sm_100a only", dev, major);
+            CUDA_TRY(cudaDeviceGetAttribute(&st.sm_count, cudaDevAttrMultiProcessorCount, dev));
+            void* ptr = nullptr;
+            CUDA_TRY(cudaGetSymbolAddress(&ptr, g_noalloc_scratch));
+            if (!ptr || (reinterpret_cast<uintptr_t>(ptr) & 255u))
+                return fail(SPHERICART_CUDA_ECUDA, "cudaGetSymbolAddress returned %p for the scratch array", ptr);
+            st.scratch = static_cast<double*>(ptr);
+            st.ready.store(true, std::memory_order_release);
+        }
+    }
+    *out = &st;
+    return 0;
+}
+
+static int vjp_noalloc_device(const void* dsph, const void* grad_sph, void* grad_xyz, int64_t n, int l_max, int dtype,
+                              cudaStream_t stream) {
+    int rc = check_common(n, l_max, dtype);
+    if (rc) return rc;
+    if (n > SPHERICART_CUDA_NOALLOC_MAX_POINTS)
+        return fail(SPHERICART_CUDA_EINVAL,
+                    "vjp_noalloc: n = %lld exceeds SPHERICART_CUDA_NOALLOC_MAX_POINTS = %d (the static scratch holds "
+                    "no more); split the batch or call sphericart_cuda_vjp",
+                    (long long)n, SPHERICART_CUDA_NOALLOC_MAX_POINTS);
+    if (n == 0) return 0;
+    if (!dsph || !grad_sph || !grad_xyz)
+        return fail(SPHERICART_CUDA_EINVAL, "dsph, grad_sph and grad_xyz must not be NULL when n > 0");
+    if (misaligned(dsph) || misaligned(grad_sph) || misaligned(grad_xyz))
+        return fail(SPHERICART_CUDA_EALIGN, "device pointers must be 16-byte aligned");
+    NoallocState* st = nullptr;
+    rc = noalloc_state(&st);
+    if (rc) return rc;
+    const int L = (l_max + 1) * (l_max + 1);
+    // slices: enough (point, slice) warps for ~16 per SM, at least 32 harmonics per slice
+    int S = (int)(((int64_t)st->sm_count * 16 + n - 1) / n);
+    if (S > L / 32) S = L / 32;
+    if (S > NOALLOC_MAX_SLICES) S = NOALLOC_MAX_SLICES;
+    if (S < 1) S = 1;
+    const int64_t units = n * S;
+    const int warps_per_cta = 8;
+    const int64_t ctas = (units + warps_per_cta - 1) / warps_per_cta;
+    const int64_t sum_ctas = (3 * n + 255) / 256;
+    if (dtype == SPHERICART_CUDA_F32) {
+        sph_vjp_split_kernel<float><<<(unsigned)ctas, warps_per_cta * 32, 0, stream>>>(
+            static_cast<const float*>(dsph), static_cast<const float*>(grad_sph), st->scratch, n, L, S);
+        sph_vjp_split_sum_kernel<float><<<(unsigned)sum_ctas, 256, 0, stream>>>(st->scratch, static_cast<float*>(grad_xyz), n, S);
+    } else {
+        sph_vjp_split_kernel<double><<<(unsigned)ctas, warps_per_cta * 32, 0, stream>>>(
+            static_cast<const double*>(dsph), static_cast<const double*>(grad_sph), st->scratch, n, L, S);
+        sph_vjp_split_sum_kernel<double><<<(unsigned)sum_ctas, 256, 0, stream>>>(st->scratch, static_cast<double*>(grad_xyz), n, S);
+    }
+    launched("vjp_split");
+    launched("vjp_split_sum");
+    CUDA_TRY(cudaGetLastError());
+    return 0;
+}
+
 }  // namespace sphb200
 
 using namespace sphb200;
@@ -720,6 +856,11 @@ int sphericart_cuda_set_option(const char* name, const char* value) {
             return 0;
         }
     return fail(SPHERICART_CUDA_EINVAL, "set_option: unknown option '%s'", name);
+}
+
+int sphericart_cuda_vjp_noalloc(const void* dsph, const void* grad_sph, void* grad_xyz, int64_t n, int l_max,
+                                int dtype, void* stream) {
+    return vjp_noalloc_device(dsph, grad_sph, grad_xyz, n, l_max, dtype, static_cast<cudaStream_t>(stream));
 }
 
 const char* sphericart_cuda_last_kernel(void) { return g_last_kernel; }
