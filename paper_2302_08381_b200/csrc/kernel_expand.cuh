@@ -63,22 +63,26 @@ __device__ __forceinline__ void dmma_m8n8k4(double (&d)[2], double a, double b) 
 template <int ESIZE, int LMAX> struct ExpandShape {
     static constexpr int L = (LMAX + 1) * (LMAX + 1);
     static constexpr int passes = (L + 31) / 32;
-    // per warp: Y image [16][L] + TWO radial images [16][n_rad][LMAX+1], all in the I/O type (the
-    // next tile's radial values arrive by cp.async while this tile is evaluated and contracted),
-    // each radial image followed by nrad_max rows of padding (the unrolled contraction reads
+    // per warp: Y image [16][L] + ONE radial image [16][n_rad][LMAX+1], both in the I/O type (the
+    // next tile's radial values are requested after this tile's contraction and arrive -- one bulk load
+    // -- while the next tile's harmonics are evaluated),
+    // the radial image followed by nrad_max rows of padding (the unrolled contraction reads
     // nrad_max rows per point whatever n_rad is; what it reads past n_rad only reaches rows of C
     // that are dropped), + the warp's segment offsets
     static constexpr int y_bytes = (TPB_PTS * L * ESIZE + 15) & ~15;
     __host__ __device__ static constexpr int r_bytes(int n_rad, int nrad_max) {
         return ((TPB_PTS * n_rad + nrad_max) * (LMAX + 1) * ESIZE + 15) & ~15;
     }
+    // + a staging image of one segment's coefficients [n_rad][L] (leaves as one bulk store) + two
+    // mbarriers (one per radial image: the image arrives as ONE bulk load)
+    __host__ __device__ static constexpr int c_bytes(int n_rad) { return (n_rad * L * ESIZE + 15) & ~15; }
     __host__ __device__ static constexpr int warp_bytes(int n_rad, int nrad_max) {
-        return y_bytes + 2 * r_bytes(n_rad, nrad_max) + (EXP_SPW + 1) * 8 + 8;
+        return y_bytes + r_bytes(n_rad, nrad_max) + c_bytes(n_rad) + (EXP_SPW + 1) * 8 + 8 + 16;
     }
 };
 
 template <typename T, typename R, int LMAX, int NRAD_MAX>
-__global__ void __launch_bounds__(128) sph_expand_kernel(const ExpandParams prm) {
+__global__ void __launch_bounds__(128, 4) sph_expand_kernel(const ExpandParams prm) {
     using RT = rec<R>;
     using Shape = ExpandShape<sizeof(T), LMAX>;
     constexpr int L = Shape::L;
@@ -91,15 +95,29 @@ __global__ void __launch_bounds__(128) sph_expand_kernel(const ExpandParams prm)
     if (seg0 >= prm.n_seg) return;
     unsigned char* my = smem + (size_t)warp * Shape::warp_bytes(n_rad, NRAD_MAX);
     T* Ys = reinterpret_cast<T*>(my);
-    T* Rbuf[2] = {reinterpret_cast<T*>(my + Shape::y_bytes),
-                  reinterpret_cast<T*>(my + Shape::y_bytes + Shape::r_bytes(n_rad, NRAD_MAX))};
-    int64_t* sp = reinterpret_cast<int64_t*>(my + Shape::y_bytes + 2 * Shape::r_bytes(n_rad, NRAD_MAX));
+    // ONE radial image: the next tile's values are requested right after this tile's contraction and
+    // land while the next tile's harmonics are evaluated (a second image would cost a resident CTA)
+    T* Rs = reinterpret_cast<T*>(my + Shape::y_bytes);
+    T* Cs = reinterpret_cast<T*>(my + Shape::y_bytes + Shape::r_bytes(n_rad, NRAD_MAX));
+    int64_t* sp = reinterpret_cast<int64_t*>(my + Shape::y_bytes + Shape::r_bytes(n_rad, NRAD_MAX) + Shape::c_bytes(n_rad));
+    uint64_t* bar = reinterpret_cast<uint64_t*>(sp + EXP_SPW + 2);
     const int pl = lane & (TPB_PTS - 1);   // point inside the tile
     const bool sinb = lane >= TPB_PTS;     // branch
     const T* __restrict__ xyz = static_cast<const T*>(prm.xyz);
     const T* __restrict__ radial = static_cast<const T*>(prm.radial);
     T* __restrict__ coeff = static_cast<T*>(prm.coeff);
     const int rstride = n_rad * (LMAX + 1);   // radial values per point
+    // a tile's radial values are one contiguous range of global memory: where a point's share is a
+    // multiple of 16 bytes the range is 16-byte aligned whatever its first point, and it arrives as ONE
+    // bulk load (TMA) signalled on an mbarrier; otherwise element by element (cp.async)
+    const bool r_bulk = (rstride * (int)sizeof(T)) % 16 == 0;
+    // likewise a segment's coefficients leave as ONE bulk store from the staging image
+    const bool c_bulk = (n_rad * L * (int)sizeof(T)) % 16 == 0;
+    if (lane == 0) {
+        mbar_init(bar, 1);
+        fence_mbar_init();
+    }
+    uint32_t phase = 0u;   // parity of the mbarrier
     // this warp's segments j = 0 .. EXP_SPW-1 are the points sp[j] .. sp[j+1]-1 (segments past the
     // end are empty)
     if (lane <= EXP_SPW) {
@@ -127,6 +145,33 @@ __global__ void __launch_bounds__(128) sph_expand_kernel(const ExpandParams prm)
     // c[seg, n, lm] of segment j: lane holds C[n = fr + 8 mt][m-index 8 t + 2 fk + {0, 1}] of every tile
     auto flush = [&](int j) {
         const int64_t seg = seg0 + j;
+        if (c_bulk) {
+            if (lane == 0) bulk_wait_read<0>();   // the previous segment's store has read the staging image
+            __syncwarp();
+            static_for<0, LMAX + 1>([&](auto lc) {
+                constexpr int l = decltype(lc)::value;
+                constexpr int NTL = Tiles::of(l), T0 = Tiles::first(l);
+                static_for<0, NTL>([&](auto tc) {
+                    constexpr int t = decltype(tc)::value;
+#pragma unroll
+                    for (int mt = 0; mt < MT; ++mt) {
+                        const int n = fr + 8 * mt;
+#pragma unroll
+                        for (int e = 0; e < 2; ++e) {
+                            const int jm = 8 * t + 2 * fk + e;
+                            if (n < n_rad && jm < 2 * l + 1) Cs[n * L + l * l + jm] = static_cast<T>(acc[mt][T0 + t][e]);
+                        }
+                    }
+                });
+            });
+            fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) {
+                bulk_store(coeff + seg * n_rad * L, Cs, (uint32_t)(n_rad * L * (int)sizeof(T)));
+                bulk_commit();
+            }
+            return;
+        }
         static_for<0, LMAX + 1>([&](auto lc) {
             constexpr int l = decltype(lc)::value;
             constexpr int NTL = Tiles::of(l), T0 = Tiles::first(l);
@@ -153,14 +198,24 @@ __global__ void __launch_bounds__(128) sph_expand_kernel(const ExpandParams prm)
             if (j < EXP_SPW) k0 = sp[j];
         }
     };
-    // inputs of a tile: radial values by cp.async into image b (absent points' rows zeroed: they
-    // contribute 0), xyz into registers
-    auto fetch = [&](int j, int64_t k0, int b, T& xa, T& ya, T& za) {
+    // inputs of a tile: its radial values into the image (absent points' rows zeroed: they contribute
+    // 0), its points into registers
+    auto fetch_radial = [&](int j, int64_t k0) {
         const int np = (int)((sp[j + 1] - k0 < TPB_PTS) ? sp[j + 1] - k0 : TPB_PTS);
-        T* dst = Rbuf[b];
-        for (int i = lane; i < np * rstride; i += 32) cp_async_elem(dst + i, radial + k0 * rstride + i);
-        cp_async_commit();
-        for (int i = np * rstride + lane; i < TPB_PTS * rstride; i += 32) dst[i] = T(0);
+        if (r_bulk) {
+            if (lane == 0) {
+                const uint32_t bytes = (uint32_t)(np * rstride * (int)sizeof(T));
+                mbar_arrive_expect_tx(bar, bytes);
+                bulk_load(Rs, radial + k0 * rstride, bytes, bar);
+            }
+        } else {
+            for (int i = lane; i < np * rstride; i += 32) cp_async_elem(Rs + i, radial + k0 * rstride + i);
+            cp_async_commit();
+        }
+        for (int i = np * rstride + lane; i < TPB_PTS * rstride; i += 32) Rs[i] = T(0);
+    };
+    auto fetch_xyz = [&](int j, int64_t k0, T& xa, T& ya, T& za) {
+        const int np = (int)((sp[j + 1] - k0 < TPB_PTS) ? sp[j + 1] - k0 : TPB_PTS);
         xa = T(0), ya = T(0), za = T(1);   // lanes past the end compute a harmless point
         if (pl < np) {
             xa = __ldg(xyz + 3 * (k0 + pl) + 0);
@@ -173,25 +228,20 @@ __global__ void __launch_bounds__(128) sph_expand_kernel(const ExpandParams prm)
     int64_t k0 = sp[0];
     settle(j, k0);
     T xn = T(0), yn = T(0), zn = T(1);
-    int buf = 0;
-    if (j < EXP_SPW) fetch(j, k0, 0, xn, yn, zn);
+    if (j < EXP_SPW) {
+        fetch_radial(j, k0);
+        fetch_xyz(j, k0, xn, yn, zn);
+    }
     zero_acc();
     while (j < EXP_SPW) {
         const int np = (int)((sp[j + 1] - k0 < TPB_PTS) ? sp[j + 1] - k0 : TPB_PTS);
         const double x = static_cast<double>(xn), y = static_cast<double>(yn), z = static_cast<double>(zn);
-        const T* Rs = Rbuf[buf];
         // the next tile (of this segment or of the warp's next non-empty one): its inputs are in
         // flight while this tile is evaluated and contracted
         int jn = j;
         int64_t kn = k0 + TPB_PTS;
         settle(jn, kn);
-        __syncwarp();   // the previous tile's contraction is done with the Y image and the other R image
-        if (jn < EXP_SPW) {
-            fetch(jn, kn, buf ^ 1, xn, yn, zn);
-            cp_async_wait_but_one();
-        } else {
-            cp_async_wait_all();
-        }
+        if (jn < EXP_SPW) fetch_xyz(jn, kn, xn, yn, zn);   // in flight through this tile
         // ---- harmonics of the tile: two lanes per point ----------------------------------------
         R X, Y, Z;
         double rinv;
@@ -232,6 +282,12 @@ __global__ void __launch_bounds__(128) sph_expand_kernel(const ExpandParams prm)
                 s = sn;
             }
         });
+        if (r_bulk) {   // this tile's radial image has landed (it was in flight through this evaluation)
+            mbar_wait(bar, phase);
+            phase ^= 1u;
+        } else {
+            cp_async_wait_all();
+        }
         __syncwarp();
         // ---- contract over the tile's points, 4 at a time (K of the DMMA) --------------------------
         // What a fragment reads outside the valid ranges (n >= n_rad: the next point's radial values
@@ -256,14 +312,16 @@ __global__ void __launch_bounds__(128) sph_expand_kernel(const ExpandParams prm)
                 });
             }
         }
-            if (jn != j) {   // the segment is complete
+        __syncwarp();   // every lane is done with the radial image and the Y image
+        if (jn < EXP_SPW) fetch_radial(jn, kn);   // lands while the next tile's harmonics are evaluated
+        if (jn != j) {   // the segment is complete
             flush(j);
             zero_acc();
         }
         j = jn;
         k0 = kn;
-        buf ^= 1;
     }
+    if (c_bulk && lane == 0) bulk_wait_read<0>();   // shared memory must outlive the bulk stores' reads of it
     // empty segments: zeros
     for (int je = 0; je < EXP_SPW; ++je) {
         if (seg0 + je < prm.n_seg && sp[je] == sp[je + 1])
