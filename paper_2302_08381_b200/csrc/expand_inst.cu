@@ -36,9 +36,20 @@ template <int LMAX, int NRAD_MAX> static int launch_nr(int smem_optin, ExpandPar
         if (dev >= 0 && dev < 64) attr_bytes[dev] = smem;
     }
     prm.warps_per_cta = warps;
-    const int64_t per_cta = (int64_t)warps * EXP_SPW;   // segments per CTA
-    const int64_t ctas = (prm.n_seg + per_cta - 1) / per_cta;
-    if (ctas > 0x7fffffff) return 1;
+    // persistent grid: as many CTAs as are resident at once (the kernel shares the segments among them by
+    // point count), fewer when there are fewer segments than warps
+    static int resident[64] = {0}, resident_smem[64] = {0};     // per device, for the last shared-memory size (benign race, idempotent)
+    if (dev < 0 || dev >= 64) return -1;
+    if (resident[dev] == 0 || resident_smem[dev] != smem) {
+        int sms = 0, per_sm = 0;
+        if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return -1;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, warps * 32, smem) != cudaSuccess) return -1;
+        if (per_sm < 1) per_sm = 1;
+        resident[dev] = sms * per_sm;
+        resident_smem[dev] = smem;
+    }
+    int64_t ctas = (prm.n_seg + warps - 1) / warps;
+    if (ctas > resident[dev]) ctas = resident[dev];
     kern<<<(unsigned)ctas, warps * 32, smem, stream>>>(prm);
     return cudaGetLastError() == cudaSuccess ? 0 : -1;
 }

@@ -39,7 +39,6 @@ struct ExpandParams {
 };
 
 constexpr int EXP_MAX_RAD = 16;   // two M-tiles of 8 radial indices
-constexpr int EXP_SPW = 4;        // consecutive segments one warp works through
 
 // N-tiles of the contraction: degree l has ceil((2l+1)/8) tiles of 8 consecutive m
 template <int LMAX> struct ExpandTiles {
@@ -77,7 +76,7 @@ template <int ESIZE, int LMAX> struct ExpandShape {
     // mbarriers (one per radial image: the image arrives as ONE bulk load)
     __host__ __device__ static constexpr int c_bytes(int n_rad) { return (n_rad * L * ESIZE + 15) & ~15; }
     __host__ __device__ static constexpr int warp_bytes(int n_rad, int nrad_max) {
-        return y_bytes + r_bytes(n_rad, nrad_max) + c_bytes(n_rad) + (EXP_SPW + 1) * 8 + 8 + 16;
+        return y_bytes + r_bytes(n_rad, nrad_max) + c_bytes(n_rad) + 16;
     }
 };
 
@@ -91,16 +90,33 @@ __global__ void __launch_bounds__(128, 4) sph_expand_kernel(const ExpandParams p
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
     const int n_rad = prm.n_rad;
-    const int64_t seg0 = ((int64_t)blockIdx.x * prm.warps_per_cta + warp) * EXP_SPW;
-    if (seg0 >= prm.n_seg) return;
+    // Persistent grid: the warps share the segments in contiguous ranges of (nearly) equal POINT counts
+    // -- warp w of W takes the segments whose first point lies in [w n / W, (w+1) n / W) -- so that all
+    // of them finish together whatever the segment lengths (a grid of one CTA per few segments ran 3.5
+    // waves and idled through the last one).  Two binary searches over seg_ptr per warp.
+    const int64_t W = (int64_t)gridDim.x * prm.warps_per_cta, w = (int64_t)blockIdx.x * prm.warps_per_cta + warp;
+    const int64_t n_pts = __ldg(prm.seg_ptr + prm.n_seg);
+    auto first_at_or_after = [&](int64_t v) {   // first segment whose first point is >= v
+        int64_t lo = 0, hi = prm.n_seg;
+        while (lo < hi) {
+            const int64_t mid = (lo + hi) >> 1;
+            if (__ldg(prm.seg_ptr + mid) >= v) hi = mid;
+            else lo = mid + 1;
+        }
+        return lo;
+    };
+    const int64_t seg0 = w == 0 ? 0 : first_at_or_after((n_pts * w + W - 1) / W);
+    const int64_t seg1 = w == W - 1 ? prm.n_seg : first_at_or_after((n_pts * (w + 1) + W - 1) / W);
+    const int cnt = (int)(seg1 - seg0);   // this warp's segments j = 0 .. cnt-1 are the points SP(j) .. SP(j+1)-1
+    if (cnt <= 0) return;
+    auto SP = [&](int j) { return __ldg(prm.seg_ptr + seg0 + j); };
     unsigned char* my = smem + (size_t)warp * Shape::warp_bytes(n_rad, NRAD_MAX);
     T* Ys = reinterpret_cast<T*>(my);
     // ONE radial image: the next tile's values are requested right after this tile's contraction and
     // land while the next tile's harmonics are evaluated (a second image would cost a resident CTA)
     T* Rs = reinterpret_cast<T*>(my + Shape::y_bytes);
     T* Cs = reinterpret_cast<T*>(my + Shape::y_bytes + Shape::r_bytes(n_rad, NRAD_MAX));
-    int64_t* sp = reinterpret_cast<int64_t*>(my + Shape::y_bytes + Shape::r_bytes(n_rad, NRAD_MAX) + Shape::c_bytes(n_rad));
-    uint64_t* bar = reinterpret_cast<uint64_t*>(sp + EXP_SPW + 2);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(my + Shape::y_bytes + Shape::r_bytes(n_rad, NRAD_MAX) + Shape::c_bytes(n_rad));
     const int pl = lane & (TPB_PTS - 1);   // point inside the tile
     const bool sinb = lane >= TPB_PTS;     // branch
     const T* __restrict__ xyz = static_cast<const T*>(prm.xyz);
@@ -118,12 +134,6 @@ __global__ void __launch_bounds__(128, 4) sph_expand_kernel(const ExpandParams p
         fence_mbar_init();
     }
     uint32_t phase = 0u;   // parity of the mbarrier
-    // this warp's segments j = 0 .. EXP_SPW-1 are the points sp[j] .. sp[j+1]-1 (segments past the
-    // end are empty)
-    if (lane <= EXP_SPW) {
-        const int64_t sidx = seg0 + lane < prm.n_seg ? seg0 + lane : prm.n_seg;
-        sp[lane] = prm.seg_ptr[sidx];
-    }
     __syncwarp();
 
     using Tiles = ExpandTiles<LMAX>;
@@ -191,17 +201,17 @@ __global__ void __launch_bounds__(128, 4) sph_expand_kernel(const ExpandParams p
         });
     };
     // the tiles of this warp in order: (segment j, first point k0); advance() steps to the next one
-    // (j == EXP_SPW: none left).  Empty segments are skipped here and zero-filled at the end.
+    // (j == cnt: none left).  Empty segments are skipped here and zero-filled at the end.
     auto settle = [&](int& j, int64_t& k0) {
-        while (j < EXP_SPW && k0 >= sp[j + 1]) {
+        while (j < cnt && k0 >= SP(j + 1)) {
             ++j;
-            if (j < EXP_SPW) k0 = sp[j];
+            if (j < cnt) k0 = SP(j);
         }
     };
     // inputs of a tile: its radial values into the image (absent points' rows zeroed: they contribute
     // 0), its points into registers
     auto fetch_radial = [&](int j, int64_t k0) {
-        const int np = (int)((sp[j + 1] - k0 < TPB_PTS) ? sp[j + 1] - k0 : TPB_PTS);
+        const int np = (int)min((int64_t)TPB_PTS, SP(j + 1) - k0);
         if (r_bulk) {
             if (lane == 0) {
                 const uint32_t bytes = (uint32_t)(np * rstride * (int)sizeof(T));
@@ -215,7 +225,7 @@ __global__ void __launch_bounds__(128, 4) sph_expand_kernel(const ExpandParams p
         for (int i = np * rstride + lane; i < TPB_PTS * rstride; i += 32) Rs[i] = T(0);
     };
     auto fetch_xyz = [&](int j, int64_t k0, T& xa, T& ya, T& za) {
-        const int np = (int)((sp[j + 1] - k0 < TPB_PTS) ? sp[j + 1] - k0 : TPB_PTS);
+        const int np = (int)min((int64_t)TPB_PTS, SP(j + 1) - k0);
         xa = T(0), ya = T(0), za = T(1);   // lanes past the end compute a harmless point
         if (pl < np) {
             xa = __ldg(xyz + 3 * (k0 + pl) + 0);
@@ -225,23 +235,23 @@ __global__ void __launch_bounds__(128, 4) sph_expand_kernel(const ExpandParams p
     };
 
     int j = 0;
-    int64_t k0 = sp[0];
+    int64_t k0 = SP(0);
     settle(j, k0);
     T xn = T(0), yn = T(0), zn = T(1);
-    if (j < EXP_SPW) {
+    if (j < cnt) {
         fetch_radial(j, k0);
         fetch_xyz(j, k0, xn, yn, zn);
     }
     zero_acc();
-    while (j < EXP_SPW) {
-        const int np = (int)((sp[j + 1] - k0 < TPB_PTS) ? sp[j + 1] - k0 : TPB_PTS);
+    while (j < cnt) {
+        const int np = (int)min((int64_t)TPB_PTS, SP(j + 1) - k0);
         const double x = static_cast<double>(xn), y = static_cast<double>(yn), z = static_cast<double>(zn);
         // the next tile (of this segment or of the warp's next non-empty one): its inputs are in
         // flight while this tile is evaluated and contracted
         int jn = j;
         int64_t kn = k0 + TPB_PTS;
         settle(jn, kn);
-        if (jn < EXP_SPW) fetch_xyz(jn, kn, xn, yn, zn);   // in flight through this tile
+        if (jn < cnt) fetch_xyz(jn, kn, xn, yn, zn);   // in flight through this tile
         // ---- harmonics of the tile: two lanes per point ----------------------------------------
         R X, Y, Z;
         double rinv;
@@ -313,7 +323,7 @@ __global__ void __launch_bounds__(128, 4) sph_expand_kernel(const ExpandParams p
             }
         }
         __syncwarp();   // every lane is done with the radial image and the Y image
-        if (jn < EXP_SPW) fetch_radial(jn, kn);   // lands while the next tile's harmonics are evaluated
+        if (jn < cnt) fetch_radial(jn, kn);   // lands while the next tile's harmonics are evaluated
         if (jn != j) {   // the segment is complete
             flush(j);
             zero_acc();
@@ -323,8 +333,8 @@ __global__ void __launch_bounds__(128, 4) sph_expand_kernel(const ExpandParams p
     }
     if (c_bulk && lane == 0) bulk_wait_read<0>();   // shared memory must outlive the bulk stores' reads of it
     // empty segments: zeros
-    for (int je = 0; je < EXP_SPW; ++je) {
-        if (seg0 + je < prm.n_seg && sp[je] == sp[je + 1])
+    for (int je = 0; je < cnt; ++je) {
+        if (SP(je) == SP(je + 1))
             for (int i = lane; i < n_rad * L; i += 32) coeff[(seg0 + je) * n_rad * L + i] = T(0);
     }
 }
