@@ -33,10 +33,10 @@ template <int MODE, bool CONV> static TqKernel pick(int deriv, int norm) {
     }
 }
 
-static TqKernel pick_direct(int deriv, int norm) {
-    if (deriv == 0) return norm ? sph_tq_kernel<tq_T, tq_R, 0, true, 0, false, true> : sph_tq_kernel<tq_T, tq_R, 0, false, 0, false, true>;
-    if (deriv == 1) return norm ? sph_tq_kernel<tq_T, tq_R, 1, true, 0, false, true> : sph_tq_kernel<tq_T, tq_R, 1, false, 0, false, true>;
-    return norm ? sph_tq_kernel<tq_T, tq_R, 2, true, 0, false, true> : sph_tq_kernel<tq_T, tq_R, 2, false, 0, false, true>;
+template <bool CONV> static TqKernel pick_direct(int deriv, int norm) {
+    if (deriv == 0) return norm ? sph_tq_kernel<tq_T, tq_R, 0, true, 0, CONV, true> : sph_tq_kernel<tq_T, tq_R, 0, false, 0, CONV, true>;
+    if (deriv == 1) return norm ? sph_tq_kernel<tq_T, tq_R, 1, true, 0, CONV, true> : sph_tq_kernel<tq_T, tq_R, 1, false, 0, CONV, true>;
+    return norm ? sph_tq_kernel<tq_T, tq_R, 2, true, 0, CONV, true> : sph_tq_kernel<tq_T, tq_R, 2, false, 0, CONV, true>;
 }
 
 // Launch shape: points per phase-A batch B (32, 16, 8), points per tile P, warps per CTA W, images
@@ -107,8 +107,18 @@ int TQ_NAME(sph_tq_launch)(const TqArgs& a) {
     if (!tab && (a.l_max + 1) * (a.l_max + 2) / 2 <= 64) bP = 8, bW = 4;   // short triangles: fewer, fuller warps
     int bN = tab ? shape[3] : 1;
     // direct stores (no staging image): table entries {B, 0, W, 0}, or the tq_direct option (1: on, 2: off)
-    bool direct = a.mode == 0 && !a.conv && ((tab && shape[3] == 0 && g_opt.tq_direct != 2) || g_opt.tq_direct == 1);
+    bool direct = a.mode == 0 && ((tab && shape[3] == 0 && g_opt.tq_direct != 2) || g_opt.tq_direct == 1);
     if (tab && shape[3] == 0) bP = 2, bN = 1;   // (used only when tq_direct = 2 turns the entry's direct stores off)
+    // Cells the table leaves to the unrolled kernels reach this one through sphericart_cuda_compute_ex (another
+    // convention) or when forced.  Measured there (e3nn axes, l_max 1-11): direct stores from 32-point batches
+    // with 2 warps (4 from l_max = 9) run 1.3-2.5x faster than the staged shapes above (f32 gradients
+    // l_max 4 / 10: 1.7 / 1.9 -> 2.7 / 3.9 TB/s); f64 with derivatives prefers 16-point staged tiles.
+    if (!tab && a.mode == 0 && g_opt.tq_direct == 0 && g_opt.tq_points == 0 && g_opt.tq_images == 0) {
+        const int T = (a.l_max + 1) * (a.l_max + 2) / 2;
+        bB = 32, bW = T <= 45 ? 2 : 4;
+        if (TQ_F64 && deriv >= 1) bP = 16, bN = 1, bW = a.l_max <= 5 ? 2 : 4;
+        else direct = true;
+    }
     // contracting modes: little or nothing staged: tiles of 16 points (8 pairs x chunks divide evenly among 8 warps)
     if (a.mode != 0) bP = 16, bN = a.mode == 1 ? 2 : 1, bW = 8, bB = 32;
     if (g_opt.tq_batch > 0) bB = g_opt.tq_batch;
@@ -134,8 +144,8 @@ int TQ_NAME(sph_tq_launch)(const TqArgs& a) {
 
     TqKernel kern = a.mode == 1 ? pick<1, false>(deriv, a.normalized)
                   : a.mode == 2 ? pick<2, false>(deriv, a.normalized)
-                  : a.conv ? pick<0, true>(deriv, a.normalized)
-                  : direct ? pick_direct(deriv, a.normalized) : pick<0, false>(deriv, a.normalized);
+                  : a.conv ? (direct ? pick_direct<true>(deriv, a.normalized) : pick<0, true>(deriv, a.normalized))
+                  : direct ? pick_direct<false>(deriv, a.normalized) : pick<0, false>(deriv, a.normalized);
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, a.smem_optin) != cudaSuccess) return -1;
 
     TqParams prm{};
