@@ -172,13 +172,13 @@ __device__ __forceinline__ void tq_sts2(uint32_t a, double x, double y) {
 // (lanes = consecutive (l, m) of one point: runs of consecutive words for +m, descending ones for -m).
 // Where one tile image leaves room for a single CTA per SM (long rows), the shared memory this frees
 // buys resident warps, and the kernel is latency-bound there.
-template <typename T, typename R, int DERIV, bool NORM, int MODE, bool CONV, bool DIRECT = false>
+template <typename T, typename R, int DERIV, bool NORM, int MODE, bool CONV, int DIRECT = 0>
 __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 1) sph_tq_kernel(const TqParams prm) {
     using RT = rec<R>;
     constexpr int ES = (int)sizeof(T);
     constexpr int PTB = tq_pt_bytes(MODE);
     static_assert(MODE == 0 || (MODE == 1 && DERIV == 2) || (MODE == 2 && DERIV == 1), "mode / derivative order");
-    static_assert(!DIRECT || MODE == 0, "direct stores: forward mode only");
+    static_assert(DIRECT == 0 || ((DIRECT == 2 || DIRECT == 4) && MODE == 0), "direct stores (2 or 4 points per lane): forward mode only");
     extern __shared__ __align__(128) unsigned char smem[];
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
@@ -186,7 +186,7 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 1) sph_tq_kernel(const TqPa
     const int l_max = prm.l_max;
     const int L = (l_max + 1) * (l_max + 1);
     const int B = prm.batch, P = DIRECT ? prm.batch : prm.pts_tile;   // (DIRECT: the batch is the one tile)
-    const TqSmem lay(l_max, DERIV, tq_img_rows(MODE, DERIV), PTB, ES, B, P, prm.n_images, DIRECT);
+    const TqSmem lay(l_max, DERIV, tq_img_rows(MODE, DERIV), PTB, ES, B, P, prm.n_images, DIRECT != 0);
     const int TT = lay.T, TP = lay.TP, CP = lay.CP;
     const uint32_t s0 = smem_u32(smem);
     const uint32_t sGT = s0 + (uint32_t)lay.gt_off, sHT = s0 + (uint32_t)lay.ht_off, sLM = s0 + (uint32_t)lay.lm_off;
@@ -225,7 +225,10 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 1) sph_tq_kernel(const TqPa
     const int NCH = (TT + 31) >> 5;                    // 32-pair chunks of one point's triangle
     const int d_pl = W / NCH, d_ch = W - d_pl * NCH;   // one step of a warp through the (point pair, chunk) units
     const int w_pl0 = warp / NCH, w_ch0 = warp - w_pl0 * NCH;
-    const int PP = (P + 1) >> 1;                       // pairs of points per tile (the last one may hold one point)
+    // points one lane takes through phase B with the same (l, m): 2, or DIRECT = 4 (the per-(l, m) decode and
+    // table loads are then shared by four points; which of the two is faster depends on the cell: tq_table.h)
+    constexpr int NPL = DIRECT == 4 ? 4 : 2;
+    const int PP = (P + NPL - 1) / NPL;               // groups of NPL points per tile (the last one may hold fewer)
     const uint32_t row_b = (uint32_t)L * ES;          // bytes of one row of one point
     const uint32_t s_bytes = (uint32_t)P * row_b;     // bytes of the tile's sph image
     // derivative axis a of the evaluation frame is row `row[a]` of the caller's arrays
@@ -254,7 +257,7 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 1) sph_tq_kernel(const TqPa
         if constexpr (CONV) sl = tq_lds(sSL + l * 8);
         const double dmm = dm * (dm - 1.0);
 #pragma unroll
-        for (int j = 0; j < 2; ++j) {
+        for (int j = 0; j < NPL; ++j) {
             if (j >= npt) break;
             const int pl = plb + j;   // point inside the image
             const int pb = pbb + j;   // ... inside the batch
@@ -621,9 +624,9 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 1) sph_tq_kernel(const TqPa
                 while (pp < PP) {
                     const int t = ch * 32 + lane;
                     if constexpr (DIRECT) {   // straight to the caller's arrays; points past the end are skipped here
-                        const int left = (int)min((int64_t)P, n - p0) - 2 * pp;
+                        const int left = (int)min((int64_t)P, n - p0) - NPL * pp;
                         if (t < TT && left > 0)
-                            assemble(t, 2 * pp, 2 * pp, left, nullptr, reinterpret_cast<unsigned char*>(sph + p0 * L),
+                            assemble(t, NPL * pp, NPL * pp, left, nullptr, reinterpret_cast<unsigned char*>(sph + p0 * L),
                                      reinterpret_cast<unsigned char*>(dsph + (DERIV >= 1 ? p0 * 3 * L : 0)),
                                      reinterpret_cast<unsigned char*>(ddsph + (DERIV >= 2 ? p0 * 9 * L : 0)), acc);
                     } else if (t < TT) assemble(t, 2 * pp, ti * P + 2 * pp, P - 2 * pp, nullptr, sS, sG, sH, acc);

@@ -33,7 +33,7 @@ struct SphOptions {
     int tq_warps = 0;        // warps per CTA of the tq kernel (0: the planner's choice)
     int tq_images = 0;       // staging images per CTA of the tq kernel (0: two unless only one fits)
     int tq_cs_warps = 0;     // f64 I/O: warps of the tq kernel's recurrence phase that run Eq. 9 only (0: balanced by the planner)
-    int tq_direct = 0;       // tq forward: 1 = store straight to global memory (no staging image), 2 = never, 0 = the table's choice
+    int tq_direct = 0;       // tq forward: 1 / 4 = store straight to global memory (no staging image), two / four points per lane; 2 = never; 0 = the table's choice
     int tq_batch = 0;        // points per phase-A batch of the tq kernel (0: the planner's choice)
     int64_t host_chunk_bytes = (int64_t)256 << 20;   // _host entry points: bytes per chunk and stream
 };

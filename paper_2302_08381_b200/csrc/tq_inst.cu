@@ -33,10 +33,10 @@ template <int MODE, bool CONV> static TqKernel pick(int deriv, int norm) {
     }
 }
 
-template <bool CONV> static TqKernel pick_direct(int deriv, int norm) {
-    if (deriv == 0) return norm ? sph_tq_kernel<tq_T, tq_R, 0, true, 0, CONV, true> : sph_tq_kernel<tq_T, tq_R, 0, false, 0, CONV, true>;
-    if (deriv == 1) return norm ? sph_tq_kernel<tq_T, tq_R, 1, true, 0, CONV, true> : sph_tq_kernel<tq_T, tq_R, 1, false, 0, CONV, true>;
-    return norm ? sph_tq_kernel<tq_T, tq_R, 2, true, 0, CONV, true> : sph_tq_kernel<tq_T, tq_R, 2, false, 0, CONV, true>;
+template <bool CONV, int NPL> static TqKernel pick_direct(int deriv, int norm) {
+    if (deriv == 0) return norm ? sph_tq_kernel<tq_T, tq_R, 0, true, 0, CONV, NPL> : sph_tq_kernel<tq_T, tq_R, 0, false, 0, CONV, NPL>;
+    if (deriv == 1) return norm ? sph_tq_kernel<tq_T, tq_R, 1, true, 0, CONV, NPL> : sph_tq_kernel<tq_T, tq_R, 1, false, 0, CONV, NPL>;
+    return norm ? sph_tq_kernel<tq_T, tq_R, 2, true, 0, CONV, NPL> : sph_tq_kernel<tq_T, tq_R, 2, false, 0, CONV, NPL>;
 }
 
 // Launch shape: points per phase-A batch B (32, 16, 8), points per tile P, warps per CTA W, images
@@ -106,9 +106,11 @@ int TQ_NAME(sph_tq_launch)(const TqArgs& a) {
     int bW = tab ? shape[2] : 8;
     if (!tab && (a.l_max + 1) * (a.l_max + 2) / 2 <= 64) bP = 8, bW = 4;   // short triangles: fewer, fuller warps
     int bN = tab ? shape[3] : 1;
-    // direct stores (no staging image): table entries {B, 0, W, 0}, or the tq_direct option (1: on, 2: off)
-    bool direct = a.mode == 0 && ((tab && shape[3] == 0 && g_opt.tq_direct != 2) || g_opt.tq_direct == 1);
-    if (tab && shape[3] == 0) bP = 2, bN = 1;   // (used only when tq_direct = 2 turns the entry's direct stores off)
+    // direct stores (no staging image): table entries {B, 0, W, 0 | 4} (two or four points per lane in phase B), or
+    // the tq_direct option (1: on with two points per lane, 4: on with four, 2: off)
+    bool direct = a.mode == 0 && ((tab && shape[1] == 0 && g_opt.tq_direct != 2) || g_opt.tq_direct == 1 || g_opt.tq_direct == 4);
+    int npl = g_opt.tq_direct == 4 ? 4 : (g_opt.tq_direct == 0 && tab && shape[1] == 0 && shape[3] == 4 ? 4 : 2);
+    if (tab && shape[1] == 0) bP = 2, bN = 1;   // (used only when tq_direct = 2 turns the entry's direct stores off)
     // Cells the table leaves to the unrolled kernels reach this one through sphericart_cuda_compute_ex (another
     // convention) or when forced.  Measured there (e3nn axes, l_max 1-11): direct stores from 32-point batches
     // with 2 warps (4 from l_max = 9) run 1.3-2.5x faster than the staged shapes above (f32 gradients
@@ -144,8 +146,10 @@ int TQ_NAME(sph_tq_launch)(const TqArgs& a) {
 
     TqKernel kern = a.mode == 1 ? pick<1, false>(deriv, a.normalized)
                   : a.mode == 2 ? pick<2, false>(deriv, a.normalized)
-                  : a.conv ? (direct ? pick_direct<true>(deriv, a.normalized) : pick<0, true>(deriv, a.normalized))
-                  : direct ? pick_direct<false>(deriv, a.normalized) : pick<0, false>(deriv, a.normalized);
+                  : a.conv ? (direct ? (npl == 4 ? pick_direct<true, 4>(deriv, a.normalized) : pick_direct<true, 2>(deriv, a.normalized))
+                                     : pick<0, true>(deriv, a.normalized))
+                  : direct ? (npl == 4 ? pick_direct<false, 4>(deriv, a.normalized) : pick_direct<false, 2>(deriv, a.normalized))
+                           : pick<0, false>(deriv, a.normalized);
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, a.smem_optin) != cudaSuccess) return -1;
 
     TqParams prm{};

@@ -398,18 +398,19 @@ def test_two_phase_kernel_direct_stores(sph, oracle, dtype, shape, option):
     all three output arrays (nothing written outside them, every element inside written)."""
     np_dt = np.float32 if dtype == "f32" else np.float64
     option("force_kernel", "tq")
-    option("tq_direct", 1)
     option("tq_batch", shape[0])
     option("tq_warps", shape[1])
     for l_max, n in ((0, 5), (3, 70), (9, 203), (14, 77), (16, 1), (23, 70), (32, 45)):
         xyz = W.make_xyz("C2" if l_max <= 16 else "C4", n, seed=l_max).astype(np_dt)
         for normalized, deriv in ((True, 2), (False, 1), (True, 0), (False, 2)):
+            option("tq_direct", 4 if (l_max + deriv) % 2 else 1)      # four / two points per lane in phase B
             before = sph.sphericart_cuda_launch_count()
             s, d, h = _run_gpu(sph, xyz, l_max, normalized, deriv >= 1, deriv >= 2)
             assert sph.sphericart_cuda_launch_count() == before + 1
             assert sph.sphericart_cuda_last_kernel() == "tq"
             _compare(oracle, xyz, l_max, normalized, dtype, s, d, h,
                      f"tq direct shape={shape} {dtype} l_max={l_max} n={n} norm={normalized} deriv={deriv}")
+    option("tq_direct", 4)
     l_max, n = 21, 45
     L = (l_max + 1) ** 2
     t_dt = torch.float32 if dtype == "f32" else torch.float64
