@@ -87,10 +87,16 @@ template <int ESIZE, int DERIV, int LMAX, int SPLIT, bool BB = false> struct Tpb
     // 16-way when the pitch in 32-bit words is 0 or 16 modulo 32, i.e. for l_max = 3 (mod 4)
     // (measured: f32 l_max = 7 ran at 2.0 TB/s where l_max = 6 and 8 reach 6.7 and 6.9).  Those row
     // lengths get 16 bytes of padding per point (pitch = 4 or 20 mod 32: 2-way), the image is then
-    // no longer byte-identical to global memory and leaves by 16-byte vector stores instead of TMA.
+    // no longer byte-identical to global memory and leaves as one bulk store per point and array where a
+    // point's rows are long enough (`row_bulk`), by 16-byte vector stores otherwise.  Measured, vector ->
+    // bulk rows: f32 V+G l_max 7 / 11: 6.2 / 4.4 -> 6.9 / 5.2 TB/s, f32 V l_max 15: 5.7 -> 6.2, f32 V+G+H
+    // l_max 3: 5.2 -> 6.0, f64 V+G l_max 7: 5.3 -> 5.9; but f32 V l_max 3 / 7 / 11 (rows of 64-576 bytes):
+    // 4.2 / 6.1 / 5.4 -> 3.3 / 5.5 / 5.0, f64 V+G l_max 3: 6.2 -> 5.5, f64 V l_max 11: 4.7 -> 4.5.
     static constexpr int words = L * ESIZE / 4;
     static constexpr bool pad = (words % 32 == 0) || (words % 32 == 16);
     static constexpr int pad_elems = pad ? 16 / ESIZE : 0;
+    static constexpr int point_bytes = L * ESIZE * (DERIV == 0 ? 1 : (DERIV == 1 ? 4 : 13));
+    static constexpr bool row_bulk = pad && (DERIV == 0 ? (ESIZE == 4 && point_bytes >= 1024) : point_bytes >= 800);
     static constexpr int pitch_s = L + pad_elems;          // elements between the points' rows of sph
     static constexpr int pitch_g = 3 * L + pad_elems;      // ... of dsph
     static constexpr int s_bytes = pts * pitch_s * ESIZE;
@@ -175,7 +181,8 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
 
         // the image we are about to overwrite must have been read out by its bulk store
         if (tile > t_begin) {
-            if (threadIdx.x == 0) bulk_wait_read<0>();
+            // (padded images: one thread per point has issued stores; the others wait on nothing)
+            if (Shape::row_bulk || threadIdx.x == 0) bulk_wait_read<0>();
             cta_sync();
         }
         T* S = reinterpret_cast<T*>(smem) + pl * PS;
@@ -354,8 +361,20 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
         T* S0 = reinterpret_cast<T*>(smem);
         T* G0 = reinterpret_cast<T*>(smem + S_BYTES);
         T* H0 = reinterpret_cast<T*>(smem + S_BYTES + G_BYTES);
-        if constexpr (Shape::pad) {
-            // padded image: rows leave as 16-byte vectors (row lengths are multiples of 16 bytes here)
+        if constexpr (Shape::row_bulk) {
+            // padded image (rows 16 bytes further apart than in global memory; row lengths are multiples of
+            // 64 bytes here), long rows: every point's rows leave as bulk stores of their own, issued by one
+            // thread per point
+            const int np = (int)((n - p0 < PTS) ? n - p0 : PTS);
+            if ((int)threadIdx.x < np) {
+                const int r = threadIdx.x;
+                bulk_store_hint(sph + (p0 + r) * L, S0 + r * PS, (uint32_t)(L * sizeof(T)), policy);
+                if (DERIV >= 1) bulk_store_hint(dsph + (p0 + r) * 3 * L, G0 + r * PG, (uint32_t)(3 * L * sizeof(T)), policy);
+                if (DERIV >= 2) bulk_store_hint(ddsph + (p0 + r) * 9 * L, H0 + r * PH, (uint32_t)(9 * L * sizeof(T)), policy);
+                bulk_commit();
+            }
+        } else if constexpr (Shape::pad) {
+            // padded image, short rows: 16-byte vectors (row lengths are multiples of 16 bytes here)
             constexpr int VE = 16 / (int)sizeof(T);        // elements per vector
             const int np = (int)((n - p0 < PTS) ? n - p0 : PTS);
             constexpr int VS = L / VE, VG = 3 * L / VE;    // vectors per point
@@ -396,7 +415,7 @@ __global__ void __launch_bounds__(SPLIT * 32, TpbShape<sizeof(T), DERIV, LMAX, S
         }
     }
     // shared memory must outlive the bulk stores' reads of it
-    if (threadIdx.x == 0) bulk_wait_read<0>();
+    if (Shape::row_bulk || threadIdx.x == 0) bulk_wait_read<0>();
 }
 
 }  // namespace sphb200
