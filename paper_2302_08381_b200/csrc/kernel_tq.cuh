@@ -223,7 +223,7 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 1) sph_tq_kernel(const TqPa
     for (int i = threadIdx.x; i < B * 2; i += blockDim.x) tq_sts2(sCS + ((i >> 1) * CP + (i & 1)) * 16, 0.0, 0.0);
 
     const int NCH = (TT + 31) >> 5;                    // 32-pair chunks of one point's triangle
-    const int d_pl = W / NCH, d_ch = W - d_pl * NCH;   // one step of a warp through the (point pair, chunk) units
+    const int d_pl = W / NCH, d_ch = W - d_pl * NCH;   // one step of a warp through the (point group, chunk) units
     const int w_pl0 = warp / NCH, w_ch0 = warp - w_pl0 * NCH;
     // points one lane takes through phase B with the same (l, m): 2, or DIRECT = 4 (the per-(l, m) decode and
     // table loads are then shared by four points; which of the two is faster depends on the cell: tq_table.h)
@@ -620,21 +620,41 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 1) sph_tq_kernel(const TqPa
                 __syncwarp();
             }
             if constexpr (MODE == 0) {
-                int pp = w_pl0, ch = w_ch0;   // pp: PAIR of points of the tile (a lane does the same (l, m) for both)
-                while (pp < PP) {
-                    const int t = ch * 32 + lane;
-                    if constexpr (DIRECT) {   // straight to the caller's arrays; points past the end are skipped here
-                        const int left = (int)min((int64_t)P, n - p0) - NPL * pp;
-                        if (t < TT && left > 0)
-                            assemble(t, NPL * pp, NPL * pp, left, nullptr, reinterpret_cast<unsigned char*>(sph + p0 * L),
-                                     reinterpret_cast<unsigned char*>(dsph + (DERIV >= 1 ? p0 * 3 * L : 0)),
-                                     reinterpret_cast<unsigned char*>(ddsph + (DERIV >= 2 ? p0 * 9 * L : 0)), acc);
-                    } else if (t < TT) assemble(t, 2 * pp, ti * P + 2 * pp, P - 2 * pp, nullptr, sS, sG, sH, acc);
-                    ch += d_ch;
-                    pp += d_pl;
-                    if (ch >= NCH) {
-                        ch -= NCH;
-                        ++pp;
+                // work units = (group of NPL points of the tile, 32 consecutive (l, m) pairs of the triangle), dealt
+                // to the warps round-robin; group and chunk advance incrementally (warp-uniform, no division), so
+                // that everything derived from them stays in uniform registers.  The last chunk of every group is
+                // partly empty (56 % of the lanes busy at l_max = 7, 69 % at 8 and 10, 82-86 % at 9, 11, 13, 15).
+                // FLAT: the items (group, pair) flattened instead, i = group * TT + t in runs of 32 lanes -- every
+                // lane busy, but group and pair are per-lane values then.  Measured over all cells: it pays for the
+                // f32 Hessians through an image (l_max 7 / 8 / 10 / 13: 3.9 / 4.6 / 4.3 / 4.9 -> 4.7 / 5.0 / 4.7 /
+                // 5.2 TB/s) and loses 3-15 % elsewhere (f64: at the HBM roof already; direct stores: more address
+                // arithmetic per lane), so it is compiled in for those kernels only.  group = floor(i / TT) by a
+                // float reciprocal, exact here: i < 16 * 561 and the fraction keeps 0.5 / TT clear of an integer.
+                constexpr bool FLAT = sizeof(T) == 4 && DERIV == 2 && DIRECT == 0;
+                if constexpr (FLAT) {
+                    const int items = PP * TT;
+                    const float rcp_tt = 1.0f / (float)TT;
+                    for (int i = warp * 32 + lane; i < items; i += W * 32) {
+                        const int pp = (int)(((float)i + 0.5f) * rcp_tt);
+                        assemble(i - pp * TT, 2 * pp, ti * P + 2 * pp, P - 2 * pp, nullptr, sS, sG, sH, acc);
+                    }
+                } else {
+                    int pp = w_pl0, ch = w_ch0;
+                    while (pp < PP) {
+                        const int t = ch * 32 + lane;
+                        if constexpr (DIRECT) {   // straight to the caller's arrays; points past the end are skipped here
+                            const int left = (int)min((int64_t)P, n - p0) - NPL * pp;
+                            if (t < TT && left > 0)
+                                assemble(t, NPL * pp, NPL * pp, left, nullptr, reinterpret_cast<unsigned char*>(sph + p0 * L),
+                                         reinterpret_cast<unsigned char*>(dsph + (DERIV >= 1 ? p0 * 3 * L : 0)),
+                                         reinterpret_cast<unsigned char*>(ddsph + (DERIV >= 2 ? p0 * 9 * L : 0)), acc);
+                        } else if (t < TT) assemble(t, 2 * pp, ti * P + 2 * pp, P - 2 * pp, nullptr, sS, sG, sH, acc);
+                        ch += d_ch;
+                        pp += d_pl;
+                        if (ch >= NCH) {
+                            ch -= NCH;
+                            ++pp;
+                        }
                     }
                 }
             } else {
