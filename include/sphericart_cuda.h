@@ -150,6 +150,7 @@ int sphericart_cuda_vjp2(const void* xyz, const void* grad_sph, const void* v, v
  * harmonics are evaluated inside the kernel and never written to memory.
  *   xyz      [N,3]               in   the points r_k (e.g. neighbour vectors), N = seg_ptr[n_seg]
  *   radial   [N, n_rad, l_max+1] in   R_nl(r_k): the radial basis is the caller's (the paper fixes none)
+ *                                     (xyz and radial may both be NULL when N = 0: every segment empty, coeff = 0)
  *   seg_ptr  [n_seg+1] int64     in   DEVICE array of ascending offsets into the points: segment s
  *                                     (e.g. the neighbours of centre s) is seg_ptr[s] .. seg_ptr[s+1]-1;
  *                                     an empty segment gives zeros

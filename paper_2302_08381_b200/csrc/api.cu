@@ -681,8 +681,11 @@ int sphericart_cuda_expand(const void* xyz, const void* radial, const int64_t* s
     if (rc) return rc;
     if (n_rad < 1) return fail(SPHERICART_CUDA_EINVAL, "n_rad = %d must be at least 1", n_rad);
     if (n_seg == 0) return 0;
-    if (!xyz || !radial || !seg_ptr || !coeff)
-        return fail(SPHERICART_CUDA_EINVAL, "xyz, radial, seg_ptr and coeff must not be NULL when n_seg > 0");
+    if (!seg_ptr || !coeff) return fail(SPHERICART_CUDA_EINVAL, "seg_ptr and coeff must not be NULL when n_seg > 0");
+    // (xyz and radial are read for the points of non-empty segments only: both may be NULL when every
+    // segment is empty, i.e. seg_ptr[n_seg] = 0, which the host cannot see without a synchronisation)
+    if ((xyz == nullptr) != (radial == nullptr))
+        return fail(SPHERICART_CUDA_EINVAL, "xyz and radial must both be given, or both be NULL when there are no points");
     if (misaligned(xyz) || misaligned(radial) || misaligned(coeff) || (reinterpret_cast<uintptr_t>(seg_ptr) & 7u))
         return fail(SPHERICART_CUDA_EALIGN, "device pointers must be 16-byte aligned (seg_ptr: 8)");
     DeviceState* st = nullptr;

@@ -488,6 +488,38 @@ def test_stream_order_with_programmatic_dependent_launch(sph):
 
 
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_expand_segment_layouts(sph, oracle, dtype):
+    """N2, the layouts that stress how the persistent grid shares the segments among its warps (by point
+    count, two binary searches over seg_ptr): one long segment among empty ones, every segment empty,
+    a single segment, far more segments than points, far more warps than segments, a first segment that
+    is empty; with a radial row of 16-byte multiples (one bulk load per tile) and without (cp.async)."""
+    np_dt = np.float32 if dtype == "f32" else np.float64
+    rng = np.random.default_rng(77)
+
+    def run(counts, l_max, n_rad, what):
+        seg = np.concatenate([[0], np.cumsum(counts)]).astype(np.int64)
+        n = int(seg[-1])
+        xyz_all = rng.standard_normal((max(n, 1), 3)).astype(np_dt)
+        rad_all = rng.standard_normal((max(n, 1), n_rad, l_max + 1)).astype(np_dt)
+        xyz, rad = xyz_all[:n], rad_all[:n]
+        # (no points at all: the C entry still wants non-NULL pointers, so views of a one-row allocation)
+        x_d, r_d = torch.from_numpy(xyz_all).cuda()[:n], torch.from_numpy(rad_all).cuda()[:n]
+        c = sph.expand(x_d, r_d, torch.from_numpy(seg).cuda())
+        torch.cuda.synchronize()
+        parity.check_expand(c.cpu().numpy(), oracle.expand(xyz, rad, seg, l_max), rad, seg, l_max, dtype,
+                            f"expand {dtype} {what} l_max={l_max} n_rad={n_rad}")
+        assert np.all(c.cpu().numpy()[np.nonzero(np.diff(seg) == 0)[0]] == 0)
+
+    for l_max, n_rad in ((8, 8), (5, 3), (6, 7)):          # 72 / 18 / 49 radial values per point
+        run([0] * 40 + [5003] + [0] * 60, l_max, n_rad, "one long segment among empty ones")
+        run([0] * 500, l_max, n_rad, "every segment empty")
+        run([37], l_max, n_rad, "a single segment")
+        run(rng.integers(0, 2, size=20000), l_max, n_rad, "more segments than points")
+        run([700, 0, 1, 16, 17, 15], l_max, n_rad, "few segments, many warps")
+        run([0, 0, 33, 4], l_max, n_rad, "leading empty segments")
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
 def test_expand_eq1(sph, oracle, dtype):
     """N2: the fused density expansion against the oracle; every l_max with a kernel, n_rad across
     the three register variants, ragged / empty / long segments."""
