@@ -137,6 +137,14 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 1) sph_tv_kernel(const TvPa
         if (col_lane) {
             R X, Y, Z, r2;
             load_point(b0, X, Y, Z, r2);
+            // The previous batch's rows must have been read out of the image before anyone writes there again:
+            // the threads that issued their bulk stores wait for that HERE, after this batch's points are
+            // loaded and normalised (the stores' reads run under that work), and only the column warps meet at
+            // a barrier of their own -- the warps that run Eq. 9 never touch the image and are not held up.
+            if (bi > 0) {
+                if ((int)threadIdx.x < B) bulk_wait_read<0>();
+                named_bar_sync(1, Wq * 32);
+            }
             // this point's row, staged at the offset its global address has from a 16-byte boundary
             const uint32_t shift = (uint32_t)(((b0 + pt_l) & 15) * row_b) & 15u;
             const uint32_t row = sIMG + pt_l * lay.pitch + shift;
@@ -233,15 +241,15 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 1) sph_tv_kernel(const TvPa
                 if (body) bulk_store_hint(g + head / ES, src + head / ES, body, policy);
                 for (uint32_t i = (head + body) / ES; i < row_b / ES; ++i) st_cs(g + i, src[i]);
                 bulk_commit();
-                bulk_wait_read<0>();   // the row has been read: the image may be overwritten
             }
         }
-        __syncthreads();
         // (the points parked in shared memory two batches ahead, so that no lane waits on global memory at the
         // top of a batch, were measured: 3 % slower -- other CTAs cover that latency already)
         // (two images, so that a batch drains while the next is computed, were measured: slower everywhere --
         // the shared memory they take costs more resident CTAs than the second barrier costs time)
     }
+    // shared memory must outlive the bulk stores' reads of it
+    if ((int)threadIdx.x < B) bulk_wait_read<0>();
 }
 
 }  // namespace sphb200

@@ -93,9 +93,6 @@ struct WcParams {
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ void named_bar_sync(int id, int threads) {
-    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
-}
 
 template <typename T, typename R, int DERIV, bool NORM, bool LODD>
 __global__ void __launch_bounds__(WC_THREADS, 1) sph_wc_kernel(const WcParams prm) {
