@@ -691,9 +691,8 @@ int sphericart_cuda_expand(const void* xyz, const void* radial, const int64_t* s
     DeviceState* st = nullptr;
     rc = device_state(&st);
     if (rc) return rc;
-    // the compile-time kernel (DMMA contraction) where it has an instantiation; l_max <= 3 goes to the
-    // generic kernel, whose image of the harmonics is f64 (the tolerance is tightest there)
-    if (g_opt.force_kernel != FORCE_GENERIC && l_max > 3) {
+    // the compile-time kernel (DMMA contraction) where it has an instantiation (l_max <= 8, n_rad <= 16)
+    if (g_opt.force_kernel != FORCE_GENERIC) {
         const int r = (dtype == SPHERICART_CUDA_F32 ? sph_expand_launch_f32 : sph_expand_launch_f64)(
             st->smem_optin, xyz, radial, seg_ptr, n_seg, l_max, n_rad, coeff, static_cast<cudaStream_t>(stream));
         if (r < 0) return fail(SPHERICART_CUDA_ECUDA, "expand launch failed: %s", cudaGetErrorString(cudaGetLastError()));

@@ -68,7 +68,13 @@ template <int ESIZE, int LMAX> struct ExpandShape {
     // the radial image followed by nrad_max rows of padding (the unrolled contraction reads
     // nrad_max rows per point whatever n_rad is; what it reads past n_rad only reaches rows of C
     // that are dropped), + the warp's segment offsets
-    static constexpr int y_bytes = (TPB_PTS * L * ESIZE + 15) & ~15;
+    // The image of the harmonics is held in the I/O type, except for l_max <= 3 where it is f64 (rows an odd
+    // number of doubles apart): the tolerance 5e-6 (l_max + 1) is tightest there, an f32 image alone uses it up
+    // (measured: l_max = 1, n_rad = 16: 1.001e-5 against 1.0e-5), and the image is at most 2 KB anyway.
+    static constexpr bool y_f64 = LMAX <= 3;
+    static constexpr int y_size = y_f64 ? 8 : ESIZE;
+    static constexpr int y_pitch = y_f64 ? (L | 1) : L;
+    static constexpr int y_bytes = (TPB_PTS * y_pitch * y_size + 15) & ~15;
     __host__ __device__ static constexpr int r_bytes(int n_rad, int nrad_max) {
         return ((TPB_PTS * n_rad + nrad_max) * (LMAX + 1) * ESIZE + 15) & ~15;
     }
@@ -111,7 +117,9 @@ __global__ void __launch_bounds__(128, 4) sph_expand_kernel(const ExpandParams p
     if (cnt <= 0) return;
     auto SP = [&](int j) { return __ldg(prm.seg_ptr + seg0 + j); };
     unsigned char* my = smem + (size_t)warp * Shape::warp_bytes(n_rad, NRAD_MAX);
-    T* Ys = reinterpret_cast<T*>(my);
+    using YT = std::conditional_t<Shape::y_f64, double, T>;   // element type of the image of the harmonics
+    constexpr int LY = Shape::y_pitch;
+    YT* Ys = reinterpret_cast<YT*>(my);
     // ONE radial image: the next tile's values are requested right after this tile's contraction and
     // land while the next tile's harmonics are evaluated (a second image would cost a resident CTA)
     T* Rs = reinterpret_cast<T*>(my + Shape::y_bytes);
@@ -256,7 +264,7 @@ __global__ void __launch_bounds__(128, 4) sph_expand_kernel(const ExpandParams p
         R X, Y, Z;
         double rinv;
         RT::normalize(x, y, z, X, Y, Z, rinv);
-        T* S = Ys + pl * L;
+        YT* S = Ys + pl * LY;
         double Qc[LMAX + 1];
         R c = RT::make(1.0, 0.0), s = RT::make(0.0, 0.0);
         static_for<0, LMAX + 1>([&](auto mc) {
@@ -283,7 +291,7 @@ __global__ void __launch_bounds__(128, 4) sph_expand_kernel(const ExpandParams p
             static_for<m, LMAX + 1>([&](auto lc) {
                 constexpr int l = decltype(lc)::value;
                 constexpr int kc = l * (l + 1) + m, ks = l * (l + 1) - m;
-                if (emit) S[sinb ? ks : kc] = static_cast<T>(Qc[l] * A);   // Eq. 5
+                if (emit) S[sinb ? ks : kc] = static_cast<YT>(Qc[l] * A);   // Eq. 5
             });
             if constexpr (m < LMAX) {   // Eq. 9
                 const R cn = X * c - Y * s;
@@ -315,7 +323,7 @@ __global__ void __launch_bounds__(128, 4) sph_expand_kernel(const ExpandParams p
                     constexpr int NTL = Tiles::of(l), T0 = Tiles::first(l);
                     static_for<0, NTL>([&](auto tc) {
                         constexpr int t = decltype(tc)::value;
-                        const double bv = static_cast<double>(Ys[p * L + l * l + 8 * t + fr]);
+                        const double bv = static_cast<double>(Ys[p * LY + l * l + 8 * t + fr]);
 #pragma unroll
                         for (int mt = 0; mt < MT; ++mt) dmma_m8n8k4(acc[mt][T0 + t], a[mt], bv);
                     });
