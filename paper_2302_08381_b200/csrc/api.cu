@@ -701,6 +701,16 @@ int sphericart_cuda_expand(const void* xyz, const void* radial, const int64_t* s
             return 0;
         }
     }
+    // any l_max with n_rad <= 16: the run-time-l_max DMMA kernel, degrees in bands
+    if (g_opt.force_kernel != FORCE_GENERIC) {
+        const int r = (dtype == SPHERICART_CUDA_F32 ? sph_expand_rt_launch_f32 : sph_expand_rt_launch_f64)(
+            st->smem_optin, xyz, radial, seg_ptr, n_seg, l_max, n_rad, coeff, static_cast<cudaStream_t>(stream));
+        if (r < 0) return fail(SPHERICART_CUDA_ECUDA, "expand launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+        if (r == 0) {
+            launched("expand_rt");
+            return 0;
+        }
+    }
     // every other (l_max, n_rad): run-time sizes, one CTA per (segment, slice of the radial rows)
     const int L = (l_max + 1) * (l_max + 1);
     if (n_seg > 0x7fffffff) return fail(SPHERICART_CUDA_EINVAL, "n_seg = %lld is too large", (long long)n_seg);

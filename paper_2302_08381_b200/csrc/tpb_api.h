@@ -30,7 +30,10 @@ SPH_VJPR_DECL(f64)
 #define SPH_EXPAND_DECL(sfx)                                                                                   \
     int sph_expand_launch_##sfx(int smem_optin, const void* xyz, const void* radial, const int64_t* seg_ptr,  \
                                 int64_t n_seg, int l_max, int n_rad, void* coeff, cudaStream_t stream);       \
-    int sph_expand_upload_##sfx(const SphTables* host_tables);
+    int sph_expand_upload_##sfx(const SphTables* host_tables);                                                \
+    /* run-time l_max <= 32, n_rad <= 16 (kernel_expand_rt.cuh): 1 if n_rad is larger, -1 CUDA error */      \
+    int sph_expand_rt_launch_##sfx(int smem_optin, const void* xyz, const void* radial, const int64_t* seg_ptr, \
+                                   int64_t n_seg, int l_max, int n_rad, void* coeff, cudaStream_t stream);
 SPH_EXPAND_DECL(f32)
 SPH_EXPAND_DECL(f64)
 #undef SPH_EXPAND_DECL
