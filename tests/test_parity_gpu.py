@@ -510,7 +510,8 @@ def test_expand_segment_layouts(sph, oracle, dtype):
                             f"expand {dtype} {what} l_max={l_max} n_rad={n_rad}")
         assert np.all(c.cpu().numpy()[np.nonzero(np.diff(seg) == 0)[0]] == 0)
 
-    for l_max, n_rad in ((8, 8), (5, 3), (6, 7)):          # 72 / 18 / 49 radial values per point
+    # (l_max <= 8: the compile-time kernel; above: the banded run-time kernel, n_rad <= 8 and 9..16)
+    for l_max, n_rad in ((8, 8), (5, 3), (6, 7), (12, 8), (10, 3), (17, 12)):   # radial rows with and without 16-byte multiples
         run([0] * 40 + [5003] + [0] * 60, l_max, n_rad, "one long segment among empty ones")
         run([0] * 500, l_max, n_rad, "every segment empty")
         run([37], l_max, n_rad, "a single segment")
