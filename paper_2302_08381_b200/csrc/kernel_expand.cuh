@@ -6,23 +6,24 @@
 // writes n_rad L values per SEGMENT -- against L values written and read back per POINT when
 // sphericart_cuda_compute is followed by a separate contraction.
 //
-// One warp per segment.  Per tile of 16 points of the segment
+// Persistent grid: every warp takes a contiguous range of segments of (nearly) equal POINT count.  Per
+// tile of 16 points of a segment
 //   1. two lanes per point (cos | sin branch of Eq. 5, as in kernel_tpb.cuh, l_max compile-time)
 //      evaluate the normalised harmonics into a [16][L] image in shared memory (f64 / double-double
-//      recurrences, stored in the I/O type), while the tile's radial values ([16][n_rad][l_max+1],
-//      one contiguous range) are copied next to it, widened to double ONCE here: the contraction
-//      runs in f64 and reads every radial value 2l+1 times (ncu on the first version, which widened
-//      each operand where it was used: the XU pipe of the f32->f64 conversions 63 % busy, the top
-//      pipe of the kernel);
+//      recurrences, stored in the I/O type; in f64 for l_max <= 3), while the tile's radial values
+//      ([16][n_rad][l_max+1], one contiguous range of global memory) land next to it as ONE bulk load
+//      (TMA, mbarrier), requested right after the previous tile's contraction;
 //   2. the contraction over the tile's points is, for every degree l, a small dense product
 //          C_l [n_rad x (2l+1)]  +=  R_l^T [n_rad x 16]  .  Y_l [16 x (2l+1)]
 //      and runs on the f64 tensor-core path: mma.sync m8n8k4 (SASS DMMA), M = radial index n, N = 8
-//      consecutive m of one l, K = 4 points per step; fragments come straight from the two images,
-//      accumulators stay in registers for the whole segment.  (Measured on B200: DMMA sustains the
-//      same 18 T FMA/s as DFMA, but one instruction does 256 FMAs instead of 32 and needs 2 operand
-//      loads instead of 2 per 32: the first version of this kernel, lane = harmonic with one LDS per
-//      DFMA, was bound by the LSU pipe and by issue slots, not by f64 throughput.)
-// At the end of the segment the accumulators go out.
+//      consecutive m of one l, K = 4 points per step; fragments come straight from the two images
+//      (widened to f64 as they are read), accumulators stay in registers for the whole segment.
+//      (Measured on B200: DMMA sustains the same 18 T FMA/s as DFMA, but one instruction does 256 FMAs
+//      instead of 32 and needs 2 operand loads instead of 2 per 32: the first version of this kernel,
+//      lane = harmonic with one LDS per DFMA, was bound by the LSU pipe and by issue slots, not by f64
+//      throughput.)
+// At the end of a segment the accumulators are staged in shared memory and leave as one bulk store.
+// l_max > 8: kernel_expand_rt.cuh (the degrees in bands, run-time loops).
 #pragma once
 #include "kernel_tpb.cuh"
 
