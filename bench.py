@@ -401,18 +401,27 @@ LMAX_FULL = (1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12, 13, 14, 15, 16, 20, 24, 28, 
 LMAX_BRIEF = (8, 12, 16, 20, 24, 28, 32)       # the cells of the default run (the >= 70 % clause: l_max >= 8)
 
 
+def lmax_cell_points(bytes_per_point):
+    """Points of one cell of the l_max axis: ~1.5 GB of output per call, at most 4 M points, at least 256
+    per SM.  (The floor was 64 per SM at first: the long rows then ran calls of a few CTAs per SM whose
+    ramp and tail cost them 5-30 % -- f64 Hessians at l_max = 32: 4.2 TB/s at 13 k points, 5.8 at 38 k,
+    6.0 at 76 k; C4, the configuration with such rows, has 262 k.  Sizing EVERY cell for ~3.2 GB instead
+    was measured too: the sweep then runs power-capped, median SM clock 1826 MHz instead of 1935-1965,
+    and the compute-heavy f64 cells lose 7-15 %.)"""
+    n = int(min(4_000_000, 1.5e9 // bytes_per_point)) // 256 * 256
+    return max(n, 148 * 256)
+
+
 def lmax_cell(torch, pkg, device, peak, dtype, deriv, l_max, normalized=1, n=None, reps=None):
-    """One cell of the metric's axis: xyz ~ N(0,1) on the device, n sized for ~1.5 GB of output (at
-    most 4 M points, at least 64 per SM), two rotating output sets where they fit; CUDA events."""
+    """One cell of the metric's axis: xyz ~ N(0,1) on the device, n from lmax_cell_points, two rotating
+    output sets where they fit; CUDA events."""
     st = torch.cuda.current_stream().cuda_stream
     tdt, es = (torch.float32, 4) if dtype == "f32" else (torch.float64, 8)
     mult = (1, 4, 13)[deriv]
     L = (l_max + 1) ** 2
     per_pt = L * es * mult
     if n is None:
-        n = int(min(4_000_000, 1.5e9 // per_pt)) // 256 * 256
-        if n < 148 * 64:          # too few points to fill the machine within the byte budget:
-            n = 148 * 64          # (Hessians at l_max >= 20) take more memory instead
+        n = lmax_cell_points(per_pt)
     x = torch.randn(n, 3, device=device, dtype=tdt)
     n_sets = 2 if n * per_pt < 3e9 else 1
     outs = [(torch.empty((n, L), device=device, dtype=tdt),
@@ -545,7 +554,7 @@ def workload_config(args):
         return W.CONFIGS[args.workload]
     es = 4 if args.dtype == "f32" else 8
     per_pt = (args.l_max + 1) ** 2 * es * (1, 4, 13)[args.deriv]
-    n = args.n or max(148 * 64, int(min(4_000_000, 1.5e9 // per_pt)) // 256 * 256)
+    n = args.n or lmax_cell_points(per_pt)
     what = (f"custom: N={n} {args.dtype} l_max={args.l_max} {'solid' if args.solid else 'normalized'} "
             f"{('Y', 'Y+grad', 'Y+grad+Hessian')[args.deriv]}, xyz~N(0,1)")
     return W.Config("C9", n, args.dtype, args.l_max, not args.solid, args.deriv >= 1, args.deriv >= 2, False, what)
@@ -785,7 +794,7 @@ def main():
     ap.add_argument("--l-max", type=int, default=8, help="--workload custom")
     ap.add_argument("--deriv", type=int, choices=[0, 1, 2], default=1, help="--workload custom: 0 Y, 1 +grad, 2 +Hessian")
     ap.add_argument("--solid", action="store_true", help="--workload custom: solid harmonics instead of normalised")
-    ap.add_argument("--n", type=int, default=0, help="--workload custom: points (default: ~1.5 GB of output)")
+    ap.add_argument("--n", type=int, default=0, help="--workload custom: points (default: as the l_max sweep, ~1.5 GB of output)")
     ap.add_argument("--op", choices=["forward", "vjp_recompute", "vjp2", "expand"], default="forward",
                     help="--workload custom --kernels-only: the entry point the step calls")
     ap.add_argument("--option", action="append", default=[], metavar="NAME=VALUE",

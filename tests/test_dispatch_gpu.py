@@ -93,14 +93,16 @@ def test_default_dispatch_expand(sph, oracle, dtype, l_max):
                                                ("f64", 14, 0), ("f32", 28, 0), ("f64", 20, 1), ("f32", 20, 2)])
 def test_sweep_cells_at_bench_size(sph, oracle, dtype, l_max, deriv):
     """Cells of the l_max sweep at the size and launch configuration bench.py times them in (n sized for
-    ~1.5 GB of output: several batches per CTA, every SM busy), default dispatch: sampled points against the
+    ~1.5 GB of output, at least 256 points per SM: several batches per CTA, every SM busy), default dispatch: sampled points against the
     oracle (first / last points and tile edges included) and, on EVERY point, properties that hold at any
     size: the addition theorem sum_m Y_lm^2 = (2l+1)/4pi, Euler's x . grad Y = 0 for the normalised
     harmonics, and trace(Hessian) = -l(l+1) Y / r^2."""
     es = 4 if dtype == "f32" else 8
     L = (l_max + 1) ** 2
     per_pt = L * es * (1, 4, 13)[deriv]
-    n = max(148 * 64, int(min(4_000_000, 1.5e9 // per_pt)) // 256 * 256) + 37          # + a ragged tail
+    import bench
+
+    n = bench.lmax_cell_points(per_pt) + 37          # bench.py's size for the cell + a ragged tail
     tdt = torch.float32 if dtype == "f32" else torch.float64
     g = torch.Generator(device="cuda").manual_seed(1000 + l_max)
     x_d = torch.randn(n, 3, device="cuda", dtype=tdt, generator=g)
