@@ -1,7 +1,7 @@
 // "wc" forward kernel: the warps of a CTA work TOGETHER on one point at a time, so that a staged
 // chunk is a third of a row (<= 368 harmonics) and every bulk store is ~3 KB.  Works for
-// l_max >= 19 and any derivative order; used by default where it wins: f64 at l_max = 32 --
-// config C4.  (Measured, Hessians, 131 072-262 144 points: f64 l_max = 32 5.0 TB/s against 4.7 for the
+// l_max >= 19 and any derivative order; used by default where it wins: f64 Hessians from l_max = 24
+// and every f64 output set at l_max = 32 -- config C4.  (Measured, Hessians, 131 072-262 144 points: f64 l_max = 32 5.0 TB/s against 4.7 for the
 // one-warp-per-point kernel -- 6.2 against 4.9 at C4's full size with rotating outputs -- but
 // 4.4-4.9 against 4.7-5.1 at l_max 28-31, whose rows split less evenly into chunks and, for even L,
 // are 128-byte aligned anyway; f32: 1.9-2.8 against 2.7-2.9 at every l_max.)
@@ -370,8 +370,13 @@ static inline int wc_plan(int min_l, int sm_count, int smem_optin, int64_t n, in
     out->prm.row0[nc] = (unsigned char)(l_max + 1);
     for (int e = l_max + 1, i = nc; e > 0; e = from[e]) out->prm.row0[--i] = (unsigned char)from[e];
     out->prm.n_chunks = nc;
-    int64_t ppc = n / ((int64_t)sm_count * 4);   // >= 4 CTAs per SM where n allows
-    if (ppc > WC_PTS) ppc = WC_PTS;
+    // One CTA per SM is resident: the grid is sized in WHOLE waves -- k = the fewest that keep a CTA at
+    // <= WC_PTS points, at least 4 where n allows -- and the points dealt evenly over k * sm_count CTAs.
+    // (n / (4 SMs) points per CTA, capped, left a last wave of a few CTAs at some sizes: n = 131 072 ran
+    // 594 CTAs = 4 waves + 2 CTAs, 3.7-4.9 TB/s where 37 888 and 262 144 points reached 4.3-6.0.)
+    int64_t waves = (n + (int64_t)WC_PTS * sm_count - 1) / ((int64_t)WC_PTS * sm_count);
+    if (waves < 4) waves = 4;
+    int64_t ppc = (n + waves * sm_count - 1) / (waves * sm_count);
     if (ppc < 16) ppc = 16;
     out->prm.pts_per_cta = (int)ppc;
     out->grid = (n + ppc - 1) / ppc;
