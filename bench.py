@@ -230,6 +230,30 @@ def time_loop(torch, fn, steps):
     return e0, e1
 
 
+def capture_steps(torch, wl, steps):
+    """The `steps` calls of the timed region captured ONCE into a CUDA graph (on a side stream, the
+    workload's launches pointed at it for the capture).  Replaying it inside the timed region submits
+    exactly the same kernels in the same order with no host launch latency between the timing events
+    and the first kernel -- with K host launches that gap and the first launches' ramp are ~25 us of a
+    460 us region at C2 (23.0 us per step at K = 20, 21.6 at K = 160).  Returns (graph, kernels in it)."""
+    pkg = wl.pkg
+    graph = torch.cuda.CUDAGraph()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    saved = wl.stream
+    before = pkg.sphericart_cuda_launch_count()
+    try:
+        with torch.cuda.stream(side):
+            wl.stream = side.cuda_stream
+            with torch.cuda.graph(graph, stream=side):
+                for i in range(steps):
+                    wl.step(i)
+    finally:
+        wl.stream = saved
+    torch.cuda.current_stream().wait_stream(side)
+    return graph, pkg.sphericart_cuda_launch_count() - before
+
+
 def n_sets_for(cfg, free_bytes):
     per_set = cfg.n * cfg.out_bytes_per_point
     want = N_SETS if per_set < (2 << 30) else 2
@@ -651,14 +675,32 @@ def run_cuda(args):
     for i in range(max(args.warmup, 3)):
         wl.step(i)
     barrier()
+    # the K steps of the timed region: one CUDA graph replay (default), or K host launches (--submit eager)
+    graph, eager_ms_step, graph_note = None, None, None
+    if args.submit == "graph" and not args.kernels_only:     # (profiling runs keep plain launches)
+        e0, e1 = time_loop(torch, wl.step, args.steps)      # the eager number, reported beside the graph's
+        barrier()
+        eager_ms_step = e0.elapsed_time(e1) / args.steps
+        try:
+            graph, graph_kernels = capture_steps(torch, wl, args.steps)
+            graph.replay()                                   # (untimed: instantiation and upload of the graph)
+        except Exception as exc:                             # capture refused: time the host launches instead
+            graph, graph_note = None, f"graph capture failed ({type(exc).__name__}): K host launches timed"
+        barrier()
     clocks = ClockSampler(local_rank)
     clocks.start()
     launches0 = pkg.sphericart_cuda_launch_count()
-    e0, e1 = time_loop(torch, wl.step, args.steps)
+    if graph is not None:
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        graph.replay()
+        e1.record()
+    else:
+        e0, e1 = time_loop(torch, wl.step, args.steps)
     clocks.sample()                              # the GPU is still draining the queue here
     barrier()
     clocks.stop()
-    launches = pkg.sphericart_cuda_launch_count() - launches0
+    launches = graph_kernels if graph is not None else pkg.sphericart_cuda_launch_count() - launches0
     ms_total = e0.elapsed_time(e1)
     if dist is not None:
         t = torch.tensor([ms_total], device=device, dtype=torch.float64)
@@ -697,7 +739,11 @@ def run_cuda(args):
                        "vjp": cfg.vjp, "parallelism": f"points sharded over {world} GPU(s), no collective",
                        "l2": f"outputs rotate over {len(wl.sets)} buffer sets "
                              f"({len(wl.sets) * cfg.n * cfg.out_bytes_per_point / 1e6:.0f} MB written before reuse "
-                             "> 126 MB L2)"},
+                             "> 126 MB L2)",
+                       "submission": ("the K steps are captured once into a CUDA graph and replayed inside the timed "
+                                      "region (same kernels, same order, no host launch latency between the events); "
+                                      f"K host launches instead: {eager_ms_step * 1e3:.2f} us per step (--submit eager)")
+                                     if graph is not None else (graph_note or "K host launches inside the timed region")},
             "clocks": clocks.summary(), "gpu_launches": int(launches), "roofline": roofline}
     if rank == 0 and not args.kernels_only:
         line["roofline"]["store_ceiling_gbs"] = store_ceiling_gbs(torch, cfg.n * cfg.out_bytes_per_point, device)
@@ -801,6 +847,8 @@ def main():
                     help="sphericart_cuda_set_option(NAME, VALUE) before anything runs (experiments)")
     ap.add_argument("--e2e-steps", type=int, default=20)
     ap.add_argument("--no-sweep", action="store_true", help="skip the brief timing of the other configurations")
+    ap.add_argument("--submit", choices=("graph", "eager"), default="graph",
+                    help="the K timed steps as one CUDA graph replay (default) or as K host launches")
     ap.add_argument("--lmax-sweep", action="store_true",
                     help="print output GB/s against l_max (f32/f64, +-gradients) as one JSON object and exit")
     ap.add_argument("--render-lmax-table", metavar="FILE", default=None,
