@@ -32,6 +32,7 @@ struct TvParams {
 struct TvSmem {
     int CP;                 // (c, s) pairs per point and set
     uint32_t pitch;         // bytes between the rows of the image
+    bool contig;            // rows end to end (odd L)
     size_t cs_off, img_off, total;
     __host__ __device__ TvSmem(int l_max, int esize, int batch) {
         CP = (l_max + 1) | 1;   // odd pitch: conflict-free lane = point stores
@@ -41,6 +42,12 @@ struct TvSmem {
         uint32_t units = (L * esize + 16 + 15) / 16;
         units |= 1;
         pitch = units * 16;
+        // Odd L (even l_max): the rows are an odd number of elements long, so laid end to end -- the image
+        // byte-identical to global memory -- lane = point stores are conflict-free as they are, no row needs
+        // staging at an offset, and a whole batch leaves as ONE bulk store (a batch starts at a multiple of
+        // 8 points: 16-byte aligned).  Even L keeps the padded rows above, each its own (aligned) bulk store.
+        contig = (L & 1u) != 0;
+        if (contig) pitch = L * esize;
         cs_off = 0;
         img_off = ((size_t)2 * batch * CP * 16 + 127) & ~(size_t)127;
         total = img_off + (size_t)batch * pitch;
@@ -146,7 +153,7 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 1) sph_tv_kernel(const TvPa
                 named_bar_sync(1, Wq * 32);
             }
             // this point's row, staged at the offset its global address has from a 16-byte boundary
-            const uint32_t shift = (uint32_t)(((b0 + pt_l) & 15) * row_b) & 15u;
+            const uint32_t shift = lay.contig ? 0u : (uint32_t)(((b0 + pt_l) & 15) * row_b) & 15u;
             const uint32_t row = sIMG + pt_l * lay.pitch + shift;
             const uint32_t cs_row = sCS + ((set * B + pt_l) * CP) * 16;
             // one entry of column m at row l: the harmonics (l, +m) and (l, -m); the sin one first, so that
@@ -228,7 +235,18 @@ __global__ void __launch_bounds__(TQ_MAX_WARPS * 32, 1) sph_tv_kernel(const TvPa
         }
         fence_proxy_async_smem();
         __syncthreads();   // the image is complete; so are the next batch's powers
-        if (threadIdx.x < B) {
+        if (lay.contig) {
+            const int np = (int)min((int64_t)B, n - b0);
+            const T* src = reinterpret_cast<const T*>(smem + lay.img_off);
+            if (np == B) {   // (B x L x ES is a multiple of 16 bytes: B >= 8)
+                if (threadIdx.x == 0) {
+                    bulk_store_hint(sph + b0 * L, src, (uint32_t)B * row_b, policy);
+                    bulk_commit();
+                }
+            } else {         // ragged last batch: plain stores (read before the next barrier: nothing left in flight)
+                for (int i = threadIdx.x; i < np * L; i += blockDim.x) st_cs(sph + b0 * L + i, src[i]);
+            }
+        } else if (threadIdx.x < B) {
             const int64_t p = b0 + threadIdx.x;
             if (p < n) {
                 const uint32_t d = (uint32_t)((p & 15) * row_b) & 15u;

@@ -35,10 +35,11 @@ static const unsigned char TQ_SHAPE[2][3][33][4] = {
 // Launch shapes of the values-only kernel (kernel_tv.cuh), and where the default dispatch uses it:
 // TV_SHAPE[f64][l_max] = {B, W, C}: points per batch, warps per CTA, warps that run Eq. 9 only (f64);
 // {0,0,0}: another family is at least as fast.  Same protocol as above, l_max = 10..32, over
-// B in {32,16,8} x W in {4,6,8} x C in {1,2}.
+// B in {32,16,8} x W in {4,6,8} x C in {1,2}; re-measured over W in {2..6,8,10,12} after the kernel's image became
+// contiguous for odd L (one bulk store per batch).
 static const unsigned char TV_SHAPE[2][33][3] = {
-    /* f32 */ {{0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {16,3,1}, {0,0,0}, {8,2,1}, {16,5,1}, {16,4,1}, {8,3,1}, {8,3,1}, {8,3,1}, {8,3,1}, {8,4,1}, {8,3,1}, {8,3,1}, {8,4,1}, {8,5,1}},
-    /* f64 */ {{0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {32,5,1}, {32,5,1}, {16,3,1}, {16,4,1}, {16,4,1}, {16,4,1}, {16,4,1}, {16,5,1}, {16,5,1}, {0,0,0}, {8,3,1}, {16,6,2}, {16,6,2}, {0,0,0}, {16,6,1}, {0,0,0}, {8,4,1}, {0,0,0}, {8,4,1}, {0,0,0}},
+    /* f32 */ {{0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {16,3,1}, {16,4,1}, {8,2,1}, {16,5,1}, {16,4,1}, {16,5,1}, {8,3,1}, {8,3,1}, {8,3,1}, {16,5,1}, {8,3,1}, {8,3,1}, {8,3,1}, {8,3,1}},
+    /* f64 */ {{0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {0,0,0}, {32,4,1}, {32,5,1}, {32,5,1}, {16,3,1}, {16,4,1}, {16,4,1}, {16,4,1}, {16,4,1}, {16,5,1}, {16,5,1}, {16,6,2}, {8,3,1}, {16,6,2}, {16,6,2}, {16,6,2}, {16,6,1}, {8,4,1}, {8,4,1}, {8,4,1}, {8,4,1}, {8,6,1}},
 };
 
 }  // namespace sphb200
