@@ -21,7 +21,7 @@
 
 namespace sphb200 {
 
-constexpr int EXRT_MAX_BANDS = 20;   // l_max = 32: 153 N-tiles; bands of >= 8 tiles
+constexpr int EXRT_MAX_BANDS = 24;   // l_max = 32: 153 N-tiles in 11 bands of <= 16; 22 bands of <= 9 (n_rad > 8)
 constexpr int EXRT_MAX_NTB = 16;     // N-tiles per band at most
 
 struct ExpandRtParams {
