@@ -150,9 +150,9 @@ static int launch_w(const DeviceState& st, const void* xyz, int64_t n, int l_max
         // the longest f64 rows: the warps of a CTA share one point, chunks of a third of a row, ~3 KB
         // bulk stores (kernel_wc.cuh says where it wins); FORCE_WC takes it wherever it can run
         const bool force_wc = g_opt.force_kernel == FORCE_WC;
-        // (default: f64 with Hessians from l_max = 24 -- measured at 38 k / 131 k / 262 k points: 4.3-6.0 TB/s
-        // against 3.7-5.1 of the two-phase and the warp-per-point kernels -- and every f64 output set at l_max = 32)
-        int min_l = force_wc ? 19 : (dtype == SPHERICART_CUDA_F64 ? (ddsph ? 24 : 32) : SPHERICART_CUDA_MAX_L + 1);
+        // (default: f64 with Hessians from l_max = 29 -- 5.1-5.8 TB/s at 38 k points against 4.2 of the two-phase
+        // kernel's one-point tiles, which win below -- and every f64 output set at l_max = 32)
+        int min_l = force_wc ? 19 : (dtype == SPHERICART_CUDA_F64 ? (ddsph ? 29 : 32) : SPHERICART_CUDA_MAX_L + 1);
         if (g_opt.wc_min_l > 0) min_l = g_opt.wc_min_l;
         WcLaunch lc{};
         if (wc_plan(min_l, st.sm_count, st.smem_optin, n, l_max, normalized, dtype, sph, dsph, ddsph, xyz, st.d_tables, &lc) == 0) {

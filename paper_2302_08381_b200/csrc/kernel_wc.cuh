@@ -1,6 +1,6 @@
 // "wc" forward kernel: the warps of a CTA work TOGETHER on one point at a time, so that a staged
 // chunk is a third of a row (<= 368 harmonics) and every bulk store is ~3 KB.  Works for
-// l_max >= 19 and any derivative order; used by default where it wins: f64 Hessians from l_max = 24
+// l_max >= 19 and any derivative order; used by default where it wins: f64 Hessians from l_max = 29
 // and every f64 output set at l_max = 32 -- config C4.  (Measured, Hessians, 131 072-262 144 points: f64 l_max = 32 5.0 TB/s against 4.7 for the
 // one-warp-per-point kernel -- 6.2 against 4.9 at C4's full size with rotating outputs -- but
 // 4.4-4.9 against 4.7-5.1 at l_max 28-31, whose rows split less evenly into chunks and, for even L,

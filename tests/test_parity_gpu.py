@@ -371,16 +371,17 @@ def test_two_phase_kernel(sph, oracle, dtype, l_max, option):
 
 
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
-@pytest.mark.parametrize("shape", [(32, 2, 4, 2), (16, 2, 8, 1), (8, 2, 6, 2), (8, 2, 3, 1), (16, 8, 5, 2), (32, 4, 8, 1)])
+@pytest.mark.parametrize("shape", [(32, 2, 4, 2), (16, 2, 8, 1), (8, 2, 6, 2), (8, 2, 3, 1), (16, 8, 5, 2), (32, 4, 8, 1),
+                                   (8, 1, 4, 1), (16, 1, 6, 2), (32, 1, 12, 2)])
 def test_two_phase_kernel_shapes(sph, oracle, dtype, shape, option):
     """Every launch shape of kernel_tq.cuh the shape table can name: batches of 32 / 16 / 8 points
-    (1 / 2 / 4 lanes per point in the recurrence phase), tiles of 2 / 4 / 8 points, one or two
+    (1 / 2 / 4 lanes per point in the recurrence phase), tiles of 1 / 2 / 4 / 8 points, one or two
     images; ragged n, odd and even row lengths."""
     np_dt = np.float32 if dtype == "f32" else np.float64
     option("force_kernel", "tq")
     for name, value in zip(("tq_batch", "tq_points", "tq_warps", "tq_images"), shape):
         option(name, value)
-    for l_max, n in ((9, 203), (12, 77), (15, 131), (16, 1), (22, 70)):
+    for l_max, n in ((9, 203), (12, 77), (15, 131), (16, 1), (22, 70), (27, 41)):
         xyz = W.make_xyz("C2" if l_max <= 16 else "C4", n, seed=l_max).astype(np_dt)
         for normalized, deriv in ((True, 2), (False, 1), (True, 0)):
             s, d, h = _run_gpu(sph, xyz, l_max, normalized, deriv >= 1, deriv >= 2)
