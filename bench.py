@@ -770,6 +770,9 @@ def run_cuda(args):
         line["cpu_baseline"] = base
         if not args.no_sweep:
             line["sweep"] = {}
+            # the l_max axis first: it follows the oracle's seconds on the host, i.e. a GPU that is not yet
+            # power-capped by the large configurations below (their cells are HBM-bound and do not care)
+            lmax_rows = lmax_sweep(torch, pkg, device, peak, LMAX_BRIEF)
             for name in ("C1", "C2", "C3", "C4", "C5"):
                 c = W.CONFIGS[name]
                 free, _ = torch.cuda.mem_get_info()
@@ -778,7 +781,7 @@ def run_cuda(args):
                     continue
                 line["sweep"][name] = sweep_one(c, torch, pkg, device, peak)
             line["sweep"]["N2_expand"] = sweep_expand(torch, pkg, device, peak)
-            line["sweep"]["lmax"] = lmax_sweep(torch, pkg, device, peak, LMAX_BRIEF)
+            line["sweep"]["lmax"] = lmax_rows
             line["sweep"]["backward"] = sweep_backward(torch, pkg, device, peak)
     if dist is not None:
         dist.barrier()
